@@ -1,0 +1,418 @@
+/*
+ * psg_oracle.c -- ORACLE. Test infrastructure, not the product.
+ *
+ * A plain, slow, fp64 CPU restatement of the per-MD-step enhanced-sampling hot
+ * path that PySAGES (arXiv 2301.04835; /root/reference/PAPER.md) defines:
+ *   gather CV atoms -> collective variables + analytic Jacobians -> bias energy
+ *   and gradient -> F_i += -dV/dxi * dxi/dr_i.
+ *
+ * Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl
+ * reference legs may build, load or call this file.  It shares no code, header,
+ * table or constant with paper_2301_04835_b200/csrc (the CUDA path) and neither
+ * side includes the other.
+ *
+ * The paper names the quantities but prints no formula for them (the only
+ * equations are Eq. 1-3, and the interface CV Eq. 4-8), so
+ * each function below is the textbook definition of the quantity the cited
+ * passage names, under the readings listed in DESIGN.md ("Readings").
+ * Inputs arrive as IEEE binary32 (the engine's arrays) and are widened exactly
+ * to binary64; every operation is binary64 except the ABF bin index, which
+ * DESIGN.md reading R-ABF-1 defines in binary32 so that "bit-exact" is
+ * meaningful.  Compile with -O2 -ffp-contract=off, no fast-math.
+ *
+ * Pins (tests/test_oracle_*.py, run with -m "not gpu"): closed-form geometries,
+ * central finite differences, translation/rotation invariance of forces,
+ * periodicity, single-hill closed forms, hand-computed ABF tables.
+ * Parity unpinned (no passage, closed form or invariant fixes them; they follow
+ * DESIGN.md readings only): the order of simultaneous deposits by several
+ * walkers (orc_deposit_hills), the two-phase mean-force read of a shared ABF
+ * grid (orc_abf_update), the stride phase of deposits.
+ */
+#include <math.h>
+#include <stdlib.h>
+#include <string.h>
+#ifdef _OPENMP
+#include <omp.h>
+#endif
+
+enum { ORC_DISTANCE = 1, ORC_ANGLE = 2, ORC_DIHEDRAL = 3, ORC_COMPONENT = 4, ORC_RGYR = 5 };
+
+/* One collective variable: a function of 1..4 *groups* of atoms, each group
+ * reduced to its (weighted) barycenter -- PAPER.md:L185-L189 (Sec. 2.2:
+ * TwoPointCV/ThreePointCV/FourPointCV/AxisCV "groups"), L227-L229 (Fig. 3,
+ * barycenter(p1)).  A group is either an explicit slice [begin, begin+size) of
+ * the slot list, or a contiguous atom range of the replica's array. */
+typedef struct {
+    int type;
+    int n_groups;
+    int is_range[4];
+    int slot_begin[4];
+    int slot_size[4];
+    long long range_begin[4];
+    long long range_size[4];
+    int axis;       /* ORC_COMPONENT: 0, 1 or 2 */
+    double period;  /* 0 = not periodic */
+} orc_cv;
+
+/* Where the engine's arrays are: PAPER.md:L37 (Snapshot: positions, forces). */
+typedef struct {
+    int n_replicas;
+    long long n_atoms;
+    long long replica_stride_atoms; /* 0: every replica indexes ONE shared array */
+    int pos_stride;                 /* floats per atom in pos: 3 or 4 */
+    int n_cv;
+    int n_slots;
+    int per_replica_slots;          /* 0: slot_atom[n_slots]; 1: slot_atom[R][n_slots] */
+} orc_layout;
+
+int orc_num_threads(void) {
+#ifdef _OPENMP
+    return omp_get_max_threads();
+#else
+    return 1;
+#endif
+}
+
+void orc_set_threads(int n) {
+#ifdef _OPENMP
+    if (n > 0) omp_set_num_threads(n);
+#else
+    (void)n;
+#endif
+}
+
+/* ---------- small vector helpers (fp64) ---------- */
+static void v_sub(const double *a, const double *b, double *o) { o[0] = a[0] - b[0]; o[1] = a[1] - b[1]; o[2] = a[2] - b[2]; }
+static double v_dot(const double *a, const double *b) { return a[0] * b[0] + a[1] * b[1] + a[2] * b[2]; }
+static void v_cross(const double *a, const double *b, double *o) {
+    o[0] = a[1] * b[2] - a[2] * b[1];
+    o[1] = a[2] * b[0] - a[0] * b[2];
+    o[2] = a[0] * b[1] - a[1] * b[0];
+}
+
+/* Nearest-image difference for a periodic CV: d <- d - P*rint(d/P).
+ * DESIGN.md reading R-PER (the paper is silent; Grid(..., periodic=True),
+ * PAPER.md:L82). */
+static double wrap_period(double d, double period) {
+    if (period > 0.0) d -= period * rint(d / period);
+    return d;
+}
+
+/* number of atoms of group g of a CV and the i-th atom's index and weight */
+static long long group_count(const orc_cv *cv, int g) { return cv->is_range[g] ? cv->range_size[g] : (long long)cv->slot_size[g]; }
+
+static long long group_atom(const orc_cv *cv, int g, long long i, const int *slot_atom) {
+    return cv->is_range[g] ? cv->range_begin[g] + i : (long long)slot_atom[cv->slot_begin[g] + i];
+}
+
+/* weight of the i-th atom of group g: explicit groups index slot_weight by slot,
+ * range groups index atom_weight by atom; NULL => 1 (barycenter, Fig. 3). */
+static double group_weight(const orc_cv *cv, int g, long long i, const float *slot_weight, const float *atom_weight) {
+    if (cv->is_range[g]) return atom_weight ? (double)atom_weight[cv->range_begin[g] + i] : 1.0;
+    return slot_weight ? (double)slot_weight[cv->slot_begin[g] + i] : 1.0;
+}
+
+/* c_g = sum_i w_i r_i / sum_i w_i  (PAPER.md:L227-L229 barycenter; with masses
+ * as weights the "center of mass" of L332, L408). */
+static void group_center(const orc_cv *cv, int g, const float *pos, int ps, const int *slot_atom,
+                         const float *slot_weight, const float *atom_weight, double *c, double *wsum) {
+    double s[3] = {0, 0, 0}, W = 0;
+    long long n = group_count(cv, g);
+    for (long long i = 0; i < n; ++i) {
+        long long a = group_atom(cv, g, i, slot_atom);
+        double w = group_weight(cv, g, i, slot_weight, atom_weight);
+        s[0] += w * (double)pos[a * ps + 0];
+        s[1] += w * (double)pos[a * ps + 1];
+        s[2] += w * (double)pos[a * ps + 2];
+        W += w;
+    }
+    c[0] = s[0] / W; c[1] = s[1] / W; c[2] = s[2] / W;
+    *wsum = W;
+}
+
+/* xi and d(xi)/d(c_g) for the CVs that are functions of group centers only. */
+static double point_cv(const orc_cv *cv, double c[4][3], double dc[4][3]) {
+    memset(dc, 0, sizeof(double) * 12);
+    switch (cv->type) {
+    case ORC_DISTANCE: { /* PAPER.md:L185 Distance: xi = |c2 - c1| */
+        double d[3]; v_sub(c[1], c[0], d);
+        double r = sqrt(v_dot(d, d));
+        if (r > 0) for (int x = 0; x < 3; ++x) { dc[1][x] = d[x] / r; dc[0][x] = -d[x] / r; }
+        return r;
+    }
+    case ORC_ANGLE: { /* PAPER.md:L186 Angle; vertex at the second group (reading R-ANG) */
+        double q[3], s[3], n[3], t[3];
+        v_sub(c[0], c[1], q); v_sub(c[2], c[1], s); v_cross(q, s, n);
+        double nn = sqrt(v_dot(n, n));
+        double th = atan2(nn, v_dot(q, s));
+        if (nn > 0) {
+            double q2 = v_dot(q, q), s2 = v_dot(s, s);
+            v_cross(q, n, t); for (int x = 0; x < 3; ++x) dc[0][x] = t[x] / (q2 * nn);
+            v_cross(s, n, t); for (int x = 0; x < 3; ++x) dc[2][x] = -t[x] / (s2 * nn);
+            for (int x = 0; x < 3; ++x) dc[1][x] = -(dc[0][x] + dc[2][x]);
+        }
+        return th;
+    }
+    case ORC_DIHEDRAL: { /* PAPER.md:L187 DihedralAngle, L81; IUPAC sign (reading R-DIH) */
+        double b1[3], b2[3], b3[3], n1[3], n2[3];
+        v_sub(c[1], c[0], b1); v_sub(c[2], c[1], b2); v_sub(c[3], c[2], b3);
+        v_cross(b1, b2, n1); v_cross(b2, b3, n2);
+        double lb2 = sqrt(v_dot(b2, b2));
+        double phi = atan2(lb2 * v_dot(b1, n2), v_dot(n1, n2));
+        double n1s = v_dot(n1, n1), n2s = v_dot(n2, n2);
+        if (n1s > 0 && n2s > 0) {
+            double a = v_dot(b1, b2) / (lb2 * lb2), e = v_dot(b3, b2) / (lb2 * lb2);
+            for (int x = 0; x < 3; ++x) {
+                dc[0][x] = -(lb2 / n1s) * n1[x];
+                dc[3][x] = (lb2 / n2s) * n2[x];
+            }
+            for (int x = 0; x < 3; ++x) {
+                dc[1][x] = -(1.0 + a) * dc[0][x] + e * dc[3][x];
+                dc[2][x] = -(1.0 + e) * dc[3][x] + a * dc[0][x];
+            }
+        }
+        return phi;
+    }
+    case ORC_COMPONENT: /* PAPER.md:L188 Component: barycenter coordinate along an axis */
+        dc[0][cv->axis] = 1.0;
+        return c[0][cv->axis];
+    }
+    return NAN;
+}
+
+/* Evaluate one CV of one replica.  jac (nullable) receives d(xi)/d(r_i), three
+ * doubles per atom, for the atoms of group 0, then group 1, ... in group order.
+ * Returns xi. */
+static double cv_one(const orc_cv *cv, const float *pos, int ps, const int *slot_atom,
+                     const float *slot_weight, const float *atom_weight, double *jac) {
+    if (cv->type == ORC_RGYR) {
+        /* PAPER.md:L189 RadiusofGyration. Reading R-RG: Rg^2 = sum w|r-c|^2 / sum w,
+         * same weights as the barycenter; dRg/dr_i = w_i (r_i - c)/(W Rg). */
+        double c[3], W;
+        group_center(cv, 0, pos, ps, slot_atom, slot_weight, atom_weight, c, &W);
+        long long n = group_count(cv, 0);
+        double s2 = 0;
+        for (long long i = 0; i < n; ++i) {
+            long long a = group_atom(cv, 0, i, slot_atom);
+            double w = group_weight(cv, 0, i, slot_weight, atom_weight);
+            double d[3] = {(double)pos[a * ps] - c[0], (double)pos[a * ps + 1] - c[1], (double)pos[a * ps + 2] - c[2]};
+            s2 += w * v_dot(d, d);
+        }
+        double rg = sqrt(s2 / W);
+        if (jac) for (long long i = 0; i < n; ++i) {
+            long long a = group_atom(cv, 0, i, slot_atom);
+            double w = group_weight(cv, 0, i, slot_weight, atom_weight);
+            for (int x = 0; x < 3; ++x)
+                jac[3 * i + x] = rg > 0 ? w * ((double)pos[a * ps + x] - c[x]) / (W * rg) : 0.0;
+        }
+        return rg;
+    }
+    double c[4][3], W[4], dc[4][3];
+    for (int g = 0; g < cv->n_groups; ++g) group_center(cv, g, pos, ps, slot_atom, slot_weight, atom_weight, c[g], &W[g]);
+    double xi = point_cv(cv, c, dc);
+    if (jac) {
+        long long o = 0;
+        for (int g = 0; g < cv->n_groups; ++g) {
+            long long n = group_count(cv, g);
+            for (long long i = 0; i < n; ++i, ++o) {
+                /* chain rule through the barycenter: d xi/d r_i = (w_i/W_g) d xi/d c_g */
+                double w = group_weight(cv, g, i, slot_weight, atom_weight) / W[g];
+                for (int x = 0; x < 3; ++x) jac[3 * o + x] = w * dc[g][x];
+            }
+        }
+    }
+    return xi;
+}
+
+static long long cv_natoms(const orc_cv *cv) {
+    long long n = 0;
+    for (int g = 0; g < cv->n_groups; ++g) n += group_count(cv, g);
+    return n;
+}
+
+/* Total Jacobian rows per replica (sum over CVs of atoms in their groups). */
+long long orc_jac_rows(const orc_layout *L, const orc_cv *cvs) {
+    long long n = 0;
+    for (int k = 0; k < L->n_cv; ++k) n += cv_natoms(&cvs[k]);
+    return n;
+}
+
+/* cv_eval: xi[R][n_cv]; jac (nullable) [R][jac_rows][3], rows ordered CV by CV,
+ * group by group, atom by atom.  PAPER.md:L39 ("computes the CVs"), L185-L189. */
+void orc_cv_eval(const orc_layout *L, const orc_cv *cvs, const int *slot_atom, const float *slot_weight,
+                 const float *atom_weight, const float *pos, double *xi, double *jac) {
+    long long rows = orc_jac_rows(L, cvs);
+#pragma omp parallel for schedule(static)
+    for (int r = 0; r < L->n_replicas; ++r) {
+        const float *p = pos + (long long)r * L->replica_stride_atoms * L->pos_stride;
+        const int *sa = slot_atom + (L->per_replica_slots ? (long long)r * L->n_slots : 0);
+        long long o = 0;
+        for (int k = 0; k < L->n_cv; ++k) {
+            double *j = jac ? jac + ((long long)r * rows + o) * 3 : NULL;
+            xi[(long long)r * L->n_cv + k] = cv_one(&cvs[k], p, L->pos_stride, sa, slot_weight, atom_weight, j);
+            o += cv_natoms(&cvs[k]);
+        }
+    }
+}
+
+/* Harmonic bias, PAPER.md:L125 (Sec. 2.1.1): H_b = H + k/2 (xi - xi0)^2.
+ * Multi-CV: V = 1/2 sum_k k_k D_k^2, dV/dxi_k = k_k D_k, D wrapped for periodic CVs. */
+void orc_harmonic(int n_replicas, int n_cv, const double *xi, const double *kspring, const double *center,
+                  const double *period, double *V, double *dVdxi) {
+    for (int r = 0; r < n_replicas; ++r) {
+        double v = 0;
+        for (int k = 0; k < n_cv; ++k) {
+            double d = wrap_period(xi[r * n_cv + k] - center[r * n_cv + k], period[k]);
+            v += 0.5 * kspring[k] * d * d;
+            dVdxi[r * n_cv + k] = kspring[k] * d;
+        }
+        V[r] = v;
+    }
+}
+
+/* Metadynamics bias, PAPER.md:L147 (Sec. 2.1.5): a sum of Gaussians of user
+ * height and width.  V(xi) = sum_h W_h exp(-1/2 sum_k (d_hk/sigma_k)^2),
+ * dV/dxi_k = -sum_h W_h exp(..) d_hk/sigma_k^2, d_hk = wrap(xi_k - s_hk).
+ * Tabs[R][n_cv] (nullable) = sum_h |term| of the gradient sum: its conditioning. */
+void orc_metad(int n_replicas, int n_cv, const double *xi, long long n_hills, const float *centers /*[n][n_cv]*/,
+               const float *heights, const double *sigma, const double *period, double *V, double *dVdxi, double *Tabs) {
+#pragma omp parallel for schedule(static)
+    for (int r = 0; r < n_replicas; ++r) {
+        double v = 0, g[8] = {0}, t[8] = {0}, d[8];
+        for (long long h = 0; h < n_hills; ++h) {
+            double e = 0;
+            for (int k = 0; k < n_cv; ++k) {
+                d[k] = wrap_period(xi[r * n_cv + k] - (double)centers[h * n_cv + k], period[k]);
+                e += (d[k] / sigma[k]) * (d[k] / sigma[k]);
+            }
+            double w = (double)heights[h] * exp(-0.5 * e);
+            v += w;
+            for (int k = 0; k < n_cv; ++k) {
+                double term = -w * d[k] / (sigma[k] * sigma[k]);
+                g[k] += term;
+                t[k] += fabs(term);
+            }
+        }
+        if (V) V[r] = v;
+        for (int k = 0; k < n_cv; ++k) {
+            if (dVdxi) dVdxi[r * n_cv + k] = g[k];
+            if (Tabs) Tabs[r * n_cv + k] = t[k];
+        }
+    }
+}
+
+/* Hill deposition.  Standard: W = w0.  Well-tempered
+ * (kB_deltaT > 0): W = w0 exp(-V_old(xi)/(kB dT)), V_old from the list BEFORE
+ * this event (reading R-WT).  Several walkers deposit synchronously and append
+ * in replica order (reading R-MW, parity unpinned).  Centres and heights are
+ * stored as binary32 (the hill store's type).  Returns the new hill count. */
+long long orc_deposit_hills(int n_replicas, int n_cv, const float *xi /*[R][n_cv]*/, const unsigned char *mask,
+                            double w0, double kB_deltaT, const double *sigma, const double *period,
+                            long long n_hills, float *centers, float *heights) {
+    double *xd = (double *)malloc(sizeof(double) * (size_t)n_replicas * n_cv);
+    double *V = (double *)malloc(sizeof(double) * (size_t)n_replicas);
+    for (long long i = 0; i < (long long)n_replicas * n_cv; ++i) xd[i] = (double)xi[i];
+    if (kB_deltaT > 0) orc_metad(n_replicas, n_cv, xd, n_hills, centers, heights, sigma, period, V, NULL, NULL);
+    long long n = n_hills;
+    for (int r = 0; r < n_replicas; ++r) {
+        if (mask && !mask[r]) continue;
+        for (int k = 0; k < n_cv; ++k) centers[n * n_cv + k] = xi[r * n_cv + k];
+        heights[n] = (float)(kB_deltaT > 0 ? w0 * exp(-V[r] / kB_deltaT) : w0);
+        ++n;
+    }
+    free(xd); free(V);
+    return n;
+}
+
+/* ABF bin index of one CV value, DEFINED IN BINARY32 (reading R-ABF-1):
+ * t = fl32(fl32(xi - lower) * invd), I = (int)floorf(t), two separately rounded
+ * operations (this file is compiled with -ffp-contract=off).  invd =
+ * (float)((double)shape / ((double)upper - (double)lower)).  Grid(lower, upper,
+ * shape, periodic): PAPER.md:L82 (Fig. 2). */
+static int abf_bin_1d(float xi, float lower, float upper, int shape, int periodic) {
+    volatile float invd = (float)((double)shape / ((double)upper - (double)lower));
+    volatile float d = xi - lower;
+    volatile float t = d * invd;
+    float f = floorf(t);
+    if (!(f == f)) return -1; /* NaN is outside */
+    if (periodic) {
+        double m = fmod((double)f, (double)shape);
+        if (m < 0) m += shape;
+        return (int)m;
+    }
+    if (f < 0.0f || f >= (float)shape) return -1;
+    return (int)f;
+}
+
+/* ABF grid update, PAPER.md:L143 (Sec. 2.1.4), L501/L507 (N = threshold before
+ * the full average is used).  For every replica: bin xi; in-grid -> hist[bin]+=1,
+ * Fsum[bin][k] += f_k.  After ALL replicas have accumulated (two-phase, reading
+ * R-ABF-3, parity unpinned) each reads Fbar_k = Fsum[bin][k]/max(hist[bin], N);
+ * outside -> bin = -1 and Fbar = 0.  dVdxi := Fbar (reading R-ABF-4). */
+void orc_abf_update(int n_replicas, int n_cv, const float *xi, const float *fsample, const float *lower,
+                    const float *upper, const int *shape, const int *periodic, int n_threshold,
+                    int *hist, double *fsum /*[nbins][n_cv]*/, int *bin_out, double *dVdxi) {
+    int *bins = (int *)malloc(sizeof(int) * (size_t)n_replicas);
+    for (int r = 0; r < n_replicas; ++r) {
+        long long flat = 0;
+        int inside = 1;
+        for (int k = 0; k < n_cv; ++k) {
+            int i = abf_bin_1d(xi[r * n_cv + k], lower[k], upper[k], shape[k], periodic[k]);
+            if (i < 0) { inside = 0; break; }
+            flat = flat * shape[k] + i; /* row-major, last CV fastest */
+        }
+        bins[r] = inside ? (int)flat : -1;
+        if (inside) {
+            hist[flat] += 1;
+            for (int k = 0; k < n_cv; ++k) fsum[flat * n_cv + k] += (double)fsample[r * n_cv + k];
+        }
+    }
+    for (int r = 0; r < n_replicas; ++r) {
+        int b = bins[r];
+        if (bin_out) bin_out[r] = b;
+        for (int k = 0; k < n_cv; ++k) {
+            double m = 0;
+            if (b >= 0) {
+                int cnt = hist[b] > n_threshold ? hist[b] : n_threshold;
+                m = fsum[(long long)b * n_cv + k] / (double)cnt;
+            }
+            dVdxi[r * n_cv + k] = m;
+        }
+    }
+    free(bins);
+}
+
+/* Bias forces, PAPER.md:L39 ("computed biasing forces are added to the backend
+ * net forces"): force[i] += -sum_k dVdxi_k d(xi_k)/d(r_i), summed over every CV
+ * and every replica that references atom i of that array.
+ * force: fp64 [n_arrays][N][3], n_arrays = R (own arrays) or 1 (shared). */
+void orc_apply_forces(const orc_layout *L, const orc_cv *cvs, const int *slot_atom, const float *slot_weight,
+                      const float *atom_weight, const float *pos, const double *dVdxi, double *force) {
+    int shared = L->replica_stride_atoms == 0;
+    long long maxrows = 0;
+    for (int k = 0; k < L->n_cv; ++k) { long long n = cv_natoms(&cvs[k]); if (n > maxrows) maxrows = n; }
+#pragma omp parallel if (!shared)
+    {
+        double *jac = (double *)malloc(sizeof(double) * 3 * (size_t)maxrows);
+#pragma omp for schedule(static)
+        for (int r = 0; r < L->n_replicas; ++r) {
+            const float *p = pos + (long long)r * L->replica_stride_atoms * L->pos_stride;
+            double *f = force + (shared ? 0 : (long long)r * L->n_atoms * 3);
+            const int *sa = slot_atom + (L->per_replica_slots ? (long long)r * L->n_slots : 0);
+            for (int k = 0; k < L->n_cv; ++k) {
+                const orc_cv *cv = &cvs[k];
+                cv_one(cv, p, L->pos_stride, sa, slot_weight, atom_weight, jac);
+                double dv = dVdxi[(long long)r * L->n_cv + k];
+                long long o = 0;
+                for (int g = 0; g < cv->n_groups; ++g) {
+                    long long n = group_count(cv, g);
+                    for (long long i = 0; i < n; ++i, ++o) {
+                        long long a = group_atom(cv, g, i, sa);
+                        for (int x = 0; x < 3; ++x) f[a * 3 + x] += -dv * jac[3 * o + x];
+                    }
+                }
+            }
+        }
+        free(jac);
+    }
+}
