@@ -1,0 +1,183 @@
+/*
+ * psg.h -- C ABI of libpsg.so: the per-MD-step enhanced-sampling hot path of
+ * PySAGES (arXiv 2301.04835; citations are lines of /root/reference/PAPER.md),
+ * batched over replicas / walkers / windows, as hand-written sm_100a CUDA.
+ *
+ *   gather CV atoms in place  ->  collective variables + analytic Jacobians
+ *   ->  bias energy and gradient  ->  force[i] += -dV/dxi * dxi/dr_i
+ *
+ * The paper's hook "gets called as part of the time integration routine ...
+ * computes the collective variables ... the computed biasing forces are added to
+ * the backend net forces" on engine-owned buffers reached without
+ * a copy (DLPack).  Here the engine hands over raw DEVICE pointers.
+ *
+ * Conventions
+ *  - Every function is extern "C", never throws, returns an int status
+ *    (PSG_OK = 0, errors < 0).  psg_last_error() gives the message.
+ *  - "host" / "device" in a parameter comment says where the pointer must live.
+ *  - Setup calls (psg_set_*, psg_load_hills) copy their host arrays, may allocate
+ *    and may synchronise the ctx stream; they are not on the hot path.
+ *  - Hot-path calls take device pointers only, enqueue work on the ctx stream and
+ *    return immediately: no allocation, no host synchronisation, CUDA-graph
+ *    capturable.  Arguments are validated on the host BEFORE anything is launched.
+ *  - Ownership: the caller owns positions and forces.  Positions are read only.
+ *    The force array is modified ONLY at atoms that belong to a CV group, ONLY by
+ *    adding to x, y, z; w (stride 4) keeps its bits.  The ctx owns the hill store,
+ *    the ABF grid (unless caller-provided), and all scratch.
+ *  - Layout: positions / forces are float32, `stride` floats per atom (3 or 4;
+ *    4 = float4 x,y,z,w, 16-byte aligned).  Replica r's array starts at
+ *    base + r * replica_stride_atoms * stride floats; replica_stride_atoms = 0
+ *    means all replicas index ONE shared array.
+ *  - Degenerate geometry (coincident points, collinear bonds, Rg = 0) and CVs
+ *    outside the ABF grid are NOT errors: the Jacobian / mean force is defined 0.
+ *  - One ctx per stream; calls on one ctx are not thread-safe.
+ *  - There is no CPU fallback: without a CUDA device psg_create fails.
+ */
+#ifndef PSG_H
+#define PSG_H
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct psg_ctx psg_ctx;
+
+enum { PSG_OK = 0, PSG_EINVAL = -1, PSG_ENOMEM = -2, PSG_ECUDA = -3, PSG_ECAPACITY = -4, PSG_ESTATE = -5 };
+
+/* Collective variables, PAPER.md:L185-L189 (Sec. 2.2). Every argument is a GROUP of
+ * atoms reduced to its weighted barycenter (barycenter(p)). */
+enum {
+    PSG_CV_DISTANCE = 1,      /* TwoPointCV Distance: |c2 - c1|                         (L185) */
+    PSG_CV_ANGLE = 2,         /* ThreePointCV Angle at the 2nd group, in [0, pi]        (L186) */
+    PSG_CV_DIHEDRAL = 3,      /* FourPointCV DihedralAngle in (-pi, pi], IUPAC sign     (L187, L81) */
+    PSG_CV_COM_COMPONENT = 4, /* AxisCV Component: barycenter coordinate along an axis  (L188) */
+    PSG_CV_RGYR = 5           /* RadiusofGyration: sqrt(sum w|r-c|^2 / sum w)           (L189) */
+};
+
+enum { PSG_METHOD_NONE = 0, PSG_METHOD_HARMONIC = 1, PSG_METHOD_METAD = 2, PSG_METHOD_ABF = 3 };
+
+/* precision of the metadynamics hill sum */
+enum {
+    PSG_HILLS_F32 = 0, /* binary32 terms on the FP32/SFU pipes, binary64 accumulation (default) */
+    PSG_HILLS_F64 = 1  /* binary64 terms: meets 1e-5 rel / 1e-6 abs on ill-conditioned gradients too */
+};
+
+#define PSG_MAX_CV 4
+#define PSG_MAX_GROUPS 4
+#define PSG_MAX_SLOTS 64
+#define PSG_MAX_RANGE_GROUPS 8
+
+typedef struct {
+    int type;                            /* PSG_CV_* */
+    int n_groups;                        /* 2, 3, 4, 1, 1 for the five types */
+    int group_is_range[PSG_MAX_GROUPS];  /* 0: explicit atoms (a slice of the slot list); 1: contiguous atom range */
+    int group_begin[PSG_MAX_GROUPS];     /* explicit: slots [begin, begin + size) */
+    int group_size[PSG_MAX_GROUPS];
+    long long range_begin[PSG_MAX_GROUPS]; /* range: atoms [range_begin, range_begin + range_size) of the replica's array */
+    long long range_size[PSG_MAX_GROUPS];
+    int axis;                            /* PSG_CV_COM_COMPONENT: 0, 1, 2 */
+    float period;                        /* 0 = not periodic; 2*pi for a dihedral */
+} psg_cv_desc;
+
+/* ------------------------------------------------------------------ lifetime */
+/* device: CUDA ordinal.  cuda_stream: a cudaStream_t (borrowed, may be NULL = legacy default stream). */
+int psg_create(psg_ctx** out, int device, void* cuda_stream);
+int psg_destroy(psg_ctx* ctx);
+/* Change the stream later work is enqueued on (e.g. torch's current stream). */
+int psg_set_stream(psg_ctx* ctx, void* cuda_stream);
+/* Message of the last error on ctx; ctx == NULL: the last psg_create failure of this thread. Never NULL. */
+const char* psg_last_error(const psg_ctx* ctx);
+
+/* --------------------------------------------------------------------- setup */
+/* Snapshot layout: R replicas of n_atoms atoms.  Must precede psg_set_cvs. */
+int psg_set_layout(psg_ctx* ctx, int n_replicas, long long n_atoms, long long replica_stride_atoms,
+                   int pos_stride_floats, int frc_stride_floats);
+
+/* CVs over groups of atoms.  All arrays are HOST and copied.
+ *  slot_atom_idx : 0-based atom indices, [n_slots] (per_replica_indices = 0, shared by all replicas)
+ *                  or [R][n_slots] (per_replica_indices = 1); every index is range-checked here.
+ *  slot_weight   : [n_slots] weights of explicit atoms (masses), NULL = 1 (plain barycenter).
+ *  atom_weight   : [n_atoms] weights used by RANGE groups, NULL = 1.
+ * Each slot belongs to exactly one (cv, group); an atom shared by two CVs is listed twice. */
+int psg_set_cvs(psg_ctx* ctx, int n_cv, const psg_cv_desc* cvs, int n_slots, const int* slot_atom_idx,
+                int per_replica_indices, const float* slot_weight, const float* atom_weight);
+
+/* Harmonic bias, PAPER.md:L125 (Sec. 2.1.1): V = 1/2 sum_k k_k (xi_k - xi0_k)^2, differences of periodic
+ * CVs wrapped to the nearest image.  kspring [n_cv], centers [R][n_cv] (host). Selects the method. */
+int psg_set_harmonic(psg_ctx* ctx, const float* kspring, const float* centers);
+
+/* Metadynamics, PAPER.md:L147-L151 (Sec. 2.1.5): V(xi) = sum_h W_h exp(-1/2 sum_k (d_hk/sigma_k)^2).
+ *  sigma [n_cv] host; w0 initial height; kB_deltaT > 0: well-tempered, W = w0 exp(-V/(kB dT)) (L149);
+ *  <= 0: standard.  capacity: hills the store can hold.  stride: psg_step deposits when step % stride == 0
+ *  (L147 "deposited at user-defined intervals"); 0 = psg_step never deposits.  Empties the store. Selects the method. */
+int psg_set_metad(psg_ctx* ctx, const float* sigma, float w0, float kB_deltaT, int capacity, int stride);
+int psg_set_hill_precision(psg_ctx* ctx, int mode /* PSG_HILLS_* */);
+/* Replace the store's contents by n hills: centers [n][n_cv], heights [n], DEVICE pointers (copied). */
+int psg_load_hills(psg_ctx* ctx, int n, const float* d_centers, const float* d_heights);
+/* Synchronises. *n_out (host) = exact hill count; if d_centers/d_heights are non-NULL (device) and
+ * max_n >= count they receive the store's contents as [n][n_cv] / [n]. */
+int psg_get_hills(psg_ctx* ctx, int* n_out, float* d_centers, float* d_heights, int max_n);
+
+/* ABF, PAPER.md:L143 (Sec. 2.1.4), Grid(lower, upper, shape, periodic) of L82, N of L501/L507.
+ * lower, upper, shape, periodic: [n_cv] host.  d_hist int32 [prod(shape)], d_fsum float32
+ * [prod(shape)][n_cv]: device, caller-owned when non-NULL, else allocated (zeroed) and owned by ctx. */
+int psg_set_abf(psg_ctx* ctx, const float* lower, const float* upper, const int* shape, const int* periodic,
+                int n_threshold, int* d_hist, float* d_fsum);
+/* Device pointers of the grid in use (to read it back / checkpoint it). */
+int psg_abf_state(psg_ctx* ctx, int** d_hist_out, float** d_fsum_out, long long* n_bins_out);
+
+/* ------------------------------------------------ hot path (device pointers) */
+/* CVs and Jacobians of every replica ("computes the collective variables"; L185-L189).
+ *  d_pos : positions, see Layout.   d_xi : out [R][n_cv].
+ *  d_jac : out, nullable, [R][n_slots][3] = d(xi_cv(slot))/d(r_slot) for the explicit slots.
+ * The Jacobian (explicit slots and the implicit form for range groups) is also cached in ctx
+ * for the next psg_apply_bias_forces. */
+int psg_cv_eval(psg_ctx* ctx, const float* d_pos, float* d_xi, float* d_jac);
+
+/* Bias energy and gradient at given CV values for the selected method (harmonic or metadynamics).
+ *  d_xi [R][n_cv] in;  d_V [R] out, nullable;  d_dVdxi [R][n_cv] out. */
+int psg_bias_eval(psg_ctx* ctx, const float* d_xi, float* d_V, float* d_dVdxi);
+
+/* Append one hill per replica at xi: all walkers see the list as it was BEFORE this
+ * call and append in replica order.  d_mask [R] nullable (NULL = all deposit).  PSG_ECAPACITY, nothing
+ * launched, if the host-side upper bound of the count + R exceeds capacity. */
+int psg_deposit_hill(psg_ctx* ctx, const float* d_xi, const unsigned char* d_mask);
+
+/* ABF grid update for all replicas, then the mean force from the fully updated grid (two-phase):
+ *  bin in binary32: I_k = floor(fl(fl(xi_k - lower_k) * invd_k)); in-grid: hist[bin] += 1, Fsum[bin][k] += f_k;
+ *  d_dVdxi[r][k] := Fsum[bin][k] / max(hist[bin], N);  outside: bin = -1, 0.
+ *  d_fsample [R][n_cv] in;  d_bin [R] out nullable;  d_dVdxi [R][n_cv] out. */
+int psg_abf_update(psg_ctx* ctx, const float* d_xi, const float* d_fsample, int* d_bin, float* d_dVdxi);
+
+/* force[i] += -sum_k dVdxi[r][k] * d(xi_k)/d(r_i), using the Jacobian cached by the last
+ * psg_cv_eval on these positions (PSG_ESTATE if there was none).  d_force in/out. */
+int psg_apply_bias_forces(psg_ctx* ctx, const float* d_pos, const float* d_dVdxi, float* d_force);
+
+/* One whole step of the selected method, fused: gather -> CVs -> (deposit if due) -> bias -> forces.
+ *  d_fsample: ABF only, else NULL.  step: 1-based MD step number (deposit phase).
+ * Afterwards xi / V / dVdxi / bin of this step can be read with psg_step_outputs. */
+int psg_step(psg_ctx* ctx, const float* d_pos, float* d_force, const float* d_fsample, long long step);
+/* Device pointers (ctx-owned, valid until destroy/reconfigure) of the last step's per-replica results:
+ * xi [R][n_cv], V [R] (0 for ABF), dVdxi [R][n_cv], bin [R] (ABF only, else NULL). Any out may be NULL. */
+int psg_step_outputs(psg_ctx* ctx, float** d_xi, float** d_V, float** d_dVdxi, int** d_bin);
+
+/* The same step for an engine whose arrays live on the HOST (pinned memory recommended): copies
+ * h_pos (and h_force) to ctx-owned device buffers, runs psg_step, copies the forces back and waits. */
+int psg_step_host(psg_ctx* ctx, const float* h_pos, float* h_force, const float* h_fsample, long long step);
+
+/* The only other call that synchronises: waits for the ctx stream and returns sticky CUDA errors. */
+int psg_sync_check(psg_ctx* ctx);
+
+/* ------------------------------------------------------------- measurement */
+/* Measured ALU throughput of this device (register-only loops, CUDA-event timed, synchronises):
+ * which = 0: FP32 FFMA lane-ops/s; 1: packed FFMA2 (f32x2) lane-ops/s (2 per lane per instruction);
+ * 2: MUFU.EX2/s; 3: FP64 DFMA lane-ops/s; 4: F2F f32->f64->f32 round trips/s; 5: I2F.F32.S32/s;
+ * 6: packed FADD2 lane-ops/s.  Denominators for the hill-sum roofline. */
+int psg_measure_alu_peak(int device, int which, double* ops_per_second_out);
+/* Launch counter: number of kernels this ctx has enqueued since creation (for bench.py's gpu_launches). */
+long long psg_launch_count(const psg_ctx* ctx);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* PSG_H */

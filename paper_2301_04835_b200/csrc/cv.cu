@@ -1,0 +1,212 @@
+// cv.cu -- CV evaluation (psg_cv_eval) and bias-force application (psg_apply_bias_forces).
+//   k_range_moments : HBM-bound block reduction of the weighted moments of large contiguous groups
+//   k_cv_eval       : one warp per replica: gather explicit atoms, combine moments, CVs + Jacobians (fp64 regs)
+//   k_apply_sparse  : one thread per (replica, slot): red.global.add of -dV/dxi * J into the force array
+//   k_apply_dense   : HBM-bound force read-modify-write over contiguous groups (implicit Jacobian)
+#include "geom.cuh"
+
+// --------------------------------------------------------------------------------------------
+// Moments of range groups. grid = (range_blocks, R); block b covers atoms [span_begin + b*TILE, +TILE).
+// Every atom is loaded once (coalesced float4) and contributes to each range group that contains it.
+// Output: rpart[r][q][b][5] in binary64 (products of binary32 inputs are exact in binary64).
+__global__ void __launch_bounds__(256) k_range_moments(const __grid_constant__ SysParams P, const float* __restrict__ pos,
+                                                        double* __restrict__ rpart) {
+    constexpr int PER = PSG_RANGE_TILE / 256;
+    const int r = blockIdx.y, b = blockIdx.x, tid = threadIdx.x;
+    const float* p = pos + (long long)r * P.rstride * P.ps;
+    const long long t0 = P.span_begin + (long long)b * PSG_RANGE_TILE;
+    float x[PER], y[PER], z[PER], w[PER];
+    long long ai[PER];
+#pragma unroll
+    for (int i = 0; i < PER; ++i) {
+        long long a = t0 + tid + (long long)i * 256;
+        ai[i] = a;
+        x[i] = y[i] = z[i] = w[i] = 0.f;
+        if (a < P.span_end) {
+            if (P.ps == 4) {
+                float4 v = __ldg(reinterpret_cast<const float4*>(p) + a);
+                x[i] = v.x; y[i] = v.y; z[i] = v.z;
+            } else {
+                x[i] = __ldg(p + a * 3); y[i] = __ldg(p + a * 3 + 1); z[i] = __ldg(p + a * 3 + 2);
+            }
+            w[i] = P.atom_weight ? __ldg(P.atom_weight + a) : 1.f;
+        }
+    }
+    __shared__ double red[8][PSG_MOM];
+    for (int q = 0; q < P.n_ranges; ++q) {
+        const GroupDev& G = P.grp[P.range_gid[q]];
+        const long long gb = G.rbegin, ge = G.rbegin + G.rsize;
+        double m[PSG_MOM] = {0, 0, 0, 0, 0};
+        if (t0 < ge && t0 + PSG_RANGE_TILE > gb) {   // block-uniform
+#pragma unroll
+            for (int i = 0; i < PER; ++i) {
+                if (ai[i] >= gb && ai[i] < ge && ai[i] < P.span_end) {
+                    double wd = (double)w[i], xd = (double)x[i], yd = (double)y[i], zd = (double)z[i];
+                    m[0] += wd; m[1] += wd * xd; m[2] += wd * yd; m[3] += wd * zd;
+                    m[4] += wd * (xd * xd + yd * yd + zd * zd);
+                }
+            }
+        }
+#pragma unroll
+        for (int i = 0; i < PSG_MOM; ++i) m[i] = warp_sum(m[i]);
+        __syncthreads();
+        if ((tid & 31) == 0) {
+#pragma unroll
+            for (int i = 0; i < PSG_MOM; ++i) red[tid >> 5][i] = m[i];
+        }
+        __syncthreads();
+        if (tid < PSG_MOM) {
+            double s = 0;
+#pragma unroll
+            for (int wq = 0; wq < 8; ++wq) s += red[wq][tid];
+            rpart[(((long long)r * P.n_ranges + q) * P.range_blocks + b) * PSG_MOM + tid] = s;
+        }
+    }
+}
+
+// --------------------------------------------------------------------------------------------
+// One warp per replica. Writes xi (fp32), the compact Jacobian of explicit slots (fp32, to jac_user and/or
+// jac_cache) and the per-group descriptors gdesc[r][gid] = {v(3), c(3), coef, W} (fp64) for range groups.
+__global__ void __launch_bounds__(256) k_cv_eval(const __grid_constant__ SysParams P, const float* __restrict__ pos,
+                                                  const double* __restrict__ rpart, float* __restrict__ xi,
+                                                  float* __restrict__ jac_user, float* __restrict__ jac_cache,
+                                                  double* __restrict__ gdesc) {
+    __shared__ WarpCvSmem sm[8];
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+    const int r = blockIdx.x * 8 + wid;
+    if (r >= P.R) return;
+    WarpCvSmem& S = sm[wid];
+    warp_cv_eval<true>(P, r, pos, rpart, S, lane);
+    if (lane < P.n_cv) xi[(long long)r * P.n_cv + lane] = (float)S.xi[lane];
+    for (int s = lane; s < P.n_slots; s += 32) {
+        D3 j = slot_jacobian(P, r, pos, S, s);
+        long long o = ((long long)r * P.n_slots + s) * 3;
+        if (jac_user) { jac_user[o] = (float)j.x; jac_user[o + 1] = (float)j.y; jac_user[o + 2] = (float)j.z; }
+        jac_cache[o] = (float)j.x; jac_cache[o + 1] = (float)j.y; jac_cache[o + 2] = (float)j.z;
+    }
+    if (P.n_ranges > 0 && lane < P.n_groups) {
+        double* d = gdesc + ((long long)r * P.n_groups + lane) * PSG_GDESC_DOUBLES;
+        d[0] = S.v[lane][0]; d[1] = S.v[lane][1]; d[2] = S.v[lane][2];
+        d[3] = S.cen[lane][0]; d[4] = S.cen[lane][1]; d[5] = S.cen[lane][2];
+        d[6] = S.coef[lane]; d[7] = S.cen[lane][3];
+    }
+}
+
+// --------------------------------------------------------------------------------------------
+// Sparse scatter: thread per (replica, slot). Atoms shared between CVs (6, 8, 14 of phi/psi) or between
+// walkers of a shared array collide, hence red.global.add.f32 (fire-and-forget L2 atomics).
+__global__ void __launch_bounds__(256) k_apply_sparse(const __grid_constant__ SysParams P, const float* __restrict__ jac,
+                                                       const float* __restrict__ dVdxi, float* __restrict__ force) {
+    long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (t >= (long long)P.R * P.n_slots) return;
+    int r = (int)(t / P.n_slots), s = (int)(t % P.n_slots);
+    int gid = P.slot_gid[s];
+    float dv = -dVdxi[(long long)r * P.n_cv + P.grp[gid].cv];
+    int atom = P.slot_atom[(P.per_rep ? (long long)r * P.n_slots : 0) + s];
+    float* f = force + ((long long)r * P.rstride + atom) * P.fs;
+    const float* j = jac + t * 3;
+    atomicAdd(f, dv * j[0]);
+    atomicAdd(f + 1, dv * j[1]);
+    atomicAdd(f + 2, dv * j[2]);
+}
+
+// --------------------------------------------------------------------------------------------
+// Dense application over range groups: grid = (range_blocks, R). Per atom:
+//   F_i += sum_{groups containing i} -dV_cv * w_i * ( v_g  +  coef_g * (r_i - c_g) )
+// Force is read and written once (float4, w preserved bit for bit); positions are read only when an Rg
+// CV needs r_i. Each replica owns its atoms here (no atomics); with a shared array (rstride = 0) several
+// replicas would hit the same atoms, so that case uses atomics.
+__global__ void __launch_bounds__(256) k_apply_dense(const __grid_constant__ SysParams P, const float* __restrict__ pos,
+                                                      const double* __restrict__ gdesc, const float* __restrict__ dVdxi,
+                                                      float* __restrict__ force) {
+    constexpr int PER = PSG_RANGE_TILE / 256;
+    const int r = blockIdx.y, b = blockIdx.x, tid = threadIdx.x;
+    const long long t0 = P.span_begin + (long long)b * PSG_RANGE_TILE;
+    __shared__ float s_v[PSG_MAX_RANGE_GROUPS][3], s_chi[PSG_MAX_RANGE_GROUPS][3], s_clo[PSG_MAX_RANGE_GROUPS][3],
+        s_k[PSG_MAX_RANGE_GROUPS];
+    __shared__ long long s_b[PSG_MAX_RANGE_GROUPS], s_e[PSG_MAX_RANGE_GROUPS];
+    if (tid < P.n_ranges) {
+        int gid = P.range_gid[tid];
+        const GroupDev& G = P.grp[gid];
+        const double* d = gdesc + ((long long)r * P.n_groups + gid) * PSG_GDESC_DOUBLES;
+        double dv = -(double)dVdxi[(long long)r * P.n_cv + G.cv];
+#pragma unroll
+        for (int x = 0; x < 3; ++x) {
+            s_v[tid][x] = (float)(dv * d[x]);
+            float hi = (float)d[3 + x];
+            s_chi[tid][x] = hi;
+            s_clo[tid][x] = (float)(d[3 + x] - (double)hi);   // centre as hi + lo: (r - hi) - lo keeps r - c accurate
+        }
+        s_k[tid] = (float)(dv * d[6]);
+        s_b[tid] = G.rbegin; s_e[tid] = G.rbegin + G.rsize;
+    }
+    __syncthreads();
+    const float* p = pos + (long long)r * P.rstride * P.ps;
+    float* f = force + (long long)r * P.rstride * P.fs;
+    const bool shared_arr = P.rstride == 0;
+#pragma unroll
+    for (int i = 0; i < PER; ++i) {
+        long long a = t0 + tid + (long long)i * 256;
+        if (a >= P.span_end) continue;
+        float ax = 0.f, ay = 0.f, az = 0.f;
+        float px = 0.f, py = 0.f, pz = 0.f;
+        if (P.any_rgyr) {
+            if (P.ps == 4) {
+                float4 v = __ldg(reinterpret_cast<const float4*>(p) + a);
+                px = v.x; py = v.y; pz = v.z;
+            } else {
+                px = __ldg(p + a * 3); py = __ldg(p + a * 3 + 1); pz = __ldg(p + a * 3 + 2);
+            }
+        }
+        bool any = false;
+        for (int q = 0; q < P.n_ranges; ++q) {
+            if (a >= s_b[q] && a < s_e[q]) {
+                any = true;
+                float k = s_k[q];
+                ax += s_v[q][0] + k * ((px - s_chi[q][0]) - s_clo[q][0]);
+                ay += s_v[q][1] + k * ((py - s_chi[q][1]) - s_clo[q][1]);
+                az += s_v[q][2] + k * ((pz - s_chi[q][2]) - s_clo[q][2]);
+            }
+        }
+        if (!any) continue;
+        float w = P.atom_weight ? __ldg(P.atom_weight + a) : 1.f;
+        ax *= w; ay *= w; az *= w;
+        if (shared_arr) {
+            atomicAdd(f + a * P.fs, ax); atomicAdd(f + a * P.fs + 1, ay); atomicAdd(f + a * P.fs + 2, az);
+        } else if (P.fs == 4) {
+            float4* fp = reinterpret_cast<float4*>(f) + a;
+            float4 v = *fp;
+            v.x += ax; v.y += ay; v.z += az;
+            *fp = v;
+        } else {
+            f[a * 3] += ax; f[a * 3 + 1] += ay; f[a * 3 + 2] += az;
+        }
+    }
+}
+
+cudaError_t psg_launch_cv_eval(psg_ctx* c, const float* d_pos, float* d_xi, float* d_jac) {
+    const SysParams& P = c->sys;
+    if (P.n_ranges > 0) {
+        dim3 g(P.range_blocks, P.R);
+        k_range_moments<<<g, 256, 0, c->stream>>>(P, d_pos, c->d_rpart);
+        c->launches++;
+    }
+    k_cv_eval<<<(P.R + 7) / 8, 256, 0, c->stream>>>(P, d_pos, c->d_rpart, d_xi, d_jac, c->d_jac, c->d_gdesc);
+    c->launches++;
+    return cudaGetLastError();
+}
+
+cudaError_t psg_launch_apply(psg_ctx* c, const float* d_pos, const float* d_dVdxi, float* d_force) {
+    const SysParams& P = c->sys;
+    if (P.n_slots > 0) {
+        long long n = (long long)P.R * P.n_slots;
+        k_apply_sparse<<<(unsigned)((n + 255) / 256), 256, 0, c->stream>>>(P, c->d_jac, d_dVdxi, d_force);
+        c->launches++;
+    }
+    if (P.n_ranges > 0) {
+        dim3 g(P.range_blocks, P.R);
+        k_apply_dense<<<g, 256, 0, c->stream>>>(P, d_pos, c->d_gdesc, d_dVdxi, d_force);
+        c->launches++;
+    }
+    return cudaGetLastError();
+}

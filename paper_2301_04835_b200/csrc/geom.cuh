@@ -1,0 +1,190 @@
+// geom.cuh -- device-side collective variables and analytic Jacobians.
+// Inputs are binary32 coordinates; the geometry of a handful of group centres is done in
+// binary64 registers and rounded once on store: it is ~200 flops per
+// CV, invisible next to the hill sum, and removes the near-degenerate fp32 failures.
+// CVs: PAPER.md:L185-L189 (Sec. 2.2). Written from the definitions; shares nothing with oracle/.
+#pragma once
+#include "internal.h"
+
+struct D3 {
+    double x, y, z;
+};
+__device__ __forceinline__ D3 d3(double x, double y, double z) { return D3{x, y, z}; }
+__device__ __forceinline__ D3 operator-(D3 a, D3 b) { return D3{a.x - b.x, a.y - b.y, a.z - b.z}; }
+__device__ __forceinline__ D3 operator+(D3 a, D3 b) { return D3{a.x + b.x, a.y + b.y, a.z + b.z}; }
+__device__ __forceinline__ D3 operator*(double s, D3 a) { return D3{s * a.x, s * a.y, s * a.z}; }
+__device__ __forceinline__ double dot(D3 a, D3 b) { return a.x * b.x + a.y * b.y + a.z * b.z; }
+__device__ __forceinline__ D3 cross(D3 a, D3 b) {
+    return D3{a.y * b.z - a.z * b.y, a.z * b.x - a.x * b.z, a.x * b.y - a.y * b.x};
+}
+
+// xi = f(c_0..c_3) and, if JAC, dxi/dc_g into dc[0..3] (zero where undefined).
+template <bool JAC>
+__device__ __forceinline__ double cv_from_centers(int type, int axis, const D3* c, D3* dc) {
+    if (JAC) {
+#pragma unroll
+        for (int g = 0; g < 4; ++g) dc[g] = d3(0, 0, 0);
+    }
+    if (type == PSG_CV_DISTANCE) {
+        D3 d = c[1] - c[0];
+        double r = sqrt(dot(d, d));
+        if (JAC && r > 0.0) {
+            double ir = 1.0 / r;
+            dc[1] = ir * d;
+            dc[0] = (-ir) * d;
+        }
+        return r;
+    }
+    if (type == PSG_CV_ANGLE) {
+        // vertex at the second group; theta = atan2(|u x v|, u.v)
+        D3 u = c[0] - c[1], v = c[2] - c[1];
+        D3 n = cross(u, v);
+        double nn = sqrt(dot(n, n));
+        double th = atan2(nn, dot(u, v));
+        if (JAC && nn > 0.0) {
+            // moving c0 inside the plane, perpendicular to u: direction (u x n), length 1/|u|
+            dc[0] = (1.0 / (dot(u, u) * nn)) * cross(u, n);
+            dc[2] = (-1.0 / (dot(v, v) * nn)) * cross(v, n);
+            dc[1] = (-1.0) * (dc[0] + dc[2]);
+        }
+        return th;
+    }
+    if (type == PSG_CV_DIHEDRAL) {
+        D3 b1 = c[1] - c[0], b2 = c[2] - c[1], b3 = c[3] - c[2];
+        D3 m = cross(b1, b2), n = cross(b2, b3);
+        double l2 = dot(b2, b2), l = sqrt(l2);
+        double phi = atan2(l * dot(b1, n), dot(m, n));
+        if (JAC) {
+            double mm = dot(m, m), nn = dot(n, n);
+            if (mm > 0.0 && nn > 0.0) {
+                D3 f0 = (-l / mm) * m;         // end atoms move the angle only through their own plane normal
+                D3 f3 = (l / nn) * n;
+                double p = dot(b1, b2) / l2, q = dot(b3, b2) / l2;
+                dc[0] = f0;
+                dc[3] = f3;
+                dc[1] = (-(1.0 + p)) * f0 + q * f3;   // torque balance about the b2 axis
+                dc[2] = (-(1.0 + q)) * f3 + p * f0;
+            }
+        }
+        return phi;
+    }
+    if (type == PSG_CV_COM_COMPONENT) {
+        if (JAC) dc[0] = d3(axis == 0 ? 1.0 : 0.0, axis == 1 ? 1.0 : 0.0, axis == 2 ? 1.0 : 0.0);
+        return axis == 0 ? c[0].x : (axis == 1 ? c[0].y : c[0].z);
+    }
+    return 0.0;
+}
+
+__device__ __forceinline__ D3 load_pos(const float* __restrict__ p, long long atom, int ps) {
+    if (ps == 4) {
+        float4 v = __ldg(reinterpret_cast<const float4*>(p) + atom);
+        return d3((double)v.x, (double)v.y, (double)v.z);
+    }
+    const float* q = p + atom * 3;
+    return d3((double)__ldg(q), (double)__ldg(q + 1), (double)__ldg(q + 2));
+}
+
+__device__ __forceinline__ double warp_sum(double v) {
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+    return v;
+}
+
+// Per-warp shared scratch for one replica's CV evaluation.
+struct WarpCvSmem {
+    double cen[PSG_MAX_GROUPS_TOTAL][4];   // cx cy cz W
+    double m2[PSG_MAX_GROUPS_TOTAL];       // sum w |r|^2 (RGYR groups)
+    double v[PSG_MAX_GROUPS_TOTAL][3];     // dxi/dc_g / W_g
+    double coef[PSG_MAX_GROUPS_TOTAL];     // RGYR: 1/(W Rg)
+    double xi[PSG_MAX_CV];
+};
+
+// One warp evaluates all CVs of replica r.
+//  - group centres: explicit groups gathered from pos by one lane per group; range groups from the
+//    partial moments written by k_range_moments (rpart != nullptr when n_ranges > 0)
+//  - lane k < n_cv computes CV k (value, and with JAC the per-group derivative)
+// On return (after __syncwarp) sm.xi / sm.v / sm.coef / sm.cen are valid for the whole warp.
+template <bool JAC>
+__device__ __forceinline__ void warp_cv_eval(const SysParams& P, int r, const float* __restrict__ pos,
+                                             const double* __restrict__ rpart, WarpCvSmem& sm, int lane) {
+    const float* p = pos + (long long)r * P.rstride * P.ps;
+    // range groups: all lanes sum the block partials (fixed order => deterministic)
+    for (int q = 0; q < P.n_ranges; ++q) {
+        const double* src = rpart + ((long long)r * P.n_ranges + q) * P.range_blocks * PSG_MOM;
+        double a[PSG_MOM] = {0, 0, 0, 0, 0};
+        for (int b = lane; b < P.range_blocks; b += 32) {
+#pragma unroll
+            for (int i = 0; i < PSG_MOM; ++i) a[i] += __ldcg(src + (long long)b * PSG_MOM + i);
+        }
+#pragma unroll
+        for (int i = 0; i < PSG_MOM; ++i) a[i] = warp_sum(a[i]);
+        if (lane == 0) {
+            int gid = P.range_gid[q];
+            double iw = 1.0 / a[0];
+            sm.cen[gid][0] = a[1] * iw; sm.cen[gid][1] = a[2] * iw; sm.cen[gid][2] = a[3] * iw; sm.cen[gid][3] = a[0];
+            sm.m2[gid] = a[4];
+        }
+    }
+    // explicit groups: lane j gathers group j
+    if (lane < P.n_groups && !P.grp[lane].is_range) {
+        const GroupDev& G = P.grp[lane];
+        const int* sa = P.slot_atom + (P.per_rep ? (long long)r * P.n_slots : 0);
+        double sx = 0, sy = 0, sz = 0, sw = 0, s2 = 0;
+        for (int i = 0; i < G.size; ++i) {
+            int s = G.begin + i;
+            D3 x = load_pos(p, sa[s], P.ps);
+            double w = P.slot_weight ? (double)P.slot_weight[s] : 1.0;
+            sx += w * x.x; sy += w * x.y; sz += w * x.z; sw += w;
+            s2 += w * dot(x, x);
+        }
+        double iw = 1.0 / sw;
+        sm.cen[lane][0] = sx * iw; sm.cen[lane][1] = sy * iw; sm.cen[lane][2] = sz * iw; sm.cen[lane][3] = sw;
+        sm.m2[lane] = s2;
+    }
+    __syncwarp();
+    if (lane < P.n_cv) {
+        const CvDev& C = P.cv[lane];
+        int g0 = C.gid0;
+        if (C.type == PSG_CV_RGYR) {
+            // Rg^2 = sum w|r|^2 / W - |c|^2 (binary64 moments); dRg/dr_i = w_i (r_i - c) / (W Rg)
+            D3 c = d3(sm.cen[g0][0], sm.cen[g0][1], sm.cen[g0][2]);
+            double W = sm.cen[g0][3];
+            double rg2 = sm.m2[g0] / W - dot(c, c);
+            double rg = rg2 > 0.0 ? sqrt(rg2) : 0.0;
+            sm.xi[lane] = rg;
+            sm.coef[g0] = rg > 0.0 ? 1.0 / (W * rg) : 0.0;
+            sm.v[g0][0] = sm.v[g0][1] = sm.v[g0][2] = 0.0;
+        } else {
+            D3 c[4], dc[4];
+#pragma unroll
+            for (int g = 0; g < 4; ++g)
+                c[g] = g < C.n_groups ? d3(sm.cen[g0 + g][0], sm.cen[g0 + g][1], sm.cen[g0 + g][2]) : d3(0, 0, 0);
+            sm.xi[lane] = cv_from_centers<JAC>(C.type, C.axis, c, dc);
+            if (JAC) {
+#pragma unroll
+                for (int g = 0; g < 4; ++g)
+                    if (g < C.n_groups) {
+                        double iw = 1.0 / sm.cen[g0 + g][3];
+                        sm.v[g0 + g][0] = dc[g].x * iw; sm.v[g0 + g][1] = dc[g].y * iw; sm.v[g0 + g][2] = dc[g].z * iw;
+                        sm.coef[g0 + g] = 0.0;
+                    }
+            }
+        }
+    }
+    __syncwarp();
+}
+
+// d(xi)/d(r_slot) for an explicit slot s (weight w_s) given the per-group vector
+__device__ __forceinline__ D3 slot_jacobian(const SysParams& P, int r, const float* __restrict__ pos,
+                                            const WarpCvSmem& sm, int s) {
+    int gid = P.slot_gid[s];
+    double w = P.slot_weight ? (double)P.slot_weight[s] : 1.0;
+    D3 j = d3(w * sm.v[gid][0], w * sm.v[gid][1], w * sm.v[gid][2]);
+    if (sm.coef[gid] != 0.0) {   // explicit RGYR group: w (r - c) / (W Rg)
+        const int* sa = P.slot_atom + (P.per_rep ? (long long)r * P.n_slots : 0);
+        D3 x = load_pos(pos + (long long)r * P.rstride * P.ps, sa[s], P.ps);
+        double k = w * sm.coef[gid];
+        j = d3(k * (x.x - sm.cen[gid][0]), k * (x.y - sm.cen[gid][1]), k * (x.z - sm.cen[gid][2]));
+    }
+    return j;
+}

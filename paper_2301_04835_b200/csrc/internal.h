@@ -1,0 +1,122 @@
+// internal.h -- shared declarations of libpsg.so (CUDA path). Not part of the ABI.
+// Shares nothing with oracle/.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+#include <string>
+
+#include "psg.h"
+
+#define PSG_MAX_GROUPS_TOTAL (PSG_MAX_CV * PSG_MAX_GROUPS)
+#define PSG_GDESC_DOUBLES 8      // per (replica, group): vx vy vz | cx cy cz | coef | W
+#define PSG_MOM 5                // moments per range group: W, sum w x, sum w y, sum w z, sum w |r|^2
+#define PSG_RANGE_TILE 2048      // atoms per block in the range-moment / dense-apply kernels
+#define PSG_HILL_RT 8            // replicas per thread in the hill sum
+#define PSG_HILL_WARPS 8         // warps per CTA in the hill sum
+#define PSG_HILL_TILE_R (PSG_HILL_RT * PSG_HILL_WARPS)   // replicas per CTA tile (64)
+#define PSG_HILL_SUB 1024        // hills per shared-memory stage
+#define PSG_HILL_STAGES 3
+
+struct CvDev {
+    int type, n_groups, axis, gid0;   // gid0: global id of this CV's first group
+    float period;
+};
+
+struct GroupDev {
+    int cv, g;          // owner
+    int is_range;
+    int begin, size;    // explicit: slot slice
+    int range_id;       // range: index into the range table, else -1
+    long long rbegin, rsize;
+};
+
+// Everything a kernel needs to know about the system; passed by value.
+struct SysParams {
+    int R;
+    long long N, rstride;       // rstride = 0: shared array
+    int ps, fs;                 // floats per atom in pos / force
+    int n_cv, n_slots, per_rep, n_groups, n_ranges;
+    int any_rgyr;
+    CvDev cv[PSG_MAX_CV];
+    GroupDev grp[PSG_MAX_GROUPS_TOTAL];
+    int range_gid[PSG_MAX_RANGE_GROUPS];     // range id -> global group id
+    long long span_begin, span_end;          // union span of all range groups
+    int range_blocks;                        // blocks per replica over the span
+    const int* slot_atom;        // device [n_slots] or [R][n_slots]
+    const int* slot_gid;         // device [n_slots]: global group id of a slot
+    const float* slot_weight;    // device [n_slots] or nullptr
+    const float* atom_weight;    // device [N] or nullptr
+};
+
+struct HillConsts {
+    float inv_period[PSG_MAX_CV];   // 0 if not periodic
+    float p_hi[PSG_MAX_CV], p_lo[PSG_MAX_CV];
+    float cscale[PSG_MAX_CV];       // sqrt(log2(e)/2)/sigma_k : exponent = -sum (d*cscale)^2 in base 2
+    double gscale[PSG_MAX_CV];      // dV/dxi_k = -gscale_k * sum_h W e a_k
+    double period_d[PSG_MAX_CV];
+    double inv_sigma_d[PSG_MAX_CV];
+    int n_cv, pmask;
+};
+
+struct MetadState {
+    float4* hills;          // records: n_cv<=3: {s0,s1,s2,W}; n_cv==4: {s0..s3},{W,0,0,0}
+    int* n_hills;           // device counter (exact)
+    int capacity;
+    double* part;           // [max_chunks][R_padded][1+n_cv]
+    unsigned* ticket;       // [n_rtiles]
+    int max_chunks;
+    double w0, kB_deltaT;
+    int stride;
+    int precision;
+    int rec;                // float4s per hill record
+    HillConsts hc;
+};
+
+struct AbfState {
+    float lower[PSG_MAX_CV], invd[PSG_MAX_CV];
+    int shape[PSG_MAX_CV], periodic[PSG_MAX_CV];
+    int n_threshold;
+    long long n_bins;
+    int* hist;
+    float* fsum;
+    bool own;
+};
+
+struct psg_ctx {
+    int device = 0;
+    cudaStream_t stream = nullptr;
+    std::string err;
+    long long launches = 0;
+    bool have_layout = false, have_cvs = false, have_jac = false;
+    int method = PSG_METHOD_NONE;
+    SysParams sys{};
+    // device copies of setup arrays
+    int* d_slot_atom = nullptr; int* d_slot_gid = nullptr; float* d_slot_weight = nullptr; float* d_atom_weight = nullptr;
+    // per-replica scratch / step outputs
+    float* d_xi = nullptr; float* d_V = nullptr; float* d_dVdxi = nullptr; int* d_bin = nullptr;
+    double* d_V64 = nullptr;
+    float* d_jac = nullptr;          // [R][n_slots][3]
+    double* d_gdesc = nullptr;       // [R][n_groups][PSG_GDESC_DOUBLES]
+    double* d_rpart = nullptr;       // [R][n_ranges][range_blocks][PSG_MOM]
+    // harmonic
+    float* d_kspring = nullptr; float* d_centers = nullptr;
+    MetadState md{};
+    long long nh_bound = 0;          // host upper bound of the hill count
+    AbfState abf{};
+    // host-engine staging (psg_step_host)
+    float* d_pos_stage = nullptr; float* d_frc_stage = nullptr; float* d_fs_stage = nullptr;
+    int sm_count = 148;
+};
+
+// ---- launchers implemented in the .cu files (all enqueue on ctx->stream) ----
+cudaError_t psg_launch_cv_eval(psg_ctx* c, const float* d_pos, float* d_xi, float* d_jac);
+cudaError_t psg_launch_apply(psg_ctx* c, const float* d_pos, const float* d_dVdxi, float* d_force);
+cudaError_t psg_launch_harmonic(psg_ctx* c, const float* d_xi, float* d_V, float* d_dVdxi);
+cudaError_t psg_launch_hillsum(psg_ctx* c, const float* d_xi, float* d_V, float* d_dVdxi);
+cudaError_t psg_launch_deposit(psg_ctx* c, const float* d_xi, const unsigned char* d_mask);
+cudaError_t psg_launch_pack_hills(psg_ctx* c, int n, const float* d_centers, const float* d_heights);
+cudaError_t psg_launch_unpack_hills(psg_ctx* c, int n, float* d_centers, float* d_heights);
+cudaError_t psg_launch_abf(psg_ctx* c, const float* d_xi, const float* d_fsample, int* d_bin, float* d_dVdxi);
+cudaError_t psg_launch_metad_step(psg_ctx* c, const float* d_pos, float* d_force);   // fused; n_ranges == 0
+bool psg_metad_step_supported(const psg_ctx* c);
+size_t psg_hill_part_doubles(const psg_ctx* c, int* max_chunks_out, int* n_rtiles_out);

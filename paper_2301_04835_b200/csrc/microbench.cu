@@ -1,0 +1,114 @@
+// microbench.cu -- psg_measure_alu_peak: measured ALU throughputs of the device, used as roofline
+// denominators for the hill sum (MEASURED_PEAKS.json holds only HBM and bf16 tensor peaks).
+// Register-only dependent chains, 8 independent chains per thread, 1024 threads x 2 CTAs per SM.
+#include <stdint.h>
+
+#include "internal.h"
+
+#define ITERS 4096
+#define CHAINS 8
+
+template <int WHICH>
+__global__ void __launch_bounds__(1024) k_peak(float* out, float seed) {
+    float a[CHAINS];
+    double d[CHAINS / 2];
+    int q[CHAINS];
+#pragma unroll
+    for (int i = 0; i < CHAINS; ++i) { a[i] = seed + threadIdx.x * 1e-6f + i; q[i] = threadIdx.x + i; }
+#pragma unroll
+    for (int i = 0; i < CHAINS / 2; ++i) d[i] = (double)a[i];
+    const float m = 0.999f + seed * 1e-9f, b = 1e-3f;
+    for (int it = 0; it < ITERS; ++it) {
+        if (WHICH == 0) {
+#pragma unroll
+            for (int i = 0; i < CHAINS; ++i) a[i] = __fmaf_rn(a[i], m, b);
+        } else if (WHICH == 1) {
+#pragma unroll
+            for (int i = 0; i < CHAINS; i += 2)
+                asm volatile("{.reg .b64 x, y, z; mov.b64 x, {%0, %1}; mov.b64 y, {%2, %2}; mov.b64 z, {%3, %3};\n"
+                             " fma.rn.f32x2 x, x, y, z; mov.b64 {%0, %1}, x;}"
+                             : "+f"(a[i]), "+f"(a[i + 1])
+                             : "f"(m), "f"(b));
+        } else if (WHICH == 2) {
+#pragma unroll
+            for (int i = 0; i < CHAINS; ++i) asm volatile("ex2.approx.ftz.f32 %0, %0;" : "+f"(a[i]));
+        } else if (WHICH == 3) {
+#pragma unroll
+            for (int i = 0; i < CHAINS / 2; ++i) d[i] = fma(d[i], (double)m, (double)b);
+        } else if (WHICH == 4) {
+#pragma unroll
+            for (int i = 0; i < CHAINS / 2; ++i) {
+                double t;
+                asm volatile("cvt.f64.f32 %0, %1;" : "=d"(t) : "f"(a[i]));
+                asm volatile("cvt.rn.f32.f64 %0, %1;" : "=f"(a[i]) : "d"(t));
+            }
+        } else if (WHICH == 5) {
+#pragma unroll
+            for (int i = 0; i < CHAINS; ++i) {
+                asm volatile("cvt.rn.f32.s32 %0, %1;" : "=f"(a[i]) : "r"(q[i]));
+                q[i] = __float_as_int(a[i]);
+            }
+        } else if (WHICH == 6) {
+#pragma unroll
+            for (int i = 0; i < CHAINS; i += 2)
+                asm volatile("{.reg .b64 x, y; mov.b64 x, {%0, %1}; mov.b64 y, {%2, %2};\n"
+                             " add.rn.f32x2 x, x, y; mov.b64 {%0, %1}, x;}"
+                             : "+f"(a[i]), "+f"(a[i + 1])
+                             : "f"(b));
+        }
+    }
+    float s = 0.f;
+#pragma unroll
+    for (int i = 0; i < CHAINS; ++i) s += a[i] + (float)q[i];
+#pragma unroll
+    for (int i = 0; i < CHAINS / 2; ++i) s += (float)d[i];
+    if (s == 123.456f) out[0] = s;   // never true; keeps the chains alive
+}
+
+template <int WHICH>
+static cudaError_t time_one(int sms, double ops_per_thread_iter, double* out) {
+    float* d = nullptr;
+    cudaError_t e = cudaMalloc((void**)&d, 4);
+    if (e != cudaSuccess) return e;
+    cudaEvent_t t0, t1;
+    cudaEventCreate(&t0);
+    cudaEventCreate(&t1);
+    int grid = sms * 2;
+    double best = 0.0;
+    for (int rep = 0; rep < 6; ++rep) {
+        cudaEventRecord(t0);
+        k_peak<WHICH><<<grid, 1024>>>(d, 1.0f);
+        cudaEventRecord(t1);
+        e = cudaEventSynchronize(t1);
+        if (e != cudaSuccess) break;
+        float ms = 0.f;
+        cudaEventElapsedTime(&ms, t0, t1);
+        double rate = (double)grid * 1024.0 * ITERS * ops_per_thread_iter / (ms * 1e-3);
+        if (rep > 0 && rate > best) best = rate;
+    }
+    cudaEventDestroy(t0);
+    cudaEventDestroy(t1);
+    cudaFree(d);
+    *out = best;
+    return e == cudaSuccess ? cudaGetLastError() : e;
+}
+
+extern "C" int psg_measure_alu_peak(int device, int which, double* out) {
+    if (!out) return PSG_EINVAL;
+    if (cudaSetDevice(device) != cudaSuccess) return PSG_ECUDA;
+    cudaDeviceProp prop;
+    if (cudaGetDeviceProperties(&prop, device) != cudaSuccess) return PSG_ECUDA;
+    int sms = prop.multiProcessorCount;
+    cudaError_t e;
+    switch (which) {
+    case 0: e = time_one<0>(sms, CHAINS, out); break;          // FFMA lane-ops
+    case 1: e = time_one<1>(sms, CHAINS, out); break;          // FFMA2: CHAINS/2 instructions x 2 lanes-ops
+    case 2: e = time_one<2>(sms, CHAINS, out); break;          // MUFU.EX2
+    case 3: e = time_one<3>(sms, CHAINS / 2, out); break;      // DFMA
+    case 4: e = time_one<4>(sms, CHAINS / 2, out); break;      // F2F.F64.F32 (+ the way back; counts the widening only)
+    case 5: e = time_one<5>(sms, CHAINS, out); break;          // I2F.F32.S32
+    case 6: e = time_one<6>(sms, CHAINS, out); break;          // FADD2
+    default: return PSG_EINVAL;
+    }
+    return e == cudaSuccess ? PSG_OK : PSG_ECUDA;
+}
