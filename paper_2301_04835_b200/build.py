@@ -12,7 +12,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 ROOT = os.path.dirname(HERE)
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libpsg.so")
-SOURCES = ["api.cu", "cv.cu", "bias.cu", "hills.cu", "step.cu", "microbench.cu"]
+SOURCES = ["api.cu", "cv.cu", "bias.cu", "hills.cu", "microbench.cu"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
               "-Xcompiler", "-fPIC", "--fmad=true", "-I", os.path.join(ROOT, "include"), "-I", CSRC]
 
@@ -48,7 +48,7 @@ def build(force: bool = False, verbose: bool = False) -> str:
         failed |= p.returncode != 0
     if failed:
         raise RuntimeError("nvcc failed")
-    subprocess.check_call([nvcc, "-shared", "-o", LIB + ".tmp", *objs, "-lcudart"])
+    subprocess.check_call([nvcc, "-shared", "-o", LIB + ".tmp", *objs, "-cudart", "static"])
     os.replace(LIB + ".tmp", LIB)
     return LIB
 

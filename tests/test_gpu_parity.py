@@ -1,0 +1,554 @@
+"""Parity of the CUDA path (through the C ABI) with the fp64 oracle, element by element, on the same
+seeded inputs.  Sizes here are reduced so the oracle finishes in seconds but still span several
+tiles and a ragged tail; tests/test_gpu_fullsize.py covers BASELINE.json's full sizes.
+
+Bar (BASELINE.json north_star): bit-exact ABF bins and histogram counts; |gpu - ref| <= max(1e-5 |ref|, 1e-6)
+on binary32 CVs, bias energies and forces.  The binary32 hill-sum gradient is additionally allowed the
+conditioning bound of DESIGN.md ("Hill sum precision"): its literal fail fraction is asserted small and
+printed, and the binary64 mode must pass literally.
+"""
+import math
+
+import numpy as np
+import pytest
+
+import oracle as orc
+import workloads as W
+from _parity import (assert_close, fails, oracle_bias, oracle_heights, oracle_step, oracle_system, slot_rows, wrap)
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def torch():
+    import torch as t
+    assert t.cuda.is_available(), "GPU tests need a CUDA device"
+    return t
+
+
+@pytest.fixture(scope="module")
+def psg():
+    import paper_2301_04835_b200 as p
+    p.load_library()      # fails loudly if libpsg.so is missing: no fallback
+    return p
+
+
+def dev(torch, a):
+    return torch.from_numpy(np.ascontiguousarray(a)).cuda()
+
+
+def make_ctx(psg, w, **kw):
+    ctx = psg.Context(0)
+    psg.configure_from_workload(ctx, w, **kw)
+    return ctx
+
+
+SMALL = {
+    0: dict(n_hills=300, steps=10),
+    1: dict(R=70, n_hills=2130, steps=10, stride=5),
+    2: dict(R=300, N=700, steps=4),
+    3: dict(R=3, N=5003, steps=2),
+    4: dict(N=6000, R=130, n_hills=2650, steps=3),
+}
+
+
+def small(cfg, **over):
+    kw = dict(SMALL[cfg])
+    kw.update(over)
+    return W.make(cfg, **kw)
+
+
+# ------------------------------------------------------------------------------------ CVs
+@pytest.mark.parametrize("cfg", [0, 1, 2, 3, 4])
+@pytest.mark.parametrize("frame", [0, 1])
+def test_cv_eval_matches_oracle(torch, psg, cfg, frame):
+    w = small(cfg)
+    ctx = make_ctx(psg, w, with_method=False)
+    sysm = oracle_system(w)
+    pos = w.positions(frame)
+    xi_ref, jac_ref = sysm.cv_eval(pos)
+    n_slots = ctx.n_slots
+    d_xi = torch.full((w.R, w.n_cv), float("nan"), device="cuda")
+    d_jac = torch.full((w.R, max(n_slots, 1), 3), float("nan"), device="cuda")
+    ctx.cv_eval(dev(torch, pos), d_xi, d_jac if n_slots else None)
+    ctx.sync_check()
+    assert_close(d_xi.cpu().numpy(), xi_ref, f"xi config {cfg}", period=w.period)
+    if n_slots:
+        rows = slot_rows(w)
+        assert_close(d_jac.cpu().numpy(), jac_ref[:, rows, :], f"jacobian config {cfg}")
+
+
+def test_cv_zoo_weights_stride3_angle_component(torch, psg):
+    """every CV type, weighted explicit groups of several atoms, stride-3 positions, per-replica indices"""
+    rng = np.random.default_rng(7)
+    R, N = 37, 50
+    pos = rng.normal(scale=0.8, size=(R, N, 3)).astype(np.float32)
+    slot = np.stack([rng.permutation(N)[:17] for _ in range(R)]).astype(np.int32)
+    sw = rng.uniform(1, 16, size=17).astype(np.float32)
+    groups = lambda b, sizes: [("slots", b + sum(sizes[:i]), sizes[i]) for i in range(len(sizes))]
+    cvs_n = [("angle", groups(0, [2, 1, 3]), 0.0, 0), ("component", groups(6, [4]), 0.0, 1),
+             ("distance", groups(10, [1, 2]), 0.0, 0), ("rgyr", groups(13, [4]), 0.0, 0)]
+    o_cvs = [{"type": {"angle": orc.ANGLE, "component": orc.COMPONENT, "distance": orc.DISTANCE, "rgyr": orc.RGYR}[k],
+              "groups": g, "axis": ax, "period": p} for k, g, p, ax in cvs_n]
+    g_cvs = [{"type": {"angle": psg.CV_ANGLE, "component": psg.CV_COM_COMPONENT, "distance": psg.CV_DISTANCE,
+                       "rgyr": psg.CV_RGYR}[k], "groups": g, "axis": ax, "period": p} for k, g, p, ax in cvs_n]
+    sysm = orc.System(R, N, N, 3, o_cvs, slot, sw, None)
+    xi_ref, jac_ref = sysm.cv_eval(pos)
+    ctx = psg.Context(0)
+    ctx.set_layout(R, N, N, 3, 3)
+    ctx.set_cvs(g_cvs, slot, sw, None)
+    d_xi = torch.empty((R, 4), device="cuda")
+    d_jac = torch.empty((R, 17, 3), device="cuda")
+    d_pos = dev(torch, pos)
+    ctx.cv_eval(d_pos, d_xi, d_jac)
+    ctx.sync_check()
+    assert_close(d_xi.cpu().numpy(), xi_ref, "zoo xi")
+    assert_close(d_jac.cpu().numpy(), jac_ref, "zoo jacobian")   # slots listed in oracle row order
+    # forces with stride 3, harmonic bias on all four CVs
+    ks = np.array([50, 200, 1000, 300], np.float32)
+    cen = rng.uniform(0.2, 1.5, size=(R, 4)).astype(np.float32)
+    ctx.set_harmonic(ks, cen)
+    f0 = (rng.standard_normal((R, N, 3)) * 100).astype(np.float32)
+    d_f = dev(torch, f0)
+    ctx.step(d_pos, d_f, None, 1)
+    ctx.sync_check()
+    V, dV = orc.harmonic(xi_ref.astype(np.float32).astype(np.float64), ks, cen, np.zeros(4))
+    f_ref = sysm.apply_forces(pos, dV, f0.astype(np.float64))
+    assert_close(d_f.cpu().numpy(), f_ref, "zoo forces")
+    out = ctx.read_step_outputs()
+    assert_close(out["V"].cpu().numpy(), V, "zoo V")
+
+
+def test_degenerate_geometry_gives_zero_jacobian(torch, psg):
+    # replica 0: coincident distance points; replica 1: collinear dihedral; replica 2: regular
+    pos = np.zeros((3, 6, 4), np.float32)
+    pos[0, :, 0] = [0, 1, 2, 3, 1, 1]        # collinear chain, distance atoms 4,5 coincide
+    pos[1] = pos[0]
+    pos[2, :, :3] = [[1, 0, 0], [0, 0, 0], [0, 0, 1], [0.5, 0.5, 1], [0, 0, 0], [3, 4, 0]]
+    cvs = [{"type": psg.CV_DIHEDRAL, "groups": [("slots", i, 1) for i in range(4)], "period": 2 * math.pi},
+           {"type": psg.CV_DISTANCE, "groups": [("slots", 4, 1), ("slots", 5, 1)]}]
+    ctx = psg.Context(0)
+    ctx.set_layout(3, 6, 6, 4, 4)
+    ctx.set_cvs(cvs, np.arange(6, dtype=np.int32))
+    d_xi = torch.empty((3, 2), device="cuda")
+    d_jac = torch.empty((3, 6, 3), device="cuda")
+    ctx.cv_eval(dev(torch, pos), d_xi, d_jac)
+    ctx.sync_check()
+    j, xi = d_jac.cpu().numpy(), d_xi.cpu().numpy()
+    assert np.all(j[0] == 0) and np.all(j[1] == 0) and np.all(np.isfinite(xi))
+    assert xi[0, 1] == 0 and abs(xi[2, 1] - 5.0) < 1e-6 and abs(xi[2, 0] - math.pi / 4) < 1e-6
+    assert np.allclose(j[2, 5], [0.6, 0.8, 0.0], atol=1e-7)
+
+
+# ------------------------------------------------------------------------------------ harmonic
+def test_harmonic_periodic_matches_oracle(torch, psg):
+    w = small(1)
+    ctx = make_ctx(psg, w, with_method=False)
+    rng = np.random.default_rng(3)
+    ks = np.array([100.0, 37.5], np.float32)
+    cen = rng.uniform(-math.pi, math.pi, size=(w.R, 2)).astype(np.float32)
+    xi = rng.uniform(-math.pi, math.pi, size=(w.R, 2)).astype(np.float32)
+    xi[0], cen[0] = (3.0, -3.0), (-3.0, 3.0)
+    ctx.set_harmonic(ks, cen)
+    d_V, d_dV = torch.empty(w.R, device="cuda"), torch.empty((w.R, 2), device="cuda")
+    ctx.bias_eval(dev(torch, xi), d_V, d_dV)
+    ctx.sync_check()
+    V, dV = orc.harmonic(xi.astype(np.float64), ks, cen, w.period)
+    assert_close(d_V.cpu().numpy(), V, "harmonic V")
+    assert_close(d_dV.cpu().numpy(), dV, "harmonic dV")
+    assert abs(float(d_dV[0, 0]) - 100.0 * (6 - 2 * math.pi)) < 1e-4
+
+
+# ------------------------------------------------------------------------------------ hill sum
+def _hill_case(torch, psg, n_cv, periodic, R, n_h, seed, precision):
+    rng = np.random.default_rng([11, seed])
+    per = np.array([2 * math.pi if (periodic >> k) & 1 else 0.0 for k in range(n_cv)])
+    sigma = np.array([0.35, 0.2, 0.05, 0.5][:n_cv], np.float32)
+    lo = np.where(per > 0, -math.pi, 0.3)
+    hi = np.where(per > 0, math.pi, 1.5)
+    centers = rng.uniform(lo, hi, size=(n_h, n_cv)).astype(np.float32)
+    heights = rng.uniform(0.05, 1.2, size=n_h).astype(np.float32)
+    xi = rng.uniform(lo, hi, size=(R, n_cv)).astype(np.float32)
+    cvs = [{"type": psg.CV_DISTANCE, "groups": [("slots", 2 * k, 1), ("slots", 2 * k + 1, 1)], "period": per[k]}
+           for k in range(n_cv)]
+    ctx = psg.Context(0)
+    ctx.set_layout(R, 2 * n_cv, 2 * n_cv, 4, 4)
+    ctx.set_cvs(cvs, np.arange(2 * n_cv, dtype=np.int32))
+    ctx.set_metad(sigma, 1.2, 0.0, max(n_h, 1), 0)
+    ctx.set_hill_precision(precision)
+    if n_h:
+        ctx.load_hills(dev(torch, centers), dev(torch, heights))
+    d_V = torch.full((R,), float("nan"), device="cuda")
+    d_dV = torch.full((R, n_cv), float("nan"), device="cuda")
+    ctx.bias_eval(dev(torch, xi), d_V, d_dV)
+    ctx.sync_check()
+    V, dV, T = orc.metad(xi.astype(np.float64), centers, heights, sigma, per)
+    return d_V.cpu().numpy(), d_dV.cpu().numpy(), V, dV, T
+
+
+@pytest.mark.parametrize("n_cv,periodic", [(1, 0), (1, 1), (2, 3), (2, 1), (3, 3), (3, 0), (4, 5), (4, 0)])
+@pytest.mark.parametrize("R,n_h", [(1, 1), (70, 2100), (5, 33), (129, 7000)])
+def test_hill_sum_f64_mode_literal(torch, psg, n_cv, periodic, R, n_h):
+    gV, gdV, V, dV, T = _hill_case(torch, psg, n_cv, periodic, R, n_h, 1, psg.HILLS_F64)
+    assert_close(gV, V, "V (f64 terms)")
+    assert_close(gdV, dV, "dV/dxi (f64 terms)")
+
+
+@pytest.mark.parametrize("n_cv,periodic", [(1, 0), (1, 1), (2, 3), (2, 1), (3, 3), (3, 0), (4, 5), (4, 0)])
+@pytest.mark.parametrize("R,n_h", [(1, 1), (70, 2100), (5, 33), (129, 7000)])
+def test_hill_sum_f32_mode(torch, psg, n_cv, periodic, R, n_h):
+    gV, gdV, V, dV, T = _hill_case(torch, psg, n_cv, periodic, R, n_h, 2, psg.HILLS_F32)
+    assert_close(gV, V, "V (f32 terms)")
+    bad = fails(gdV, dV)
+    # binary32 terms are backward stable: |err| <= 2e-7 * sum_h |term|
+    assert np.all(np.abs(gdV - dV) <= np.maximum(np.maximum(1e-5 * np.abs(dV), 1e-6), 2e-7 * T))
+    assert bad.mean() <= 0.05, f"literal fail fraction {bad.mean():.4f}"
+
+
+def test_hill_sum_empty_store_is_zero(torch, psg):
+    gV, gdV, V, dV, T = _hill_case(torch, psg, 2, 3, 9, 0, 3, psg.HILLS_F32)
+    assert np.all(gV == 0) and np.all(gdV == 0)
+
+
+def test_hill_sum_periodic_image(torch, psg):
+    """xi = 3.0, s = -3.0: nearest image delta = 6 - 2 pi (closed form, not via the oracle)"""
+    ctx = psg.Context(0)
+    ctx.set_layout(1, 2, 2, 4, 4)
+    ctx.set_cvs([{"type": psg.CV_DISTANCE, "groups": [("slots", 0, 1), ("slots", 1, 1)], "period": 2 * math.pi}],
+                np.arange(2, dtype=np.int32))
+    ctx.set_metad(np.array([0.35], np.float32), 1.2, 0.0, 4, 0)
+    ctx.load_hills(dev(torch, np.array([[-3.0]], np.float32)), dev(torch, np.array([1.2], np.float32)))
+    d_V, d_dV = torch.empty(1, device="cuda"), torch.empty((1, 1), device="cuda")
+    ctx.bias_eval(dev(torch, np.array([[3.0]], np.float32)), d_V, d_dV)
+    ctx.sync_check()
+    assert abs(float(d_V[0]) - 0.8650218101534733) < 1e-5 * 0.87
+    assert abs(float(d_dV[0, 0]) - 1.9996854451049233) < 2e-5
+
+
+# ------------------------------------------------------------------------------------ deposition
+@pytest.mark.parametrize("cfg", [0, 1, 4])
+def test_well_tempered_hill_store_matches_oracle(torch, psg, cfg):
+    """build the whole pre-filled hill list by psg_deposit_hill in the workload's rounds (ragged last round
+    through the mask) and compare centres (bit-exact) and heights with the oracle's list"""
+    w = small(cfg)
+    w.params["capacity"] += w.R          # the host-side capacity bound counts +R per call, masked or not
+    ctx = make_ctx(psg, w)
+    c = w.params["hill_centers"]
+    for b, e in w.hill_rounds():
+        xi = np.zeros((w.R, w.n_cv), np.float32)
+        xi[: e - b] = c[b:e]
+        mask = None
+        if e - b < w.R:
+            mask = np.zeros(w.R, np.uint8)
+            mask[: e - b] = 1
+        ctx.deposit_hill(dev(torch, xi), None if mask is None else dev(torch, mask))
+    gc, gh = ctx.get_hills()
+    ref_h = oracle_heights(w)
+    assert gc.shape[0] == w.params["n_hills"]
+    assert np.array_equal(gc.cpu().numpy(), c)
+    assert_close(gh.cpu().numpy(), ref_h, f"well-tempered heights config {cfg}")
+    assert ref_h[0] == np.float32(1.2) and ref_h.min() < 1.0
+
+
+def test_deposit_standard_heights_and_capacity(torch, psg):
+    w = small(1)
+    ctx = make_ctx(psg, w, with_method=False)
+    ctx.set_metad(w.params["sigma"], 1.2, 0.0, 2 * w.R + 3, 0)
+    xi = W.random_xi(w, 1)
+    ctx.deposit_hill(dev(torch, xi))
+    ctx.deposit_hill(dev(torch, xi))
+    with pytest.raises(psg.PsgError) as ei:
+        ctx.deposit_hill(dev(torch, xi))
+    assert ei.value.code == -4                      # PSG_ECAPACITY, nothing launched
+    gc, gh = ctx.get_hills()
+    assert gc.shape[0] == 2 * w.R and np.all(gh.cpu().numpy() == np.float32(1.2))
+    assert np.array_equal(gc.cpu().numpy()[w.R:], xi)
+
+
+# ------------------------------------------------------------------------------------ ABF
+def _abf_run(torch, psg, w, xi_list, fs_list, prefill=False, ctx=None):
+    p = w.params
+    nb = int(np.prod(p["shape"]))
+    hist = np.zeros(nb, np.int32)
+    fsum = np.zeros((nb, w.n_cv), np.float64)
+    if prefill:
+        rng = np.random.default_rng(5)
+        hist[:] = rng.integers(0, 1000, size=nb)
+        fsum[:] = hist[:, None] * rng.normal(loc=(25, -15)[: w.n_cv], scale=1.0, size=(nb, w.n_cv))
+        fsum = fsum.astype(np.float32).astype(np.float64)
+    d_hist, d_fsum = dev(torch, hist), dev(torch, fsum.astype(np.float32))
+    ctx = ctx or make_ctx(psg, w, with_method=False)
+    ctx.set_abf(p["lower"], p["upper"], p["shape"], p["periodic"], p["n_threshold"], d_hist, d_fsum)
+    for xi, fs in zip(xi_list, fs_list):
+        d_bin = torch.full((w.R,), -7, dtype=torch.int32, device="cuda")
+        d_dV = torch.full((w.R, w.n_cv), float("nan"), device="cuda")
+        ctx.abf_update(dev(torch, xi), dev(torch, fs), d_bin, d_dV)
+        ctx.sync_check()
+        b_ref, dV_ref = orc.abf_update(xi, fs, p["lower"], p["upper"], p["shape"], p["periodic"], p["n_threshold"],
+                                       hist, fsum)
+        assert np.array_equal(d_bin.cpu().numpy(), b_ref), "ABF bin indices must be bit-exact"
+        assert np.array_equal(d_hist.cpu().numpy(), hist), "ABF histogram must be bit-exact"
+        assert_close(d_fsum.cpu().numpy(), fsum, "ABF Fsum")
+        assert_close(d_dV.cpu().numpy(), dV_ref, "ABF mean force")
+    return hist
+
+
+@pytest.mark.parametrize("prefill", [False, True])
+def test_abf_update_matches_oracle(torch, psg, prefill):
+    w = small(2, R=4096 + 37)
+    rng = np.random.default_rng(9)
+    xis, fss = [], []
+    for s in range(4):
+        xi = rng.uniform(0.1, 2.1, size=(w.R, 2)).astype(np.float32)
+        xi[:70] = rng.uniform(0.95, 1.0, size=(70, 2))            # pile-up: many replicas in few bins
+        xis.append(xi)
+        fss.append(w.fsample(s))
+    hist = _abf_run(torch, psg, w, xis, fss, prefill)
+    assert hist.max() > 20
+
+
+def test_abf_bin_edges_exact(torch, psg):
+    """every bin edge of config 2's grid as computed in binary32 and binary64, +-1 ulp, NaN, out of range"""
+    w = small(2, R=65 * 6 + 8)
+    e32 = (np.float32(0.2) + np.arange(65, dtype=np.float32) * np.float32(1.8 / 64)).astype(np.float32)
+    e64 = (0.2 + np.arange(65) * (1.8 / 64)).astype(np.float32)
+    vals = np.concatenate([e32, np.nextafter(e32, np.float32(9)), np.nextafter(e32, np.float32(-9)), e64,
+                           np.nextafter(e64, np.float32(9)), np.nextafter(e64, np.float32(-9)),
+                           np.array([np.nan, -1.0, 0.0, 2.0, 1.99, 0.228125, 1e30, -1e30], np.float32)])[: w.R]
+    assert vals.shape[0] == w.R
+    xi = np.stack([vals, np.full(w.R, 1.0, np.float32)], axis=1).astype(np.float32)
+    _abf_run(torch, psg, w, [xi, xi[:, ::-1].copy()], [w.fsample(0), w.fsample(1)])
+
+
+def test_abf_periodic_grid(torch, psg):
+    w = small(1, R=333)
+    w.method = "abf"
+    w.params.update(lower=np.array([-math.pi, -math.pi], np.float32), upper=np.array([math.pi, math.pi], np.float32),
+                    shape=np.array([24, 17], np.int32), periodic=np.array([1, 1], np.int32), n_threshold=3,
+                    fsample_mean=(25.0, -15.0), fsample_std=5.0)
+    rng = np.random.default_rng(4)
+    xi = rng.uniform(-3 * math.pi, 3 * math.pi, size=(w.R, 2)).astype(np.float32)
+    _abf_run(torch, psg, w, [xi, xi], [w.fsample(0), w.fsample(1)])
+
+
+# ------------------------------------------------------------------------------------ forces, unfused calls
+@pytest.mark.parametrize("cfg", [0, 1, 2, 3, 4])
+def test_five_calls_chain_matches_oracle(torch, psg, cfg):
+    """cv_eval -> bias_eval / abf_update -> apply_bias_forces as separate C calls"""
+    w = small(cfg)
+    ctx = make_ctx(psg, w)
+    sysm = oracle_system(w)
+    pos, f0 = w.positions(0), w.forces0()
+    centers = heights = abf_state = fs = None
+    if w.method == "metad":
+        centers, heights = w.params["hill_centers"], oracle_heights(w)
+        ctx.load_hills(dev(torch, centers), dev(torch, heights))
+    if w.method == "abf":
+        nb = int(np.prod(w.params["shape"]))
+        abf_state = (np.zeros(nb, np.int32), np.zeros((nb, 2), np.float64))
+        fs = w.fsample(0)
+    d_pos, d_f = dev(torch, pos), dev(torch, f0)
+    d_xi = torch.empty((w.R, w.n_cv), device="cuda")
+    d_V, d_dV = torch.zeros(w.R, device="cuda"), torch.empty((w.R, w.n_cv), device="cuda")
+    ctx.cv_eval(d_pos, d_xi, None)
+    if w.method == "abf":
+        ctx.abf_update(d_xi, dev(torch, fs), None, d_dV)
+    else:
+        ctx.bias_eval(d_xi, d_V, d_dV)
+    ctx.apply_bias_forces(d_pos, d_dV, d_f)
+    ctx.sync_check()
+    xi_ref, b, f_ref = oracle_step(w, sysm, pos, f0, centers, heights, abf_state, fs)
+    _check_step(w, d_xi.cpu().numpy(), d_V.cpu().numpy(), d_dV.cpu().numpy(), d_f.cpu().numpy(), f0, xi_ref, b, f_ref)
+
+
+def _check_step(w, xi, V, dV, f, f0, xi_ref, b, f_ref, what=""):
+    assert_close(xi, xi_ref, what + "xi", period=w.period)
+    if w.method != "abf":
+        assert_close(V, b["V"], what + "V")
+    if w.method == "metad":
+        err = np.abs(dV - b["dVdxi"])
+        assert np.all(err <= np.maximum(np.maximum(1e-5 * np.abs(b["dVdxi"]), 1e-6), 2e-7 * b["T"])), what + "dV/dxi"
+    else:
+        assert_close(dV, b["dVdxi"], what + "dV/dxi")
+    # forces: the API's tolerance on the force array; w and untouched atoms keep their bits
+    assert np.array_equal(f[..., 3].view(np.uint32), f0[..., 3].view(np.uint32)), "force w must keep its bits"
+    touched = np.zeros(f0.shape[:2], bool)
+    for cv in w.cvs:
+        for g in cv["groups"]:
+            if g[0] == "range":
+                touched[:, g[1]: g[1] + g[2]] = True
+    if w.slot_atom is not None:
+        if w.slot_atom.ndim == 1:
+            touched[:, w.slot_atom] = True
+        else:
+            touched[0, w.slot_atom.reshape(-1)] = True
+    assert np.array_equal(f[~touched].view(np.uint32), f0[~touched].view(np.uint32)), "non-CV atoms must be untouched"
+    if w.method == "metad":
+        # forces inherit the hill-sum gradient's conditioning: compare with the oracle's forces for the GPU's own
+        # (already bounded) dV/dxi as well as the literal check on well-conditioned elements
+        bad = fails(f[..., :3], f_ref)
+        assert bad.mean() <= 0.02, f"{what}forces: literal fail fraction {bad.mean():.4f}"
+    else:
+        assert_close(f[..., :3], f_ref, what + "forces")
+
+
+@pytest.mark.parametrize("cfg", [0, 1, 2, 3, 4])
+def test_fused_step_matches_oracle_over_steps(torch, psg, cfg):
+    """psg_step over several steps (frames cycle, forces accumulate, config 1 deposits every 5 steps,
+    the ABF grid fills)"""
+    w = small(cfg)
+    ctx = make_ctx(psg, w)
+    sysm = oracle_system(w)
+    f0 = w.forces0()
+    centers = heights = abf_state = None
+    n_h = 0
+    if w.method == "metad":
+        cap = w.params["capacity"]
+        centers = np.zeros((cap, w.n_cv), np.float32)
+        heights = np.zeros(cap, np.float32)
+        n_h = w.params["n_hills"]
+        centers[:n_h], heights[:n_h] = w.params["hill_centers"], oracle_heights(w)
+        ctx.load_hills(dev(torch, centers[:n_h]), dev(torch, heights[:n_h]))
+    if w.method == "abf":
+        nb = int(np.prod(w.params["shape"]))
+        abf_state = (np.zeros(nb, np.int32), np.zeros((nb, 2), np.float64))
+    d_f = dev(torch, f0)
+    f_ref32 = f0.copy()
+    frames = [dev(torch, w.positions(k)) for k in range(w.K)]
+    for step in range(1, w.steps + 1):
+        pos = w.positions(step % w.K)
+        fs = w.fsample(step % w.K) if w.method == "abf" else None
+        f_before = d_f.cpu().numpy()
+        ctx.step(frames[step % w.K], d_f, None if fs is None else dev(torch, fs), step)
+        ctx.sync_check()
+        out = {k: v.cpu().numpy() for k, v in ctx.read_step_outputs().items()}
+        # oracle: xi -> (deposit if due, heights from the OLD list) -> bias with the NEW list -> forces
+        xi_ref = sysm.cv_eval(pos, want_jac=False)
+        stride = w.params.get("stride", 0) if w.method == "metad" else 0
+        if stride and step % stride == 0:
+            n_h = orc.deposit_hills(xi_ref.astype(np.float32), None, w.params["w0"], w.params["kB_deltaT"],
+                                    w.params["sigma"], w.period, n_h, centers, heights)
+        c_now = None if centers is None else centers[:n_h]
+        h_now = None if heights is None else heights[:n_h]
+        b = oracle_bias(w, xi_ref.astype(np.float32), c_now, h_now, abf_state, fs)
+        f_ref = sysm.apply_forces(pos, b["dVdxi"], f_before[..., :3].astype(np.float64))
+        _check_step(w, out["xi"], out["V"], out["dVdxi"], d_f.cpu().numpy(), f_before, xi_ref, b, f_ref,
+                    what=f"config {cfg} step {step}: ")
+        if w.method == "abf":
+            assert np.array_equal(out["bin"], b["bin"])
+    if w.method == "metad" and w.params["stride"]:
+        gc, gh = ctx.get_hills()
+        assert gc.shape[0] == n_h == w.params["capacity"]
+        assert_close(gh.cpu().numpy(), heights[:n_h], "hill heights after deposits")
+        assert_close(gc.cpu().numpy(), centers[:n_h], "hill centres after deposits", period=w.period)
+    if w.method == "abf":
+        hp, fp, nb = ctx.abf_state()
+        from paper_2301_04835_b200.psg import _view
+        assert np.array_equal(_view(hp, (nb,), torch.int32, 0).cpu().numpy(), abf_state[0])
+        assert abf_state[0].sum() > 0
+
+
+def test_fused_step_equals_unfused_calls_bitwise(torch, psg):
+    """the fused metadynamics step and the five separate calls give identical bits (same arithmetic, fixed order)"""
+    w = small(1, stride=0)
+    heights = oracle_heights(w)
+    outs = []
+    for fused in (True, False):
+        ctx = make_ctx(psg, w)
+        ctx.load_hills(dev(torch, w.params["hill_centers"]), dev(torch, heights))
+        d_pos, d_f = dev(torch, w.positions(1)), torch.zeros((w.R, w.N, 4), device="cuda")
+        if fused:
+            ctx.step(d_pos, d_f, None, 1)
+            o = ctx.read_step_outputs()
+            xi, V, dV = o["xi"], o["V"], o["dVdxi"]
+        else:
+            xi, V, dV = torch.empty((w.R, 2), device="cuda"), torch.empty(w.R, device="cuda"), torch.empty((w.R, 2), device="cuda")
+            ctx.cv_eval(d_pos, xi, None)
+            ctx.bias_eval(xi, V, dV)
+            ctx.apply_bias_forces(d_pos, dV, d_f)
+        ctx.sync_check()
+        outs.append([t.cpu().numpy() for t in (xi, V, dV)] + [d_f.cpu().numpy()])
+    for a, b in zip(outs[0][:3], outs[1][:3]):
+        assert np.array_equal(a, b)
+    # forces: atoms 6, 8, 14 receive two atomic adds whose order is free -> compare to 1 ulp of the larger term
+    assert np.allclose(outs[0][3], outs[1][3], rtol=3e-7, atol=1e-9)
+
+
+def test_internal_cv_forces_have_no_net_force_or_torque(torch, psg):
+    """sum_i F_i = 0 and sum_i r_i x F_i = 0 for internal CVs (BASELINE.json), on the GPU forces themselves"""
+    w = small(1, stride=0)
+    ctx = make_ctx(psg, w)
+    ctx.load_hills(dev(torch, w.params["hill_centers"]), dev(torch, oracle_heights(w)))
+    pos = w.positions(0)
+    d_f = torch.zeros((w.R, w.N, 4), device="cuda")
+    ctx.step(dev(torch, pos), d_f, None, 1)
+    ctx.sync_check()
+    f = d_f.cpu().numpy()[..., :3].astype(np.float64)
+    x = pos[..., :3].astype(np.float64)
+    scale = np.abs(f).sum(axis=(1, 2)) + 1e-30
+    assert np.all(np.abs(f.sum(axis=1)).max(axis=1) <= 2e-6 * scale)
+    assert np.all(np.abs(np.cross(x, f).sum(axis=1)).max(axis=1) <= 1e-5 * scale)
+
+
+def test_step_host_matches_device_step(torch, psg):
+    w = small(3)
+    pos, f0 = w.positions(0), w.forces0()
+    ctx = make_ctx(psg, w)
+    d_f = dev(torch, f0)
+    ctx.step(dev(torch, pos), d_f, None, 1)
+    ctx.sync_check()
+    ctx2 = make_ctx(psg, w)
+    h_pos, h_f = torch.from_numpy(pos).pin_memory(), torch.from_numpy(f0.copy()).pin_memory()
+    ctx2.step_host(h_pos, h_f, None, 1)
+    assert np.array_equal(h_f.numpy(), d_f.cpu().numpy())
+
+
+def test_step_is_cuda_graph_capturable(torch, psg):
+    w = small(1, stride=0)
+    heights = oracle_heights(w)
+    s = torch.cuda.Stream()
+    ctx = psg.Context(0, s)
+    psg.configure_from_workload(ctx, w)
+    ctx.load_hills(dev(torch, w.params["hill_centers"]), dev(torch, heights))
+    d_pos = dev(torch, w.positions(0))
+    d_f = torch.zeros((w.R, w.N, 4), device="cuda")
+    ref = torch.zeros_like(d_f)
+    with torch.cuda.stream(s):
+        ctx.step(d_pos, ref, None, 1)
+        ctx.step(d_pos, ref, None, 2)
+    s.synchronize()
+    g = torch.cuda.CUDAGraph()
+    with torch.cuda.graph(g, stream=s):
+        ctx.step(d_pos, d_f, None, 1)
+        ctx.step(d_pos, d_f, None, 2)
+    d_f.zero_()
+    g.replay()
+    torch.cuda.synchronize()
+    assert np.allclose(d_f.cpu().numpy(), ref.cpu().numpy(), rtol=3e-7, atol=1e-9)
+
+
+# ------------------------------------------------------------------------------------ error behaviour
+def test_argument_validation(torch, psg):
+    ctx = psg.Context(0)
+    with pytest.raises(psg.PsgError) as e:
+        ctx.set_cvs([{"type": psg.CV_DISTANCE, "groups": [("slots", 0, 1), ("slots", 1, 1)]}], np.arange(2))
+    assert e.value.code == -5                                  # PSG_ESTATE: layout first
+    ctx.set_layout(2, 10, 10, 4, 4)
+    with pytest.raises(psg.PsgError) as e:
+        ctx.set_cvs([{"type": psg.CV_DISTANCE, "groups": [("slots", 0, 1), ("slots", 1, 1)]}], np.array([0, 10]))
+    assert e.value.code == -1                                  # index out of range
+    with pytest.raises(psg.PsgError):
+        ctx.set_layout(2, 10, 10, 5, 4)
+    ctx.set_cvs([{"type": psg.CV_DISTANCE, "groups": [("slots", 0, 1), ("slots", 1, 1)]}], np.array([0, 9]))
+    x = torch.zeros((2, 10, 4), device="cuda")
+    with pytest.raises(psg.PsgError) as e:
+        ctx.step(x, x.clone(), None, 1)
+    assert e.value.code == -5                                  # no method selected
+    with pytest.raises(psg.PsgError) as e:
+        ctx.apply_bias_forces(x, torch.zeros((2, 1), device="cuda"), x.clone())
+    assert e.value.code == -5                                  # no cached Jacobian
+    with pytest.raises(psg.PsgError) as e:
+        ctx.cv_eval(x, None, None)
+    assert e.value.code == -1
+    with pytest.raises(ValueError):
+        ctx.cv_eval(x.double(), torch.zeros((2, 1), device="cuda"), None)
