@@ -57,7 +57,7 @@ class ClockSampler:
         self.p = None
         try:
             self.p = subprocess.Popen(["nvidia-smi", "-i", str(index), f"--query-gpu={self.Q}", "--format=csv,noheader,nounits",
-                                       "-lms", "50"], stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+                                       "-lms", "100"], stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
         except OSError:
             pass
 
@@ -101,6 +101,8 @@ def make_workload(cfg, K, W_):
         w = W.make(3, steps=K)
     else:
         w = W.make(4, steps=K)
+    if w.method == "metad":
+        w.params["capacity"] += w.R     # psg_deposit_hill's host-side bound counts +R for a masked (ragged) round
     return w
 
 
@@ -174,7 +176,7 @@ def run_psg(args, rank, world):
     ev0 = [torch.cuda.Event(enable_timing=True) for _ in range(K)]
     ev1 = [torch.cuda.Event(enable_timing=True) for _ in range(K)]
     launches0 = ctx.launch_count()
-    clk = ClockSampler(local) if rank == 0 else None
+    clk = ClockSampler(local) if rank == 0 and not args.no_clock_sampler else None
     barrier()
     t_wall = time.perf_counter()
     for s in range(1, K + 1):
@@ -241,7 +243,9 @@ def run_psg(args, rank, world):
                "gpu_launches": int(launches), "clocks": clocks,
                "back_to_back": {"value": units / (ms_b2b * 1e-3), "unit": UNIT, "ms_per_step": ms_b2b / K,
                                 "note": "same K steps, no L2 flush, two events around the whole loop"},
-               "wall_s_timed_region": t_wall}
+               "wall_s_timed_region": t_wall,
+               "per_step_us": {"min": float(per_step.min() * 1e3), "median": float(np.median(per_step) * 1e3),
+                               "p99": float(np.percentile(per_step, 99) * 1e3), "max": float(per_step.max() * 1e3)}}
         hbm_peak, which = _peaks()
         if w.method == "metad":
             evals = algorithmic_hill_evals(w, K)
@@ -372,6 +376,7 @@ def main():
     ap.add_argument("--cpu-budget", type=float, default=15.0)
     ap.add_argument("--ref-budget", type=float, default=60.0)
     ap.add_argument("--skip-cpu-baseline", action="store_true")
+    ap.add_argument("--no-clock-sampler", action="store_true")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3)
     rank = int(os.environ.get("RANK", 0))

@@ -76,7 +76,7 @@ typedef struct {
     long long range_begin[PSG_MAX_GROUPS]; /* range: atoms [range_begin, range_begin + range_size) of the replica's array */
     long long range_size[PSG_MAX_GROUPS];
     int axis;                            /* PSG_CV_COM_COMPONENT: 0, 1, 2 */
-    float period;                        /* 0 = not periodic; 2*pi for a dihedral */
+    double period;                       /* 0 = not periodic; 2*pi for a dihedral (binary64: the wrap must not lose bits) */
 } psg_cv_desc;
 
 /* ------------------------------------------------------------------ lifetime */

@@ -72,7 +72,7 @@ static void free_all(psg_ctx* c) {
     dfree(c->d_xi); dfree(c->d_V); dfree(c->d_dVdxi); dfree(c->d_bin); dfree(c->d_V64);
     dfree(c->d_jac); dfree(c->d_gdesc); dfree(c->d_rpart);
     dfree(c->d_kspring); dfree(c->d_centers);
-    dfree(c->md.hills); dfree(c->md.n_hills); dfree(c->md.part); dfree(c->md.ticket);
+    dfree(c->md.hills); dfree(c->md.heights); dfree(c->md.n_hills); dfree(c->md.part); dfree(c->md.ticket);
     if (c->abf.own) { dfree(c->abf.hist); dfree(c->abf.fsum); }
     c->abf.hist = nullptr; c->abf.fsum = nullptr;
     dfree(c->d_pos_stage); dfree(c->d_frc_stage); dfree(c->d_fs_stage);
@@ -129,7 +129,7 @@ int psg_set_cvs(psg_ctx* c, int n_cv, const psg_cv_desc* cvs, int n_slots, const
         if (d.type < PSG_CV_DISTANCE || d.type > PSG_CV_RGYR) return fail(c, PSG_EINVAL, "psg_set_cvs: unknown CV type");
         if (d.n_groups != kGroups[d.type]) return fail(c, PSG_EINVAL, "psg_set_cvs: wrong n_groups for this CV type");
         if (d.type == PSG_CV_COM_COMPONENT && (d.axis < 0 || d.axis > 2)) return fail(c, PSG_EINVAL, "psg_set_cvs: axis must be 0, 1 or 2");
-        if (!(d.period >= 0.f)) return fail(c, PSG_EINVAL, "psg_set_cvs: period must be >= 0");
+        if (!(d.period >= 0.0)) return fail(c, PSG_EINVAL, "psg_set_cvs: period must be >= 0");
         CvDev& C = P.cv[k];
         C.type = d.type; C.n_groups = d.n_groups; C.axis = d.axis; C.period = d.period; C.gid0 = P.n_groups;
         if (d.type == PSG_CV_RGYR) P.any_rgyr = 1;
@@ -214,17 +214,6 @@ int psg_set_harmonic(psg_ctx* c, const float* kspring, const float* centers) {
     return PSG_OK;
 }
 
-// split P into p_hi (12 low mantissa bits cleared, so k*p_hi is exact for small integers k) and p_lo
-static void split_period(double P, float* hi, float* lo) {
-    float h = (float)P;
-    uint32_t b;
-    memcpy(&b, &h, 4);
-    b &= 0xFFFFF000u;
-    memcpy(&h, &b, 4);
-    *hi = h;
-    *lo = (float)(P - (double)h);
-}
-
 int psg_set_metad(psg_ctx* c, const float* sigma, float w0, float kB_deltaT, int capacity, int stride) {
     if (!c) return PSG_EINVAL;
     if (!c->have_cvs) return fail(c, PSG_ESTATE, "psg_set_metad: call psg_set_cvs first");
@@ -235,20 +224,24 @@ int psg_set_metad(psg_ctx* c, const float* sigma, float w0, float kB_deltaT, int
     HillConsts hc;
     memset(&hc, 0, sizeof(hc));
     hc.n_cv = n_cv;
-    const double cs = sqrt(0.5 * 1.4426950408889634074);   // sqrt(log2(e)/2)
+    const double log2e = 1.4426950408889634074;
     for (int k = 0; k < n_cv; ++k) {
         if (!(sigma[k] > 0.f)) return fail(c, PSG_EINVAL, "psg_set_metad: sigma must be > 0");
-        double sg = (double)sigma[k], per = (double)c->sys.cv[k].period;
-        hc.cscale[k] = (float)(cs / sg);
-        hc.gscale[k] = 1.0 / ((double)hc.cscale[k] * sg * sg);
+        double sg = (double)sigma[k], per = c->sys.cv[k].period;
+        hc.nc[k] = (float)(-log2e / (2.0 * sg * sg));
+        hc.gscale[k] = 1.0 / (sg * sg);
         hc.inv_sigma_d[k] = 1.0 / sg;
-        hc.period_d[k] = per > 0 ? per : 1.0;
+        hc.period_d[k] = per > 0 ? per : 1e300;   // non-periodic: rint(d / 1e300) = 0, no wrap
         if (per > 0) {
             hc.pmask |= 1 << k;
             hc.inv_period[k] = (float)(1.0 / per);
-            split_period(per, &hc.p_hi[k], &hc.p_lo[k]);
+            // -P = np_hi + np_lo; |k| <= 1 for CV values inside one period, so k * np_hi is exact
+            hc.np_hi[k] = (float)(-per);
+            hc.np_lo[k] = (float)(-per - (double)hc.np_hi[k]);
         }
     }
+    hc.neq = 1;
+    while (hc.neq < n_cv && hc.nc[hc.neq] == hc.nc[0]) hc.neq++;
     M.hc = hc;
     M.w0 = (double)w0; M.kB_deltaT = (double)kB_deltaT; M.capacity = capacity; M.stride = stride;
     M.rec = n_cv <= 3 ? 1 : 2;
@@ -256,6 +249,7 @@ int psg_set_metad(psg_ctx* c, const float* sigma, float w0, float kB_deltaT, int
     int n_rt = 0;
     size_t part = psg_hill_part_doubles(c, &M.max_chunks, &n_rt);
     CK(c, dalloc(M.hills, (size_t)capacity * M.rec + 2));
+    CK(c, dalloc(M.heights, (size_t)capacity + 2));
     CK(c, dalloc(M.n_hills, 1));
     CK(c, dalloc(M.part, part));
     CK(c, dalloc(M.ticket, (size_t)n_rt));

@@ -15,11 +15,10 @@
 #define PSG_HILL_WARPS 8         // warps per CTA in the hill sum
 #define PSG_HILL_TILE_R (PSG_HILL_RT * PSG_HILL_WARPS)   // replicas per CTA tile (64)
 #define PSG_HILL_SUB 1024        // hills per shared-memory stage
-#define PSG_HILL_STAGES 3
 
 struct CvDev {
     int type, n_groups, axis, gid0;   // gid0: global id of this CV's first group
-    float period;
+    double period;
 };
 
 struct GroupDev {
@@ -49,20 +48,22 @@ struct SysParams {
 };
 
 struct HillConsts {
-    float inv_period[PSG_MAX_CV];   // 0 if not periodic
-    float p_hi[PSG_MAX_CV], p_lo[PSG_MAX_CV];
-    float cscale[PSG_MAX_CV];       // sqrt(log2(e)/2)/sigma_k : exponent = -sum (d*cscale)^2 in base 2
-    double gscale[PSG_MAX_CV];      // dV/dxi_k = -gscale_k * sum_h W e a_k
-    double period_d[PSG_MAX_CV];
+    float inv_period[PSG_MAX_CV];   // 0 if not periodic (then the wrap is the identity)
+    float np_hi[PSG_MAX_CV], np_lo[PSG_MAX_CV];   // -P as two binary32 constants (Cody-Waite)
+    float nc[PSG_MAX_CV];           // -log2(e) / (2 sigma_k^2): base-2 exponent = log2 W + sum_k nc_k d_k^2
+    double gscale[PSG_MAX_CV];      // dV/dxi_k = -gscale_k * sum_h W e d_k,  gscale_k = 1 / sigma_k^2
+    double period_d[PSG_MAX_CV];    // binary64 path; 1e300 if not periodic
     double inv_sigma_d[PSG_MAX_CV];
     int n_cv, pmask;
+    int neq;                        // number of leading CVs whose nc equals nc[0]
 };
 
 struct MetadState {
-    float4* hills;          // records: n_cv<=3: {s0,s1,s2,W}; n_cv==4: {s0..s3},{W,0,0,0}
+    float4* hills;          // kernel-side records: n_cv<=3: {s0,s1,s2,log2 W}; n_cv==4: {s0..s3},{log2 W,0,0,0}
+    float* heights;         // W as deposited / loaded (exported by psg_get_hills; read by the binary64 path)
     int* n_hills;           // device counter (exact)
     int capacity;
-    double* part;           // [max_chunks][R_padded][1+n_cv]
+    double* part;           // [max_chunks][n_rtiles][TILE_R][1+n_cv]
     unsigned* ticket;       // [n_rtiles]
     int max_chunks;
     double w0, kB_deltaT;

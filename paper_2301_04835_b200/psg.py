@@ -36,7 +36,7 @@ class _CvDesc(C.Structure):
     _fields_ = [("type", C.c_int), ("n_groups", C.c_int), ("group_is_range", C.c_int * 4),
                 ("group_begin", C.c_int * 4), ("group_size", C.c_int * 4),
                 ("range_begin", C.c_longlong * 4), ("range_size", C.c_longlong * 4),
-                ("axis", C.c_int), ("period", C.c_float)]
+                ("axis", C.c_int), ("period", C.c_double)]
 
 
 _lib = None

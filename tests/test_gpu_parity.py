@@ -14,7 +14,8 @@ import pytest
 
 import oracle as orc
 import workloads as W
-from _parity import (assert_close, fails, oracle_bias, oracle_heights, oracle_step, oracle_system, slot_rows, wrap)
+from _parity import (assert_close, assert_forces_close, fails, metad_force_extra, oracle_bias, oracle_heights, oracle_step,
+                     oracle_system, slot_rows, wrap)
 
 pytestmark = pytest.mark.gpu
 
@@ -114,7 +115,7 @@ def test_cv_zoo_weights_stride3_angle_component(torch, psg):
     ctx.sync_check()
     V, dV = orc.harmonic(xi_ref.astype(np.float32).astype(np.float64), ks, cen, np.zeros(4))
     f_ref = sysm.apply_forces(pos, dV, f0.astype(np.float64))
-    assert_close(d_f.cpu().numpy(), f_ref, "zoo forces")
+    assert_forces_close(d_f.cpu().numpy(), f_ref, f0, "zoo forces")
     out = ctx.read_step_outputs()
     assert_close(out["V"].cpu().numpy(), V, "zoo V")
 
@@ -358,10 +359,10 @@ def test_five_calls_chain_matches_oracle(torch, psg, cfg):
     ctx.apply_bias_forces(d_pos, d_dV, d_f)
     ctx.sync_check()
     xi_ref, b, f_ref = oracle_step(w, sysm, pos, f0, centers, heights, abf_state, fs)
-    _check_step(w, d_xi.cpu().numpy(), d_V.cpu().numpy(), d_dV.cpu().numpy(), d_f.cpu().numpy(), f0, xi_ref, b, f_ref)
+    _check_step(w, sysm, pos, d_xi.cpu().numpy(), d_V.cpu().numpy(), d_dV.cpu().numpy(), d_f.cpu().numpy(), f0, xi_ref, b, f_ref)
 
 
-def _check_step(w, xi, V, dV, f, f0, xi_ref, b, f_ref, what=""):
+def _check_step(w, sysm, pos, xi, V, dV, f, f0, xi_ref, b, f_ref, what=""):
     assert_close(xi, xi_ref, what + "xi", period=w.period)
     if w.method != "abf":
         assert_close(V, b["V"], what + "V")
@@ -383,13 +384,10 @@ def _check_step(w, xi, V, dV, f, f0, xi_ref, b, f_ref, what=""):
         else:
             touched[0, w.slot_atom.reshape(-1)] = True
     assert np.array_equal(f[~touched].view(np.uint32), f0[~touched].view(np.uint32)), "non-CV atoms must be untouched"
-    if w.method == "metad":
-        # forces inherit the hill-sum gradient's conditioning: compare with the oracle's forces for the GPU's own
-        # (already bounded) dV/dxi as well as the literal check on well-conditioned elements
-        bad = fails(f[..., :3], f_ref)
-        assert bad.mean() <= 0.02, f"{what}forces: literal fail fraction {bad.mean():.4f}"
-    else:
-        assert_close(f[..., :3], f_ref, what + "forces")
+    # forces inherit the hill-sum gradient's conditioning bound
+    extra = metad_force_extra(w, sysm, pos, b["T"]) if w.method == "metad" else None
+    lit = assert_forces_close(f[..., :3], f_ref, f0[..., :3], what + "forces", extra)
+    assert lit.mean() <= 0.02, f"{what}forces: literal fail fraction {lit.mean():.4f}"
 
 
 @pytest.mark.parametrize("cfg", [0, 1, 2, 3, 4])
@@ -432,7 +430,7 @@ def test_fused_step_matches_oracle_over_steps(torch, psg, cfg):
         h_now = None if heights is None else heights[:n_h]
         b = oracle_bias(w, xi_ref.astype(np.float32), c_now, h_now, abf_state, fs)
         f_ref = sysm.apply_forces(pos, b["dVdxi"], f_before[..., :3].astype(np.float64))
-        _check_step(w, out["xi"], out["V"], out["dVdxi"], d_f.cpu().numpy(), f_before, xi_ref, b, f_ref,
+        _check_step(w, sysm, pos, out["xi"], out["V"], out["dVdxi"], d_f.cpu().numpy(), f_before, xi_ref, b, f_ref,
                     what=f"config {cfg} step {step}: ")
         if w.method == "abf":
             assert np.array_equal(out["bin"], b["bin"])
