@@ -184,6 +184,7 @@ int psg_set_cvs(psg_ctx* c, int n_cv, const psg_cv_desc* cvs, int n_slots, const
         CK(c, dalloc(c->d_atom_weight, (size_t)P.N));
         CK(c, cudaMemcpy(c->d_atom_weight, atom_weight, (size_t)P.N * sizeof(float), cudaMemcpyHostToDevice));
     }
+    for (int i = 0; i < PSG_MAX_SLOTS; ++i) P.slot_atom_c[i] = (!per_rep && i < n_slots) ? slot_atom[i] : 0;
     P.slot_atom = c->d_slot_atom; P.slot_gid = c->d_slot_gid; P.slot_weight = c->d_slot_weight; P.atom_weight = c->d_atom_weight;
     // scratch
     size_t R = (size_t)P.R;
@@ -255,6 +256,7 @@ int psg_set_metad(psg_ctx* c, const float* sigma, float w0, float kB_deltaT, int
     CK(c, dalloc(M.ticket, (size_t)n_rt));
     CK(c, cudaMemset(M.n_hills, 0, sizeof(int)));
     CK(c, cudaMemset(M.ticket, 0, n_rt * sizeof(unsigned)));
+    CK(c, psg_launch_null_hills(c, 0, capacity));   // invariant: records beyond the count are null (contribute 0)
     c->nh_bound = 0;
     c->method = PSG_METHOD_METAD;
     return PSG_OK;
@@ -275,6 +277,7 @@ int psg_load_hills(psg_ctx* c, int n, const float* d_centers, const float* d_hei
     if (n > c->md.capacity) return fail(c, PSG_ECAPACITY, "psg_load_hills: more hills than capacity");
     cudaSetDevice(c->device);
     CK(c, psg_launch_pack_hills(c, n, d_centers, d_heights));
+    if (c->nh_bound > n) CK(c, psg_launch_null_hills(c, n, (int)c->nh_bound));
     CK(c, cudaMemcpyAsync(c->md.n_hills, &n, sizeof(int), cudaMemcpyHostToDevice, c->stream));
     CK(c, cudaStreamSynchronize(c->stream));   // n is a stack variable
     c->nh_bound = n;

@@ -82,6 +82,19 @@ __global__ void k_unpack_hills(int n, int n_cv, int rec, const float4* __restric
     heights[h] = heights_in[h];
 }
 
+// null records: centre 0, log2 W = -inf, W = 0: ex2(-inf) = 0, so they add exactly 0 to V and to the gradient
+__global__ void k_null_hills(int begin, int end, int rec, float4* __restrict__ hills, float* __restrict__ heights) {
+    int h = begin + blockIdx.x * blockDim.x + threadIdx.x;
+    if (h >= end) return;
+    const float ninf = __int_as_float(0xff800000);
+    heights[h] = 0.f;
+    if (rec == 1) hills[h] = make_float4(0.f, 0.f, 0.f, ninf);
+    else {
+        hills[2 * h] = make_float4(0.f, 0.f, 0.f, 0.f);
+        hills[2 * h + 1] = make_float4(ninf, 0.f, 0.f, 0.f);
+    }
+}
+
 // ---------------------------------------------------------------- host side
 static int hills_grid(const psg_ctx* c) { return c->sm_count * 2; }
 
@@ -119,7 +132,20 @@ static HillKernelArgs base_args(psg_ctx* c) {
     HillKernelArgs A{};
     A.hills = c->md.hills; A.heights = c->md.heights; A.n_hills = c->md.n_hills; A.part = c->md.part; A.ticket = c->md.ticket;
     A.R = c->sys.R;
+    // The host's upper bound of the hill count saves the kernel a dependent global load. Under stream capture the
+    // launch may be replayed with a longer list than the one seen now, so the kernel reads the device counter.
+    cudaStreamCaptureStatus st = cudaStreamCaptureStatusNone;
+    if (cudaStreamIsCapturing(c->stream, &st) != cudaSuccess) { st = cudaStreamCaptureStatusNone; (void)cudaGetLastError(); }
+    A.n_h_host = st == cudaStreamCaptureStatusNone ? (int)c->nh_bound : -1;
     return A;
+}
+
+cudaError_t psg_launch_null_hills(psg_ctx* c, int begin, int end) {
+    if (end > begin) {
+        k_null_hills<<<(end - begin + 255) / 256, 256, 0, c->stream>>>(begin, end, c->md.rec, c->md.hills, c->md.heights);
+        c->launches++;
+    }
+    return cudaGetLastError();
 }
 
 cudaError_t psg_launch_hillsum(psg_ctx* c, const float* d_xi, float* d_V, float* d_dVdxi) {

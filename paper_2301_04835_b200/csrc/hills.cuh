@@ -223,12 +223,13 @@ __device__ __forceinline__ double thread_cv(const SysParams& P, int r, int k, co
         if (g < C.n_groups) {
             const GroupDev& G = P.grp[C.gid0 + g];
             if (G.size == 1 && !P.slot_weight) {
-                c[g] = load_pos(p, sa[G.begin], P.ps);   // a single unweighted atom is its own barycenter
+                // a single unweighted atom is its own barycenter; shared index lists come from kernel parameters
+                c[g] = load_pos(p, P.per_rep ? sa[G.begin] : P.slot_atom_c[G.begin], P.ps);
             } else {
                 double sx = 0, sy = 0, sz = 0, sw = 0;
                 for (int i = 0; i < G.size; ++i) {
                     int s = G.begin + i;
-                    D3 x = load_pos(p, sa[s], P.ps);
+                    D3 x = load_pos(p, P.per_rep ? sa[s] : P.slot_atom_c[s], P.ps);
                     double w = P.slot_weight ? (double)P.slot_weight[s] : 1.0;
                     sx += w * x.x; sy += w * x.y; sz += w * x.z; sw += w;
                 }
@@ -248,7 +249,8 @@ __device__ __forceinline__ double thread_cv(const SysParams& P, int r, int k, co
 struct HillKernelArgs {
     const float4* hills;     // packed records {s0, s1, s2, log2 W} (n_cv == 4: two float4)
     const float* heights;    // W, as exported
-    const int* n_hills;
+    const int* n_hills;      // device counter (exact), read only when n_h_host < 0 (stream capture)
+    int n_h_host;            // host upper bound of the count; records beyond the exact count are null (contribute 0)
     double* part;
     unsigned* ticket;
     const float* xi_in;      // not fused: [R][n_cv]
@@ -294,7 +296,7 @@ __global__ void __launch_bounds__(HWARPS * 32, 2) k_hills(const __grid_constant_
     const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
     const int R = A.R;
     const int n_rt = (R + TILE_R - 1) / TILE_R;
-    const int n_h = *A.n_hills;
+    const int n_h = A.n_h_host >= 0 ? A.n_h_host : *A.n_hills;
     // chunking: as many chunks per tile as the grid allows, chunk length a multiple of 32
     int cpt = (int)gridDim.x / n_rt;
     if (cpt < 1) cpt = 1;
@@ -309,7 +311,8 @@ __global__ void __launch_bounds__(HWARPS * 32, 2) k_hills(const __grid_constant_
         for (int s = 0; s < STG; ++s) mbar_init(&full[s], 1);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
-    __syncthreads();
+    // no CTA-wide sync here: thread 0 issues the first TMA loads itself; everybody else first meets the barriers
+    // after the __syncthreads that follows the CV prologue
     unsigned seq = 0;   // sub-tiles consumed so far by this CTA (stage = seq % STG, parity = (seq / STG) & 1)
 
     for (int item = blockIdx.x; item < items; item += gridDim.x) {
@@ -373,9 +376,9 @@ __global__ void __launch_bounds__(HWARPS * 32, 2) k_hills(const __grid_constant_
                 int s = seq % STG;
                 mbar_wait(&full[s], (seq / STG) & 1);
                 int cnt = min(SUB, len - t * SUB);
-                if (warp_active) {
-                    accumulate_f32<NCV, PM, NEQ>(stage + s * SUB * REC, cnt, lane, X, hc, a32);
-                    // flush the binary32 partial sums (<= 32 hills per lane) into the binary64 slots
+                if (warp_active) accumulate_f32<NCV, PM, NEQ>(stage + s * SUB * REC, cnt, lane, X, hc, a32);
+                if (warp_active && ((t & 1) || t == n_st - 1)) {
+                    // flush the binary32 partial sums (<= 64 hills per lane) into the binary64 slots
 #pragma unroll
                     for (int p = 0; p < RT / 2; ++p)
 #pragma unroll
@@ -429,15 +432,15 @@ __global__ void __launch_bounds__(HWARPS * 32, 2) k_hills(const __grid_constant_
             for (int i = 0; i < 32; ++i) sum += src[(i + lane) & 31];
             dst[v] = sum;
         }
-        __threadfence();
         __syncthreads();
         if (tid == 0) {
-            unsigned old = atomicAdd(&A.ticket[tile], 1u);
+            // release: the CTA's partials (ordered before this by the barrier) are visible to whoever acquires the ticket
+            unsigned old;
+            asm volatile("atom.acq_rel.gpu.global.add.u32 %0, [%1], 1;" : "=r"(old) : "l"(A.ticket + tile) : "memory");
             s_last = (old == (unsigned)(n_chunks - 1));
         }
         __syncthreads();
         if (s_last) {   // block-uniform: this CTA finishes the tile
-            __threadfence();
             for (int t = tid; t < TILE_R * NV; t += NT) {
                 const double* src = A.part + ((size_t)tile * TILE_R) * NV + t;
                 const size_t cstride = (size_t)n_rt * TILE_R * NV;

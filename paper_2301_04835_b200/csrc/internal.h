@@ -41,6 +41,7 @@ struct SysParams {
     int range_gid[PSG_MAX_RANGE_GROUPS];     // range id -> global group id
     long long span_begin, span_end;          // union span of all range groups
     int range_blocks;                        // blocks per replica over the span
+    int slot_atom_c[PSG_MAX_SLOTS];          // shared index list (per_rep == 0): read from kernel parameters
     const int* slot_atom;        // device [n_slots] or [R][n_slots]
     const int* slot_gid;         // device [n_slots]: global group id of a slot
     const float* slot_weight;    // device [n_slots] or nullptr
@@ -117,6 +118,7 @@ cudaError_t psg_launch_hillsum(psg_ctx* c, const float* d_xi, float* d_V, float*
 cudaError_t psg_launch_deposit(psg_ctx* c, const float* d_xi, const unsigned char* d_mask);
 cudaError_t psg_launch_pack_hills(psg_ctx* c, int n, const float* d_centers, const float* d_heights);
 cudaError_t psg_launch_unpack_hills(psg_ctx* c, int n, float* d_centers, float* d_heights);
+cudaError_t psg_launch_null_hills(psg_ctx* c, int begin, int end);   // records [begin, end) := null
 cudaError_t psg_launch_abf(psg_ctx* c, const float* d_xi, const float* d_fsample, int* d_bin, float* d_dVdxi);
 cudaError_t psg_launch_metad_step(psg_ctx* c, const float* d_pos, float* d_force);   // fused; n_ranges == 0
 bool psg_metad_step_supported(const psg_ctx* c);

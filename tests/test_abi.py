@@ -43,9 +43,9 @@ def test_library_is_sm100a_and_uses_tma_bulk_copies():
     so = build.build()
     out = subprocess.run(["cuobjdump", "-lelf", so], capture_output=True, text=True).stdout
     assert "sm_100a" in out
-    sass = subprocess.run(["cuobjdump", "-sass", "-fun", "_Z7k_hillsILi2ELi3ELb0ELb1EEv9SysParams10HillConsts14HillKernelArgs", so],
+    sass = subprocess.run(["cuobjdump", "-sass", "-fun", "_Z7k_hillsILi2ELi3ELi2ELb0EEv9SysParams10HillConsts14HillKernelArgs", so],
                           capture_output=True, text=True).stdout
-    assert "UBLKCP" in sass and "MUFU.EX2" in sass and "SYNCS" in sass
+    assert "UBLKCP" in sass and "MUFU.EX2" in sass and "SYNCS" in sass and "FFMA2" in sass
 
 
 def test_no_cpu_fallback(lib):
