@@ -3,6 +3,7 @@
 #include <math.h>
 #include <string.h>
 
+#include <algorithm>
 #include <new>
 #include <vector>
 
@@ -70,7 +71,7 @@ int psg_create(psg_ctx** out, int device, void* cuda_stream) {
 static void free_all(psg_ctx* c) {
     dfree(c->d_slot_atom); dfree(c->d_slot_gid); dfree(c->d_slot_weight); dfree(c->d_atom_weight);
     dfree(c->d_xi); dfree(c->d_V); dfree(c->d_dVdxi); dfree(c->d_bin); dfree(c->d_V64);
-    dfree(c->d_jac); dfree(c->d_gdesc); dfree(c->d_rpart);
+    dfree(c->d_jac); dfree(c->d_gdesc); dfree(c->d_rpart); dfree(c->d_arrive); dfree(c->d_rdesc);
     dfree(c->d_kspring); dfree(c->d_centers);
     dfree(c->md.hills); dfree(c->md.heights); dfree(c->md.n_hills); dfree(c->md.part); dfree(c->md.ticket);
     if (c->abf.own) { dfree(c->abf.hist); dfree(c->abf.fsum); }
@@ -193,6 +194,10 @@ int psg_set_cvs(psg_ctx* c, int n_cv, const psg_cv_desc* cvs, int n_slots, const
     CK(c, dalloc(c->d_jac, R * (size_t)n_slots * 3));
     CK(c, dalloc(c->d_gdesc, R * P.n_groups * PSG_GDESC_DOUBLES));
     CK(c, dalloc(c->d_rpart, R * P.n_ranges * (size_t)P.range_blocks * PSG_MOM));
+    CK(c, dalloc(c->d_arrive, 2 * R));
+    CK(c, cudaMemset(c->d_arrive, 0, 2 * R * sizeof(unsigned)));
+    CK(c, dalloc(c->d_rdesc, R * P.n_ranges * 4));
+    CK(c, cudaMemset(c->d_rdesc, 0, std::max<size_t>(R * P.n_ranges * 4, 1) * sizeof(float4)));
     CK(c, cudaMemset(c->d_V, 0, R * sizeof(float)));
     CK(c, cudaMemset(c->d_bin, 0xff, R * sizeof(int)));
     c->sys = P;
@@ -413,6 +418,11 @@ int psg_step(psg_ctx* c, const float* d_pos, float* d_force, const float* d_fsam
         CK(c, psg_launch_cv_eval(c, d_pos, c->d_xi, nullptr));
         CK(c, psg_launch_hillsum(c, c->d_xi, c->d_V, c->d_dVdxi));
     } else if (c->method == PSG_METHOD_HARMONIC) {
+        if (psg_range_step_supported(c, d_pos, d_force)) {
+            CK(c, psg_launch_range_step(c, d_pos, d_force));   // large contiguous groups: one persistent launch
+            c->have_jac = false;
+            return PSG_OK;
+        }
         CK(c, psg_launch_cv_eval(c, d_pos, c->d_xi, nullptr));
         CK(c, psg_launch_harmonic(c, c->d_xi, c->d_V, c->d_dVdxi));
     } else {

@@ -96,6 +96,16 @@ __global__ void k_null_hills(int begin, int end, int rec, float4* __restrict__ h
 }
 
 // ---------------------------------------------------------------- host side
+#ifdef PSG_TRACE
+static long long* g_trace = nullptr;
+long long* psg_trace_buffer() {
+    if (!g_trace) { cudaMalloc(&g_trace, 4096 * 8 * sizeof(long long)); cudaMemset(g_trace, 0, 4096 * 8 * sizeof(long long)); }
+    return g_trace;
+}
+extern "C" int psg_debug_trace(long long* host_out, int n_ctas) {
+    return (int)cudaMemcpy(host_out, psg_trace_buffer(), (size_t)n_ctas * 8 * sizeof(long long), cudaMemcpyDeviceToHost);
+}
+#endif
 static int hills_grid(const psg_ctx* c) { return c->sm_count * 2; }
 
 size_t psg_hill_part_doubles(const psg_ctx* c, int* max_chunks_out, int* n_rtiles_out) {
@@ -137,6 +147,9 @@ static HillKernelArgs base_args(psg_ctx* c) {
     cudaStreamCaptureStatus st = cudaStreamCaptureStatusNone;
     if (cudaStreamIsCapturing(c->stream, &st) != cudaSuccess) { st = cudaStreamCaptureStatusNone; (void)cudaGetLastError(); }
     A.n_h_host = st == cudaStreamCaptureStatusNone ? (int)c->nh_bound : -1;
+#ifdef PSG_TRACE
+    A.trace = psg_trace_buffer();
+#endif
     return A;
 }
 

@@ -263,7 +263,15 @@ struct HillKernelArgs {
     int R;
     int fused;
     int stages;              // shared-memory stages of SUB hills
+#ifdef PSG_TRACE
+    long long* trace;        // [grid][8] clock64 stamps of the first item of every CTA (debug builds only)
+#endif
 };
+#ifdef PSG_TRACE
+#define PSG_STAMP(i) do { if (threadIdx.x == 0 && item == (int)blockIdx.x && A.trace) A.trace[blockIdx.x * 8 + (i)] = clock64(); } while (0)
+#else
+#define PSG_STAMP(i) do { } while (0)
+#endif
 
 __host__ __device__ inline size_t hills_smem_bytes(int n_cv, int stages, int n_groups, bool fused) {
     int rec = n_cv <= 3 ? 1 : 2;
@@ -323,6 +331,7 @@ __global__ void __launch_bounds__(HWARPS * 32, 2) k_hills(const __grid_constant_
         if (len > Lc) len = Lc;
         if (len < 0) len = 0;
         const int n_st = (len + SUB - 1) / SUB;
+        PSG_STAMP(0);
         // producer prologue
         if (tid == 0) {
             for (int t = 0; t < n_st && t < STG; ++t) {
@@ -361,6 +370,7 @@ __global__ void __launch_bounds__(HWARPS * 32, 2) k_hills(const __grid_constant_
             }
         }
         __syncthreads();
+        PSG_STAMP(1);
         const bool warp_active = r0 + wid * RT < R;
         if (!F64) {
             u64 X[RT / 2][NCV], a32[RT / 2][NV];
@@ -421,6 +431,7 @@ __global__ void __launch_bounds__(HWARPS * 32, 2) k_hills(const __grid_constant_
                 ++seq;
             }
         }
+        PSG_STAMP(2);
         // lanes -> warp totals through the shared accumulators: lane v (< RT*NV) sums value v over the 32 lanes
         // (rotated start => no bank conflicts; the order is fixed per lane => deterministic)
         __syncwarp();
@@ -433,6 +444,7 @@ __global__ void __launch_bounds__(HWARPS * 32, 2) k_hills(const __grid_constant_
             dst[v] = sum;
         }
         __syncthreads();
+        PSG_STAMP(3);
         if (tid == 0) {
             // release: the CTA's partials (ordered before this by the barrier) are visible to whoever acquires the ticket
             unsigned old;
@@ -440,6 +452,7 @@ __global__ void __launch_bounds__(HWARPS * 32, 2) k_hills(const __grid_constant_
             s_last = (old == (unsigned)(n_chunks - 1));
         }
         __syncthreads();
+        PSG_STAMP(4);
         if (s_last) {   // block-uniform: this CTA finishes the tile
             for (int t = tid; t < TILE_R * NV; t += NT) {
                 const double* src = A.part + ((size_t)tile * TILE_R) * NV + t;
@@ -463,6 +476,7 @@ __global__ void __launch_bounds__(HWARPS * 32, 2) k_hills(const __grid_constant_
             if (tid == 0) A.ticket[tile] = 0u;   // ready for the next launch
             if (A.fused) {
                 __syncthreads();
+                PSG_STAMP(5);
                 // forces: one thread per (replica, slot); red.global.add (atoms shared by CVs / walkers collide)
                 for (int t = tid; t < TILE_R * P.n_slots; t += NT) {
                     int rr = t / P.n_slots, s = t % P.n_slots, r = r0 + rr;
@@ -481,5 +495,12 @@ __global__ void __launch_bounds__(HWARPS * 32, 2) k_hills(const __grid_constant_
             }
         }
         __syncthreads();   // s_xi / s_out / s_acc / s_last are reused by the next item
+        PSG_STAMP(6);
+#ifdef PSG_TRACE
+        if (threadIdx.x == 0 && item == (int)blockIdx.x && A.trace) {
+            unsigned smid; asm volatile("mov.u32 %0, %%smid;" : "=r"(smid));
+            A.trace[blockIdx.x * 8 + 7] = smid;
+        }
+#endif
     }
 }

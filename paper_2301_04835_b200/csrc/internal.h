@@ -10,7 +10,7 @@
 #define PSG_MAX_GROUPS_TOTAL (PSG_MAX_CV * PSG_MAX_GROUPS)
 #define PSG_GDESC_DOUBLES 8      // per (replica, group): vx vy vz | cx cy cz | coef | W
 #define PSG_MOM 5                // moments per range group: W, sum w x, sum w y, sum w z, sum w |r|^2
-#define PSG_RANGE_TILE 2048      // atoms per block in the range-moment / dense-apply kernels
+#define PSG_RANGE_TILE 2048      // atoms per block / slice in the range-moment, dense-apply and fused range-step kernels
 #define PSG_HILL_RT 8            // replicas per thread in the hill sum
 #define PSG_HILL_WARPS 8         // warps per CTA in the hill sum
 #define PSG_HILL_TILE_R (PSG_HILL_RT * PSG_HILL_WARPS)   // replicas per CTA tile (64)
@@ -100,6 +100,8 @@ struct psg_ctx {
     float* d_jac = nullptr;          // [R][n_slots][3]
     double* d_gdesc = nullptr;       // [R][n_groups][PSG_GDESC_DOUBLES]
     double* d_rpart = nullptr;       // [R][n_ranges][range_blocks][PSG_MOM]
+    unsigned* d_arrive = nullptr;    // [2][R]: arrive / done counters of the fused range step (zero between launches)
+    float4* d_rdesc = nullptr;       // [R][n_ranges][4]: tagged force descriptors of the fused range step (zero between launches)
     // harmonic
     float* d_kspring = nullptr; float* d_centers = nullptr;
     MetadState md{};
@@ -122,4 +124,10 @@ cudaError_t psg_launch_null_hills(psg_ctx* c, int begin, int end);   // records 
 cudaError_t psg_launch_abf(psg_ctx* c, const float* d_xi, const float* d_fsample, int* d_bin, float* d_dVdxi);
 cudaError_t psg_launch_metad_step(psg_ctx* c, const float* d_pos, float* d_force);   // fused; n_ranges == 0
 bool psg_metad_step_supported(const psg_ctx* c);
+bool psg_range_step_supported(const psg_ctx* c, const float* d_pos, const float* d_force);
+cudaError_t psg_launch_range_step(psg_ctx* c, const float* d_pos, float* d_force);   // fused harmonic step over range groups
 size_t psg_hill_part_doubles(const psg_ctx* c, int* max_chunks_out, int* n_rtiles_out);
+
+#ifdef PSG_TRACE
+long long* psg_trace_buffer();   // debug builds: [4096][8] clock64 stamps
+#endif

@@ -472,6 +472,62 @@ def test_fused_step_equals_unfused_calls_bitwise(torch, psg):
     assert np.allclose(outs[0][3], outs[1][3], rtol=3e-7, atol=1e-9)
 
 
+@pytest.mark.parametrize("R,N,weighted", [(3, 5003, False), (2, 2048, False), (5, 6161, True), (1, 100, False), (40, 33000, False)])
+def test_fused_range_step_equals_unfused_calls_bitwise(torch, psg, R, N, weighted):
+    """config 3 (umbrella windows over large contiguous groups): the one-launch persistent step (TMA-staged slices,
+    inter-CTA window reduction) and the separate calls use the same arithmetic in the same order -> same bits;
+    several steps in a row check that the window counters re-arm"""
+    w = W.make(3, R=R, N=N, steps=3, weighted=weighted)
+    f0 = w.forces0()
+    res = []
+    for fused in (True, False):
+        ctx = make_ctx(psg, w)
+        d_f = dev(torch, f0)
+        launches = []
+        for step in (1, 2, 3):
+            d_pos = dev(torch, w.positions(step % w.K))
+            n0 = ctx.launch_count()
+            if fused:
+                ctx.step(d_pos, d_f, None, step)
+                o = ctx.read_step_outputs()
+                xi, V, dV = o["xi"], o["V"], o["dVdxi"]
+            else:
+                xi, V, dV = (torch.empty((w.R, 2), device="cuda"), torch.empty(w.R, device="cuda"),
+                             torch.empty((w.R, 2), device="cuda"))
+                ctx.cv_eval(d_pos, xi, None)
+                ctx.bias_eval(xi, V, dV)
+                ctx.apply_bias_forces(d_pos, dV, d_f)
+            launches.append(ctx.launch_count() - n0)
+        ctx.sync_check()
+        res.append([t.cpu().numpy() for t in (xi, V, dV, d_f)])
+        if fused:
+            assert launches == [1, 1, 1], f"the umbrella step must be ONE launch, got {launches}"
+    for name, a, b in zip(("xi", "V", "dVdxi", "force"), res[0], res[1]):
+        assert np.array_equal(a.view(np.uint32), b.view(np.uint32)), f"{name}: fused and unfused bits differ"
+
+
+def test_fused_range_step_is_cuda_graph_capturable(torch, psg):
+    w = W.make(3, R=4, N=9000, steps=2)
+    s = torch.cuda.Stream()
+    ctx = psg.Context(0, s)
+    psg.configure_from_workload(ctx, w)
+    d_pos = dev(torch, w.positions(0))
+    d_f = torch.zeros((w.R, w.N, 4), device="cuda")
+    ref = torch.zeros_like(d_f)
+    with torch.cuda.stream(s):
+        ctx.step(d_pos, ref, None, 1)
+        ctx.step(d_pos, ref, None, 2)
+    s.synchronize()
+    g = torch.cuda.CUDAGraph()
+    with torch.cuda.graph(g, stream=s):
+        ctx.step(d_pos, d_f, None, 1)
+        ctx.step(d_pos, d_f, None, 2)
+    d_f.zero_()
+    g.replay()
+    torch.cuda.synchronize()
+    assert np.array_equal(d_f.cpu().numpy(), ref.cpu().numpy())
+
+
 def test_internal_cv_forces_have_no_net_force_or_torque(torch, psg):
     """sum_i F_i = 0 and sum_i r_i x F_i = 0 for internal CVs (BASELINE.json), on the GPU forces themselves"""
     w = small(1, stride=0)
