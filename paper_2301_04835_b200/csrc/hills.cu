@@ -102,6 +102,7 @@ long long* psg_trace_buffer() {
     if (!g_trace) { cudaMalloc(&g_trace, 4096 * 8 * sizeof(long long)); cudaMemset(g_trace, 0, 4096 * 8 * sizeof(long long)); }
     return g_trace;
 }
+extern "C" int psg_debug_trace_clear() { return (int)cudaMemset(psg_trace_buffer(), 0, 4096 * 8 * sizeof(long long)); }
 extern "C" int psg_debug_trace(long long* host_out, int n_ctas) {
     return (int)cudaMemcpy(host_out, psg_trace_buffer(), (size_t)n_ctas * 8 * sizeof(long long), cudaMemcpyDeviceToHost);
 }

@@ -2,37 +2,41 @@
 // A1, A3a, A3b, A4, A8, A9; the paper's measured instance of this path is a COM-distance CV over 1,600-bead
 // groups with a harmonic bias).  ONE persistent, warp-specialised launch per MD step;
 // one CTA per SM; item = (window r, slice s of RS_SLICE atoms); CTA b owns items b, b + grid, b + 2 grid, ...
+// Every byte of the two big arrays enters the SM by 1-D TMA bulk copies (cp.async.bulk + mbarrier, SASS UBLKCP).
 //
-//   producer warp : positions of the CTA's next items -> a ring of RS_STAGES shared-memory stages, one 1-D TMA
-//                   bulk copy per slice (cp.async.bulk + mbarrier, SASS UBLKCP), up to RS_STAGES - 1 items ahead.
-//   A group (8 warps): weighted moments {W, sum w r, sum w |r|^2} of every range group over the slice, binary64,
-//                   reduced in fixed order -> rpart; one acq_rel ticket per item.  Whoever takes the LAST ticket
-//                   of a window hands the window to its CTA's window warp and moves on.
-//   window warp   : combines the window's partials in fixed order, evaluates the CVs (center-of-mass distance /
-//                   angle / dihedral / component, radius of gyration) and the harmonic bias in binary64, and
-//                   publishes per-group force descriptors (16-byte records carrying a valid tag).
-//   B groups (2 x 8 warps, alternating items): wait for the window's descriptors, then
-//                   F_i += -dV/dxi_k * w_i (v_g + coef_g (r_i - c_g))  with r_i from the stage STILL RESIDENT in
-//                   shared memory and the force streamed through registers (ld.global.cs / st.global.cs float4);
-//                   then the stage is handed back to the producer.
-//   Positions cross HBM once, forces are read once and written once = 48 B/atom, the algorithmic minimum.  The
-//   three roles are decoupled by the stage ring, so the inter-CTA dependency (B needs every A of its window) is
-//   absorbed by the A group running several items ahead of the B groups.
-// A never waits on another CTA, so the wait in B cannot deadlock as long as the grid is co-resident and a window
-// has at most `grid` slices: the kernel is launched cooperatively (the launch fails instead of hanging).
-// Results are bitwise reproducible and equal to the unfused calls: fixed thread -> atom map, fixed reduction
-// order, one writer per atom.
+//   PA warp  : positions of the next items -> ring A (L2 policy evict_last), throttled to stay at most `lag`
+//              items ahead of the B group, so the slices it brought in are still in L2 when B wants them.
+//   A group  (8 warps): weighted moments {W, sum w r, sum w |r|^2} of every range group over the slice, binary64,
+//              per-warp partials -> a small shared-memory ring; the stage goes straight back to PA.
+//   T warps  (2, alternating items): sum the 8 warp partials in fixed order -> rpart (global); one release
+//              ticket per item on the window's counter.
+//   W warp   : owns the windows r = b, b + grid, ... (an even share, whoever finishes them): waits until a window
+//              has all its tickets (acquire), combines its partials in fixed order, evaluates the CVs (center-of-mass distance / angle /
+//              dihedral / component, radius of gyration) and the harmonic bias in binary64, publishes per-group
+//              force descriptors (16-byte records carrying a valid tag).
+//   PB warp  : positions (now an L2 hit) and forces of the B group's next items -> ring B.
+//   B group  (8 warps): waits for the window's descriptors, then
+//              F_i += -dV/dxi_k * w_i (v_g + coef_g (r_i - c_g))  out of shared memory, st.global.cs float4.
+//   HBM traffic: positions once (the second read is served by L2 while `lag` x grid x 32 KB fits), forces read
+//   once and written once = 48 B/atom, the algorithmic minimum; 64 B/atom if L2 keeps nothing.
+// The window dependency (B needs every A of its window, from ~49 other CTAs, plus the window warp's work) is a
+// chain of several L2 round trips; it is absorbed by B simply running `lag` items behind A -- no shared-memory
+// stage is held across it.  A, T and W never wait on another CTA, so the wait in B cannot deadlock as long as the
+// grid is co-resident and a window has at most `grid` slices: the kernel is launched cooperatively (the launch
+// fails instead of hanging).  Results are bitwise reproducible and equal to the unfused calls: fixed
+// thread -> atom map, fixed reduction order, one writer per atom.
 #include <stdlib.h>
 
 #include "geom.cuh"
 
-#define RS_SLICE PSG_RANGE_TILE   // atoms per slice (2048): 32 KB of float4 positions per stage
-#define RS_STAGES 6
-#define RS_GT 256                 // threads of the A group and of each B group
-#define RS_NB 2                   // B groups
-#define RS_LEAD 64                 // producer warp + window warp
-#define RS_THREADS (RS_LEAD + RS_GT * (1 + RS_NB))
-#define RS_WQ 8                    // ring of windows handed from the A group to the window warp
+#define RS_SLICE PSG_RANGE_TILE   // atoms per slice (2048): 32 KB of float4 per array and stage
+#define RS_ASTAGES 2              // ring A: positions
+#define RS_BSTAGES 2              // ring B: positions + forces
+#define RS_RED 4                  // ring of per-warp partial moments between the A group and the T warps
+#define RS_NT 2                   // T warps
+#define RS_GT 256                 // threads of the A group and of the B group
+#define RS_LEAD (32 * (3 + RS_NT))   // PA, PB, W, T warps
+#define RS_THREADS (RS_LEAD + 2 * RS_GT)
 #define RS_PER (RS_SLICE / RS_GT)
 #define RS_DESC 4                 // float4 records per (window, range group): {v, tag} {c_hi, tag} {c_lo, tag} {k, 0, 0, tag}
 #define RS_TAG 1.0f
@@ -47,9 +51,10 @@ struct RangeStepArgs {
     double* V64_out;        // [R]
     float* dV_out;          // [R][n_cv]
     double* rpart;          // [R][n_ranges][n_slices][PSG_MOM]
-    unsigned* arrive;       // [R]  tickets of phase A
-    unsigned* done;         // [R]  finished phase B
+    unsigned* arrive;       // [R]  tickets
+    unsigned* done;         // [R]  slices whose forces are written
     float4* desc;           // [R][n_ranges][RS_DESC]
+    int lag;                // items PA may run ahead of the B group
 #ifdef PSG_TRACE
     long long* trace;
 #endif
@@ -65,9 +70,20 @@ __device__ __forceinline__ void rs_mbar_expect_tx(uint64_t* bar, uint32_t bytes)
 __device__ __forceinline__ void rs_mbar_arrive(uint64_t* bar) {
     asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(rs_smem_u32(bar)) : "memory");
 }
-__device__ __forceinline__ void rs_tma_load_1d(void* dst, const void* src, uint32_t bytes, uint64_t* bar) {
-    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(rs_smem_u32(dst)),
-                 "l"(src), "r"(bytes), "r"(rs_smem_u32(bar))
+__device__ __forceinline__ uint64_t rs_policy_evict_last() {
+    uint64_t p;
+    asm volatile("createpolicy.fractional.L2::evict_last.b64 %0, 1.0;" : "=l"(p));
+    return p;
+}
+__device__ __forceinline__ uint64_t rs_policy_evict_first() {
+    uint64_t p;
+    asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(p));
+    return p;
+}
+__device__ __forceinline__ void rs_tma_load_1d(void* dst, const void* src, uint32_t bytes, uint64_t* bar, uint64_t policy) {
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes.L2::cache_hint [%0], [%1], %2, [%3], %4;" ::"r"(
+                     rs_smem_u32(dst)),
+                 "l"(src), "r"(bytes), "r"(rs_smem_u32(bar)), "l"(policy)
                  : "memory");
 }
 __device__ __forceinline__ void rs_mbar_wait(uint64_t* bar, uint32_t parity) {
@@ -90,18 +106,31 @@ __device__ __forceinline__ float4 rs_ld_relaxed_f4(const float4* p) {   // one 1
     return v;
 }
 
+#ifdef PSG_TRACE
+// debug builds: cycles each role spends waiting, summed over the launch, [grid][16] (lane 0 / thread 0 of the role)
+#define RS_T0 long long rs_t0_ = clock64()
+#define RS_ACC(slot) do { rs_acc_[slot] += clock64() - rs_t0_; } while (0)
+#define RS_DECL long long rs_acc_[3] = {0, 0, 0}; const long long rs_start_ = clock64()
+#define RS_FLUSH(cond, base) do { if ((cond) && A.trace) { for (int z_ = 0; z_ < 3; ++z_) A.trace[blockIdx.x * 32 + (base) + z_] = rs_acc_[z_]; A.trace[blockIdx.x * 32 + (base) + 3] = clock64() - rs_start_; } } while (0)
+#else
+#define RS_T0 do { } while (0)
+#define RS_ACC(slot) do { } while (0)
+#define RS_DECL do { } while (0)
+#define RS_FLUSH(cond, base) do { } while (0)
+#endif
+
 struct RsShared {
-    double red[2][RS_GT / 32][PSG_MAX_RANGE_GROUPS][PSG_MOM];    // A: per-warp partial moments, double-buffered by item parity
-    double mom[PSG_MAX_RANGE_GROUPS][PSG_MOM];                    // window warp: moments
-    double cen[PSG_MAX_RANGE_GROUPS][4];                          // window warp: centre, W per range group
+    double red[RS_RED][RS_GT / 32][PSG_MAX_RANGE_GROUPS][PSG_MOM];   // A group -> T warps: per-warp partial moments
+    double mom[PSG_MAX_RANGE_GROUPS][PSG_MOM];                    // W warp: the window's moments
+    double cen[PSG_MAX_RANGE_GROUPS][4];                          // W warp: centre, W per range group
     double gv[PSG_MAX_RANGE_GROUPS][3], gcoef[PSG_MAX_RANGE_GROUPS];   // d xi / d c_g / W_g,  Rg: 1/(W Rg)
     double dv[PSG_MAX_CV];                                        // -(dV/dxi_k), through binary32 like the unfused path
     double vk[PSG_MAX_CV];                                        // 1/2 k_k D_k^2
-    float4 desc[RS_NB][PSG_MAX_RANGE_GROUPS][RS_DESC];            // B groups: the window's force descriptors
-    uint64_t full[RS_STAGES], empty[RS_STAGES];
-    int wq[RS_WQ];                    // windows waiting for the window warp
-    volatile int wq_head, wq_tail;    // written by A's warp 0 / by the window warp
-    volatile int a_done;              // the A group has processed its last item
+    float4 desc[PSG_MAX_RANGE_GROUPS][RS_DESC];                   // B group: the window's force descriptors
+    int blo[PSG_MAX_RANGE_GROUPS], bhi[PSG_MAX_RANGE_GROUPS];     // B group: slice-local atom bounds of every group
+    uint64_t a_full[RS_ASTAGES], a_empty[RS_ASTAGES], b_full[RS_BSTAGES], b_empty[RS_BSTAGES];
+    uint64_t red_full[RS_RED], red_empty[RS_RED];
+    volatile long long b_prog;                  // items the B group has finished
 };
 
 struct RsItem {
@@ -121,23 +150,43 @@ __device__ __forceinline__ RsItem rs_item(const SysParams& P, long long it, long
     return I;
 }
 
-// Window-level work, done ONCE per window by warp 0 of the A group of the CTA that took its last ticket: combine
-// partials, CVs, harmonic bias, outputs, and the per-group force descriptors published for every CTA of the window.
+// Window-level work, done ONCE per window by the W warp of the CTA that took its last ticket: combine partials,
+// CVs, harmonic bias, outputs, and the per-group force descriptors published for every CTA of the window.
 __device__ __forceinline__ void rs_window(const SysParams& P, const RangeStepArgs& A, RsShared& S, int r, int lane) {
     const int n_slices = P.range_blocks;
-    // fixed-order combination per value: lanes stride the slices (increasing), then an xor tree
-    for (int q = 0; q < P.n_ranges; ++q) {
-        const double* src = A.rpart + (((long long)r * P.n_ranges + q) * n_slices) * PSG_MOM;
-        double sum[PSG_MOM] = {0, 0, 0, 0, 0};
+    // operands of the bias, requested early: their latency hides behind the combination
+    float h_center = 0.f, h_k = 0.f;
+    if (lane < P.n_cv) {
+        h_center = __ldg(A.centers + (long long)r * P.n_cv + lane);
+        h_k = __ldg(A.kspring + lane);
+    }
+    // fixed-order combination per value: lanes stride the slices (increasing), then an xor tree. Three groups
+    // at a time, so that all their loads (L2, written by other SMs) are in flight together: this latency is
+    // what every CTA of the window waits for.
+    for (int q0 = 0; q0 < P.n_ranges; q0 += 3) {
+        double sum[3][PSG_MOM];
+#pragma unroll
+        for (int j = 0; j < 3; ++j)
+#pragma unroll
+            for (int i = 0; i < PSG_MOM; ++i) sum[j][i] = 0.0;
+#pragma unroll 2
         for (int b = lane; b < n_slices; b += 32) {
 #pragma unroll
-            for (int i = 0; i < PSG_MOM; ++i) sum[i] += __ldcg(src + (long long)b * PSG_MOM + i);
+            for (int j = 0; j < 3; ++j) {
+                if (q0 + j < P.n_ranges) {
+                    const double* src = A.rpart + (((long long)r * P.n_ranges + q0 + j) * n_slices + b) * PSG_MOM;
+#pragma unroll
+                    for (int i = 0; i < PSG_MOM; ++i) sum[j][i] += __ldcg(src + i);
+                }
+            }
         }
 #pragma unroll
-        for (int i = 0; i < PSG_MOM; ++i) {
-            sum[i] = warp_sum(sum[i]);
-            if (lane == 0) S.mom[q][i] = sum[i];
-        }
+        for (int j = 0; j < 3; ++j)
+#pragma unroll
+            for (int i = 0; i < PSG_MOM; ++i) {
+                const double t = warp_sum(sum[j][i]);
+                if (lane == 0 && q0 + j < P.n_ranges) S.mom[q0 + j][i] = t;
+            }
     }
     __syncwarp();
     if (lane < P.n_ranges) {
@@ -179,10 +228,10 @@ __device__ __forceinline__ void rs_window(const SysParams& P, const RangeStepArg
         }
         // harmonic bias at the CV rounded to binary32, as the unfused calls see it
         const float xif = (float)xi;
-        double d = (double)xif - (double)A.centers[(long long)r * P.n_cv + lane];
+        double d = (double)xif - (double)h_center;
         const double per = C.period;
         if (per > 0.0) d -= per * rint(d / per);
-        const double ks = (double)A.kspring[lane];
+        const double ks = (double)h_k;
         const float dVf = (float)(ks * d);
         S.dv[lane] = -(double)dVf;
         S.vk[lane] = 0.5 * ks * d * d;
@@ -216,11 +265,11 @@ __device__ __forceinline__ void rs_window(const SysParams& P, const RangeStepArg
     __syncwarp();
 }
 
-// A group, one item: moments of the slice in shared memory -> rpart -> ticket (-> window work)
-__device__ __forceinline__ void rs_phase_a(const SysParams& P, const RangeStepArgs& A, RsShared& S, const float4* __restrict__ sp,
-                                           const RsItem& I, int buf, int tid) {
+// A group, one item: per-warp moments of the slice in shared memory -> S.red[buf]. Warps do not synchronise with
+// each other: each reports to the T warp (red_full) and hands the stage back (a_empty) on its own.
+__device__ __forceinline__ void rs_phase_a(const SysParams& P, RsShared& S, const float4* __restrict__ sp, const RsItem& I, int buf,
+                                           int tid) {
     const int lane = tid & 31, wid = tid >> 5;
-    const int n_slices = P.range_blocks;
     const long long t0 = P.span_begin + (long long)I.s * RS_SLICE;
     const long long t1 = t0 + (I.bytes >> 4);
     bool have_full = false;           // moments over the WHOLE slice, shared by every group that contains it
@@ -229,7 +278,7 @@ __device__ __forceinline__ void rs_phase_a(const SysParams& P, const RangeStepAr
         const GroupDev& G = P.grp[P.range_gid[q]];
         const long long gb = G.rbegin, ge = G.rbegin + G.rsize;
         double m[PSG_MOM] = {0, 0, 0, 0, 0};
-        if (t0 < ge && t1 > gb) {     // group-uniform
+        if (t0 < ge && t1 > gb) {     // uniform over the group
             const bool inside = gb <= t0 && t1 <= ge;
             if (inside && have_full) {
 #pragma unroll
@@ -262,162 +311,212 @@ __device__ __forceinline__ void rs_phase_a(const SysParams& P, const RangeStepAr
             for (int i = 0; i < PSG_MOM; ++i) S.red[buf][wid][q][i] = m[i];
         }
     }
-    rs_group_sync(1);
-    if (wid == 0) {
-        // warp 0 finishes the item while warps 1..7 move on (S.red is double-buffered)
-        for (int t = lane; t < P.n_ranges * PSG_MOM; t += 32) {
-            const int q = t / PSG_MOM, i = t % PSG_MOM;
-            double sum = 0.0;
-#pragma unroll
-            for (int wq = 0; wq < RS_GT / 32; ++wq) sum += S.red[buf][wq][q][i];
-            A.rpart[(((long long)I.r * P.n_ranges + q) * n_slices + I.s) * PSG_MOM + i] = sum;
-        }
-        __syncwarp();
-        unsigned old = 0;
-        if (lane == 0) {
-            // release: the warp's partials (ordered before this by the warp barrier) become visible to whoever
-            // acquires the ticket
-            asm volatile("atom.acq_rel.gpu.global.add.u32 %0, [%1], 1;" : "=r"(old) : "l"(A.arrive + I.r) : "memory");
-        }
-        if (lane == 0 && old == (unsigned)(n_slices - 1)) {
-            // last ticket of the window: hand it to the window warp (the ring cannot realistically fill: a CTA
-            // closes a window every few items; wait if it does)
-            const int h = S.wq_head;
-            while (h - S.wq_tail >= RS_WQ) __nanosleep(100);
-            S.wq[h % RS_WQ] = I.r;
-            __threadfence_block();
-            S.wq_head = h + 1;
-        }
-    }
+    __syncwarp();
 }
 
-// B group, one item: force update of the slice; positions from shared memory, forces streamed through registers
-__device__ __forceinline__ void rs_phase_b(const SysParams& P, const RangeStepArgs& A, RsShared& S, const float4* __restrict__ sp,
-                                           const RsItem& I, int g, int tid) {
-    const int bar_id = 2 + g;
-    float4* f = reinterpret_cast<float4*>(A.force) + I.a0;
-    const int cnt = (int)(I.bytes >> 4);
-    // forces first: their latency overlaps the descriptor poll
-    float4 fv[RS_PER];
+// T warp, one item: the slice's moments (8 warp partials, fixed order) -> rpart; ticket on the window's counter
+__device__ __forceinline__ void rs_tail(const SysParams& P, const RangeStepArgs& A, RsShared& S, const RsItem& I, int buf,
+                                        int lane) {
+    const int n_slices = P.range_blocks;
+    for (int t = lane; t < P.n_ranges * PSG_MOM; t += 32) {
+        const int q = t / PSG_MOM, i = t % PSG_MOM;
+        double sum = 0.0;
 #pragma unroll
-    for (int i = 0; i < RS_PER; ++i) {
-        const int o = tid + i * RS_GT;
-        fv[i] = make_float4(0.f, 0.f, 0.f, 0.f);
-        if (o < cnt) fv[i] = __ldcs(f + o);   // streamed: read once, written once
+        for (int wq = 0; wq < RS_GT / 32; ++wq) sum += S.red[buf][wq][q][i];
+        A.rpart[(((long long)I.r * P.n_ranges + q) * n_slices + I.s) * PSG_MOM + i] = sum;
     }
+    __syncwarp();
+    if (lane == 0) {
+        rs_mbar_arrive(&S.red_empty[buf]);
+        // release: the warp's partials (ordered before this by the warp barrier) become visible to the W warp that
+        // acquires the counter
+        asm volatile("red.release.gpu.global.add.u32 [%0], 1;" ::"l"(A.arrive + I.r) : "memory");
+    }
+    __syncwarp();
+}
+
+// B group, one item: force update of the slice; positions and forces out of shared memory, result streamed to global
+__device__ __forceinline__ void rs_phase_b(const SysParams& P, const RangeStepArgs& A, RsShared& S, const float4* __restrict__ sp,
+                                           const float4* __restrict__ sf, const RsItem& I, int tid) {
+#ifdef PSG_TRACE
+    const long long rs_p0_ = clock64();
+#endif
     if (tid < P.n_ranges * RS_DESC) {
         const float4* src = A.desc + (long long)I.r * P.n_ranges * RS_DESC + tid;
         float4 d = rs_ld_relaxed_f4(src);
-        while (d.w != RS_TAG) {   // window not finished yet: only at pipeline start-up or if the A groups lag
+        while (d.w != RS_TAG) {   // window not finished yet: only at pipeline start-up or if `lag` is too short
             __nanosleep(200);
             d = rs_ld_relaxed_f4(src);
+#ifdef PSG_TRACE
+            if (tid == 0 && A.trace) A.trace[blockIdx.x * 32 + 24] += 1;   // polls that found the window unfinished
+#endif
         }
-        S.desc[g][tid / RS_DESC][tid % RS_DESC] = d;
+        S.desc[tid / RS_DESC][tid % RS_DESC] = d;
     }
-    rs_group_sync(bar_id);
+    if (tid >= 32 && tid < 32 + P.n_ranges) {
+        // slice-local bounds of every group: the atom loop compares 32-bit offsets held in shared memory
+        const GroupDev& G = P.grp[P.range_gid[tid - 32]];
+        const long long t0 = P.span_begin + (long long)I.s * RS_SLICE;
+        long long lo = G.rbegin - t0, hi = G.rbegin + G.rsize - t0;
+        const long long cnt = (long long)(I.bytes >> 4);
+        if (lo < 0) lo = 0;
+        if (hi > cnt) hi = cnt;
+        S.blo[tid - 32] = (int)lo;
+        S.bhi[tid - 32] = hi > lo ? (int)hi : (int)lo;
+    }
+    rs_group_sync(2);
+#ifdef PSG_TRACE
+    if (tid == 0 && A.trace) A.trace[blockIdx.x * 32 + 25] += clock64() - rs_p0_;   // poll + group barrier
+#endif
+    float4* f = reinterpret_cast<float4*>(A.force) + I.a0;
     const long long t0 = P.span_begin + (long long)I.s * RS_SLICE;
+    // group-major, the thread's RS_PER atoms side by side (independent chains); per atom the groups are still
+    // accumulated in increasing order, as in the unfused kernel
+    float ax[RS_PER], ay[RS_PER], az[RS_PER];
+    unsigned anym = 0u;
 #pragma unroll
-    for (int i = 0; i < RS_PER; ++i) {
-        const int o = tid + i * RS_GT;
-        if (o >= cnt) continue;
-        const long long a = t0 + o;
-        const float4 p = sp[o];
-        float ax = 0.f, ay = 0.f, az = 0.f;
-        bool any = false;
-        for (int q = 0; q < P.n_ranges; ++q) {
-            const GroupDev& G = P.grp[P.range_gid[q]];
-            if (a >= G.rbegin && a < G.rbegin + G.rsize) {
-                any = true;
-                const float4 v = S.desc[g][q][0], hi = S.desc[g][q][1], lo = S.desc[g][q][2];
-                const float k = S.desc[g][q][3].x;
-                ax += v.x + k * ((p.x - hi.x) - lo.x);
-                ay += v.y + k * ((p.y - hi.y) - lo.y);
-                az += v.z + k * ((p.z - hi.z) - lo.z);
+    for (int i = 0; i < RS_PER; ++i) ax[i] = ay[i] = az[i] = 0.f;
+    for (int q = 0; q < P.n_ranges; ++q) {
+        const int lo_o = S.blo[q], hi_o = S.bhi[q];
+        if (lo_o >= hi_o) continue;   // uniform: the slice does not touch this group
+        const float4 v = S.desc[q][0], hi = S.desc[q][1], lo = S.desc[q][2];
+        const float k = S.desc[q][3].x;
+#pragma unroll
+        for (int i = 0; i < RS_PER; ++i) {
+            const int o = tid + i * RS_GT;
+            if (o >= lo_o && o < hi_o) {
+                const float4 p = sp[o];
+                anym |= 1u << i;
+                ax[i] += v.x + k * ((p.x - hi.x) - lo.x);
+                ay[i] += v.y + k * ((p.y - hi.y) - lo.y);
+                az[i] += v.z + k * ((p.z - hi.z) - lo.z);
             }
         }
-        if (!any) continue;   // an atom of the span that belongs to no group is not written
-        const float w = P.atom_weight ? __ldg(P.atom_weight + a) : 1.f;
+    }
+#pragma unroll
+    for (int i = 0; i < RS_PER; ++i) {
+        if (!((anym >> i) & 1u)) continue;   // an atom of the span that belongs to no group is not written
+        const int o = tid + i * RS_GT;
+        const float w = P.atom_weight ? __ldg(P.atom_weight + t0 + o) : 1.f;
+        float4 fv = sf[o];
         // (no contraction: same bits as the unfused path); the record's w keeps its bits
-        fv[i].x += __fmul_rn(ax, w); fv[i].y += __fmul_rn(ay, w); fv[i].z += __fmul_rn(az, w);
-        __stcs(f + o, fv[i]);
+        fv.x += __fmul_rn(ax[i], w); fv.y += __fmul_rn(ay[i], w); fv.z += __fmul_rn(az[i], w);
+        __stcs(f + o, fv);
     }
 }
 
 __global__ void __launch_bounds__(RS_THREADS, 1) k_range_step(const __grid_constant__ SysParams P, const __grid_constant__ RangeStepArgs A) {
     extern __shared__ __align__(128) unsigned char rs_smem[];
-    float4* stage = reinterpret_cast<float4*>(rs_smem);   // RS_STAGES x RS_SLICE positions
-    RsShared& S = *reinterpret_cast<RsShared*>(rs_smem + (size_t)RS_STAGES * RS_SLICE * 16);
-    const int tid = threadIdx.x;
+    float4* ring_a = reinterpret_cast<float4*>(rs_smem);                       // RS_ASTAGES x RS_SLICE positions
+    float4* ring_b = ring_a + (size_t)RS_ASTAGES * RS_SLICE;                   // RS_BSTAGES x {RS_SLICE positions, RS_SLICE forces}
+    RsShared& S = *reinterpret_cast<RsShared*>(ring_b + (size_t)RS_BSTAGES * 2 * RS_SLICE);
+    const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
     const long long items = (long long)P.R * P.range_blocks;
     const long long G = gridDim.x;
     const long long n_mine = blockIdx.x < items ? (items - blockIdx.x + G - 1) / G : 0;
 
     if (tid == 0) {
-        for (int st = 0; st < RS_STAGES; ++st) {
-            rs_mbar_init(&S.full[st], 1);
-            rs_mbar_init(&S.empty[st], RS_GT / 32);   // one arrival per warp of the B group that used the stage
-        }
+        for (int st = 0; st < RS_ASTAGES; ++st) { rs_mbar_init(&S.a_full[st], 1); rs_mbar_init(&S.a_empty[st], RS_GT / 32); }
+        for (int st = 0; st < RS_BSTAGES; ++st) { rs_mbar_init(&S.b_full[st], 1); rs_mbar_init(&S.b_empty[st], RS_GT / 32); }
+        for (int b = 0; b < RS_RED; ++b) { rs_mbar_init(&S.red_full[b], RS_GT / 32); rs_mbar_init(&S.red_empty[b], 1); }
+        S.b_prog = 0;
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     __syncthreads();
 
-    if (tid == 0) { S.wq_head = 0; S.wq_tail = 0; S.a_done = 0; }
-    __syncthreads();
-
-    if (tid < 32) {
-        // ---------------- producer warp
-        if (tid == 0) {
+    if (warp == 0) {
+        // ---------------- PA: positions -> ring A, at most `lag` items ahead of the B group
+        if (lane == 0) {
+            const uint64_t keep = rs_policy_evict_last();
+            RS_DECL;
             for (long long it = 0; it < n_mine; ++it) {
-                const int st = (int)(it % RS_STAGES);
-                if (it >= RS_STAGES) rs_mbar_wait(&S.empty[st], (uint32_t)((it / RS_STAGES - 1) & 1));
+                const int st = (int)(it % RS_ASTAGES);
+                { RS_T0; if (it >= RS_ASTAGES) rs_mbar_wait(&S.a_empty[st], (uint32_t)((it / RS_ASTAGES - 1) & 1)); RS_ACC(0); }
+                { RS_T0; while (it - S.b_prog > A.lag) __nanosleep(200); RS_ACC(1); }
                 const RsItem I = rs_item(P, it, G);
-                rs_mbar_expect_tx(&S.full[st], I.bytes);
-                rs_tma_load_1d(stage + (size_t)st * RS_SLICE, reinterpret_cast<const float4*>(A.pos) + I.a0, I.bytes, &S.full[st]);
+                rs_mbar_expect_tx(&S.a_full[st], I.bytes);
+                rs_tma_load_1d(ring_a + (size_t)st * RS_SLICE, reinterpret_cast<const float4*>(A.pos) + I.a0, I.bytes, &S.a_full[st], keep);
             }
+            RS_FLUSH(true, 0);
         }
-    } else if (tid < RS_LEAD) {
-        // ---------------- window warp: serves the windows whose last ticket was taken by this CTA
-        const int lane = tid & 31;
-        int tail = 0;
-        for (;;) {
-            int head = S.wq_head;
-            const int fin = S.a_done;   // read AFTER head: a_done is set after the last hand-over
-            if (head == tail) {
-                if (fin && S.wq_head == tail) break;
-                __nanosleep(100);
-                continue;
+    } else if (warp == 1) {
+        // ---------------- PB: positions (L2) + forces -> ring B
+        if (lane == 0) {
+            const uint64_t once = rs_policy_evict_first();
+            RS_DECL;
+            for (long long it = 0; it < n_mine; ++it) {
+                const int st = (int)(it % RS_BSTAGES);
+                { RS_T0; if (it >= RS_BSTAGES) rs_mbar_wait(&S.b_empty[st], (uint32_t)((it / RS_BSTAGES - 1) & 1)); RS_ACC(0); }
+                const RsItem I = rs_item(P, it, G);
+                float4* dst = ring_b + (size_t)st * 2 * RS_SLICE;
+                rs_mbar_expect_tx(&S.b_full[st], 2u * I.bytes);
+                rs_tma_load_1d(dst, reinterpret_cast<const float4*>(A.pos) + I.a0, I.bytes, &S.b_full[st], once);
+                rs_tma_load_1d(dst + RS_SLICE, reinterpret_cast<const float4*>(A.force) + I.a0, I.bytes, &S.b_full[st], once);
             }
-            __threadfence_block();
-            const int r = S.wq[tail % RS_WQ];
-            __threadfence();            // acquire side of the ticket (taken by another warp of this CTA)
-            rs_window(P, A, S, r, lane);
-            ++tail;
-            if (lane == 0) S.wq_tail = tail;
+            RS_FLUSH(true, 4);
+        }
+    } else if (warp == 2) {
+        // ---------------- W: windows b, b + grid, ...
+        for (long long r = blockIdx.x; r < P.R; r += G) {
+            if (lane == 0) {
+                unsigned n;
+                do {
+                    asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(n) : "l"(A.arrive + r) : "memory");
+                    if (n < (unsigned)P.range_blocks) __nanosleep(200);
+                } while (n < (unsigned)P.range_blocks);
+            }
             __syncwarp();
+            __threadfence();
+#ifdef PSG_TRACE
+            const long long w0_ = clock64();
+#endif
+            rs_window(P, A, S, (int)r, lane);
+#ifdef PSG_TRACE
+            if (lane == 0 && A.trace) { A.trace[blockIdx.x * 32 + 28] += clock64() - w0_; A.trace[blockIdx.x * 32 + 29] += 1; }
+#endif
         }
+    } else if (warp < 3 + RS_NT) {
+        // ---------------- T warp j: items j, j + RS_NT, ...
+        const int j = warp - 3;
+        RS_DECL;
+        for (long long it = j; it < n_mine; it += RS_NT) {
+            const int buf = (int)(it % RS_RED);
+            const RsItem I = rs_item(P, it, G);
+            { RS_T0; rs_mbar_wait(&S.red_full[buf], (uint32_t)((it / RS_RED) & 1)); RS_ACC(0); }
+            { RS_T0; rs_tail(P, A, S, I, buf, lane); RS_ACC(1); }
+        }
+        RS_FLUSH(lane == 0, 8 + 4 * j);
     } else if (tid < RS_LEAD + RS_GT) {
         // ---------------- A group
         const int t = tid - RS_LEAD;
+        RS_DECL;
         for (long long it = 0; it < n_mine; ++it) {
-            const int st = (int)(it % RS_STAGES);
+            const int st = (int)(it % RS_ASTAGES), buf = (int)(it % RS_RED);
             const RsItem I = rs_item(P, it, G);
-            rs_mbar_wait(&S.full[st], (uint32_t)((it / RS_STAGES) & 1));
-            rs_phase_a(P, A, S, stage + (size_t)st * RS_SLICE, I, (int)(it & 1), t);
+            { RS_T0; rs_mbar_wait(&S.a_full[st], (uint32_t)((it / RS_ASTAGES) & 1)); RS_ACC(0); }
+            { RS_T0; if (it >= RS_RED) rs_mbar_wait(&S.red_empty[buf], (uint32_t)((it / RS_RED - 1) & 1)); RS_ACC(1); }
+            rs_phase_a(P, S, ring_a + (size_t)st * RS_SLICE, I, buf, t);
+            if ((t & 31) == 0) {
+                rs_mbar_arrive(&S.red_full[buf]);   // this warp's partials are in S.red[buf]
+                rs_mbar_arrive(&S.a_empty[st]);     // and it is done reading the stage
+            }
         }
-        rs_group_sync(1);               // warp 0 has handed over its last window
-        if (t == 0) { __threadfence_block(); S.a_done = 1; }
+        RS_FLUSH(t == 0, 16);
     } else {
-        // ---------------- B groups: group g takes the items it = g, g + RS_NB, ...
-        const int g = (tid - RS_LEAD - RS_GT) / RS_GT, t = (tid - RS_LEAD - RS_GT) % RS_GT;
-        for (long long it = g; it < n_mine; it += RS_NB) {
-            const int st = (int)(it % RS_STAGES);
+        // ---------------- B group
+        const int t = tid - RS_LEAD - RS_GT;
+        RS_DECL;
+        for (long long it = 0; it < n_mine; ++it) {
+            const int st = (int)(it % RS_BSTAGES);
             const RsItem I = rs_item(P, it, G);
-            rs_mbar_wait(&S.full[st], (uint32_t)((it / RS_STAGES) & 1));   // the stage's bytes are visible to this thread
-            rs_phase_b(P, A, S, stage + (size_t)st * RS_SLICE, I, g, t);
+            const float4* sp = ring_b + (size_t)st * 2 * RS_SLICE;
+            { RS_T0; rs_mbar_wait(&S.b_full[st], (uint32_t)((it / RS_BSTAGES) & 1)); RS_ACC(0); }
+            { RS_T0; rs_phase_b(P, A, S, sp, sp + RS_SLICE, I, t); RS_ACC(1); }
             __syncwarp();
-            if ((t & 31) == 0) rs_mbar_arrive(&S.empty[st]);   // this warp is done reading the stage
-            rs_group_sync(2 + g);                              // S.desc[g] may be overwritten by the next item
+            if ((t & 31) == 0) rs_mbar_arrive(&S.b_empty[st]);   // this warp is done reading the stage
+            rs_group_sync(2);                                    // S.desc may be overwritten by the next item
             if (t == 0) {
+                S.b_prog = it + 1;
                 // the last CTA to finish a window re-arms its counters and descriptor tags for the next launch
                 const unsigned old = atomicAdd(A.done + I.r, 1u);
                 if (old == (unsigned)(P.range_blocks - 1)) {
@@ -427,10 +526,11 @@ __global__ void __launch_bounds__(RS_THREADS, 1) k_range_step(const __grid_const
                 }
             }
         }
+        RS_FLUSH(t == 0, 20);
     }
 }
 
-static const size_t kRsSmem = (size_t)RS_STAGES * RS_SLICE * 16 + sizeof(RsShared);
+static const size_t kRsSmem = (size_t)(RS_ASTAGES + 2 * RS_BSTAGES) * RS_SLICE * 16 + sizeof(RsShared);
 
 // co-resident CTAs per SM (0 if the kernel cannot be configured)
 static int rs_blocks_per_sm() {
@@ -469,6 +569,10 @@ cudaError_t psg_launch_range_step(psg_ctx* c, const float* d_pos, float* d_force
     A.pos = d_pos; A.force = d_force; A.kspring = c->d_kspring; A.centers = c->d_centers;
     A.xi_out = c->d_xi; A.V_out = c->d_V; A.V64_out = c->d_V64; A.dV_out = c->d_dVdxi;
     A.rpart = c->d_rpart; A.arrive = c->d_arrive; A.done = c->d_arrive + P.R; A.desc = c->d_rdesc;
+    // B runs `lag` items behind A: long enough to cover the window dependency (several L2 round trips), short
+    // enough that lag x grid x 32 KB of positions stays in L2 (12 x 148 x 32 KB = 57 MB of 126 MB)
+    static const int lag_env = getenv("PSG_RANGE_LAG") ? atoi(getenv("PSG_RANGE_LAG")) : 0;
+    A.lag = lag_env > 0 ? lag_env : 12;
 #ifdef PSG_TRACE
     A.trace = psg_trace_buffer();
 #endif
