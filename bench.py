@@ -265,7 +265,7 @@ def run_psg(args, rank, world):
         elif w.method == "harmonic":
             bytes_step = 48.0 * w.R * w.N                          # read pos once + read force + write force (float4)
             ach = bytes_step * K / (ms_total * 1e-3) / 1e9
-            out["roofline"] = {"bound": "hbm", "kernel": "k_range_moments + k_apply_dense", "achieved": ach, "peak": hbm_peak,
+            out["roofline"] = {"bound": "hbm", "kernel": "k_range_step (fused umbrella step, one launch)", "achieved": ach, "peak": hbm_peak,
                                "unit": "GB/s", "frac": ach / hbm_peak, "traffic": None, "peak_source": which + " copy bandwidth",
                                "algorithmic_bytes_per_step": bytes_step,
                                "frac_back_to_back": bytes_step * K / (ms_b2b * 1e-3) / 1e9 / hbm_peak}

@@ -15,7 +15,7 @@
 //              dihedral / component, radius of gyration) and the harmonic bias in binary64, publishes per-group
 //              force descriptors (16-byte records carrying a valid tag).
 //   PB warp  : positions (now an L2 hit) and forces of the B group's next items -> ring B.
-//   B group  (8 warps): waits for the window's descriptors, then
+//   B group  (16 warps): waits for the window's descriptors, then
 //              F_i += -dV/dxi_k * w_i (v_g + coef_g (r_i - c_g))  out of shared memory, st.global.cs float4.
 //   HBM traffic: positions once (the second read is served by L2 while `lag` x grid x 32 KB fits), forces read
 //   once and written once = 48 B/atom, the algorithmic minimum; 64 B/atom if L2 keeps nothing.
@@ -34,10 +34,12 @@
 #define RS_BSTAGES 2              // ring B: positions + forces
 #define RS_RED 4                  // ring of per-warp partial moments between the A group and the T warps
 #define RS_NT 2                   // T warps
-#define RS_GT 256                 // threads of the A group and of the B group
+#define RS_GT 256                 // threads of the A group (fixes the reduction order: same map as k_range_moments)
+#define RS_GTB 512                // threads of the B group
 #define RS_LEAD (32 * (3 + RS_NT))   // PA, PB, W, T warps
-#define RS_THREADS (RS_LEAD + 2 * RS_GT)
+#define RS_THREADS (RS_LEAD + RS_GT + RS_GTB)
 #define RS_PER (RS_SLICE / RS_GT)
+#define RS_PERB (RS_SLICE / RS_GTB)
 #define RS_DESC 4                 // float4 records per (window, range group): {v, tag} {c_hi, tag} {c_lo, tag} {k, 0, 0, tag}
 #define RS_TAG 1.0f
 
@@ -99,7 +101,7 @@ __device__ __forceinline__ void rs_mbar_wait(uint64_t* bar, uint32_t parity) {
         "r"(parity)
         : "memory");
 }
-__device__ __forceinline__ void rs_group_sync(int id) { asm volatile("bar.sync %0, %1;" ::"r"(id), "n"(RS_GT) : "memory"); }
+__device__ __forceinline__ void rs_b_sync() { asm volatile("bar.sync 2, %0;" ::"n"(RS_GTB) : "memory"); }
 __device__ __forceinline__ float4 rs_ld_relaxed_f4(const float4* p) {   // one 16-byte access, always from L2
     float4 v;
     asm volatile("ld.relaxed.gpu.global.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "l"(p) : "memory");
@@ -128,6 +130,7 @@ struct RsShared {
     double vk[PSG_MAX_CV];                                        // 1/2 k_k D_k^2
     float4 desc[PSG_MAX_RANGE_GROUPS][RS_DESC];                   // B group: the window's force descriptors
     int blo[PSG_MAX_RANGE_GROUPS], bhi[PSG_MAX_RANGE_GROUPS];     // B group: slice-local atom bounds of every group
+    int bfast;                                                    // B group: the item takes the straight-line path
     uint64_t a_full[RS_ASTAGES], a_empty[RS_ASTAGES], b_full[RS_BSTAGES], b_empty[RS_BSTAGES];
     uint64_t red_full[RS_RED], red_empty[RS_RED];
     volatile long long b_prog;                  // items the B group has finished
@@ -284,15 +287,32 @@ __device__ __forceinline__ void rs_phase_a(const SysParams& P, RsShared& S, cons
 #pragma unroll
                 for (int i = 0; i < PSG_MOM; ++i) m[i] = mf[i];
             } else {
+                if (inside && (t1 - t0 == RS_SLICE) && !P.atom_weight) {
+                    // the common case, straight-line: a whole slice inside the group, unit weights
+                    // (1.0 * x + m rounds exactly like x + m: same bits as the general loop)
 #pragma unroll
-                for (int i = 0; i < RS_PER; ++i) {
-                    const long long a = t0 + tid + i * RS_GT;
-                    if (a >= gb && a < ge && a < t1) {
-                        // (re-read from shared memory per group pass: registers are the scarce resource here)
+                    for (int i = 0; i < RS_PER; ++i) {
                         const float4 v = sp[tid + i * RS_GT];
-                        const double wd = P.atom_weight ? (double)__ldg(P.atom_weight + a) : 1.0;
-                        // products of binary32 inputs are exact in binary64
                         const double xd = (double)v.x, yd = (double)v.y, zd = (double)v.z;
+                        m[0] += 1.0; m[1] += xd; m[2] += yd; m[3] += zd;
+                        m[4] += xd * xd + yd * yd + zd * zd;
+                    }
+                } else {
+                    // branch-free: an atom outside the group (or past the end of a ragged slice) enters with w = 0
+                    // and r = 0, which adds exactly +0 to every moment -- the same bits as skipping it
+#pragma unroll
+                    for (int i = 0; i < RS_PER; ++i) {
+                        const int o = tid + i * RS_GT;
+                        const long long a = t0 + o;
+                        const bool in = a >= gb && a < ge && a < t1;
+                        float4 v = make_float4(0.f, 0.f, 0.f, 0.f);
+                        float wf = 0.f;
+                        if (in) {   // predicated loads, no divergence
+                            v = sp[o];
+                            wf = P.atom_weight ? __ldg(P.atom_weight + a) : 1.f;
+                        }
+                        // products of binary32 inputs are exact in binary64
+                        const double wd = (double)wf, xd = (double)v.x, yd = (double)v.y, zd = (double)v.z;
                         m[0] += wd; m[1] += wd * xd; m[2] += wd * yd; m[3] += wd * zd;
                         m[4] += wd * (xd * xd + yd * yd + zd * zd);
                     }
@@ -364,26 +384,66 @@ __device__ __forceinline__ void rs_phase_b(const SysParams& P, const RangeStepAr
         S.blo[tid - 32] = (int)lo;
         S.bhi[tid - 32] = hi > lo ? (int)hi : (int)lo;
     }
-    rs_group_sync(2);
+    if (tid == 64) {
+        // fast path: a whole slice that every group either covers completely or does not touch, and is touched at all
+        const long long t0 = P.span_begin + (long long)I.s * RS_SLICE;
+        const long long t1 = t0 + (long long)(I.bytes >> 4);
+        bool fast = (I.bytes >> 4) == RS_SLICE, any = false;
+        for (int q = 0; q < P.n_ranges; ++q) {
+            const GroupDev& G = P.grp[P.range_gid[q]];
+            const long long gb = G.rbegin, ge = G.rbegin + G.rsize;
+            const bool touch = t0 < ge && t1 > gb, cover = gb <= t0 && t1 <= ge;
+            if (touch && !cover) fast = false;
+            any |= cover;
+        }
+        S.bfast = fast && any;
+    }
+    rs_b_sync();
 #ifdef PSG_TRACE
     if (tid == 0 && A.trace) A.trace[blockIdx.x * 32 + 25] += clock64() - rs_p0_;   // poll + group barrier
 #endif
     float4* f = reinterpret_cast<float4*>(A.force) + I.a0;
     const long long t0 = P.span_begin + (long long)I.s * RS_SLICE;
-    // group-major, the thread's RS_PER atoms side by side (independent chains); per atom the groups are still
+    // group-major, the thread's RS_PERB atoms side by side (independent chains); per atom the groups are still
     // accumulated in increasing order, as in the unfused kernel
-    float ax[RS_PER], ay[RS_PER], az[RS_PER];
-    unsigned anym = 0u;
+    float ax[RS_PERB], ay[RS_PERB], az[RS_PERB];
 #pragma unroll
-    for (int i = 0; i < RS_PER; ++i) ax[i] = ay[i] = az[i] = 0.f;
+    for (int i = 0; i < RS_PERB; ++i) ax[i] = ay[i] = az[i] = 0.f;
+    if (S.bfast && !P.atom_weight) {
+        // the common case, straight-line: a whole slice, every group either covers all of it or none of it, unit
+        // weights (x * 1.0f is x: same bits as the general loop)
+        float4 p[RS_PERB];
+#pragma unroll
+        for (int i = 0; i < RS_PERB; ++i) p[i] = sp[tid + i * RS_GTB];
+        for (int q = 0; q < P.n_ranges; ++q) {
+            if (S.blo[q] >= S.bhi[q]) continue;   // uniform
+            const float4 v = S.desc[q][0], hi = S.desc[q][1], lo = S.desc[q][2];
+            const float k = S.desc[q][3].x;
+#pragma unroll
+            for (int i = 0; i < RS_PERB; ++i) {
+                ax[i] += v.x + k * ((p[i].x - hi.x) - lo.x);
+                ay[i] += v.y + k * ((p[i].y - hi.y) - lo.y);
+                az[i] += v.z + k * ((p[i].z - hi.z) - lo.z);
+            }
+        }
+#pragma unroll
+        for (int i = 0; i < RS_PERB; ++i) {
+            const int o = tid + i * RS_GTB;
+            float4 fv = sf[o];
+            fv.x += ax[i]; fv.y += ay[i]; fv.z += az[i];   // the record's w keeps its bits
+            __stcs(f + o, fv);
+        }
+        return;
+    }
+    unsigned anym = 0u;
     for (int q = 0; q < P.n_ranges; ++q) {
         const int lo_o = S.blo[q], hi_o = S.bhi[q];
         if (lo_o >= hi_o) continue;   // uniform: the slice does not touch this group
         const float4 v = S.desc[q][0], hi = S.desc[q][1], lo = S.desc[q][2];
         const float k = S.desc[q][3].x;
 #pragma unroll
-        for (int i = 0; i < RS_PER; ++i) {
-            const int o = tid + i * RS_GT;
+        for (int i = 0; i < RS_PERB; ++i) {
+            const int o = tid + i * RS_GTB;
             if (o >= lo_o && o < hi_o) {
                 const float4 p = sp[o];
                 anym |= 1u << i;
@@ -394,9 +454,9 @@ __device__ __forceinline__ void rs_phase_b(const SysParams& P, const RangeStepAr
         }
     }
 #pragma unroll
-    for (int i = 0; i < RS_PER; ++i) {
+    for (int i = 0; i < RS_PERB; ++i) {
         if (!((anym >> i) & 1u)) continue;   // an atom of the span that belongs to no group is not written
-        const int o = tid + i * RS_GT;
+        const int o = tid + i * RS_GTB;
         const float w = P.atom_weight ? __ldg(P.atom_weight + t0 + o) : 1.f;
         float4 fv = sf[o];
         // (no contraction: same bits as the unfused path); the record's w keeps its bits
@@ -417,7 +477,7 @@ __global__ void __launch_bounds__(RS_THREADS, 1) k_range_step(const __grid_const
 
     if (tid == 0) {
         for (int st = 0; st < RS_ASTAGES; ++st) { rs_mbar_init(&S.a_full[st], 1); rs_mbar_init(&S.a_empty[st], RS_GT / 32); }
-        for (int st = 0; st < RS_BSTAGES; ++st) { rs_mbar_init(&S.b_full[st], 1); rs_mbar_init(&S.b_empty[st], RS_GT / 32); }
+        for (int st = 0; st < RS_BSTAGES; ++st) { rs_mbar_init(&S.b_full[st], 1); rs_mbar_init(&S.b_empty[st], RS_GTB / 32); }
         for (int b = 0; b < RS_RED; ++b) { rs_mbar_init(&S.red_full[b], RS_GT / 32); rs_mbar_init(&S.red_empty[b], 1); }
         S.b_prog = 0;
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
@@ -495,7 +555,7 @@ __global__ void __launch_bounds__(RS_THREADS, 1) k_range_step(const __grid_const
             const RsItem I = rs_item(P, it, G);
             { RS_T0; rs_mbar_wait(&S.a_full[st], (uint32_t)((it / RS_ASTAGES) & 1)); RS_ACC(0); }
             { RS_T0; if (it >= RS_RED) rs_mbar_wait(&S.red_empty[buf], (uint32_t)((it / RS_RED - 1) & 1)); RS_ACC(1); }
-            rs_phase_a(P, S, ring_a + (size_t)st * RS_SLICE, I, buf, t);
+            { RS_T0; rs_phase_a(P, S, ring_a + (size_t)st * RS_SLICE, I, buf, t); RS_ACC(2); }
             if ((t & 31) == 0) {
                 rs_mbar_arrive(&S.red_full[buf]);   // this warp's partials are in S.red[buf]
                 rs_mbar_arrive(&S.a_empty[st]);     // and it is done reading the stage
@@ -514,7 +574,7 @@ __global__ void __launch_bounds__(RS_THREADS, 1) k_range_step(const __grid_const
             { RS_T0; rs_phase_b(P, A, S, sp, sp + RS_SLICE, I, t); RS_ACC(1); }
             __syncwarp();
             if ((t & 31) == 0) rs_mbar_arrive(&S.b_empty[st]);   // this warp is done reading the stage
-            rs_group_sync(2);                                    // S.desc may be overwritten by the next item
+            rs_b_sync();                                    // S.desc may be overwritten by the next item
             if (t == 0) {
                 S.b_prog = it + 1;
                 // the last CTA to finish a window re-arms its counters and descriptor tags for the next launch
