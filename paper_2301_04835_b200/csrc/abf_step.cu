@@ -1,0 +1,117 @@
+// abf_step.cu -- the fused ABF step: ONE launch
+// per MD step instead of four.  A step of config 2 moves < 4 MB, so launch latency, not bandwidth, is what it costs.
+//
+//   phase 1  warp per replica: gather the CV atoms in place, CVs + Jacobians (binary64 registers), bin xi in
+//            binary32, hist[bin] += 1 (int32 atomic), Fsum[bin] += f (vector float atomic)
+//   grid barrier (all replicas have accumulated: the two-phase reading R-ABF-2 of DESIGN.md)
+//   phase 2  the same warp: Fbar = Fsum[bin] / max(hist[bin], N)  ->  dV/dxi;  force[i] += -Fbar_k * dxi_k/dr_i
+//            (red.global.add.f32: atoms shared between CVs or walkers collide)
+// The barrier is a counter in global memory, so the grid must be co-resident: the kernel is launched cooperatively
+// (the launch fails instead of hanging) with at most occupancy x SM-count CTAs; warps loop over replicas.
+// Same arithmetic as k_cv_eval + k_abf_accumulate + k_abf_mean + k_apply_sparse: bins, counts, xi, dV/dxi and the
+// Jacobian are bit-identical to the separate calls; Fsum and forces differ only by the order of the atomics.
+#include "abf.cuh"
+#include "geom.cuh"
+
+struct AbfStepArgs {
+    const float* pos;
+    const float* fsample;   // [R][n_cv]
+    float* force;
+    float* xi_out;          // [R][n_cv]
+    int* bin_out;           // [R]
+    float* dV_out;          // [R][n_cv]
+    float* jac;             // [R][n_slots][3] (the ctx cache, as after psg_cv_eval)
+    unsigned* bar;          // [2] arrive / depart counters, zero between launches
+};
+
+__global__ void __launch_bounds__(256, 4) k_abf_step(const __grid_constant__ SysParams P, const __grid_constant__ AbfState G,
+                                                  const __grid_constant__ AbfStepArgs A) {
+    __shared__ WarpCvSmem sm[8];
+    const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
+    const int warps = gridDim.x * 8, gw = blockIdx.x * 8 + wid;
+    WarpCvSmem& S = sm[wid];
+
+    for (int r = gw; r < P.R; r += warps) {
+        warp_cv_eval<true>(P, r, A.pos, nullptr, S, lane);
+        if (lane < P.n_cv) A.xi_out[(long long)r * P.n_cv + lane] = (float)S.xi[lane];
+        for (int s = lane; s < P.n_slots; s += 32) {
+            const D3 j = slot_jacobian(P, r, A.pos, S, s);
+            const long long o = ((long long)r * P.n_slots + s) * 3;
+            A.jac[o] = (float)j.x; A.jac[o + 1] = (float)j.y; A.jac[o + 2] = (float)j.z;
+        }
+        if (lane == 0) {
+            float xi[PSG_MAX_CV];
+#pragma unroll
+            for (int k = 0; k < PSG_MAX_CV; ++k) xi[k] = k < P.n_cv ? (float)S.xi[k] : 0.f;
+            A.bin_out[r] = abf_accumulate_one(G, P.n_cv, xi, A.fsample + (long long)r * P.n_cv);
+        }
+        __syncwarp();
+    }
+
+    // ---- grid barrier: every replica's atomics are performed before anyone reads the grid
+    __syncthreads();
+    if (tid == 0) {
+        __threadfence();
+        atomicAdd(A.bar, 1u);
+        unsigned n;
+        do {
+            asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(n) : "l"(A.bar) : "memory");
+        } while (n < gridDim.x);
+    }
+    __syncthreads();
+
+    for (int r = gw; r < P.R; r += warps) {
+        float* dV = A.dV_out + (long long)r * P.n_cv;
+        if (lane == 0) abf_mean_one(G, P.n_cv, A.bin_out[r], dV);
+        __syncwarp();
+        for (int s = lane; s < P.n_slots; s += 32) {
+            const int gid = P.slot_gid[s];
+            const float dv = -dV[P.grp[gid].cv];
+            const int atom = P.slot_atom[(P.per_rep ? (long long)r * P.n_slots : 0) + s];
+            float* f = A.force + ((long long)r * P.rstride + atom) * P.fs;
+            const float* j = A.jac + ((long long)r * P.n_slots + s) * 3;
+            atomicAdd(f, dv * j[0]);
+            atomicAdd(f + 1, dv * j[1]);
+            atomicAdd(f + 2, dv * j[2]);
+        }
+    }
+
+    // ---- the last CTA to leave re-arms the barrier for the next launch
+    __syncthreads();
+    if (tid == 0) {
+        const unsigned old = atomicAdd(A.bar + 1, 1u);
+        if (old == gridDim.x - 1) { A.bar[0] = 0u; A.bar[1] = 0u; }
+    }
+}
+
+static int abf_blocks_per_sm() {
+    static int n = -1;
+    if (n < 0) {
+        if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n, k_abf_step, 256, 0) != cudaSuccess) n = 0;
+        (void)cudaGetLastError();
+    }
+    return n;
+}
+
+bool psg_abf_step_supported(const psg_ctx* c) {
+    return c->method == PSG_METHOD_ABF && c->sys.n_ranges == 0 && c->d_gbar != nullptr && abf_blocks_per_sm() >= 1;
+}
+
+cudaError_t psg_launch_abf_step(psg_ctx* c, const float* d_pos, const float* d_fsample, float* d_force) {
+    const SysParams& P = c->sys;
+    AbfStepArgs A{};
+    A.pos = d_pos; A.fsample = d_fsample; A.force = d_force;
+    A.xi_out = c->d_xi; A.bin_out = c->d_bin; A.dV_out = c->d_dVdxi; A.jac = c->d_jac; A.bar = c->d_gbar;
+    long long grid = (P.R + 7) / 8;
+    const long long cap = (long long)c->sm_count * abf_blocks_per_sm();
+    if (grid > cap) grid = cap;
+    cudaLaunchConfig_t cfg{};
+    cfg.gridDim = dim3((unsigned)grid); cfg.blockDim = dim3(256); cfg.dynamicSmemBytes = 0; cfg.stream = c->stream;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeCooperative;   // co-residency is what makes the grid barrier safe
+    attr[0].val.cooperative = 1;
+    cfg.attrs = attr; cfg.numAttrs = 1;
+    cudaError_t e = cudaLaunchKernelEx(&cfg, k_abf_step, P, c->abf, A);
+    if (e == cudaSuccess) c->launches++;
+    return e;
+}

@@ -71,7 +71,7 @@ int psg_create(psg_ctx** out, int device, void* cuda_stream) {
 static void free_all(psg_ctx* c) {
     dfree(c->d_slot_atom); dfree(c->d_slot_gid); dfree(c->d_slot_weight); dfree(c->d_atom_weight);
     dfree(c->d_xi); dfree(c->d_V); dfree(c->d_dVdxi); dfree(c->d_bin); dfree(c->d_V64);
-    dfree(c->d_jac); dfree(c->d_gdesc); dfree(c->d_rpart); dfree(c->d_arrive); dfree(c->d_rdesc);
+    dfree(c->d_jac); dfree(c->d_gdesc); dfree(c->d_rpart); dfree(c->d_arrive); dfree(c->d_rdesc); dfree(c->d_gbar);
     dfree(c->d_kspring); dfree(c->d_centers);
     dfree(c->md.hills); dfree(c->md.heights); dfree(c->md.n_hills); dfree(c->md.part); dfree(c->md.ticket);
     if (c->abf.own) { dfree(c->abf.hist); dfree(c->abf.fsum); }
@@ -196,6 +196,8 @@ int psg_set_cvs(psg_ctx* c, int n_cv, const psg_cv_desc* cvs, int n_slots, const
     CK(c, dalloc(c->d_rpart, R * P.n_ranges * (size_t)P.range_blocks * PSG_MOM));
     CK(c, dalloc(c->d_arrive, 2 * R));
     CK(c, cudaMemset(c->d_arrive, 0, 2 * R * sizeof(unsigned)));
+    CK(c, dalloc(c->d_gbar, 2));
+    CK(c, cudaMemset(c->d_gbar, 0, 2 * sizeof(unsigned)));
     CK(c, dalloc(c->d_rdesc, R * P.n_ranges * 4));
     CK(c, cudaMemset(c->d_rdesc, 0, std::max<size_t>(R * P.n_ranges * 4, 1) * sizeof(float4)));
     CK(c, cudaMemset(c->d_V, 0, R * sizeof(float)));
@@ -426,6 +428,11 @@ int psg_step(psg_ctx* c, const float* d_pos, float* d_force, const float* d_fsam
         CK(c, psg_launch_cv_eval(c, d_pos, c->d_xi, nullptr));
         CK(c, psg_launch_harmonic(c, c->d_xi, c->d_V, c->d_dVdxi));
     } else {
+        if (psg_abf_step_supported(c)) {
+            CK(c, psg_launch_abf_step(c, d_pos, d_fsample, d_force));   // one launch: CVs, grid update, barrier, forces
+            c->have_jac = true;
+            return PSG_OK;
+        }
         CK(c, psg_launch_cv_eval(c, d_pos, c->d_xi, nullptr));
         CK(c, psg_launch_abf(c, c->d_xi, d_fsample, nullptr, c->d_dVdxi));
     }

@@ -101,6 +101,7 @@ struct psg_ctx {
     double* d_gdesc = nullptr;       // [R][n_groups][PSG_GDESC_DOUBLES]
     double* d_rpart = nullptr;       // [R][n_ranges][range_blocks][PSG_MOM]
     unsigned* d_arrive = nullptr;    // [2][R]: arrive / done counters of the fused range step (zero between launches)
+    unsigned* d_gbar = nullptr;      // [2]: grid-barrier counters of the fused ABF step (zero between launches)
     float4* d_rdesc = nullptr;       // [R][n_ranges][4]: tagged force descriptors of the fused range step (zero between launches)
     // harmonic
     float* d_kspring = nullptr; float* d_centers = nullptr;
@@ -124,6 +125,8 @@ cudaError_t psg_launch_null_hills(psg_ctx* c, int begin, int end);   // records 
 cudaError_t psg_launch_abf(psg_ctx* c, const float* d_xi, const float* d_fsample, int* d_bin, float* d_dVdxi);
 cudaError_t psg_launch_metad_step(psg_ctx* c, const float* d_pos, float* d_force);   // fused; n_ranges == 0
 bool psg_metad_step_supported(const psg_ctx* c);
+bool psg_abf_step_supported(const psg_ctx* c);
+cudaError_t psg_launch_abf_step(psg_ctx* c, const float* d_pos, const float* d_fsample, float* d_force);   // fused ABF step
 bool psg_range_step_supported(const psg_ctx* c, const float* d_pos, const float* d_force);
 cudaError_t psg_launch_range_step(psg_ctx* c, const float* d_pos, float* d_force);   // fused harmonic step over range groups
 size_t psg_hill_part_doubles(const psg_ctx* c, int* max_chunks_out, int* n_rtiles_out);

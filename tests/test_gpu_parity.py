@@ -528,6 +528,47 @@ def test_fused_range_step_is_cuda_graph_capturable(torch, psg):
     assert np.array_equal(d_f.cpu().numpy(), ref.cpu().numpy())
 
 
+@pytest.mark.parametrize("R,N", [(300, 700), (4100, 64), (1, 30)])
+def test_fused_abf_step_equals_unfused_calls(torch, psg, R, N):
+    """the one-launch ABF step (CVs -> grid update -> grid barrier -> mean force -> scatter) against the four
+    separate calls: xi, bins, dV/dxi inputs and histogram are identical; Fsum and forces differ only by the order
+    of the float atomics; R = 4100 makes every warp loop over several replicas"""
+    w = W.make(2, R=R, N=N, steps=3)
+    f0 = w.forces0()
+    res = []
+    for fused in (True, False):
+        ctx = make_ctx(psg, w)
+        d_f = dev(torch, f0)
+        for step in (1, 2, 3):
+            d_pos, d_fs = dev(torch, w.positions(step % w.K)), dev(torch, w.fsample(step % w.K))
+            n0 = ctx.launch_count()
+            if fused:
+                ctx.step(d_pos, d_f, d_fs, step)
+                o = ctx.read_step_outputs()
+                xi, b, dV = o["xi"], o["bin"], o["dVdxi"]
+                assert ctx.launch_count() - n0 == 1, "the ABF step must be ONE launch"
+            else:
+                xi, b, dV = (torch.empty((w.R, 2), device="cuda"), torch.empty(w.R, dtype=torch.int32, device="cuda"),
+                             torch.empty((w.R, 2), device="cuda"))
+                ctx.cv_eval(d_pos, xi, None)
+                ctx.abf_update(xi, d_fs, b, dV)
+                ctx.apply_bias_forces(d_pos, dV, d_f)
+        ctx.sync_check()
+        hp, fp, nb = ctx.abf_state()
+        from paper_2301_04835_b200.psg import _view
+        hist = _view(hp, (nb,), torch.int32, 0).cpu().numpy().copy()
+        fsum = _view(fp, (nb, 2), torch.float32, 0).cpu().numpy().copy()
+        res.append([xi.cpu().numpy(), b.cpu().numpy(), dV.cpu().numpy(), d_f.cpu().numpy(), hist, fsum])
+    a, c = res
+    assert np.array_equal(a[0].view(np.uint32), c[0].view(np.uint32)), "xi"
+    assert np.array_equal(a[1], c[1]), "bins"
+    assert np.array_equal(a[4], c[4]), "histogram"
+    assert np.allclose(a[5], c[5], rtol=2e-6, atol=1e-4), "Fsum"
+    assert np.allclose(a[2], c[2], rtol=2e-6, atol=1e-6), "dV/dxi"
+    assert np.allclose(a[3], c[3], rtol=1e-5, atol=1e-4), "forces"
+    assert np.array_equal(a[3][..., 3].view(np.uint32), f0[..., 3].view(np.uint32))
+
+
 def test_internal_cv_forces_have_no_net_force_or_torque(torch, psg):
     """sum_i F_i = 0 and sum_i r_i x F_i = 0 for internal CVs (BASELINE.json), on the GPU forces themselves"""
     w = small(1, stride=0)
