@@ -116,6 +116,23 @@ def algorithmic_hill_evals(w, K):
     return float((w.R * (n0 + (s // stride) * w.R)).sum())
 
 
+# ------------------------------------------------------------------------------------------ multi-rank plumbing
+def max_over_ranks(times_ms, world, device):
+    """element-wise MAX over ranks of a list of per-rank times (the slowest rank defines the job's time)"""
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor(list(times_ms), dtype=torch.float64, device=device)
+    if world > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return t.tolist()
+
+
+def whole_job_value(units_per_rank, world, ms):
+    """replicas are sharded by rank with no data-path collective: weak scaling, the job
+    processed world x units_per_rank units in the time of its slowest rank"""
+    return float(units_per_rank) * world / (ms * 1e-3)
+
+
 # ------------------------------------------------------------------------------------------ psg arm
 def run_psg(args, rank, world):
     import torch
@@ -222,15 +239,12 @@ def run_psg(args, rank, world):
     d2h = h_force.numel() * 4
 
     # ---- max over ranks
-    t = torch.tensor([ms_total, ms_b2b, ms_e2e], dtype=torch.float64, device=dev)
-    if world > 1:
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-    ms_total, ms_b2b, ms_e2e = t.tolist()
+    ms_total, ms_b2b, ms_e2e = max_over_ranks([ms_total, ms_b2b, ms_e2e], world, dev)
 
     out = None
     if rank == 0:
         units = float(w.R) * K * world
-        value = units / (ms_total * 1e-3)
+        value = whole_job_value(float(w.R) * K, world, ms_total)
         out = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": Wm,
                "ms_per_step": ms_total / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
                "dtype": "f32", "data": "synthetic",

@@ -1,0 +1,56 @@
+"""N > 1 plumbing of bench.py on CPU (gloo, world_size 2): the path shards replicas by rank with no data-path
+collective, so the only cross-rank logic is the max-over-ranks timing, the whole-job value,
+and the rule that rank 0 alone prints the line of the reference arm."""
+import json
+import os
+import subprocess
+import sys
+
+import pytest
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+_WORKER = r"""
+import os, sys, json
+sys.path.insert(0, {root!r})
+import torch, torch.distributed as dist
+import bench
+rank, world = int(os.environ["RANK"]), int(os.environ["WORLD_SIZE"])
+dist.init_process_group("gloo")
+mine = [10.0 + 5.0 * rank, 3.0 - rank, 7.0]            # rank 1 is slower on the first, faster on the second
+red = bench.max_over_ranks(mine, world, torch.device("cpu"))
+dist.barrier()
+if rank == 0:
+    print(json.dumps({{"red": red, "value": bench.whole_job_value(512 * 100, world, red[0])}}))
+dist.destroy_process_group()
+"""
+
+
+def _torchrun(args, timeout=300):
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", "--nproc-per-node", "2", "--master-addr", "127.0.0.1",
+           "--master-port", "29731"] + args
+    env = dict(os.environ, OMP_NUM_THREADS="2")
+    return subprocess.run(cmd, cwd=ROOT, env=env, capture_output=True, text=True, timeout=timeout)
+
+
+def test_max_over_ranks_and_whole_job_value_gloo(tmp_path):
+    script = tmp_path / "worker.py"
+    script.write_text(_WORKER.format(root=ROOT))
+    p = _torchrun([str(script)])
+    assert p.returncode == 0, p.stderr[-2000:]
+    line = [l for l in p.stdout.splitlines() if l.startswith("{")]
+    assert len(line) == 1, "exactly one rank prints"
+    d = json.loads(line[0])
+    assert d["red"] == [15.0, 3.0, 7.0]
+    assert d["value"] == pytest.approx(2 * 512 * 100 / 15e-3)
+
+
+def test_reference_arm_under_torchrun_prints_one_line_from_rank0():
+    p = _torchrun(["bench.py", "--impl", "reference", "--gpus", "2", "--config", "0", "--steps", "2", "--warmup", "3",
+                   "--ref-budget", "2"])
+    assert p.returncode == 0, p.stderr[-2000:]
+    lines = [l for l in p.stdout.splitlines() if l.startswith("{")]
+    assert len(lines) == 1
+    d = json.loads(lines[0])
+    assert d["impl"] == "reference" and d["n_gpus"] == 2 and d["cpu_baseline"]["kind"] == "oracle"
+    assert d["e2e"]["h2d_bytes_per_step"] == 0 and d["value"] > 0
