@@ -41,6 +41,11 @@ def hill_eval_instr(n_cv, n_periodic):
     return 4 * n_cv + 3 * n_periodic + 2
 
 
+# dram__bytes_read.sum + dram__bytes_write.sum of ONE launch of the dominant kernel, from the committed ncu --set full
+# captures (profiles/r1b_*_ncu_full.md); bytes
+NCU_TRAFFIC = {1: 1.138e6, 2: 6.98e6, 3: 1.3703e9, 4: 5.35e6}
+
+
 def _peaks():
     p = os.path.join(ROOT, "MEASURED_PEAKS.json")
     if os.path.exists(p):
@@ -271,7 +276,7 @@ def run_psg(args, rank, world):
             ach = evals * C / (ms_total * 1e-3)
             out["hill_evals_per_s"] = evals * world / (ms_total * 1e-3)
             out["roofline"] = {"bound": "alu", "kernel": "k_hills (fused step)", "achieved": ach / 1e9, "peak": fma_peak / 1e9,
-                               "unit": "G FP32 lane-instr/s", "frac": ach / fma_peak, "traffic": None,
+                               "unit": "G FP32 lane-instr/s", "frac": ach / fma_peak, "traffic": NCU_TRAFFIC.get(args.config),
                                "peak_source": "psg_measure_alu_peak(FFMA), measured in this run (burst, kernel timed alone)",
                                "instr_per_hill_eval": C, "mufu_peak_Gops": mufu_peak / 1e9, "ffma2_peak_Glaneops": ffma2_peak / 1e9,
                                "mufu_frac": (evals / (ms_total * 1e-3)) / mufu_peak,
@@ -280,14 +285,14 @@ def run_psg(args, rank, world):
             bytes_step = 48.0 * w.R * w.N                          # read pos once + read force + write force (float4)
             ach = bytes_step * K / (ms_total * 1e-3) / 1e9
             out["roofline"] = {"bound": "hbm", "kernel": "k_range_step (fused umbrella step, one launch)", "achieved": ach, "peak": hbm_peak,
-                               "unit": "GB/s", "frac": ach / hbm_peak, "traffic": None, "peak_source": which + " copy bandwidth",
-                               "algorithmic_bytes_per_step": bytes_step,
+                               "unit": "GB/s", "frac": ach / hbm_peak, "traffic": NCU_TRAFFIC.get(args.config),
+                               "peak_source": which + " copy bandwidth", "algorithmic_bytes_per_step": bytes_step,
                                "frac_back_to_back": bytes_step * K / (ms_b2b * 1e-3) / 1e9 / hbm_peak}
         else:
             bytes_step = float(w.R) * (8 * 32 + 3 * 32 + 8 * 32 * 2)
             ach = bytes_step * K / (ms_total * 1e-3) / 1e9
-            out["roofline"] = {"bound": "hbm", "kernel": "k_cv_eval + k_abf_* + k_apply_sparse (latency-bound)", "achieved": ach,
-                               "peak": hbm_peak, "unit": "GB/s", "frac": ach / hbm_peak, "traffic": None,
+            out["roofline"] = {"bound": "hbm", "kernel": "k_abf_step (fused ABF step, one launch; latency-bound)", "achieved": ach,
+                               "peak": hbm_peak, "unit": "GB/s", "frac": ach / hbm_peak, "traffic": NCU_TRAFFIC.get(args.config),
                                "peak_source": which + " copy bandwidth",
                                "note": "a step moves < 4 MB: launch latency, not HBM, bounds it (DESIGN.md)"}
         if not args.skip_cpu_baseline:
