@@ -569,6 +569,38 @@ def test_fused_abf_step_equals_unfused_calls(torch, psg, R, N):
     assert np.array_equal(a[3][..., 3].view(np.uint32), f0[..., 3].view(np.uint32))
 
 
+def test_fused_abf_step_is_cuda_graph_capturable(torch, psg):
+    """the cooperative one-launch ABF step replays from a CUDA graph and leaves its grid barrier re-armed"""
+    w = W.make(2, R=600, N=100, steps=2)
+    s = torch.cuda.Stream()
+    outs = []
+    for graph in (False, True):
+        ctx = psg.Context(0, s)
+        psg.configure_from_workload(ctx, w)
+        d_pos, d_fs = dev(torch, w.positions(0)), dev(torch, w.fsample(0))
+        d_f = torch.zeros((w.R, w.N, 4), device="cuda")
+        torch.cuda.synchronize()
+        if graph:
+            g = torch.cuda.CUDAGraph()
+            with torch.cuda.graph(g, stream=s):
+                ctx.step(d_pos, d_f, d_fs, 1)
+            d_f.zero_()
+            ctx.set_abf(w.params["lower"], w.params["upper"], w.params["shape"], w.params["periodic"], w.params["n_threshold"])
+            torch.cuda.synchronize()
+            for _ in range(3):
+                g.replay()
+        else:
+            with torch.cuda.stream(s):
+                for _ in range(3):
+                    ctx.step(d_pos, d_f, d_fs, 1)
+        torch.cuda.synchronize()
+        hp, fp, nb = ctx.abf_state()
+        from paper_2301_04835_b200.psg import _view
+        outs.append((_view(hp, (nb,), torch.int32, 0).cpu().numpy().copy(), d_f.cpu().numpy()))
+    assert np.array_equal(outs[0][0], outs[1][0]) and outs[0][0].sum() > 0
+    assert np.allclose(outs[0][1], outs[1][1], rtol=1e-5, atol=1e-4)
+
+
 def test_internal_cv_forces_have_no_net_force_or_torque(torch, psg):
     """sum_i F_i = 0 and sum_i r_i x F_i = 0 for internal CVs (BASELINE.json), on the GPU forces themselves"""
     w = small(1, stride=0)
