@@ -9,9 +9,9 @@
 // Moments of range groups. grid = (range_blocks, R); block b covers atoms [span_begin + b*TILE, +TILE).
 // Every atom is loaded once (coalesced float4) and contributes to each range group that contains it.
 // Output: rpart[r][q][b][5] in binary64 (products of binary32 inputs are exact in binary64).
-__global__ void __launch_bounds__(256) k_range_moments(const __grid_constant__ SysParams P, const float* __restrict__ pos,
+__global__ void __launch_bounds__(PSG_RANGE_THREADS) k_range_moments(const __grid_constant__ SysParams P, const float* __restrict__ pos,
                                                         double* __restrict__ rpart) {
-    constexpr int PER = PSG_RANGE_TILE / 256;
+    constexpr int NT = PSG_RANGE_THREADS, PER = PSG_RANGE_TILE / NT;
     const int r = blockIdx.y, b = blockIdx.x, tid = threadIdx.x;
     const float* p = pos + (long long)r * P.rstride * P.ps;
     const long long t0 = P.span_begin + (long long)b * PSG_RANGE_TILE;
@@ -19,7 +19,7 @@ __global__ void __launch_bounds__(256) k_range_moments(const __grid_constant__ S
     long long ai[PER];
 #pragma unroll
     for (int i = 0; i < PER; ++i) {
-        long long a = t0 + tid + (long long)i * 256;
+        long long a = t0 + tid + (long long)i * NT;
         ai[i] = a;
         x[i] = y[i] = z[i] = w[i] = 0.f;
         if (a < P.span_end) {
@@ -32,7 +32,7 @@ __global__ void __launch_bounds__(256) k_range_moments(const __grid_constant__ S
             w[i] = P.atom_weight ? __ldg(P.atom_weight + a) : 1.f;
         }
     }
-    __shared__ double red[8][PSG_MOM];
+    __shared__ double red[NT / 32][PSG_MOM];
     for (int q = 0; q < P.n_ranges; ++q) {
         const GroupDev& G = P.grp[P.range_gid[q]];
         const long long gb = G.rbegin, ge = G.rbegin + G.rsize;
@@ -58,7 +58,7 @@ __global__ void __launch_bounds__(256) k_range_moments(const __grid_constant__ S
         if (tid < PSG_MOM) {
             double s = 0;
 #pragma unroll
-            for (int wq = 0; wq < 8; ++wq) s += red[wq][tid];
+            for (int wq = 0; wq < NT / 32; ++wq) s += red[wq][tid];
             rpart[(((long long)r * P.n_ranges + q) * P.range_blocks + b) * PSG_MOM + tid] = s;
         }
     }
@@ -188,7 +188,7 @@ cudaError_t psg_launch_cv_eval(psg_ctx* c, const float* d_pos, float* d_xi, floa
     const SysParams& P = c->sys;
     if (P.n_ranges > 0) {
         dim3 g(P.range_blocks, P.R);
-        k_range_moments<<<g, 256, 0, c->stream>>>(P, d_pos, c->d_rpart);
+        k_range_moments<<<g, PSG_RANGE_THREADS, 0, c->stream>>>(P, d_pos, c->d_rpart);
         c->launches++;
     }
     k_cv_eval<<<(P.R + 7) / 8, 256, 0, c->stream>>>(P, d_pos, c->d_rpart, d_xi, d_jac, c->d_jac, c->d_gdesc);

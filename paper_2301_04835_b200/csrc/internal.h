@@ -11,6 +11,7 @@
 #define PSG_GDESC_DOUBLES 8      // per (replica, group): vx vy vz | cx cy cz | coef | W
 #define PSG_MOM 5                // moments per range group: W, sum w x, sum w y, sum w z, sum w |r|^2
 #define PSG_RANGE_TILE 2048      // atoms per block / slice in the range-moment, dense-apply and fused range-step kernels
+#define PSG_RANGE_THREADS 256    // threads that reduce one slice's moments (k_range_moments block = A group of k_range_step: same thread -> atom map, same bits)
 #define PSG_HILL_RT 8            // replicas per thread in the hill sum
 #define PSG_HILL_WARPS 8         // warps per CTA in the hill sum
 #define PSG_HILL_TILE_R (PSG_HILL_RT * PSG_HILL_WARPS)   // replicas per CTA tile (64)

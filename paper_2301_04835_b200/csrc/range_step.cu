@@ -34,7 +34,7 @@
 #define RS_BSTAGES 2              // ring B: positions + forces
 #define RS_RED 4                  // ring of per-warp partial moments between the A group and the T warps
 #define RS_NT 2                   // T warps
-#define RS_GT 256                 // threads of the A group (fixes the reduction order: same map as k_range_moments)
+#define RS_GT PSG_RANGE_THREADS   // threads of the A group (256; fixes the reduction order: same map as k_range_moments)
 #define RS_GTB 512                // threads of the B group
 #define RS_LEAD (32 * (3 + RS_NT))   // PA, PB, W, T warps
 #define RS_THREADS (RS_LEAD + RS_GT + RS_GTB)
@@ -110,11 +110,14 @@ __device__ __forceinline__ float4 rs_ld_relaxed_f4(const float4* p) {   // one 1
 
 #ifdef PSG_TRACE
 // debug builds: cycles each role spends waiting, summed over the launch, [grid][16] (lane 0 / thread 0 of the role)
+__device__ __forceinline__ long long rs_gt() { long long t; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t)); return t; }
+#define RS_GSTAMP(cond, i) do { if ((cond) && A.trace) A.trace[blockIdx.x * 32 + (i)] = rs_gt(); } while (0)
 #define RS_T0 long long rs_t0_ = clock64()
 #define RS_ACC(slot) do { rs_acc_[slot] += clock64() - rs_t0_; } while (0)
 #define RS_DECL long long rs_acc_[3] = {0, 0, 0}; const long long rs_start_ = clock64()
 #define RS_FLUSH(cond, base) do { if ((cond) && A.trace) { for (int z_ = 0; z_ < 3; ++z_) A.trace[blockIdx.x * 32 + (base) + z_] = rs_acc_[z_]; A.trace[blockIdx.x * 32 + (base) + 3] = clock64() - rs_start_; } } while (0)
 #else
+#define RS_GSTAMP(cond, i) do { } while (0)
 #define RS_T0 do { } while (0)
 #define RS_ACC(slot) do { } while (0)
 #define RS_DECL do { } while (0)
@@ -143,8 +146,11 @@ struct RsItem {
 };
 __device__ __forceinline__ RsItem rs_item(const SysParams& P, long long it, long long G) {
     RsItem I;
-    const long long j = blockIdx.x + it * G;
-    I.r = (int)(j / P.range_blocks); I.s = (int)(j % P.range_blocks);
+    // R <= 65535 and range_blocks <= grid, so the item index fits 32 bits: one 32-bit division, not two 64-bit ones
+    const unsigned j = (unsigned)(blockIdx.x + it * G);
+    const unsigned nb = (unsigned)P.range_blocks;
+    const unsigned r = j / nb;
+    I.r = (int)r; I.s = (int)(j - r * nb);
     const long long b = P.span_begin + (long long)I.s * RS_SLICE;
     I.a0 = (long long)I.r * P.rstride + b;
     long long cnt = P.span_end - b;
@@ -412,18 +418,16 @@ __device__ __forceinline__ void rs_phase_b(const SysParams& P, const RangeStepAr
     if (S.bfast && !P.atom_weight) {
         // the common case, straight-line: a whole slice, every group either covers all of it or none of it, unit
         // weights (x * 1.0f is x: same bits as the general loop)
-        float4 p[RS_PERB];
-#pragma unroll
-        for (int i = 0; i < RS_PERB; ++i) p[i] = sp[tid + i * RS_GTB];
         for (int q = 0; q < P.n_ranges; ++q) {
             if (S.blo[q] >= S.bhi[q]) continue;   // uniform
             const float4 v = S.desc[q][0], hi = S.desc[q][1], lo = S.desc[q][2];
             const float k = S.desc[q][3].x;
 #pragma unroll
             for (int i = 0; i < RS_PERB; ++i) {
-                ax[i] += v.x + k * ((p[i].x - hi.x) - lo.x);
-                ay[i] += v.y + k * ((p[i].y - hi.y) - lo.y);
-                az[i] += v.z + k * ((p[i].z - hi.z) - lo.z);
+                const float4 p = sp[tid + i * RS_GTB];   // re-read per group: registers are the scarce resource
+                ax[i] += v.x + k * ((p.x - hi.x) - lo.x);
+                ay[i] += v.y + k * ((p.y - hi.y) - lo.y);
+                az[i] += v.z + k * ((p.z - hi.z) - lo.z);
             }
         }
 #pragma unroll
@@ -475,6 +479,7 @@ __global__ void __launch_bounds__(RS_THREADS, 1) k_range_step(const __grid_const
     const long long G = gridDim.x;
     const long long n_mine = blockIdx.x < items ? (items - blockIdx.x + G - 1) / G : 0;
 
+    RS_GSTAMP(tid == 0, 31);
     if (tid == 0) {
         for (int st = 0; st < RS_ASTAGES; ++st) { rs_mbar_init(&S.a_full[st], 1); rs_mbar_init(&S.a_empty[st], RS_GT / 32); }
         for (int st = 0; st < RS_BSTAGES; ++st) { rs_mbar_init(&S.b_full[st], 1); rs_mbar_init(&S.b_empty[st], RS_GTB / 32); }
@@ -562,6 +567,7 @@ __global__ void __launch_bounds__(RS_THREADS, 1) k_range_step(const __grid_const
             }
         }
         RS_FLUSH(t == 0, 16);
+        RS_GSTAMP(t == 0, 26);
     } else {
         // ---------------- B group
         const int t = tid - RS_LEAD - RS_GT;
@@ -571,6 +577,8 @@ __global__ void __launch_bounds__(RS_THREADS, 1) k_range_step(const __grid_const
             const RsItem I = rs_item(P, it, G);
             const float4* sp = ring_b + (size_t)st * 2 * RS_SLICE;
             { RS_T0; rs_mbar_wait(&S.b_full[st], (uint32_t)((it / RS_BSTAGES) & 1)); RS_ACC(0); }
+            RS_GSTAMP(t == 0 && it == 0, 27);
+            RS_GSTAMP(t == 0 && it == n_mine / 2, 14);
             { RS_T0; rs_phase_b(P, A, S, sp, sp + RS_SLICE, I, t); RS_ACC(1); }
             __syncwarp();
             if ((t & 31) == 0) rs_mbar_arrive(&S.b_empty[st]);   // this warp is done reading the stage
@@ -587,6 +595,7 @@ __global__ void __launch_bounds__(RS_THREADS, 1) k_range_step(const __grid_const
             }
         }
         RS_FLUSH(t == 0, 20);
+        RS_GSTAMP(t == 0, 30);
     }
 }
 
@@ -630,9 +639,9 @@ cudaError_t psg_launch_range_step(psg_ctx* c, const float* d_pos, float* d_force
     A.xi_out = c->d_xi; A.V_out = c->d_V; A.V64_out = c->d_V64; A.dV_out = c->d_dVdxi;
     A.rpart = c->d_rpart; A.arrive = c->d_arrive; A.done = c->d_arrive + P.R; A.desc = c->d_rdesc;
     // B runs `lag` items behind A: long enough to cover the window dependency (several L2 round trips), short
-    // enough that lag x grid x 32 KB of positions stays in L2 (12 x 148 x 32 KB = 57 MB of 126 MB)
+    // enough that lag x grid x 32 KB of positions stays in L2 (10 x 148 x 32 KB = 47 MB of 126 MB; measured optimum)
     static const int lag_env = getenv("PSG_RANGE_LAG") ? atoi(getenv("PSG_RANGE_LAG")) : 0;
-    A.lag = lag_env > 0 ? lag_env : 12;
+    A.lag = lag_env > 0 ? lag_env : 10;
 #ifdef PSG_TRACE
     A.trace = psg_trace_buffer();
 #endif
