@@ -134,6 +134,8 @@ struct RsShared {
     float4 desc[PSG_MAX_RANGE_GROUPS][RS_DESC];                   // B group: the window's force descriptors
     int blo[PSG_MAX_RANGE_GROUPS], bhi[PSG_MAX_RANGE_GROUPS];     // B group: slice-local atom bounds of every group
     int bfast;                                                    // B group: the item takes the straight-line path
+    long long g_b[PSG_MAX_RANGE_GROUPS], g_e[PSG_MAX_RANGE_GROUPS];   // atom range of every range group (copied once from the
+                                                                  // kernel parameters)
     uint64_t a_full[RS_ASTAGES], a_empty[RS_ASTAGES], b_full[RS_BSTAGES], b_empty[RS_BSTAGES];
     uint64_t red_full[RS_RED], red_empty[RS_RED];
     volatile long long b_prog;                  // items the B group has finished
@@ -284,8 +286,7 @@ __device__ __forceinline__ void rs_phase_a(const SysParams& P, RsShared& S, cons
     bool have_full = false;           // moments over the WHOLE slice, shared by every group that contains it
     double mf[PSG_MOM] = {0, 0, 0, 0, 0};
     for (int q = 0; q < P.n_ranges; ++q) {
-        const GroupDev& G = P.grp[P.range_gid[q]];
-        const long long gb = G.rbegin, ge = G.rbegin + G.rsize;
+        const long long gb = S.g_b[q], ge = S.g_e[q];
         double m[PSG_MOM] = {0, 0, 0, 0, 0};
         if (t0 < ge && t1 > gb) {     // uniform over the group
             const bool inside = gb <= t0 && t1 <= ge;
@@ -381,9 +382,8 @@ __device__ __forceinline__ void rs_phase_b(const SysParams& P, const RangeStepAr
     }
     if (tid >= 32 && tid < 32 + P.n_ranges) {
         // slice-local bounds of every group: the atom loop compares 32-bit offsets held in shared memory
-        const GroupDev& G = P.grp[P.range_gid[tid - 32]];
         const long long t0 = P.span_begin + (long long)I.s * RS_SLICE;
-        long long lo = G.rbegin - t0, hi = G.rbegin + G.rsize - t0;
+        long long lo = S.g_b[tid - 32] - t0, hi = S.g_e[tid - 32] - t0;
         const long long cnt = (long long)(I.bytes >> 4);
         if (lo < 0) lo = 0;
         if (hi > cnt) hi = cnt;
@@ -396,8 +396,7 @@ __device__ __forceinline__ void rs_phase_b(const SysParams& P, const RangeStepAr
         const long long t1 = t0 + (long long)(I.bytes >> 4);
         bool fast = (I.bytes >> 4) == RS_SLICE, any = false;
         for (int q = 0; q < P.n_ranges; ++q) {
-            const GroupDev& G = P.grp[P.range_gid[q]];
-            const long long gb = G.rbegin, ge = G.rbegin + G.rsize;
+            const long long gb = S.g_b[q], ge = S.g_e[q];
             const bool touch = t0 < ge && t1 > gb, cover = gb <= t0 && t1 <= ge;
             if (touch && !cover) fast = false;
             any |= cover;
@@ -485,6 +484,10 @@ __global__ void __launch_bounds__(RS_THREADS, 1) k_range_step(const __grid_const
         for (int st = 0; st < RS_BSTAGES; ++st) { rs_mbar_init(&S.b_full[st], 1); rs_mbar_init(&S.b_empty[st], RS_GTB / 32); }
         for (int b = 0; b < RS_RED; ++b) { rs_mbar_init(&S.red_full[b], RS_GT / 32); rs_mbar_init(&S.red_empty[b], 1); }
         S.b_prog = 0;
+        for (int q = 0; q < P.n_ranges; ++q) {
+            const GroupDev& G = P.grp[P.range_gid[q]];
+            S.g_b[q] = G.rbegin; S.g_e[q] = G.rbegin + G.rsize;
+        }
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     __syncthreads();
