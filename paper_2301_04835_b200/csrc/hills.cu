@@ -107,7 +107,7 @@ extern "C" int psg_debug_trace(long long* host_out, int n_ctas) {
     return (int)cudaMemcpy(host_out, psg_trace_buffer(), (size_t)n_ctas * 8 * sizeof(long long), cudaMemcpyDeviceToHost);
 }
 #endif
-static int hills_grid(const psg_ctx* c) { return c->sm_count * 2; }
+static int hills_grid(const psg_ctx* c) { return c->sm_count; }   // one 16-warp CTA per SM
 
 size_t psg_hill_part_doubles(const psg_ctx* c, int* max_chunks_out, int* n_rtiles_out) {
     int n_rt = (c->sys.R + TILE_R - 1) / TILE_R;
@@ -115,17 +115,16 @@ size_t psg_hill_part_doubles(const psg_ctx* c, int* max_chunks_out, int* n_rtile
     if (cpt < 1) cpt = 1;
     if (max_chunks_out) *max_chunks_out = cpt;
     if (n_rtiles_out) *n_rtiles_out = n_rt;
-    return (size_t)cpt * n_rt * TILE_R * (1 + PSG_MAX_CV);
+    return (size_t)cpt * 2 * n_rt * TILE_R * (1 + PSG_MAX_CV);   // one partial per (chunk, warp half)
 }
 
 static cudaError_t launch_hills(psg_ctx* c, HillKernelArgs& A) {
     const int n_cv = c->sys.n_cv;
     const bool fused = A.fused != 0;
-    // stages: as many as still let two CTAs share an SM (227 KB, 1 KB reserved per CTA); else 3 stages, one CTA
+    // stages: up to 3, as many as fit the SM's 227 KB (1 KB reserved per CTA) beside the binary64 accumulators
     int stages = 3;
-    for (; stages >= 1; --stages)
-        if (2 * (hills_smem_bytes(n_cv, stages, c->sys.n_groups, fused) + 1024) <= 227 * 1024) break;
-    if (stages < 1) stages = 3;
+    for (; stages > 1; --stages)
+        if (hills_smem_bytes(n_cv, stages, c->sys.n_groups, fused) + 1024 <= 227 * 1024) break;
     A.stages = stages;
     const size_t smem = hills_smem_bytes(n_cv, stages, c->sys.n_groups, fused);
     const int grid = hills_grid(c);

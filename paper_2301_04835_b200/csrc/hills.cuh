@@ -4,9 +4,11 @@
 //   d_hk = nearest image of xi_k - s_hk.
 // Not a dense contraction (the wrap breaks bilinearity; the exp dominates): FP32-pipe + MUFU work, no tensor cores.
 //
-// Decomposition. CTA = (tile of 64 replicas) x (chunk of hills); 8 warps, warp w owns 8 replicas whose xi sit in
-// registers as 4 packed f32x2 pairs; its 32 lanes stride over the hills of the chunk, which is streamed through
-// shared memory by 1-D TMA bulk copies (cp.async.bulk + mbarrier). One LDS.128 hill record feeds 8 evaluations.
+// Decomposition. CTA = (tile of 64 replicas) x (chunk of hills); ONE CTA of 16 warps per SM. Warps w and w + 8 own the
+// same 8 replicas, whose xi sit in registers as 4 packed f32x2 pairs; the 64 lanes of the pair stride over the hills of
+// the chunk, which is streamed through shared memory by 1-D TMA bulk copies (cp.async.bulk + mbarrier). One LDS.128
+// hill record feeds 8 evaluations. (Two independent 8-warp CTAs per SM were measured to run unevenly -- the scheduler favours one,
+// which finishes at half time -- with the same total time; one 16-warp CTA per SM ends all its warps together.)
 // All arithmetic of an evaluation is PACKED binary32 (FADD2/FMUL2/FFMA2: two replicas per instruction), which
 // halves the issue slots per evaluation and leaves the FMA pipe as the only bound:
 //     per periodic dim  d = xi - s; t = d/P + M; k = t - M; d -= k P_hi; d -= k P_lo   (5)
@@ -24,6 +26,9 @@
 #define HWARPS PSG_HILL_WARPS
 #define TILE_R PSG_HILL_TILE_R
 #define SUB PSG_HILL_SUB
+#ifndef PSG_HILL_UNROLL
+#define PSG_HILL_UNROLL 2
+#endif
 #define MAGIC_RN 12582912.0f   // 1.5 * 2^23: (x + M) - M = rint(x) for |x| < 2^22
 
 typedef unsigned long long u64;
@@ -158,21 +163,23 @@ struct HillBody {
     }
 };
 
-// binary32 terms over one shared-memory sub-tile: lanes stride the hills; full groups of 32 run unpredicated
+// binary32 terms over one shared-memory sub-tile: the 64 lanes of a warp pair stride the hills; full groups of 64 run unpredicated
 template <int NCV, int PM, int NEQ>
-__device__ __forceinline__ void accumulate_f32(const float4* __restrict__ sm, int n_sub, int lane, const u64 (&X)[RT / 2][NCV],
+__device__ __forceinline__ void accumulate_f32(const float4* __restrict__ sm, int n_sub, int off, const u64 (&X)[RT / 2][NCV],
                                                const HillConsts& hc, u64 (&a32)[RT / 2][1 + NCV]) {
+    // off = lane + 32 * half in [0, 64): this thread takes hills off, off + 64, ...
     const HillBody<NCV, PM, NEQ> body(hc);
-    const int n_full = n_sub >> 5;
-#pragma unroll 2
-    for (int i = 0; i < n_full; ++i) body(sm, lane + 32 * i, X, a32);
-    if (lane + 32 * n_full < n_sub) body(sm, lane + 32 * n_full, X, a32);
+    const int n_full = n_sub >> 6;
+    constexpr int UNR = PSG_HILL_UNROLL;
+#pragma unroll UNR
+    for (int i = 0; i < n_full; ++i) body(sm, off + 64 * i, X, a32);
+    if (off + 64 * n_full < n_sub) body(sm, off + 64 * n_full, X, a32);
 }
 
 // binary64 terms (PSG_HILLS_F64): the definition, evaluated in double on the FP64 pipe; heights read from the
 // exported height array (global). Accumulates straight into the thread's binary64 slots.
 template <int NCV>
-__device__ __forceinline__ void accumulate_f64(const float4* __restrict__ sm, const float* __restrict__ W, int n_sub, int lane,
+__device__ __forceinline__ void accumulate_f64(const float4* __restrict__ sm, const float* __restrict__ W, int n_sub, int off,
                                                const float (&xi)[RT][NCV], const HillConsts& hc, double* __restrict__ acc,
                                                int acc_stride) {
     constexpr int NV = 1 + NCV;
@@ -182,7 +189,7 @@ __device__ __forceinline__ void accumulate_f64(const float4* __restrict__ sm, co
         for (int jj = 0; jj < 2; ++jj)
 #pragma unroll
             for (int v = 0; v < NV; ++v) a[jj][v] = 0.0;
-        for (int h = lane; h < n_sub; h += 32) {
+        for (int h = off; h < n_sub; h += 64) {
             float s[NCV], lw;
             load_rec<NCV>(sm, h, s, lw);
             const double w = (double)__ldg(W + h);
@@ -268,7 +275,7 @@ struct HillKernelArgs {
 #endif
 };
 #ifdef PSG_TRACE
-#define PSG_STAMP(i) do { if (threadIdx.x == 0 && item == (int)blockIdx.x && A.trace) A.trace[blockIdx.x * 8 + (i)] = clock64(); } while (0)
+#define PSG_STAMP(i) do { if (threadIdx.x == 0 && item == (int)blockIdx.x && A.trace) { long long t_; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t_)); A.trace[blockIdx.x * 8 + (i)] = t_; } } while (0)
 #else
 #define PSG_STAMP(i) do { } while (0)
 #endif
@@ -286,7 +293,7 @@ __host__ __device__ inline size_t hills_smem_bytes(int n_cv, int stages, int n_g
 
 // One kernel for psg_bias_eval and the whole metadynamics step (A.fused).
 template <int NCV, int PM, int NEQ, bool F64>
-__global__ void __launch_bounds__(HWARPS * 32, 2) k_hills(const __grid_constant__ SysParams P, const __grid_constant__ HillConsts hc,
+__global__ void __launch_bounds__(HWARPS * 32, 1) k_hills(const __grid_constant__ SysParams P, const __grid_constant__ HillConsts hc,
                                                            const __grid_constant__ HillKernelArgs A) {
     constexpr int REC = NCV <= 3 ? 1 : 2;
     constexpr int NV = 1 + NCV;
@@ -302,6 +309,7 @@ __global__ void __launch_bounds__(HWARPS * 32, 2) k_hills(const __grid_constant_
     __shared__ int s_last;
 
     const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
+    const int half = wid >> 3, w8 = wid & 7;   // warps w8 and w8 + 8 own the same replicas; half picks the hills
     const int R = A.R;
     const int n_rt = (R + TILE_R - 1) / TILE_R;
     const int n_h = A.n_h_host >= 0 ? A.n_h_host : *A.n_hills;
@@ -371,14 +379,14 @@ __global__ void __launch_bounds__(HWARPS * 32, 2) k_hills(const __grid_constant_
         }
         __syncthreads();
         PSG_STAMP(1);
-        const bool warp_active = r0 + wid * RT < R;
+        const bool warp_active = r0 + w8 * RT < R;
         if (!F64) {
             u64 X[RT / 2][NCV], a32[RT / 2][NV];
 #pragma unroll
             for (int p = 0; p < RT / 2; ++p) {
 #pragma unroll
                 for (int k = 0; k < NCV; ++k)
-                    X[p][k] = *reinterpret_cast<const u64*>(s_xi + k * TILE_R + wid * RT + 2 * p);   // {xi[2p][k], xi[2p+1][k]}
+                    X[p][k] = *reinterpret_cast<const u64*>(s_xi + k * TILE_R + w8 * RT + 2 * p);   // {xi[2p][k], xi[2p+1][k]}
 #pragma unroll
                 for (int v = 0; v < NV; ++v) a32[p][v] = 0ull;
             }
@@ -386,9 +394,9 @@ __global__ void __launch_bounds__(HWARPS * 32, 2) k_hills(const __grid_constant_
                 int s = seq % STG;
                 mbar_wait(&full[s], (seq / STG) & 1);
                 int cnt = min(SUB, len - t * SUB);
-                if (warp_active) accumulate_f32<NCV, PM, NEQ>(stage + s * SUB * REC, cnt, lane, X, hc, a32);
-                if (warp_active && ((t & 1) || t == n_st - 1)) {
-                    // flush the binary32 partial sums (<= 64 hills per lane) into the binary64 slots
+                if (warp_active) accumulate_f32<NCV, PM, NEQ>(stage + s * SUB * REC, cnt, lane + 32 * half, X, hc, a32);
+                if (warp_active && ((t & 3) == 3 || t == n_st - 1)) {
+                    // flush the binary32 partial sums (<= 64 hills per lane: 4 sub-tiles of 16) into the binary64 slots
 #pragma unroll
                     for (int p = 0; p < RT / 2; ++p)
 #pragma unroll
@@ -414,13 +422,13 @@ __global__ void __launch_bounds__(HWARPS * 32, 2) k_hills(const __grid_constant_
 #pragma unroll
             for (int j = 0; j < RT; ++j)
 #pragma unroll
-                for (int k = 0; k < NCV; ++k) xi[j][k] = s_xi[k * TILE_R + wid * RT + j];
+                for (int k = 0; k < NCV; ++k) xi[j][k] = s_xi[k * TILE_R + w8 * RT + j];
             for (int t = 0; t < n_st; ++t) {
                 int s = seq % STG;
                 mbar_wait(&full[s], (seq / STG) & 1);
                 int cnt = min(SUB, len - t * SUB);
                 if (warp_active)
-                    accumulate_f64<NCV>(stage + s * SUB * REC, A.heights + h0 + t * SUB, cnt, lane, xi, hc, s_acc + tid, NT);
+                    accumulate_f64<NCV>(stage + s * SUB * REC, A.heights + h0 + t * SUB, cnt, lane + 32 * half, xi, hc, s_acc + tid, NT);
                 __syncthreads();
                 if (tid == 0 && t + STG < n_st) {
                     int cn = min(SUB, len - (t + STG) * SUB);
@@ -435,7 +443,7 @@ __global__ void __launch_bounds__(HWARPS * 32, 2) k_hills(const __grid_constant_
         // lanes -> warp totals through the shared accumulators: lane v (< RT*NV) sums value v over the 32 lanes
         // (rotated start => no bank conflicts; the order is fixed per lane => deterministic)
         __syncwarp();
-        double* dst = A.part + ((size_t)(chunk * n_rt + tile) * TILE_R + wid * RT) * NV;
+        double* dst = A.part + ((size_t)((chunk * 2 + half) * n_rt + tile) * TILE_R + w8 * RT) * NV;   // one partial per (chunk, half)
         for (int v = lane; v < RT * NV; v += 32) {
             const double* src = s_acc + v * NT + wid * 32;
             double sum = 0.0;
@@ -459,7 +467,7 @@ __global__ void __launch_bounds__(HWARPS * 32, 2) k_hills(const __grid_constant_
                 const size_t cstride = (size_t)n_rt * TILE_R * NV;
                 double sum = 0.0;
 #pragma unroll 8
-                for (int c = 0; c < n_chunks; ++c) sum += __ldcg(src + c * cstride);
+                for (int c = 0; c < 2 * n_chunks; ++c) sum += __ldcg(src + c * cstride);
                 int v = t % NV;
                 if (v > 0) sum *= -hc.gscale[v - 1];
                 s_out[t] = sum;

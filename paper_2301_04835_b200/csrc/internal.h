@@ -13,8 +13,8 @@
 #define PSG_RANGE_TILE 2048      // atoms per block / slice in the range-moment, dense-apply and fused range-step kernels
 #define PSG_RANGE_THREADS 256    // threads that reduce one slice's moments (k_range_moments block = A group of k_range_step: same thread -> atom map, same bits)
 #define PSG_HILL_RT 8            // replicas per thread in the hill sum
-#define PSG_HILL_WARPS 8         // warps per CTA in the hill sum
-#define PSG_HILL_TILE_R (PSG_HILL_RT * PSG_HILL_WARPS)   // replicas per CTA tile (64)
+#define PSG_HILL_WARPS 16        // warps per CTA in the hill sum: two halves of 8 warps share the tile's replicas and split its hills
+#define PSG_HILL_TILE_R (PSG_HILL_RT * 8)   // replicas per CTA tile (64): warp w and warp w + 8 own the same 8 replicas
 #define PSG_HILL_SUB 1024        // hills per shared-memory stage
 
 struct CvDev {
