@@ -115,7 +115,7 @@ size_t psg_hill_part_doubles(const psg_ctx* c, int* max_chunks_out, int* n_rtile
     if (cpt < 1) cpt = 1;
     if (max_chunks_out) *max_chunks_out = cpt;
     if (n_rtiles_out) *n_rtiles_out = n_rt;
-    return (size_t)cpt * 2 * n_rt * TILE_R * (1 + PSG_MAX_CV);   // one partial per (chunk, warp half)
+    return (size_t)cpt * n_rt * TILE_R * (1 + PSG_MAX_CV);
 }
 
 static cudaError_t launch_hills(psg_ctx* c, HillKernelArgs& A) {

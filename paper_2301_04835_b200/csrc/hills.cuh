@@ -26,9 +26,6 @@
 #define HWARPS PSG_HILL_WARPS
 #define TILE_R PSG_HILL_TILE_R
 #define SUB PSG_HILL_SUB
-#ifndef PSG_HILL_UNROLL
-#define PSG_HILL_UNROLL 2
-#endif
 #define MAGIC_RN 12582912.0f   // 1.5 * 2^23: (x + M) - M = rint(x) for |x| < 2^22
 
 typedef unsigned long long u64;
@@ -170,8 +167,7 @@ __device__ __forceinline__ void accumulate_f32(const float4* __restrict__ sm, in
     // off = lane + 32 * half in [0, 64): this thread takes hills off, off + 64, ...
     const HillBody<NCV, PM, NEQ> body(hc);
     const int n_full = n_sub >> 6;
-    constexpr int UNR = PSG_HILL_UNROLL;
-#pragma unroll UNR
+#pragma unroll 2
     for (int i = 0; i < n_full; ++i) body(sm, off + 64 * i, X, a32);
     if (off + 64 * n_full < n_sub) body(sm, off + 64 * n_full, X, a32);
 }
@@ -217,6 +213,7 @@ __device__ __forceinline__ void accumulate_f64(const float4* __restrict__ sm, co
 }
 
 // lane-local CV of (replica r, CV k) for systems with explicit groups only; dc[g] = d xi / d c_g / W_g.
+template <bool JAC>
 __device__ __forceinline__ double thread_cv(const SysParams& P, int r, int k, const float* __restrict__ pos, D3* dc) {
     const CvDev& C = P.cv[k];
     const float* p = pos + (long long)r * P.rstride * P.ps;
@@ -246,10 +243,12 @@ __device__ __forceinline__ double thread_cv(const SysParams& P, int r, int k, co
             }
         }
     }
-    double xi = cv_from_centers<true>(C.type, C.axis, c, dc);
+    double xi = cv_from_centers<JAC>(C.type, C.axis, c, dc);
+    if (JAC) {
 #pragma unroll
-    for (int g = 0; g < 4; ++g)
-        if (W[g] != 1.0) dc[g] = (1.0 / W[g]) * dc[g];
+        for (int g = 0; g < 4; ++g)
+            if (W[g] != 1.0) dc[g] = (1.0 / W[g]) * dc[g];
+    }
     return xi;
 }
 
@@ -284,7 +283,7 @@ __host__ __device__ inline size_t hills_smem_bytes(int n_cv, int stages, int n_g
     int rec = n_cv <= 3 ? 1 : 2;
     size_t b = (size_t)stages * SUB * rec * 16;                    // hill stages
     b += (size_t)RT * (1 + n_cv) * HWARPS * 32 * 8;                // binary64 accumulators [RT*NV][256]
-    b += (size_t)TILE_R * (1 + n_cv) * 8;                          // s_out
+    b += (size_t)3 * TILE_R * (1 + n_cv) * 8;                      // s_out, s_half[2]
     b += (size_t)TILE_R * n_cv * 4;                                // s_xi
     b += fused ? (size_t)TILE_R * n_groups * 3 * 4 : 0;            // s_jv
     b += 8 * 8 + 64;                                               // barriers, pad
@@ -303,7 +302,8 @@ __global__ void __launch_bounds__(HWARPS * 32, 1) k_hills(const __grid_constant_
     float4* stage = reinterpret_cast<float4*>(smem_raw);                          // STG * SUB * REC float4
     double* s_acc = reinterpret_cast<double*>(stage + STG * SUB * REC);           // [RT*NV][NT]
     double* s_out = s_acc + RT * NV * NT;                                         // [TILE_R][NV]
-    uint64_t* full = reinterpret_cast<uint64_t*>(s_out + TILE_R * NV);            // 8 barriers
+    double* s_half = s_out + TILE_R * NV;                                         // [2][TILE_R][NV]: per-half / per-part sums
+    uint64_t* full = reinterpret_cast<uint64_t*>(s_half + 2 * TILE_R * NV);       // 8 barriers
     float* s_xi = reinterpret_cast<float*>(full + 8);                             // [NCV][TILE_R] (pairs of replicas adjacent)
     float* s_jv = s_xi + TILE_R * NCV;                                            // fused: [TILE_R][n_groups][3]
     __shared__ int s_last;
@@ -354,12 +354,23 @@ __global__ void __launch_bounds__(HWARPS * 32, 1) k_hills(const __grid_constant_
         for (int i = 0; i < RT * NV; ++i) s_acc[i * NT + tid] = 0.0;
         // CV values (and per-group Jacobian vectors) of this tile's replicas; overlaps the first TMA loads
         if (A.fused) {
-            for (int t = tid; t < TILE_R * NCV; t += NT) {
-                int rr = t / NCV, k = t % NCV, r = r0 + rr;
-                float v = 0.f;
-                if (r < R) {
+            // the value (gather, cross products, atan2) and the Jacobian (gather, cross products, divisions) of one CV are
+            // two serial binary64 chains: different threads (different warps) take them, which shortens the prologue
+            for (int t2 = tid; t2 < 2 * TILE_R * NCV; t2 += NT) {
+                const bool want_j = t2 >= TILE_R * NCV;
+                const int t = want_j ? t2 - TILE_R * NCV : t2;
+                const int rr = t / NCV, k = t % NCV, r = r0 + rr;
+                if (!want_j) {
+                    float v = 0.f;
+                    if (r < R) {
+                        D3 dc[4];
+                        v = (float)thread_cv<false>(P, r, k, A.pos, dc);
+                        if (chunk == 0 && A.xi_out) A.xi_out[(long long)r * NCV + k] = v;
+                    }
+                    s_xi[k * TILE_R + rr] = v;
+                } else if (r < R) {
                     D3 dc[4];
-                    v = (float)thread_cv(P, r, k, A.pos, dc);
+                    (void)thread_cv<true>(P, r, k, A.pos, dc);
                     const CvDev& C = P.cv[k];
 #pragma unroll
                     for (int g = 0; g < 4; ++g)
@@ -367,9 +378,7 @@ __global__ void __launch_bounds__(HWARPS * 32, 1) k_hills(const __grid_constant_
                             float* j = s_jv + (rr * P.n_groups + C.gid0 + g) * 3;
                             j[0] = (float)dc[g].x; j[1] = (float)dc[g].y; j[2] = (float)dc[g].z;
                         }
-                    if (chunk == 0 && A.xi_out) A.xi_out[(long long)r * NCV + k] = v;
                 }
-                s_xi[k * TILE_R + rr] = v;
             }
         } else {
             for (int t = tid; t < TILE_R * NCV; t += NT) {
@@ -443,7 +452,8 @@ __global__ void __launch_bounds__(HWARPS * 32, 1) k_hills(const __grid_constant_
         // lanes -> warp totals through the shared accumulators: lane v (< RT*NV) sums value v over the 32 lanes
         // (rotated start => no bank conflicts; the order is fixed per lane => deterministic)
         __syncwarp();
-        double* dst = A.part + ((size_t)((chunk * 2 + half) * n_rt + tile) * TILE_R + w8 * RT) * NV;   // one partial per (chunk, half)
+        constexpr int TV = TILE_R * NV;
+        double* dst = s_half + half * TV + w8 * RT * NV;
         for (int v = lane; v < RT * NV; v += 32) {
             const double* src = s_acc + v * NT + wid * 32;
             double sum = 0.0;
@@ -451,6 +461,9 @@ __global__ void __launch_bounds__(HWARPS * 32, 1) k_hills(const __grid_constant_
             for (int i = 0; i < 32; ++i) sum += src[(i + lane) & 31];
             dst[v] = sum;
         }
+        __syncthreads();
+        // the two warp halves in fixed order -> this chunk's partial of the tile
+        for (int t = tid; t < TV; t += NT) A.part[(size_t)(chunk * n_rt + tile) * TV + t] = s_half[t] + s_half[TV + t];
         __syncthreads();
         PSG_STAMP(3);
         if (tid == 0) {
@@ -462,12 +475,23 @@ __global__ void __launch_bounds__(HWARPS * 32, 1) k_hills(const __grid_constant_
         __syncthreads();
         PSG_STAMP(4);
         if (s_last) {   // block-uniform: this CTA finishes the tile
-            for (int t = tid; t < TILE_R * NV; t += NT) {
-                const double* src = A.part + ((size_t)tile * TILE_R) * NV + t;
-                const size_t cstride = (size_t)n_rt * TILE_R * NV;
+            // chunk partials in fixed order; two thread groups split the chunks so that more loads are in flight
+            constexpr int PARTS = NT >= 2 * TV ? 2 : 1;
+            const size_t cstride = (size_t)n_rt * TV;
+            const int cn = (n_chunks + PARTS - 1) / PARTS;
+            for (int t = tid; t < PARTS * TV; t += NT) {
+                const int pt = t / TV, v = t - pt * TV;
+                const double* src = A.part + (size_t)tile * TV + v;
+                const int c1 = min(n_chunks, (pt + 1) * cn);
                 double sum = 0.0;
-#pragma unroll 8
-                for (int c = 0; c < 2 * n_chunks; ++c) sum += __ldcg(src + c * cstride);
+#pragma unroll 9
+                for (int c = pt * cn; c < c1; ++c) sum += __ldcg(src + c * cstride);
+                s_half[pt * TV + v] = sum;
+            }
+            __syncthreads();
+            for (int t = tid; t < TV; t += NT) {
+                double sum = s_half[t];
+                if (PARTS == 2) sum += s_half[TV + t];
                 int v = t % NV;
                 if (v > 0) sum *= -hc.gscale[v - 1];
                 s_out[t] = sum;
