@@ -138,6 +138,68 @@ def whole_job_value(units_per_rank, world, ms):
     return float(units_per_rank) * world / (ms * 1e-3)
 
 
+
+def per_call_table(ctx, w, frames, fsamp, force, to_dev, hbm_peak, fma_peak, n=20, reps=3):
+    """each C-ABI call timed on its own (a CUDA graph of n calls, best of reps), with the roofline
+    that bounds it where one applies; the force array keeps accumulating (pure +=), state (hills / grid) is static."""
+    import torch
+    main = torch.cuda.current_stream()
+    s = torch.cuda.Stream()              # graphs are captured on a side stream; the ctx follows it for this table
+    s.wait_stream(main)
+    ctx.set_stream(s)
+    try:
+        with torch.cuda.stream(s):
+            return _per_call_table(ctx, w, frames, fsamp, force, hbm_peak, fma_peak, n, reps, s)
+    finally:
+        torch.cuda.synchronize()
+        ctx.set_stream(main)
+
+
+def _per_call_table(ctx, w, frames, fsamp, force, hbm_peak, fma_peak, n, reps, s):
+    import torch
+    pos = frames[0]
+    xi = torch.empty((w.R, w.n_cv), device=pos.device)
+    V = torch.empty(w.R, device=pos.device)
+    dV = torch.zeros((w.R, w.n_cv), device=pos.device)
+    ctx.cv_eval(pos, xi, None)
+    calls = {"psg_cv_eval": lambda: ctx.cv_eval(pos, xi, None)}
+    if w.method == "abf":
+        calls["psg_abf_update"] = lambda: ctx.abf_update(xi, fsamp[0], None, dV)
+    else:
+        calls["psg_bias_eval"] = lambda: ctx.bias_eval(xi, V, dV)
+    calls["psg_apply_bias_forces"] = lambda: ctx.apply_bias_forces(pos, dV, force)
+    calls["psg_step"] = lambda: ctx.step(pos, force, None if fsamp is None else fsamp[0], -1)
+    out = {}
+    for name, fn in calls.items():
+        fn(); torch.cuda.synchronize()
+        g = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(g, stream=s):
+            for _ in range(n):
+                fn()
+        g.replay(); torch.cuda.synchronize()
+        best = 1e30
+        for _ in range(reps):
+            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            a.record(); g.replay(); b.record(); torch.cuda.synchronize()
+            best = min(best, a.elapsed_time(b) / n * 1e3)
+        out[name] = {"us": round(best, 2)}
+    n_range_atoms = sum(g[2] for cv in w.cvs for g in cv["groups"] if g[0] == "range")
+    if n_range_atoms and not w.shared_array:
+        span = w.R * w.N
+        out["psg_cv_eval"].update(bound="hbm", frac=round(16.0 * span / (out["psg_cv_eval"]["us"] * 1e-6) / 1e9 / hbm_peak, 3),
+                                  algorithmic_bytes=16.0 * span)
+        out["psg_apply_bias_forces"].update(bound="hbm", algorithmic_bytes=48.0 * span,
+                                            frac=round(48.0 * span / (out["psg_apply_bias_forces"]["us"] * 1e-6) / 1e9 / hbm_peak, 3))
+        out["psg_step"].update(bound="hbm", algorithmic_bytes=48.0 * span,
+                               frac=round(48.0 * span / (out["psg_step"]["us"] * 1e-6) / 1e9 / hbm_peak, 3))
+    if w.method == "metad":
+        C = hill_eval_instr(w.n_cv, int((w.period > 0).sum()))
+        work = float(w.R) * ctx.n_hills() * C
+        for k in ("psg_bias_eval", "psg_step"):
+            out[k].update(bound="alu", frac=round(work / (out[k]["us"] * 1e-6) / fma_peak, 3))
+    return out
+
+
 # ------------------------------------------------------------------------------------------ psg arm
 def run_psg(args, rank, world):
     import torch
@@ -295,6 +357,11 @@ def run_psg(args, rank, world):
                                "peak": hbm_peak, "unit": "GB/s", "frac": ach / hbm_peak, "traffic": NCU_TRAFFIC.get(args.config),
                                "peak_source": which + " copy bandwidth",
                                "note": "a step moves < 4 MB: launch latency, not HBM, bounds it (DESIGN.md)"}
+        if world == 1 and not args.skip_per_call:
+            reset_state()
+            out["per_call"] = per_call_table(ctx, w, frames, fsamp, force, to_dev, hbm_peak,
+                                             psg.measure_alu_peak(0, local) if w.method == "metad" else 1.0)
+            out["per_call"]["note"] = "graph replay of 20 calls each, L2 warm; us per call"
         if not args.skip_cpu_baseline:
             out["cpu_baseline"] = cpu_baseline(w, budget_s=args.cpu_budget)
     if world > 1:
@@ -395,6 +462,7 @@ def main():
     ap.add_argument("--cpu-budget", type=float, default=15.0)
     ap.add_argument("--ref-budget", type=float, default=60.0)
     ap.add_argument("--skip-cpu-baseline", action="store_true")
+    ap.add_argument("--skip-per-call", action="store_true")
     ap.add_argument("--no-clock-sampler", action="store_true")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3)

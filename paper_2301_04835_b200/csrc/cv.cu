@@ -9,19 +9,17 @@
 // Moments of range groups. grid = (range_blocks, R); block b covers atoms [span_begin + b*TILE, +TILE).
 // Every atom is loaded once (coalesced float4) and contributes to each range group that contains it.
 // Output: rpart[r][q][b][5] in binary64 (products of binary32 inputs are exact in binary64).
-__global__ void __launch_bounds__(PSG_RANGE_THREADS) k_range_moments(const __grid_constant__ SysParams P, const float* __restrict__ pos,
+__global__ void __launch_bounds__(PSG_RANGE_THREADS, 4) k_range_moments(const __grid_constant__ SysParams P, const float* __restrict__ pos,
                                                         double* __restrict__ rpart) {
     constexpr int NT = PSG_RANGE_THREADS, PER = PSG_RANGE_TILE / NT;
     const int r = blockIdx.y, b = blockIdx.x, tid = threadIdx.x;
     const float* p = pos + (long long)r * P.rstride * P.ps;
     const long long t0 = P.span_begin + (long long)b * PSG_RANGE_TILE;
-    float x[PER], y[PER], z[PER], w[PER];
-    long long ai[PER];
+    float x[PER], y[PER], z[PER];
 #pragma unroll
     for (int i = 0; i < PER; ++i) {
         long long a = t0 + tid + (long long)i * NT;
-        ai[i] = a;
-        x[i] = y[i] = z[i] = w[i] = 0.f;
+        x[i] = y[i] = z[i] = 0.f;
         if (a < P.span_end) {
             if (P.ps == 4) {
                 float4 v = __ldg(reinterpret_cast<const float4*>(p) + a);
@@ -29,38 +27,57 @@ __global__ void __launch_bounds__(PSG_RANGE_THREADS) k_range_moments(const __gri
             } else {
                 x[i] = __ldg(p + a * 3); y[i] = __ldg(p + a * 3 + 1); z[i] = __ldg(p + a * 3 + 2);
             }
-            w[i] = P.atom_weight ? __ldg(P.atom_weight + a) : 1.f;
         }
     }
-    __shared__ double red[NT / 32][PSG_MOM];
+    // per group: skip blocks that do not touch it; a block that lies wholly inside several groups is reduced once and
+    // the moments are copied (the same bits); one pair of barriers for all groups. k_range_step's A group does the same.
+    __shared__ double red[NT / 32][PSG_MAX_RANGE_GROUPS][PSG_MOM];
+    const long long t1 = t0 + PSG_RANGE_TILE < P.span_end ? t0 + PSG_RANGE_TILE : P.span_end;
+    bool have_full = false;
+    double mf[PSG_MOM] = {0, 0, 0, 0, 0};
     for (int q = 0; q < P.n_ranges; ++q) {
         const GroupDev& G = P.grp[P.range_gid[q]];
         const long long gb = G.rbegin, ge = G.rbegin + G.rsize;
         double m[PSG_MOM] = {0, 0, 0, 0, 0};
-        if (t0 < ge && t0 + PSG_RANGE_TILE > gb) {   // block-uniform
+        if (t0 < ge && t1 > gb) {   // block-uniform
+            const bool inside = gb <= t0 && t1 <= ge;
+            if (inside && have_full) {
 #pragma unroll
-            for (int i = 0; i < PER; ++i) {
-                if (ai[i] >= gb && ai[i] < ge && ai[i] < P.span_end) {
-                    double wd = (double)w[i], xd = (double)x[i], yd = (double)y[i], zd = (double)z[i];
+                for (int i = 0; i < PSG_MOM; ++i) m[i] = mf[i];
+            } else {
+#pragma unroll
+                for (int i = 0; i < PER; ++i) {
+                    // branch-free: an atom outside the group enters with w = 0 and r = 0, which adds exactly +0
+                    const long long a = t0 + tid + (long long)i * NT;
+                    const bool in = a >= gb && a < ge && a < t1;
+                    float wf = 0.f;
+                    if (in) wf = P.atom_weight ? __ldg(P.atom_weight + a) : 1.f;   // (weights are re-read per group pass: L1/L2 hits)
+                    const double wd = (double)wf, xd = in ? (double)x[i] : 0.0, yd = in ? (double)y[i] : 0.0,
+                                 zd = in ? (double)z[i] : 0.0;
                     m[0] += wd; m[1] += wd * xd; m[2] += wd * yd; m[3] += wd * zd;
                     m[4] += wd * (xd * xd + yd * yd + zd * zd);
                 }
+#pragma unroll
+                for (int i = 0; i < PSG_MOM; ++i) m[i] = warp_sum(m[i]);
+                if (inside) {
+                    have_full = true;
+#pragma unroll
+                    for (int i = 0; i < PSG_MOM; ++i) mf[i] = m[i];
+                }
             }
         }
-#pragma unroll
-        for (int i = 0; i < PSG_MOM; ++i) m[i] = warp_sum(m[i]);
-        __syncthreads();
         if ((tid & 31) == 0) {
 #pragma unroll
-            for (int i = 0; i < PSG_MOM; ++i) red[tid >> 5][i] = m[i];
+            for (int i = 0; i < PSG_MOM; ++i) red[tid >> 5][q][i] = m[i];
         }
-        __syncthreads();
-        if (tid < PSG_MOM) {
-            double s = 0;
+    }
+    __syncthreads();
+    if (tid < P.n_ranges * PSG_MOM) {
+        const int q = tid / PSG_MOM, i = tid % PSG_MOM;
+        double s = 0;
 #pragma unroll
-            for (int wq = 0; wq < NT / 32; ++wq) s += red[wq][tid];
-            rpart[(((long long)r * P.n_ranges + q) * P.range_blocks + b) * PSG_MOM + tid] = s;
-        }
+        for (int wq = 0; wq < NT / 32; ++wq) s += red[wq][q][i];
+        rpart[(((long long)r * P.n_ranges + q) * P.range_blocks + b) * PSG_MOM + i] = s;
     }
 }
 
