@@ -3,7 +3,7 @@
 // Register-only dependent chains, 8 independent chains per thread, 1024 threads x 2 CTAs per SM.
 #include <stdint.h>
 
-#include "internal.h"
+#include "hills.cuh"
 
 #define ITERS 4096
 #define CHAINS 8
@@ -65,6 +65,69 @@ __global__ void __launch_bounds__(1024) k_peak(float* out, float seed) {
     if (s == 123.456f) out[0] = s;   // never true; keeps the chains alive
 }
 
+// The hill loop alone: HillBody on a shared-memory table of 1,024 hill records, no TMA, no barriers, no flush, no
+// reduction -- the ceiling of the kernel's own instruction mix (per hill and replica pair: 16 packed FMA-pipe
+// instructions, 2 MUFU.EX2; one LDS.128 per 8 evaluations), with the launch shape of k_hills (512 threads, 1 CTA/SM).
+template <int NCV, int PM, int NEQ>
+__global__ void __launch_bounds__(HWARPS * 32, 1) k_hill_loop_peak(const __grid_constant__ HillConsts hc, float* out, int iters) {
+    __shared__ float4 tab[1024];
+    for (int i = threadIdx.x; i < 1024; i += blockDim.x)
+        tab[i] = make_float4(-3.f + 0.005f * i, 2.9f - 0.004f * i, 0.3f + 0.001f * i, -1.f - 0.001f * i);
+    __syncthreads();
+    u64 X[RT / 2][NCV], a32[RT / 2][1 + NCV];
+#pragma unroll
+    for (int p = 0; p < RT / 2; ++p) {
+#pragma unroll
+        for (int k = 0; k < NCV; ++k) X[p][k] = pk(-3.f + 0.01f * threadIdx.x + p, 3.f - 0.01f * threadIdx.x - p);
+#pragma unroll
+        for (int v = 0; v < 1 + NCV; ++v) a32[p][v] = 0ull;
+    }
+    const int off = threadIdx.x & 63;
+    for (int it = 0; it < iters; ++it) accumulate_f32<NCV, PM, NEQ>(tab, 1024, off, X, hc, a32);
+    float s = 0.f;
+#pragma unroll
+    for (int p = 0; p < RT / 2; ++p)
+#pragma unroll
+        for (int v = 0; v < 1 + NCV; ++v) { float lo, hi; upk(a32[p][v], lo, hi); s += lo + hi; }
+    if (s == 123.456f) out[0] = s;
+}
+
+template <int NCV, int PM, int NEQ>
+static cudaError_t time_hill_loop(int sms, double* out) {
+    float* d = nullptr;
+    cudaError_t e = cudaMalloc((void**)&d, 4);
+    if (e != cudaSuccess) return e;
+    HillConsts hc{};
+    for (int k = 0; k < NCV; ++k) {
+        hc.inv_period[k] = (PM >> k) & 1 ? 0.15915494f : 0.f;
+        hc.np_hi[k] = (PM >> k) & 1 ? -6.2831855f : 0.f;
+        hc.np_lo[k] = (PM >> k) & 1 ? 1.7484555e-7f : 0.f;
+        hc.nc[k] = k < NEQ ? -5.888f : -288.5f;
+    }
+    cudaEvent_t t0, t1;
+    cudaEventCreate(&t0);
+    cudaEventCreate(&t1);
+    const int iters = 64;
+    double best = 0.0;
+    for (int rep = 0; rep < 6; ++rep) {
+        cudaEventRecord(t0);
+        k_hill_loop_peak<NCV, PM, NEQ><<<sms, HWARPS * 32>>>(hc, d, iters);
+        cudaEventRecord(t1);
+        e = cudaEventSynchronize(t1);
+        if (e != cudaSuccess) break;
+        float ms = 0.f;
+        cudaEventElapsedTime(&ms, t0, t1);
+        // every thread: iters x 16 hills (1,024 / 64) x RT replicas
+        double rate = (double)sms * HWARPS * 32 * iters * 16.0 * RT / (ms * 1e-3);
+        if (rep > 0 && rate > best) best = rate;
+    }
+    cudaEventDestroy(t0);
+    cudaEventDestroy(t1);
+    cudaFree(d);
+    *out = best;
+    return e == cudaSuccess ? cudaGetLastError() : e;
+}
+
 template <int WHICH>
 static cudaError_t time_one(int sms, double ops_per_thread_iter, double* out) {
     float* d = nullptr;
@@ -108,6 +171,8 @@ extern "C" int psg_measure_alu_peak(int device, int which, double* out) {
     case 4: e = time_one<4>(sms, CHAINS / 2, out); break;      // F2F.F64.F32 (+ the way back; counts the widening only)
     case 5: e = time_one<5>(sms, CHAINS, out); break;          // I2F.F32.S32
     case 6: e = time_one<6>(sms, CHAINS, out); break;          // FADD2
+    case 7: e = time_hill_loop<2, 3, 2>(sms, out); break;      // hill evaluations/s of the bare loop, 2-D periodic (C = 16)
+    case 8: e = time_hill_loop<3, 3, 2>(sms, out); break;      // hill evaluations/s of the bare loop, 3-D, 2 periodic (C = 20)
     default: return PSG_EINVAL;
     }
     return e == cudaSuccess ? PSG_OK : PSG_ECUDA;
