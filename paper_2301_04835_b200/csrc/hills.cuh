@@ -27,7 +27,7 @@
 #define TILE_R PSG_HILL_TILE_R
 #define SUB PSG_HILL_SUB
 #ifndef PSG_FLUSH_EVERY
-#define PSG_FLUSH_EVERY 4        // sub-tiles (16 hills per lane each) between binary32 -> binary64 flushes
+#define PSG_FLUSH_EVERY 2        // sub-tiles (32 hills per lane each) between binary32 -> binary64 flushes
 #endif
 #define MAGIC_RN 12582912.0f   // 1.5 * 2^23: (x + M) - M = rint(x) for |x| < 2^22
 
@@ -271,7 +271,7 @@ struct HillKernelArgs {
     float* force;            // fused
     int R;
     int fused;
-    int stages;              // shared-memory stages of SUB hills
+    int stages;              // shared-memory stages of SUB x 16 bytes
 #ifdef PSG_TRACE
     long long* trace;        // [grid][8] clock64 stamps of the first item of every CTA (debug builds only)
 #endif
@@ -284,7 +284,8 @@ struct HillKernelArgs {
 
 __host__ __device__ inline size_t hills_smem_bytes(int n_cv, int stages, int n_groups, bool fused) {
     int rec = n_cv <= 3 ? 1 : 2;
-    size_t b = (size_t)stages * SUB * rec * 16;                    // hill stages
+    (void)rec;
+    size_t b = (size_t)stages * SUB * 16;                          // hill stages (SUB / rec hills each)
     b += (size_t)RT * (1 + n_cv) * HWARPS * 32 * 8;                // binary64 accumulators [RT*NV][256]
     b += (size_t)3 * TILE_R * (1 + n_cv) * 8;                      // s_out, s_half[2]
     b += (size_t)TILE_R * n_cv * 4;                                // s_xi
@@ -298,12 +299,13 @@ template <int NCV, int PM, int NEQ, bool F64>
 __global__ void __launch_bounds__(HWARPS * 32, 1) k_hills(const __grid_constant__ SysParams P, const __grid_constant__ HillConsts hc,
                                                            const __grid_constant__ HillKernelArgs A) {
     constexpr int REC = NCV <= 3 ? 1 : 2;
+    constexpr int SUBH = SUB / REC;   // hills per stage: a stage is always SUB x 16 bytes
     constexpr int NV = 1 + NCV;
     constexpr int NT = HWARPS * 32;
     extern __shared__ __align__(128) unsigned char smem_raw[];
     const int STG = A.stages;
-    float4* stage = reinterpret_cast<float4*>(smem_raw);                          // STG * SUB * REC float4
-    double* s_acc = reinterpret_cast<double*>(stage + STG * SUB * REC);           // [RT*NV][NT]
+    float4* stage = reinterpret_cast<float4*>(smem_raw);                          // STG * SUBH * REC float4
+    double* s_acc = reinterpret_cast<double*>(stage + STG * SUBH * REC);           // [RT*NV][NT]
     double* s_out = s_acc + RT * NV * NT;                                         // [TILE_R][NV]
     double* s_half = s_out + TILE_R * NV;                                         // [2][TILE_R][NV]: per-half / per-part sums
     uint64_t* full = reinterpret_cast<uint64_t*>(s_half + 2 * TILE_R * NV);       // 8 barriers
@@ -343,15 +345,15 @@ __global__ void __launch_bounds__(HWARPS * 32, 1) k_hills(const __grid_constant_
         int len = n_h - h0;
         if (len > Lc) len = Lc;
         if (len < 0) len = 0;
-        const int n_st = (len + SUB - 1) / SUB;
+        const int n_st = (len + SUBH - 1) / SUBH;
         PSG_STAMP(0);
         // producer prologue
         if (tid == 0) {
             for (int t = 0; t < n_st && t < STG; ++t) {
                 int s = (seq + t) % STG;
-                int cnt = min(SUB, len - t * SUB);
+                int cnt = min(SUBH, len - t * SUBH);
                 mbar_expect_tx(&full[s], (uint32_t)cnt * REC * 16u);
-                tma_load_1d(stage + s * SUB * REC, A.hills + (size_t)(h0 + t * SUB) * REC, (uint32_t)cnt * REC * 16u, &full[s]);
+                tma_load_1d(stage + s * SUBH * REC, A.hills + (size_t)(h0 + t * SUBH) * REC, (uint32_t)cnt * REC * 16u, &full[s]);
             }
         }
         // binary64 accumulators of this item
@@ -407,11 +409,11 @@ __global__ void __launch_bounds__(HWARPS * 32, 1) k_hills(const __grid_constant_
             for (int t = 0; t < n_st; ++t) {
                 int s = seq % STG;
                 mbar_wait(&full[s], (seq / STG) & 1);
-                int cnt = min(SUB, len - t * SUB);
+                int cnt = min(SUBH, len - t * SUBH);
                 if (warp_active) {
                     // a full sub-tile gets a compile-time trip count (the compiler then schedules across iterations)
-                    if (cnt == SUB) accumulate_f32<NCV, PM, NEQ>(stage + s * SUB * REC, SUB, lane + 32 * half, X, hc, a32);
-                    else accumulate_f32<NCV, PM, NEQ>(stage + s * SUB * REC, cnt, lane + 32 * half, X, hc, a32);
+                    if (cnt == SUBH) accumulate_f32<NCV, PM, NEQ>(stage + s * SUBH * REC, SUBH, lane + 32 * half, X, hc, a32);
+                    else accumulate_f32<NCV, PM, NEQ>(stage + s * SUBH * REC, cnt, lane + 32 * half, X, hc, a32);
                 }
                 if (warp_active && ((t % PSG_FLUSH_EVERY) == PSG_FLUSH_EVERY - 1 || t == n_st - 1)) {
                     // flush the binary32 partial sums (<= 64 hills per lane: 4 sub-tiles of 16) into the binary64 slots
@@ -433,10 +435,10 @@ __global__ void __launch_bounds__(HWARPS * 32, 1) k_hills(const __grid_constant_
                     if (atomicAdd(&s_cnt[s], 1) == HWARPS - 1) {
                         s_cnt[s] = 0;
                         if (t + STG < n_st) {
-                            int cn = min(SUB, len - (t + STG) * SUB);
+                            int cn = min(SUBH, len - (t + STG) * SUBH);
                             asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
                             mbar_expect_tx(&full[s], (uint32_t)cn * REC * 16u);
-                            tma_load_1d(stage + s * SUB * REC, A.hills + (size_t)(h0 + (t + STG) * SUB) * REC,
+                            tma_load_1d(stage + s * SUBH * REC, A.hills + (size_t)(h0 + (t + STG) * SUBH) * REC,
                                         (uint32_t)cn * REC * 16u, &full[s]);
                         }
                     }
@@ -452,18 +454,18 @@ __global__ void __launch_bounds__(HWARPS * 32, 1) k_hills(const __grid_constant_
             for (int t = 0; t < n_st; ++t) {
                 int s = seq % STG;
                 mbar_wait(&full[s], (seq / STG) & 1);
-                int cnt = min(SUB, len - t * SUB);
+                int cnt = min(SUBH, len - t * SUBH);
                 if (warp_active)
-                    accumulate_f64<NCV>(stage + s * SUB * REC, A.heights + h0 + t * SUB, cnt, lane + 32 * half, xi, hc, s_acc + tid, NT);
+                    accumulate_f64<NCV>(stage + s * SUBH * REC, A.heights + h0 + t * SUBH, cnt, lane + 32 * half, xi, hc, s_acc + tid, NT);
                 __syncwarp();
                 if (lane == 0) {
                     if (atomicAdd(&s_cnt[s], 1) == HWARPS - 1) {
                         s_cnt[s] = 0;
                         if (t + STG < n_st) {
-                            int cn = min(SUB, len - (t + STG) * SUB);
+                            int cn = min(SUBH, len - (t + STG) * SUBH);
                             asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
                             mbar_expect_tx(&full[s], (uint32_t)cn * REC * 16u);
-                            tma_load_1d(stage + s * SUB * REC, A.hills + (size_t)(h0 + (t + STG) * SUB) * REC,
+                            tma_load_1d(stage + s * SUBH * REC, A.hills + (size_t)(h0 + (t + STG) * SUBH) * REC,
                                         (uint32_t)cn * REC * 16u, &full[s]);
                         }
                     }

@@ -15,7 +15,7 @@
 #define PSG_HILL_RT 8            // replicas per thread in the hill sum
 #define PSG_HILL_WARPS 16        // warps per CTA in the hill sum: two halves of 8 warps share the tile's replicas and split its hills
 #define PSG_HILL_TILE_R (PSG_HILL_RT * 8)   // replicas per CTA tile (64): warp w and warp w + 8 own the same 8 replicas
-#define PSG_HILL_SUB 1024        // hills per shared-memory stage
+#define PSG_HILL_SUB 2048        // hills per shared-memory stage
 
 struct CvDev {
     int type, n_groups, axis, gid0;   // gid0: global id of this CV's first group
