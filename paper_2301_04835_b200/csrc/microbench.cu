@@ -93,7 +93,7 @@ __global__ void __launch_bounds__(HWARPS * 32, 1) k_hill_loop_peak(const __grid_
 }
 
 template <int NCV, int PM, int NEQ>
-static cudaError_t time_hill_loop(int sms, double* out) {
+static cudaError_t time_hill_loop(int sms, double* out, int iters = 64) {
     float* d = nullptr;
     cudaError_t e = cudaMalloc((void**)&d, 4);
     if (e != cudaSuccess) return e;
@@ -107,7 +107,6 @@ static cudaError_t time_hill_loop(int sms, double* out) {
     cudaEvent_t t0, t1;
     cudaEventCreate(&t0);
     cudaEventCreate(&t1);
-    const int iters = 64;
     double best = 0.0;
     for (int rep = 0; rep < 6; ++rep) {
         cudaEventRecord(t0);
@@ -173,7 +172,9 @@ extern "C" int psg_measure_alu_peak(int device, int which, double* out) {
     case 6: e = time_one<6>(sms, CHAINS, out); break;          // FADD2
     case 7: e = time_hill_loop<2, 3, 2>(sms, out); break;      // hill evaluations/s of the bare loop, 2-D periodic (C = 16)
     case 8: e = time_hill_loop<3, 3, 2>(sms, out); break;      // hill evaluations/s of the bare loop, 3-D, 2 periodic (C = 20)
-    default: return PSG_EINVAL;
+    default:
+        if (which >= 100 && which < 200) { e = time_hill_loop<2, 3, 2>(sms, out, which - 100); break; }   // short runs: which - 100 passes
+        return PSG_EINVAL;
     }
     return e == cudaSuccess ? PSG_OK : PSG_ECUDA;
 }
