@@ -155,7 +155,15 @@ int psg_apply_bias_forces(psg_ctx* ctx, const float* d_pos, const float* d_dVdxi
 
 /* One whole step of the selected method, fused: gather -> CVs -> (deposit if due) -> bias -> forces.
  *  d_fsample: ABF only, else NULL.  step: 1-based MD step number (deposit phase).
- * Afterwards xi / V / dVdxi / bin of this step can be read with psg_step_outputs. */
+ * Afterwards xi / V / dVdxi / bin of this step can be read with psg_step_outputs.
+ * ONE kernel launch per step where a fused kernel covers the configuration, with the same results as the
+ * separate calls: metadynamics over explicit groups (k_hills); ABF over explicit groups (k_abf_step);
+ * harmonic windows whose groups are all contiguous ranges, float4 positions and forces 16-byte aligned, one
+ * array per window, at most (SM count) slices of 2,048 atoms per window (k_range_step).  Anything else runs the
+ * kernels of the separate calls in sequence.  k_abf_step and k_range_step contain inter-CTA waits and are
+ * launched cooperatively: the launch fails (PSG_ECUDA) rather than hangs if the grid cannot be co-resident.
+ * Environment (read once, for experiments): PSG_RANGE_LAG = items the position producer of k_range_step may
+ * run ahead of the force group (default 10); PSG_DISABLE_RANGE_STEP = take the separate kernels instead. */
 int psg_step(psg_ctx* ctx, const float* d_pos, float* d_force, const float* d_fsample, long long step);
 /* Device pointers (ctx-owned, valid until destroy/reconfigure) of the last step's per-replica results:
  * xi [R][n_cv], V [R] (0 for ABF), dVdxi [R][n_cv], bin [R] (ABF only, else NULL). Any out may be NULL. */
@@ -172,7 +180,10 @@ int psg_sync_check(psg_ctx* ctx);
 /* Measured ALU throughput of this device (register-only loops, CUDA-event timed, synchronises):
  * which = 0: FP32 FFMA lane-ops/s; 1: packed FFMA2 (f32x2) lane-ops/s (2 per lane per instruction);
  * 2: MUFU.EX2/s; 3: FP64 DFMA lane-ops/s; 4: F2F f32->f64->f32 round trips/s; 5: I2F.F32.S32/s;
- * 6: packed FADD2 lane-ops/s.  Denominators for the hill-sum roofline. */
+ * 6: packed FADD2 lane-ops/s.  Denominators for the hill-sum roofline.
+ * 7 / 8: hill evaluations/s of the BARE hill loop (k_hills' own inner loop on a shared-memory table, nothing
+ * else; 2-D periodic / 3-D with 2 periodic CVs): the ceiling of the kernel's instruction mix.
+ * 100 + n: the same as 7 with only n passes of 1,024 hills (short-run behaviour). */
 int psg_measure_alu_peak(int device, int which, double* ops_per_second_out);
 /* Launch counter: number of kernels this ctx has enqueued since creation (for bench.py's gpu_launches). */
 long long psg_launch_count(const psg_ctx* ctx);
