@@ -601,6 +601,45 @@ def test_fused_abf_step_is_cuda_graph_capturable(torch, psg):
     assert np.allclose(outs[0][1], outs[1][1], rtol=1e-5, atol=1e-4)
 
 
+def test_metad_step_more_tiles_than_ctas(torch, psg):
+    """20,000 walkers = 313 replica tiles for ~148 CTAs: every CTA of the persistent k_hills loops over several
+    (tile, chunk) items (stage ring, tickets and partial buffers are reused across items); R is not a multiple of 64"""
+    w = W.make(1, R=20000, n_hills=2600, steps=2, stride=0)
+    ctx = make_ctx(psg, w)
+    sysm = oracle_system(w)
+    centers, heights = w.params["hill_centers"], oracle_heights(w)
+    ctx.load_hills(dev(torch, centers), dev(torch, heights))
+    pos, f0 = w.positions(1), w.forces0()
+    d_f = dev(torch, f0)
+    for _ in range(2):                      # twice: the second launch must find tickets / counters re-armed
+        d_f.copy_(dev(torch, f0))
+        ctx.step(dev(torch, pos), d_f, None, 1)
+    ctx.sync_check()
+    out = {k: v.cpu().numpy() for k, v in ctx.read_step_outputs().items()}
+    xi_ref, b, f_ref = oracle_step(w, sysm, pos, f0, centers, heights)
+    _check_step(w, sysm, pos, out["xi"], out["V"], out["dVdxi"], d_f.cpu().numpy(), f0, xi_ref, b, f_ref, what="R=20000: ")
+
+
+def test_abf_step_at_the_replica_limit(torch, psg):
+    """65,535 replicas (the ctx maximum): every warp of the cooperative k_abf_step loops over many replicas"""
+    w = W.make(2, R=65535, N=40, steps=2)
+    ctx = make_ctx(psg, w)
+    sysm = oracle_system(w)
+    pos, f0, fs = w.positions(0), w.forces0(), w.fsample(0)
+    nb = int(np.prod(w.params["shape"]))
+    abf = (np.zeros(nb, np.int32), np.zeros((nb, 2), np.float64))
+    d_f = dev(torch, f0)
+    ctx.step(dev(torch, pos), d_f, dev(torch, fs), 1)
+    ctx.sync_check()
+    out = {k: v.cpu().numpy() for k, v in ctx.read_step_outputs().items()}
+    xi_ref, b, f_ref = oracle_step(w, sysm, pos, f0, None, None, abf, fs)
+    assert np.array_equal(out["bin"], b["bin"])
+    hp, fp, nbins = ctx.abf_state()
+    from paper_2301_04835_b200.psg import _view
+    assert np.array_equal(_view(hp, (nbins,), torch.int32, 0).cpu().numpy(), abf[0])
+    _check_step(w, sysm, pos, out["xi"], None, out["dVdxi"], d_f.cpu().numpy(), f0, xi_ref, b, f_ref, what="R=65535: ")
+
+
 def test_internal_cv_forces_have_no_net_force_or_torque(torch, psg):
     """sum_i F_i = 0 and sum_i r_i x F_i = 0 for internal CVs (BASELINE.json), on the GPU forces themselves"""
     w = small(1, stride=0)
