@@ -640,6 +640,50 @@ def test_abf_step_at_the_replica_limit(torch, psg):
     _check_step(w, sysm, pos, out["xi"], None, out["dVdxi"], d_f.cpu().numpy(), f0, xi_ref, b, f_ref, what="R=65535: ")
 
 
+def _range_workload(R, N, cvs, weighted=False):
+    """config-3 geometry with a custom list of range-group CVs (windows' centres re-cut to the number of CVs)"""
+    w = W.make(3, R=R, N=N, steps=2, weighted=weighted)
+    w.cvs = cvs
+    c = 1.0 + 4.0 * np.arange(R) / max(R - 1, 1)
+    w.params = {"kspring": np.full(len(cvs), 1000.0, np.float32),
+                "centers": np.stack([c] * len(cvs), axis=1).astype(np.float32)}
+    return w
+
+
+@pytest.mark.parametrize("case", ["gap", "angle3", "limit", "over_limit"])
+def test_fused_range_step_shapes(torch, psg, case):
+    """k_range_step on shapes config 3 does not have: groups that leave a GAP in their span (those atoms must keep
+    their force bits), a three-group CV with an Rg CV on an overlapping range, a window of exactly `grid` slices,
+    and one slice more than that (falls back to the separate kernels); all against the oracle"""
+    props = torch.cuda.get_device_properties(0)
+    n_lim = props.multi_processor_count * 2048
+    if case == "gap":
+        R, N, want = 5, 9000, 1
+        cvs = [W._cv("distance", [("range", 100, 1900), ("range", 5000, 3500)])]
+    elif case == "angle3":
+        R, N, want = 4, 12000, 1
+        cvs = [W._cv("angle", [("range", 0, 4000), ("range", 4000, 4000), ("range", 8000, 4000)]),
+               W._cv("rgyr", [("range", 2000, 9000)])]
+    elif case == "limit":
+        R, N, want = 1, n_lim, 1
+        cvs = [W._cv("rgyr", [("range", 0, N)]), W._cv("distance", [("range", 0, N // 2), ("range", N // 2, N - N // 2)])]
+    else:
+        R, N, want = 1, n_lim + 1, 4
+        cvs = [W._cv("rgyr", [("range", 0, N)]), W._cv("distance", [("range", 0, N // 2), ("range", N // 2, N - N // 2)])]
+    w = _range_workload(R, N, cvs, weighted=(case == "angle3"))
+    ctx = make_ctx(psg, w)
+    sysm = oracle_system(w)
+    pos, f0 = w.positions(1), w.forces0()
+    d_f = dev(torch, f0)
+    n0 = ctx.launch_count()
+    ctx.step(dev(torch, pos), d_f, None, 1)
+    ctx.sync_check()
+    assert ctx.launch_count() - n0 == want
+    out = {k: v.cpu().numpy() for k, v in ctx.read_step_outputs().items()}
+    xi_ref, b, f_ref = oracle_step(w, sysm, pos, f0)
+    _check_step(w, sysm, pos, out["xi"], out["V"], out["dVdxi"], d_f.cpu().numpy(), f0, xi_ref, b, f_ref, what=case + ": ")
+
+
 def test_internal_cv_forces_have_no_net_force_or_torque(torch, psg):
     """sum_i F_i = 0 and sum_i r_i x F_i = 0 for internal CVs (BASELINE.json), on the GPU forces themselves"""
     w = small(1, stride=0)
