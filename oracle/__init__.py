@@ -42,7 +42,8 @@ class _CV(C.Structure):
 
 class _Layout(C.Structure):
     _fields_ = [("n_replicas", C.c_int), ("n_atoms", C.c_longlong), ("replica_stride_atoms", C.c_longlong),
-                ("pos_stride", C.c_int), ("n_cv", C.c_int), ("n_slots", C.c_int), ("per_replica_slots", C.c_int)]
+                ("pos_stride", C.c_int), ("n_cv", C.c_int), ("n_slots", C.c_int), ("per_replica_slots", C.c_int),
+                ("box", C.c_double * 3)]
 
 
 _lib = None
@@ -92,7 +93,7 @@ class System:
     """
 
     def __init__(self, n_replicas, n_atoms, replica_stride_atoms, pos_stride, cvs, slot_atom,
-                 slot_weight=None, atom_weight=None):
+                 slot_weight=None, atom_weight=None, box=None):
         self.cvs_py = cvs
         self.n_cv = len(cvs)
         arr = (_CV * self.n_cv)()
@@ -117,6 +118,8 @@ class System:
         n_slots = self.slot_atom.shape[-1] if self.slot_atom.size else 0
         self.layout = _Layout(int(n_replicas), int(n_atoms), int(replica_stride_atoms), int(pos_stride),
                               self.n_cv, int(n_slots), per_rep)
+        for x in range(3):      # orthorhombic box lengths for the minimum-image convention; 0 = open (reading R-MI)
+            self.layout.box[x] = float(box[x]) if box is not None else 0.0
         self.slot_weight = _f32(slot_weight)
         self.atom_weight = _f32(atom_weight)
         self.R = int(n_replicas)

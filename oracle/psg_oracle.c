@@ -63,6 +63,8 @@ typedef struct {
     int n_cv;
     int n_slots;
     int per_replica_slots;          /* 0: slot_atom[n_slots]; 1: slot_atom[R][n_slots] */
+    double box[3];                  /* orthorhombic box lengths for the minimum-image convention; 0 = open in that direction
+                                     * (reading R-MI of DESIGN.md; the paper is silent on periodic positions) */
 } orc_layout;
 
 int orc_num_threads(void) {
@@ -99,6 +101,23 @@ static double wrap_period(double d, double period) {
 }
 
 /* number of atoms of group g of a CV and the i-th atom's index and weight */
+/* nearest image of a displacement vector in an orthorhombic box: d <- d - L rint(d / L) per periodic direction */
+static void min_image(double *d, const double *box) {
+    if (!box) return;
+    for (int x = 0; x < 3; ++x)
+        if (box[x] > 0) d[x] -= box[x] * rint(d[x] / box[x]);
+}
+
+/* position of atom a as the image nearest to ref (ref == NULL: as stored) */
+static void atom_image(const float *pos, int ps, long long a, const double *ref, const double *box, double *r) {
+    for (int x = 0; x < 3; ++x) r[x] = (double)pos[a * ps + x];
+    if (ref && box) {
+        double d[3] = {r[0] - ref[0], r[1] - ref[1], r[2] - ref[2]};
+        min_image(d, box);
+        for (int x = 0; x < 3; ++x) r[x] = ref[x] + d[x];
+    }
+}
+
 static long long group_count(const orc_cv *cv, int g) { return cv->is_range[g] ? cv->range_size[g] : (long long)cv->slot_size[g]; }
 
 static long long group_atom(const orc_cv *cv, int g, long long i, const int *slot_atom) {
@@ -115,15 +134,17 @@ static double group_weight(const orc_cv *cv, int g, long long i, const float *sl
 /* c_g = sum_i w_i r_i / sum_i w_i  (PAPER.md:L227-L229 barycenter; with masses
  * as weights the "center of mass" of L332, L408). */
 static void group_center(const orc_cv *cv, int g, const float *pos, int ps, const int *slot_atom,
-                         const float *slot_weight, const float *atom_weight, double *c, double *wsum) {
-    double s[3] = {0, 0, 0}, W = 0;
+                         const float *slot_weight, const float *atom_weight, const double *box, double *c, double *wsum) {
+    double s[3] = {0, 0, 0}, W = 0, first[3];
     long long n = group_count(cv, g);
+    atom_image(pos, ps, group_atom(cv, g, 0, slot_atom), NULL, NULL, first);
     for (long long i = 0; i < n; ++i) {
         long long a = group_atom(cv, g, i, slot_atom);
-        double w = group_weight(cv, g, i, slot_weight, atom_weight);
-        s[0] += w * (double)pos[a * ps + 0];
-        s[1] += w * (double)pos[a * ps + 1];
-        s[2] += w * (double)pos[a * ps + 2];
+        double w = group_weight(cv, g, i, slot_weight, atom_weight), r[3];
+        atom_image(pos, ps, a, first, box, r);   /* with a box: the image nearest to the group's first atom (R-MI) */
+        s[0] += w * r[0];
+        s[1] += w * r[1];
+        s[2] += w * r[2];
         W += w;
     }
     c[0] = s[0] / W; c[1] = s[1] / W; c[2] = s[2] / W;
@@ -131,18 +152,18 @@ static void group_center(const orc_cv *cv, int g, const float *pos, int ps, cons
 }
 
 /* xi and d(xi)/d(c_g) for the CVs that are functions of group centers only. */
-static double point_cv(const orc_cv *cv, double c[4][3], double dc[4][3]) {
+static double point_cv(const orc_cv *cv, double c[4][3], double dc[4][3], const double *box) {
     memset(dc, 0, sizeof(double) * 12);
     switch (cv->type) {
     case ORC_DISTANCE: { /* PAPER.md:L185 Distance: xi = |c2 - c1| */
-        double d[3]; v_sub(c[1], c[0], d);
+        double d[3]; v_sub(c[1], c[0], d); min_image(d, box);
         double r = sqrt(v_dot(d, d));
         if (r > 0) for (int x = 0; x < 3; ++x) { dc[1][x] = d[x] / r; dc[0][x] = -d[x] / r; }
         return r;
     }
     case ORC_ANGLE: { /* PAPER.md:L186 Angle; vertex at the second group (reading R-ANG) */
         double q[3], s[3], n[3], t[3];
-        v_sub(c[0], c[1], q); v_sub(c[2], c[1], s); v_cross(q, s, n);
+        v_sub(c[0], c[1], q); v_sub(c[2], c[1], s); min_image(q, box); min_image(s, box); v_cross(q, s, n);
         double nn = sqrt(v_dot(n, n));
         double th = atan2(nn, v_dot(q, s));
         if (nn > 0) {
@@ -156,6 +177,7 @@ static double point_cv(const orc_cv *cv, double c[4][3], double dc[4][3]) {
     case ORC_DIHEDRAL: { /* PAPER.md:L187 DihedralAngle, L81; IUPAC sign (reading R-DIH) */
         double b1[3], b2[3], b3[3], n1[3], n2[3];
         v_sub(c[1], c[0], b1); v_sub(c[2], c[1], b2); v_sub(c[3], c[2], b3);
+        min_image(b1, box); min_image(b2, box); min_image(b3, box);
         v_cross(b1, b2, n1); v_cross(b2, b3, n2);
         double lb2 = sqrt(v_dot(b2, b2));
         double phi = atan2(lb2 * v_dot(b1, n2), v_dot(n1, n2));
@@ -184,32 +206,35 @@ static double point_cv(const orc_cv *cv, double c[4][3], double dc[4][3]) {
  * doubles per atom, for the atoms of group 0, then group 1, ... in group order.
  * Returns xi. */
 static double cv_one(const orc_cv *cv, const float *pos, int ps, const int *slot_atom,
-                     const float *slot_weight, const float *atom_weight, double *jac) {
+                     const float *slot_weight, const float *atom_weight, const double *box, double *jac) {
     if (cv->type == ORC_RGYR) {
         /* PAPER.md:L189 RadiusofGyration. Reading R-RG: Rg^2 = sum w|r-c|^2 / sum w,
          * same weights as the barycenter; dRg/dr_i = w_i (r_i - c)/(W Rg). */
-        double c[3], W;
-        group_center(cv, 0, pos, ps, slot_atom, slot_weight, atom_weight, c, &W);
+        double c[3], W, first[3], r[3];
+        group_center(cv, 0, pos, ps, slot_atom, slot_weight, atom_weight, box, c, &W);
         long long n = group_count(cv, 0);
+        atom_image(pos, ps, group_atom(cv, 0, 0, slot_atom), NULL, NULL, first);
         double s2 = 0;
         for (long long i = 0; i < n; ++i) {
             long long a = group_atom(cv, 0, i, slot_atom);
             double w = group_weight(cv, 0, i, slot_weight, atom_weight);
-            double d[3] = {(double)pos[a * ps] - c[0], (double)pos[a * ps + 1] - c[1], (double)pos[a * ps + 2] - c[2]};
+            atom_image(pos, ps, a, first, box, r);
+            double d[3] = {r[0] - c[0], r[1] - c[1], r[2] - c[2]};
             s2 += w * v_dot(d, d);
         }
         double rg = sqrt(s2 / W);
         if (jac) for (long long i = 0; i < n; ++i) {
             long long a = group_atom(cv, 0, i, slot_atom);
             double w = group_weight(cv, 0, i, slot_weight, atom_weight);
+            atom_image(pos, ps, a, first, box, r);
             for (int x = 0; x < 3; ++x)
-                jac[3 * i + x] = rg > 0 ? w * ((double)pos[a * ps + x] - c[x]) / (W * rg) : 0.0;
+                jac[3 * i + x] = rg > 0 ? w * (r[x] - c[x]) / (W * rg) : 0.0;
         }
         return rg;
     }
     double c[4][3], W[4], dc[4][3];
-    for (int g = 0; g < cv->n_groups; ++g) group_center(cv, g, pos, ps, slot_atom, slot_weight, atom_weight, c[g], &W[g]);
-    double xi = point_cv(cv, c, dc);
+    for (int g = 0; g < cv->n_groups; ++g) group_center(cv, g, pos, ps, slot_atom, slot_weight, atom_weight, box, c[g], &W[g]);
+    double xi = point_cv(cv, c, dc, box);
     if (jac) {
         long long o = 0;
         for (int g = 0; g < cv->n_groups; ++g) {
@@ -222,6 +247,11 @@ static double cv_one(const orc_cv *cv, const float *pos, int ps, const int *slot
         }
     }
     return xi;
+}
+
+/* NULL when no direction is periodic */
+static const double *orc_box(const orc_layout *L) {
+    return (L->box[0] > 0 || L->box[1] > 0 || L->box[2] > 0) ? L->box : NULL;
 }
 
 static long long cv_natoms(const orc_cv *cv) {
@@ -249,7 +279,7 @@ void orc_cv_eval(const orc_layout *L, const orc_cv *cvs, const int *slot_atom, c
         long long o = 0;
         for (int k = 0; k < L->n_cv; ++k) {
             double *j = jac ? jac + ((long long)r * rows + o) * 3 : NULL;
-            xi[(long long)r * L->n_cv + k] = cv_one(&cvs[k], p, L->pos_stride, sa, slot_weight, atom_weight, j);
+            xi[(long long)r * L->n_cv + k] = cv_one(&cvs[k], p, L->pos_stride, sa, slot_weight, atom_weight, orc_box(L), j);
             o += cv_natoms(&cvs[k]);
         }
     }
@@ -401,7 +431,7 @@ void orc_apply_forces(const orc_layout *L, const orc_cv *cvs, const int *slot_at
             const int *sa = slot_atom + (L->per_replica_slots ? (long long)r * L->n_slots : 0);
             for (int k = 0; k < L->n_cv; ++k) {
                 const orc_cv *cv = &cvs[k];
-                cv_one(cv, p, L->pos_stride, sa, slot_weight, atom_weight, jac);
+                cv_one(cv, p, L->pos_stride, sa, slot_weight, atom_weight, orc_box(L), jac);
                 double dv = dVdxi[(long long)r * L->n_cv + k];
                 long long o = 0;
                 for (int g = 0; g < cv->n_groups; ++g) {
