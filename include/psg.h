@@ -102,6 +102,16 @@ int psg_set_layout(psg_ctx* ctx, int n_replicas, long long n_atoms, long long re
 int psg_set_cvs(psg_ctx* ctx, int n_cv, const psg_cv_desc* cvs, int n_slots, const int* slot_atom_idx,
                 int per_replica_indices, const float* slot_weight, const float* atom_weight);
 
+/* Minimum-image convention for periodic POSITIONS (the paper is silent: Fig. 3 and App. A subtract raw coordinates,
+ * PAPER.md:L230, L466, reading R-MI).  box [3] (host): orthorhombic box lengths, 0 = open
+ * in that direction; NULL or all zeros switches it off (the default after psg_set_layout).  With a box, (i) the atoms of
+ * an explicit group are taken as the images nearest to the group's FIRST atom before the barycenter / radius of gyration
+ * is formed (a molecule split by wrapping is made whole; the group must be smaller than half the box), and (ii) the
+ * displacement vectors between group centres in Distance, Angle and Dihedral are nearest images.  Component reads the
+ * centre as is.  Explicit groups only: PSG_EINVAL if a CV has a contiguous-range group (large groups are taken as
+ * given); call after psg_set_cvs. */
+int psg_set_box(psg_ctx* ctx, const double* box);
+
 /* Harmonic bias, PAPER.md:L125 (Sec. 2.1.1): V = 1/2 sum_k k_k (xi_k - xi0_k)^2, differences of periodic
  * CVs wrapped to the nearest image.  kspring [n_cv], centers [R][n_cv] (host). Selects the method. */
 int psg_set_harmonic(psg_ctx* ctx, const float* kspring, const float* centers);

@@ -123,6 +123,7 @@ int psg_set_cvs(psg_ctx* c, int n_cv, const psg_cv_desc* cvs, int n_slots, const
     SysParams P = c->sys;
     P.n_cv = n_cv; P.n_slots = n_slots; P.per_rep = per_rep ? 1 : 0;
     P.n_groups = 0; P.n_ranges = 0; P.any_rgyr = 0;
+    P.has_box = 0; P.box[0] = P.box[1] = P.box[2] = 0.0;   // psg_set_box comes after psg_set_cvs
     P.span_begin = P.N; P.span_end = 0;
     std::vector<int> slot_gid(n_slots > 0 ? n_slots : 1, -1);
     for (int k = 0; k < n_cv; ++k) {
@@ -204,6 +205,23 @@ int psg_set_cvs(psg_ctx* c, int n_cv, const psg_cv_desc* cvs, int n_slots, const
     CK(c, cudaMemset(c->d_bin, 0xff, R * sizeof(int)));
     c->sys = P;
     c->have_cvs = true; c->have_jac = false; c->method = PSG_METHOD_NONE;
+    return PSG_OK;
+}
+
+int psg_set_box(psg_ctx* c, const double* box) {
+    if (!c) return PSG_EINVAL;
+    if (!c->have_cvs) return fail(c, PSG_ESTATE, "psg_set_box: call psg_set_cvs first");
+    bool on = false;
+    if (box)
+        for (int x = 0; x < 3; ++x) {
+            if (!(box[x] >= 0.0)) return fail(c, PSG_EINVAL, "psg_set_box: box lengths must be >= 0");
+            on |= box[x] > 0.0;
+        }
+    if (on && c->sys.n_ranges > 0)
+        return fail(c, PSG_EINVAL, "psg_set_box: the minimum-image convention covers explicit groups only; this ctx has range groups");
+    c->sys.has_box = on ? 1 : 0;
+    for (int x = 0; x < 3; ++x) c->sys.box[x] = on ? box[x] : 0.0;
+    c->have_jac = false;
     return PSG_OK;
 }
 

@@ -18,15 +18,28 @@ __device__ __forceinline__ D3 cross(D3 a, D3 b) {
     return D3{a.y * b.z - a.z * b.y, a.z * b.x - a.x * b.z, a.x * b.y - a.y * b.x};
 }
 
-// xi = f(c_0..c_3) and, if JAC, dxi/dc_g into dc[0..3] (zero where undefined).
+// Minimum-image convention (reading R-MI; the paper is silent on periodic positions): box = nullptr or the three
+// orthorhombic box lengths, 0 = open in that direction.  d <- d - L rint(d / L).
+__device__ __forceinline__ D3 min_image(D3 d, const double* box) {
+    if (box) {
+        if (box[0] > 0.0) d.x -= box[0] * rint(d.x / box[0]);
+        if (box[1] > 0.0) d.y -= box[1] * rint(d.y / box[1]);
+        if (box[2] > 0.0) d.z -= box[2] * rint(d.z / box[2]);
+    }
+    return d;
+}
+__device__ __forceinline__ const double* sys_box(const SysParams& P) { return P.has_box ? P.box : nullptr; }
+
+// xi = f(c_0..c_3) and, if JAC, dxi/dc_g into dc[0..3] (zero where undefined). Displacements between centres are nearest
+// images when a box is given.
 template <bool JAC>
-__device__ __forceinline__ double cv_from_centers(int type, int axis, const D3* c, D3* dc) {
+__device__ __forceinline__ double cv_from_centers(int type, int axis, const D3* c, D3* dc, const double* box = nullptr) {
     if (JAC) {
 #pragma unroll
         for (int g = 0; g < 4; ++g) dc[g] = d3(0, 0, 0);
     }
     if (type == PSG_CV_DISTANCE) {
-        D3 d = c[1] - c[0];
+        D3 d = min_image(c[1] - c[0], box);
         double r = sqrt(dot(d, d));
         if (JAC && r > 0.0) {
             double ir = 1.0 / r;
@@ -37,7 +50,7 @@ __device__ __forceinline__ double cv_from_centers(int type, int axis, const D3* 
     }
     if (type == PSG_CV_ANGLE) {
         // vertex at the second group; theta = atan2(|u x v|, u.v)
-        D3 u = c[0] - c[1], v = c[2] - c[1];
+        D3 u = min_image(c[0] - c[1], box), v = min_image(c[2] - c[1], box);
         D3 n = cross(u, v);
         double nn = sqrt(dot(n, n));
         double th = atan2(nn, dot(u, v));
@@ -50,7 +63,7 @@ __device__ __forceinline__ double cv_from_centers(int type, int axis, const D3* 
         return th;
     }
     if (type == PSG_CV_DIHEDRAL) {
-        D3 b1 = c[1] - c[0], b2 = c[2] - c[1], b3 = c[3] - c[2];
+        D3 b1 = min_image(c[1] - c[0], box), b2 = min_image(c[2] - c[1], box), b3 = min_image(c[3] - c[2], box);
         D3 m = cross(b1, b2), n = cross(b2, b3);
         double l2 = dot(b2, b2), l = sqrt(l2);
         double phi = atan2(l * dot(b1, n), dot(m, n));
@@ -130,9 +143,12 @@ __device__ __forceinline__ void warp_cv_eval(const SysParams& P, int r, const fl
         const GroupDev& G = P.grp[lane];
         const int* sa = P.slot_atom + (P.per_rep ? (long long)r * P.n_slots : 0);
         double sx = 0, sy = 0, sz = 0, sw = 0, s2 = 0;
+        const double* box = sys_box(P);
+        const D3 first = load_pos(p, sa[G.begin], P.ps);
         for (int i = 0; i < G.size; ++i) {
             int s = G.begin + i;
             D3 x = load_pos(p, sa[s], P.ps);
+            if (box) x = first + min_image(x - first, box);   // the image nearest to the group's first atom
             double w = P.slot_weight ? (double)P.slot_weight[s] : 1.0;
             sx += w * x.x; sy += w * x.y; sz += w * x.z; sw += w;
             s2 += w * dot(x, x);
@@ -159,7 +175,7 @@ __device__ __forceinline__ void warp_cv_eval(const SysParams& P, int r, const fl
 #pragma unroll
             for (int g = 0; g < 4; ++g)
                 c[g] = g < C.n_groups ? d3(sm.cen[g0 + g][0], sm.cen[g0 + g][1], sm.cen[g0 + g][2]) : d3(0, 0, 0);
-            sm.xi[lane] = cv_from_centers<JAC>(C.type, C.axis, c, dc);
+            sm.xi[lane] = cv_from_centers<JAC>(C.type, C.axis, c, dc, sys_box(P));
             if (JAC) {
 #pragma unroll
                 for (int g = 0; g < 4; ++g)
@@ -183,6 +199,10 @@ __device__ __forceinline__ D3 slot_jacobian(const SysParams& P, int r, const flo
     if (sm.coef[gid] != 0.0) {   // explicit RGYR group: w (r - c) / (W Rg)
         const int* sa = P.slot_atom + (P.per_rep ? (long long)r * P.n_slots : 0);
         D3 x = load_pos(pos + (long long)r * P.rstride * P.ps, sa[s], P.ps);
+        if (P.has_box) {
+            const D3 first = load_pos(pos + (long long)r * P.rstride * P.ps, sa[P.grp[gid].begin], P.ps);
+            x = first + min_image(x - first, P.box);
+        }
         double k = w * sm.coef[gid];
         j = d3(k * (x.x - sm.cen[gid][0]), k * (x.y - sm.cen[gid][1]), k * (x.z - sm.cen[gid][2]));
     }

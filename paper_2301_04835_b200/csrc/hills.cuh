@@ -234,9 +234,11 @@ __device__ __forceinline__ double thread_cv(const SysParams& P, int r, int k, co
                 c[g] = load_pos(p, P.per_rep ? sa[G.begin] : P.slot_atom_c[G.begin], P.ps);
             } else {
                 double sx = 0, sy = 0, sz = 0, sw = 0;
+                const D3 first = load_pos(p, P.per_rep ? sa[G.begin] : P.slot_atom_c[G.begin], P.ps);
                 for (int i = 0; i < G.size; ++i) {
                     int s = G.begin + i;
                     D3 x = load_pos(p, P.per_rep ? sa[s] : P.slot_atom_c[s], P.ps);
+                    if (P.has_box) x = first + min_image(x - first, P.box);   // the image nearest to the group's first atom
                     double w = P.slot_weight ? (double)P.slot_weight[s] : 1.0;
                     sx += w * x.x; sy += w * x.y; sz += w * x.z; sw += w;
                 }
@@ -246,7 +248,7 @@ __device__ __forceinline__ double thread_cv(const SysParams& P, int r, int k, co
             }
         }
     }
-    double xi = cv_from_centers<JAC>(C.type, C.axis, c, dc);
+    double xi = cv_from_centers<JAC>(C.type, C.axis, c, dc, sys_box(P));
     if (JAC) {
 #pragma unroll
         for (int g = 0; g < 4; ++g)

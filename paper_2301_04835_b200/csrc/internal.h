@@ -37,6 +37,8 @@ struct SysParams {
     int ps, fs;                 // floats per atom in pos / force
     int n_cv, n_slots, per_rep, n_groups, n_ranges;
     int any_rgyr;
+    int has_box;                // minimum-image convention on (psg_set_box); explicit groups only
+    double box[3];              // orthorhombic box lengths, 0 = open in that direction
     CvDev cv[PSG_MAX_CV];
     GroupDev grp[PSG_MAX_GROUPS_TOTAL];
     int range_gid[PSG_MAX_RANGE_GROUPS];     // range id -> global group id

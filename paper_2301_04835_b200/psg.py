@@ -20,7 +20,7 @@ _KIND = {"distance": CV_DISTANCE, "angle": CV_ANGLE, "dihedral": CV_DIHEDRAL, "c
 
 # every symbol include/psg.h declares
 EXPORTS = ["psg_create", "psg_destroy", "psg_set_stream", "psg_last_error", "psg_set_layout", "psg_set_cvs",
-           "psg_set_harmonic", "psg_set_metad", "psg_set_hill_precision", "psg_load_hills", "psg_get_hills",
+           "psg_set_box", "psg_set_harmonic", "psg_set_metad", "psg_set_hill_precision", "psg_load_hills", "psg_get_hills",
            "psg_set_abf", "psg_abf_state", "psg_cv_eval", "psg_bias_eval", "psg_deposit_hill", "psg_abf_update",
            "psg_apply_bias_forces", "psg_step", "psg_step_outputs", "psg_step_host", "psg_sync_check",
            "psg_measure_alu_peak", "psg_launch_count"]
@@ -64,6 +64,7 @@ def load_library():
         L.psg_set_stream.argtypes = [vp, vp]
         L.psg_set_layout.argtypes = [vp, i, ll, ll, i, i]
         L.psg_set_cvs.argtypes = [vp, i, C.POINTER(_CvDesc), i, vp, i, vp, vp]
+        L.psg_set_box.argtypes = [vp, vp]
         L.psg_set_harmonic.argtypes = [vp, vp, vp]
         L.psg_set_metad.argtypes = [vp, vp, f, f, i, i]
         L.psg_set_hill_precision.argtypes = [vp, i]
@@ -180,6 +181,11 @@ class Context:
         k3, p_aw = _hp(atom_weight, np.float32)
         self._ck(self._L.psg_set_cvs(self._h, len(cvs), arr, n_slots, p_sa, per_rep, p_sw, p_aw))
         self.n_cv, self.n_slots = len(cvs), n_slots
+
+    def set_box(self, box):
+        """orthorhombic box lengths [3] for the minimum-image convention (0 = open); None switches it off"""
+        k1, p1 = _hp(None if box is None else np.asarray(box, np.float64), np.float64)
+        self._ck(self._L.psg_set_box(self._h, p1))
 
     def set_harmonic(self, kspring, centers):
         k1, p1 = _hp(kspring, np.float32)

@@ -737,6 +737,74 @@ def test_step_is_cuda_graph_capturable(torch, psg):
     assert np.allclose(d_f.cpu().numpy(), ref.cpu().numpy(), rtol=3e-7, atol=1e-9)
 
 
+# ------------------------------------------------------------------------------------ minimum image
+def _wrapped(w, pos, box):
+    """the same atoms as an engine with periodic boundaries stores them: every coordinate wrapped into [0, L)"""
+    p = pos.copy()
+    p[..., :3] = np.mod(p[..., :3].astype(np.float64), np.asarray(box)).astype(np.float32)
+    return p
+
+
+@pytest.mark.parametrize("cfg", [1, 2, 4])
+def test_minimum_image_step_matches_oracle(torch, psg, cfg):
+    """psg_set_box: with every atom wrapped into a box SMALLER than the molecules' excursions, the fused steps (k_hills
+    prologue, k_abf_step) and psg_cv_eval give the oracle's minimum-image CVs, Jacobians and forces; ADP chains are
+    ~0.5 nm across, the box is 1.3 nm, so most replicas have groups on both sides of a face"""
+    w = small(cfg)
+    box = (1.3, 1.45, 1.6) if cfg != 2 else (4.7, 5.1, 4.9)
+    if cfg == 4:
+        box = (3.9, 4.1, 4.3)       # the distance pair of config 4 is up to 1.5 nm apart: L/2 must exceed it
+    ctx = make_ctx(psg, w)
+    ctx.set_box(box)
+    cvs = [{"type": {"distance": orc.DISTANCE, "angle": orc.ANGLE, "dihedral": orc.DIHEDRAL, "component": orc.COMPONENT,
+                     "rgyr": orc.RGYR}[cv["kind"]], "groups": cv["groups"], "axis": cv["axis"], "period": cv["period"]}
+           for cv in w.cvs]
+    sysm = orc.System(w.R, w.N, 0 if w.shared_array else w.N, 4, cvs, w.slot_atom, None, w.atom_weight, box=box)
+    pos = _wrapped(w, w.positions(1), box)
+    f0 = w.forces0()
+    centers = heights = abf_state = fs = None
+    if w.method == "metad":
+        centers, heights = w.params["hill_centers"], oracle_heights(w)
+        ctx.load_hills(dev(torch, centers), dev(torch, heights))
+    if w.method == "abf":
+        nb = int(np.prod(w.params["shape"]))
+        abf_state, fs = (np.zeros(nb, np.int32), np.zeros((nb, 2), np.float64)), w.fsample(1)
+    # separate call first: CVs and the compact Jacobian
+    d_pos = dev(torch, pos)
+    d_xi = torch.empty((w.R, w.n_cv), device="cuda")
+    d_jac = torch.empty((w.R, w.slot_atom.shape[-1], 3), device="cuda")
+    ctx.cv_eval(d_pos, d_xi, d_jac)
+    xi_ref, jac_ref = sysm.cv_eval(pos)
+    assert_close(d_xi.cpu().numpy(), xi_ref, "xi (minimum image)", period=w.period)
+    assert_close(d_jac.cpu().numpy(), jac_ref[:, slot_rows(w)], "Jacobian (minimum image)")
+    # the open-boundary result differs for the replicas that straddle a face: the box is really in play
+    open_sys = oracle_system(w)
+    assert np.abs(wrap(open_sys.cv_eval(pos, want_jac=False) - xi_ref, w.period)).max() > 1e-2
+    # fused step
+    d_f = dev(torch, f0)
+    ctx.step(d_pos, d_f, None if fs is None else dev(torch, fs), 1)
+    ctx.sync_check()
+    out = {k: v.cpu().numpy() for k, v in ctx.read_step_outputs().items()}
+    xi_ref, b, f_ref = oracle_step(w, sysm, pos, f0, centers, heights, abf_state, fs)
+    if w.method == "abf":
+        assert np.array_equal(out["bin"], b["bin"])
+    _check_step(w, sysm, pos, out["xi"], out.get("V"), out["dVdxi"], d_f.cpu().numpy(), f0, xi_ref, b, f_ref,
+                what=f"minimum image, config {cfg}: ")
+
+
+def test_set_box_validation(torch, psg):
+    w = small(3)
+    ctx = make_ctx(psg, w)
+    with pytest.raises(psg.PsgError):
+        ctx.set_box((3.0, 3.0, 3.0))          # range groups are taken as given
+    ctx.set_box(None)                          # switching it off is always fine
+    w1 = small(1)
+    c1 = make_ctx(psg, w1)
+    with pytest.raises(psg.PsgError):
+        c1.set_box((3.0, -1.0, 3.0))
+    c1.set_box((0.0, 0.0, 0.0))
+
+
 # ------------------------------------------------------------------------------------ error behaviour
 def test_argument_validation(torch, psg):
     ctx = psg.Context(0)
