@@ -26,7 +26,11 @@
  * Parity unpinned (no passage, closed form or invariant fixes them; they follow
  * DESIGN.md readings only): the order of simultaneous deposits by several
  * walkers (orc_deposit_hills), the two-phase mean-force read of a shared ABF
- * grid (orc_abf_update), the stride phase of deposits.
+ * grid (orc_abf_update), the stride phase of deposits.  The minimum-image
+ * convention (orc_layout.box, reading R-MI) is a reading too -- the paper is
+ * silent on periodic positions -- but its arithmetic is pinned
+ * (tests/test_oracle_minimum_image.py: geometries across a face, box-vector
+ * shift invariance, finite differences).
  */
 #include <math.h>
 #include <stdlib.h>
