@@ -223,16 +223,32 @@ __device__ __forceinline__ double thread_cv(const SysParams& P, int r, int k, co
     const int* sa = P.slot_atom + (P.per_rep ? (long long)r * P.n_slots : 0);
     D3 c[4];
     double W[4];
+    // Fast path (measured: the gather, not the arithmetic, was half of the prologue): every group a single unweighted
+    // atom -- a single atom is its own barycenter -- so all indices are formed first and the four position loads are in
+    // flight together instead of one dependent (index -> position) chain per group.
+    bool single = !P.slot_weight;
 #pragma unroll
-    for (int g = 0; g < 4; ++g) {
-        c[g] = d3(0, 0, 0);
-        W[g] = 1.0;
-        if (g < C.n_groups) {
-            const GroupDev& G = P.grp[C.gid0 + g];
-            if (G.size == 1 && !P.slot_weight) {
-                // a single unweighted atom is its own barycenter; shared index lists come from kernel parameters
-                c[g] = load_pos(p, P.per_rep ? sa[G.begin] : P.slot_atom_c[G.begin], P.ps);
-            } else {
+    for (int g = 0; g < 4; ++g)
+        if (g < C.n_groups) single = single && P.grp[C.gid0 + g].size == 1;
+    if (single) {
+        long long a[4];
+#pragma unroll
+        for (int g = 0; g < 4; ++g) {
+            const int s = P.grp[C.gid0 + (g < C.n_groups ? g : 0)].begin;   // unused groups re-read group 0 (no branch)
+            a[g] = P.per_rep ? sa[s] : P.slot_atom_c[s];                    // shared index lists come from kernel parameters
+        }
+#pragma unroll
+        for (int g = 0; g < 4; ++g) {
+            c[g] = load_pos(p, a[g], P.ps);
+            W[g] = 1.0;
+        }
+    } else {
+#pragma unroll
+        for (int g = 0; g < 4; ++g) {
+            c[g] = d3(0, 0, 0);
+            W[g] = 1.0;
+            if (g < C.n_groups) {
+                const GroupDev& G = P.grp[C.gid0 + g];
                 double sx = 0, sy = 0, sz = 0, sw = 0;
                 const D3 first = load_pos(p, P.per_rep ? sa[G.begin] : P.slot_atom_c[G.begin], P.ps);
                 for (int i = 0; i < G.size; ++i) {
