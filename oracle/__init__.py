@@ -138,6 +138,20 @@ class System:
                           _p(pos, C.c_float), _p(xi, C.c_double), _p(jac, C.c_double))
         return (xi, jac) if want_jac else xi
 
+    def abf_estimate(self, pos, vel, mass, dt, fbias_prev, whist, first):
+        """ABF instantaneous-force estimator (reading R-ABF-EST): returns (fsample [R][n_cv], W [R][n_cv]); ``whist``
+        [R][2][n_cv] float64 is advanced in place; ``fbias_prev`` [R][n_cv] or None."""
+        pos, vel, mass = _f32(pos), _f32(vel), _f32(mass)
+        assert whist.dtype == np.float64 and whist.flags.c_contiguous and whist.shape == (self.R, 2, self.n_cv)
+        fb = None if fbias_prev is None else _f64(fbias_prev)
+        fs = np.empty((self.R, self.n_cv), np.float64)
+        w = np.empty((self.R, self.n_cv), np.float64)
+        lib().orc_abf_estimate(C.byref(self.layout), self.cvs, _p(self.slot_atom, C.c_int), _p(self.slot_weight, C.c_float),
+                               _p(self.atom_weight, C.c_float), _p(pos, C.c_float), _p(vel, C.c_float), _p(mass, C.c_float),
+                               C.c_double(float(dt)), _p(fb, C.c_double), _p(whist, C.c_double), C.c_int(1 if first else 0),
+                               _p(fs, C.c_double), _p(w, C.c_double))
+        return fs, w
+
     def apply_forces(self, pos, dVdxi, force):
         """force: fp64 [n_arrays][N][3] (n_arrays = 1 if shared else R); returns the updated copy."""
         pos = _f32(pos)

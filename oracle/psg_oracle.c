@@ -30,7 +30,10 @@
  * convention (orc_layout.box, reading R-MI) is a reading too -- the paper is
  * silent on periodic positions -- but its arithmetic is pinned
  * (tests/test_oracle_minimum_image.py: geometries across a face, box-vector
- * shift invariance, finite differences).
+ * shift invariance, finite differences).  The ABF force estimator
+ * (orc_abf_estimate, reading R-ABF-EST) is a reading as well -- the paper only
+ * cites its reference [43] -- with its arithmetic pinned by closed-form
+ * trajectories and numpy's least squares (tests/test_oracle_abf_estimator.py).
  */
 #include <math.h>
 #include <stdlib.h>
@@ -448,5 +451,81 @@ void orc_apply_forces(const orc_layout *L, const orc_cv *cvs, const int *slot_at
             }
         }
         free(jac);
+    }
+}
+
+/* ABF instantaneous-force estimator.  PAPER.md:L143 says only "based on the algorithm described
+ * in [43]" (Darve et al. 2008, not available here), so this follows SURVEY.md 8(f) / DESIGN.md reading R-ABF-EST:
+ *   J[k][i] = d xi_k / d r_i over the atoms of the CVs (contributions of one atom to one CV through several slots add),
+ *   p_i = m_i v_i,   G = J J^T  (n_cv x n_cv),   b = J p,   solve G W = b,
+ *   dW/dt = (3/2 W(t) - 2 W(t - dt) + 1/2 W(t - 2 dt)) / dt      (second-order backward difference),
+ *   fsample = dW/dt + Fbias_prev       (Fbias_prev = the mean force dV/dxi applied at the previous step: the atoms felt
+ *                                       -Fbias_prev J, which is added back to recover the unbiased generalized force).
+ * whist [R][2][n_cv] holds W(t - dt), W(t - 2 dt) and is advanced; first != 0 initialises both to W(t) (dW/dt = 0).
+ * vel has the layout of pos; mass [n_atoms] is shared by the replicas.  A singular G gives W = 0 for that replica.
+ * Pins: a constant and a linearly growing force on a free particle are recovered exactly (the difference formula is exact
+ * for quadratics), W equals the least-squares solution of J^T W = p, momentum orthogonal to every row of J gives 0. */
+void orc_abf_estimate(const orc_layout *L, const orc_cv *cvs, const int *slot_atom, const float *slot_weight,
+                      const float *atom_weight, const float *pos, const float *vel, const float *mass, double dt,
+                      const double *fbias_prev /*[R][n_cv], nullable = 0*/, double *whist /*[R][2][n_cv]*/, int first,
+                      double *fsample /*[R][n_cv]*/, double *w_out /*[R][n_cv], nullable*/) {
+    const int n_cv = L->n_cv;
+    long long maxrows = 0;
+    for (int k = 0; k < n_cv; ++k) { long long n = cv_natoms(&cvs[k]); if (n > maxrows) maxrows = n; }
+    for (int r = 0; r < L->n_replicas; ++r) {
+        const float *p = pos + (long long)r * L->replica_stride_atoms * L->pos_stride;
+        const float *v = vel + (long long)r * L->replica_stride_atoms * L->pos_stride;
+        const int *sa = slot_atom + (L->per_replica_slots ? (long long)r * L->n_slots : 0);
+        /* dense rows of J over the atoms of this replica's array would be huge: keep (atom, vector) lists per CV */
+        double *jac[4]; long long *atoms[4]; long long na[4];
+        for (int k = 0; k < n_cv; ++k) {
+            na[k] = cv_natoms(&cvs[k]);
+            jac[k] = (double *)malloc(sizeof(double) * 3 * (size_t)na[k]);
+            atoms[k] = (long long *)malloc(sizeof(long long) * (size_t)na[k]);
+            cv_one(&cvs[k], p, L->pos_stride, sa, slot_weight, atom_weight, orc_box(L), jac[k]);
+            long long o = 0;
+            for (int g = 0; g < cvs[k].n_groups; ++g)
+                for (long long i = 0; i < group_count(&cvs[k], g); ++i) atoms[k][o++] = group_atom(&cvs[k], g, i, sa);
+        }
+        double G[4][4] = {{0}}, b[4] = {0}, W[4] = {0};
+        for (int k = 0; k < n_cv; ++k) {
+            for (long long i = 0; i < na[k]; ++i) {
+                long long a = atoms[k][i];
+                double m = (double)mass[a];
+                for (int x = 0; x < 3; ++x) b[k] += jac[k][3 * i + x] * m * (double)v[a * L->pos_stride + x];
+                for (int l = 0; l < n_cv; ++l)
+                    for (long long j = 0; j < na[l]; ++j)
+                        if (atoms[l][j] == a)
+                            for (int x = 0; x < 3; ++x) G[k][l] += jac[k][3 * i + x] * jac[l][3 * j + x];
+            }
+        }
+        /* Gaussian elimination with partial pivoting on the augmented matrix */
+        double A[4][5];
+        int ok = 1;
+        for (int k = 0; k < n_cv; ++k) { for (int l = 0; l < n_cv; ++l) A[k][l] = G[k][l]; A[k][n_cv] = b[k]; }
+        for (int c = 0; c < n_cv && ok; ++c) {
+            int piv = c;
+            for (int k = c + 1; k < n_cv; ++k) if (fabs(A[k][c]) > fabs(A[piv][c])) piv = k;
+            if (!(fabs(A[piv][c]) > 0)) { ok = 0; break; }
+            if (piv != c) for (int l = 0; l <= n_cv; ++l) { double t = A[c][l]; A[c][l] = A[piv][l]; A[piv][l] = t; }
+            for (int k = c + 1; k < n_cv; ++k) {
+                double f = A[k][c] / A[c][c];
+                for (int l = c; l <= n_cv; ++l) A[k][l] -= f * A[c][l];
+            }
+        }
+        if (ok) for (int k = n_cv - 1; k >= 0; --k) {
+            double s = A[k][n_cv];
+            for (int l = k + 1; l < n_cv; ++l) s -= A[k][l] * W[l];
+            W[k] = s / A[k][k];
+        }
+        double *h1 = whist + ((long long)r * 2 + 0) * n_cv, *h2 = whist + ((long long)r * 2 + 1) * n_cv;
+        for (int k = 0; k < n_cv; ++k) {
+            if (first) { h1[k] = W[k]; h2[k] = W[k]; }
+            double dW = (1.5 * W[k] - 2.0 * h1[k] + 0.5 * h2[k]) / dt;
+            fsample[(long long)r * n_cv + k] = dW + (fbias_prev ? fbias_prev[(long long)r * n_cv + k] : 0.0);
+            if (w_out) w_out[(long long)r * n_cv + k] = W[k];
+            h2[k] = h1[k]; h1[k] = W[k];
+        }
+        for (int k = 0; k < n_cv; ++k) { free(jac[k]); free(atoms[k]); }
     }
 }
