@@ -159,6 +159,18 @@ int psg_deposit_hill(psg_ctx* ctx, const float* d_xi, const unsigned char* d_mas
  *  d_fsample [R][n_cv] in;  d_bin [R] out nullable;  d_dVdxi [R][n_cv] out. */
 int psg_abf_update(psg_ctx* ctx, const float* d_xi, const float* d_fsample, int* d_bin, float* d_dVdxi);
 
+/* ABF instantaneous generalized-force estimator.  The paper says only "based on the algorithm
+ * described in [43]"; this is DESIGN.md reading R-ABF-EST: with J[k][i] = d xi_k/d r_i and momenta
+ * p_i = m_i v_i of the CV atoms, solve (J J^T) W = J p per replica; d_fsample[r][k] := (3/2 W(t) - 2 W(t - dt)
+ * + 1/2 W(t - 2 dt)) / dt + d_fbias_prev[r][k], the last term being the mean force dV/dxi applied at the previous step
+ * (NULL = 0).  The result is the `d_fsample` input of psg_abf_update / psg_step.  The history W(t - dt), W(t - 2 dt) is
+ * ctx-owned; the first call after setup or psg_abf_estimate_reset initialises it to W(t) (so the first sample is
+ * d_fbias_prev alone).  d_vel has the layout of d_pos; d_mass [n_atoms] (device) is shared by the replicas.  A singular
+ * J J^T gives W = 0 for that replica.  Explicit groups only (PSG_EINVAL with range groups). */
+int psg_abf_estimate(psg_ctx* ctx, const float* d_pos, const float* d_vel, const float* d_mass, double dt,
+                     const float* d_fbias_prev, float* d_fsample);
+int psg_abf_estimate_reset(psg_ctx* ctx);
+
 /* force[i] += -sum_k dVdxi[r][k] * d(xi_k)/d(r_i), using the Jacobian cached by the last
  * psg_cv_eval on these positions (PSG_ESTATE if there was none).  d_force in/out. */
 int psg_apply_bias_forces(psg_ctx* ctx, const float* d_pos, const float* d_dVdxi, float* d_force);

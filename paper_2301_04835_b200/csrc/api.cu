@@ -71,7 +71,7 @@ int psg_create(psg_ctx** out, int device, void* cuda_stream) {
 static void free_all(psg_ctx* c) {
     dfree(c->d_slot_atom); dfree(c->d_slot_gid); dfree(c->d_slot_weight); dfree(c->d_atom_weight);
     dfree(c->d_xi); dfree(c->d_V); dfree(c->d_dVdxi); dfree(c->d_bin); dfree(c->d_V64);
-    dfree(c->d_jac); dfree(c->d_gdesc); dfree(c->d_rpart); dfree(c->d_arrive); dfree(c->d_rdesc); dfree(c->d_gbar);
+    dfree(c->d_jac); dfree(c->d_gdesc); dfree(c->d_rpart); dfree(c->d_arrive); dfree(c->d_rdesc); dfree(c->d_gbar); dfree(c->d_whist);
     dfree(c->d_kspring); dfree(c->d_centers);
     dfree(c->md.hills); dfree(c->md.heights); dfree(c->md.n_hills); dfree(c->md.part); dfree(c->md.ticket);
     if (c->abf.own) { dfree(c->abf.hist); dfree(c->abf.fsum); }
@@ -197,6 +197,9 @@ int psg_set_cvs(psg_ctx* c, int n_cv, const psg_cv_desc* cvs, int n_slots, const
     CK(c, dalloc(c->d_rpart, R * P.n_ranges * (size_t)P.range_blocks * PSG_MOM));
     CK(c, dalloc(c->d_arrive, 2 * R));
     CK(c, cudaMemset(c->d_arrive, 0, 2 * R * sizeof(unsigned)));
+    CK(c, dalloc(c->d_whist, R * 2 * n_cv));
+    CK(c, cudaMemset(c->d_whist, 0, R * 2 * n_cv * sizeof(double)));
+    c->est_first = true;
     CK(c, dalloc(c->d_gbar, 2));
     CK(c, cudaMemset(c->d_gbar, 0, 2 * sizeof(unsigned)));
     CK(c, dalloc(c->d_rdesc, R * P.n_ranges * 4));
@@ -405,6 +408,23 @@ int psg_abf_update(psg_ctx* c, const float* d_xi, const float* d_fsample, int* d
     if (c->method != PSG_METHOD_ABF) return fail(c, PSG_ESTATE, "psg_abf_update: ABF is not selected");
     if (!d_xi || !d_fsample || !d_dVdxi) return fail(c, PSG_EINVAL, "psg_abf_update: NULL pointer");
     CK(c, psg_launch_abf(c, d_xi, d_fsample, d_bin, d_dVdxi));
+    return PSG_OK;
+}
+
+int psg_abf_estimate(psg_ctx* c, const float* d_pos, const float* d_vel, const float* d_mass, double dt, const float* d_fbias_prev,
+                     float* d_fsample) {
+    if (!c) return PSG_EINVAL;
+    if (!c->have_cvs) return fail(c, PSG_ESTATE, "psg_abf_estimate: no CVs configured");
+    if (!d_pos || !d_vel || !d_mass || !d_fsample) return fail(c, PSG_EINVAL, "psg_abf_estimate: NULL pointer");
+    if (!(dt > 0.0)) return fail(c, PSG_EINVAL, "psg_abf_estimate: dt must be > 0");
+    if (c->sys.n_ranges > 0) return fail(c, PSG_EINVAL, "psg_abf_estimate: explicit groups only (this ctx has range groups)");
+    CK(c, psg_launch_abf_estimate(c, d_pos, d_vel, d_mass, dt, d_fbias_prev, d_fsample));
+    return PSG_OK;
+}
+
+int psg_abf_estimate_reset(psg_ctx* c) {
+    if (!c) return PSG_EINVAL;
+    c->est_first = true;
     return PSG_OK;
 }
 

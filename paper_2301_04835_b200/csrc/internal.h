@@ -104,6 +104,8 @@ struct psg_ctx {
     double* d_gdesc = nullptr;       // [R][n_groups][PSG_GDESC_DOUBLES]
     double* d_rpart = nullptr;       // [R][n_ranges][range_blocks][PSG_MOM]
     unsigned* d_arrive = nullptr;    // [2][R]: arrive / done counters of the fused range step (zero between launches)
+    double* d_whist = nullptr;       // [R][2][n_cv]: W(t - dt), W(t - 2 dt) of the ABF force estimator
+    bool est_first = true;           // the next psg_abf_estimate initialises the history
     unsigned* d_gbar = nullptr;      // [2]: grid-barrier counters of the fused ABF step (zero between launches)
     float4* d_rdesc = nullptr;       // [R][n_ranges][4]: tagged force descriptors of the fused range step (zero between launches)
     // harmonic
@@ -128,6 +130,8 @@ cudaError_t psg_launch_null_hills(psg_ctx* c, int begin, int end);   // records 
 cudaError_t psg_launch_abf(psg_ctx* c, const float* d_xi, const float* d_fsample, int* d_bin, float* d_dVdxi);
 cudaError_t psg_launch_metad_step(psg_ctx* c, const float* d_pos, float* d_force);   // fused; n_ranges == 0
 bool psg_metad_step_supported(const psg_ctx* c);
+cudaError_t psg_launch_abf_estimate(psg_ctx* c, const float* d_pos, const float* d_vel, const float* d_mass, double dt,
+                                    const float* d_fbias_prev, float* d_fsample);
 bool psg_abf_step_supported(const psg_ctx* c);
 cudaError_t psg_launch_abf_step(psg_ctx* c, const float* d_pos, const float* d_fsample, float* d_force);   // fused ABF step
 bool psg_range_step_supported(const psg_ctx* c, const float* d_pos, const float* d_force);

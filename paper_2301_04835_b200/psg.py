@@ -22,7 +22,7 @@ _KIND = {"distance": CV_DISTANCE, "angle": CV_ANGLE, "dihedral": CV_DIHEDRAL, "c
 EXPORTS = ["psg_create", "psg_destroy", "psg_set_stream", "psg_last_error", "psg_set_layout", "psg_set_cvs",
            "psg_set_box", "psg_set_harmonic", "psg_set_metad", "psg_set_hill_precision", "psg_load_hills", "psg_get_hills",
            "psg_set_abf", "psg_abf_state", "psg_cv_eval", "psg_bias_eval", "psg_deposit_hill", "psg_abf_update",
-           "psg_apply_bias_forces", "psg_step", "psg_step_outputs", "psg_step_host", "psg_sync_check",
+           "psg_abf_estimate", "psg_abf_estimate_reset", "psg_apply_bias_forces", "psg_step", "psg_step_outputs", "psg_step_host", "psg_sync_check",
            "psg_measure_alu_peak", "psg_launch_count"]
 
 
@@ -76,6 +76,8 @@ def load_library():
         L.psg_bias_eval.argtypes = [vp, vp, vp, vp]
         L.psg_deposit_hill.argtypes = [vp, vp, vp]
         L.psg_abf_update.argtypes = [vp, vp, vp, vp, vp]
+        L.psg_abf_estimate.argtypes = [vp, vp, vp, vp, C.c_double, vp, vp]
+        L.psg_abf_estimate_reset.argtypes = [vp]
         L.psg_apply_bias_forces.argtypes = [vp, vp, vp, vp]
         L.psg_step.argtypes = [vp, vp, vp, vp, ll]
         L.psg_step_outputs.argtypes = [vp, C.POINTER(vp), C.POINTER(vp), C.POINTER(vp), C.POINTER(vp)]
@@ -252,6 +254,14 @@ class Context:
         t = self._torch
         self._ck(self._L.psg_abf_update(self._h, _dp(d_xi, t.float32), _dp(d_fsample, t.float32), _dp(d_bin, t.int32),
                                         _dp(d_dVdxi, t.float32)))
+
+    def abf_estimate(self, d_pos, d_vel, d_mass, dt, d_fbias_prev, d_fsample):
+        t = self._torch
+        self._ck(self._L.psg_abf_estimate(self._h, _dp(d_pos, t.float32), _dp(d_vel, t.float32), _dp(d_mass, t.float32),
+                                          float(dt), _dp(d_fbias_prev, t.float32), _dp(d_fsample, t.float32)))
+
+    def abf_estimate_reset(self):
+        self._ck(self._L.psg_abf_estimate_reset(self._h))
 
     def apply_bias_forces(self, d_pos, d_dVdxi, d_force):
         t = self._torch

@@ -805,6 +805,82 @@ def test_set_box_validation(torch, psg):
     c1.set_box((0.0, 0.0, 0.0))
 
 
+# ------------------------------------------------------------------------------------ ABF force estimator
+@pytest.mark.parametrize("cfg,R", [(1, 70), (2, 300), (4, 130)])
+def test_abf_force_estimator_matches_oracle(torch, psg, cfg, R):
+    """psg_abf_estimate over five MD steps of a synthetic trajectory (positions and velocities change every step, a bias is
+    fed back from the second step on) against the oracle's reading R-ABF-EST: dihedral pairs that share three atoms
+    (config 1), barycenter groups (config 2), per-replica index lists on a shared array with colliding walkers (config 4).
+    The sample is a difference quotient of W over dt, so its rounding floor is ~ulp(W)/dt: compared with
+    |d| <= max(1e-5 |ref|, 1e-6, 4e-7 * max|W| / dt)."""
+    w = small(cfg) if cfg != 1 else small(cfg, R=R)
+    ctx = make_ctx(psg, w, with_method=False)
+    sysm = oracle_system(w)
+    rng = np.random.default_rng(1000 + cfg)
+    n_arr = 1 if w.shared_array else w.R
+    mass = rng.uniform(1.0, 16.0, size=w.N).astype(np.float32)
+    dt = 0.002
+    hist = np.zeros((w.R, 2, w.n_cv))
+    d_fs = torch.empty((w.R, w.n_cv), device="cuda")
+    d_mass = dev(torch, mass)
+    vel0 = rng.normal(scale=0.5, size=(n_arr, w.N, 4)).astype(np.float32)
+    for step in range(5):
+        pos = w.positions(step % w.K)
+        vel = (vel0 + 0.05 * step * rng.normal(size=vel0.shape)).astype(np.float32)
+        fb = None if step == 0 else rng.normal(scale=20.0, size=(w.R, w.n_cv)).astype(np.float32)
+        ctx.abf_estimate(dev(torch, pos), dev(torch, vel), d_mass, dt, None if fb is None else dev(torch, fb), d_fs)
+        ctx.sync_check()
+        ref, W = sysm.abf_estimate(pos, vel, mass, dt, fb, hist, first=(step == 0))
+        got = d_fs.cpu().numpy()
+        tol = np.maximum(np.maximum(1e-5 * np.abs(ref), 1e-6), 4e-7 * np.abs(W).max(axis=0) / dt)
+        assert np.all(np.abs(got - ref) <= tol), f"step {step}: max err {np.abs(got - ref).max()}"
+    # after a reset the history starts again: the sample is the fed-back bias alone
+    ctx.abf_estimate_reset()
+    fb = np.full((w.R, w.n_cv), 3.5, np.float32)
+    ctx.abf_estimate(dev(torch, pos), dev(torch, vel), d_mass, dt, dev(torch, fb), d_fs)
+    assert np.array_equal(d_fs.cpu().numpy(), fb)
+
+
+def test_abf_estimator_feeds_the_abf_step(torch, psg):
+    """estimator -> psg_step (ABF) -> the mean force of that step fed back to the next estimate: the chained device path
+    against the same chain in the oracle, bins and histogram bit-exact"""
+    w = small(2)
+    ctx = make_ctx(psg, w)
+    sysm = oracle_system(w)
+    rng = np.random.default_rng(77)
+    mass = rng.uniform(1.0, 16.0, size=w.N).astype(np.float32)
+    dt = 0.002
+    nb = int(np.prod(w.params["shape"]))
+    abf = (np.zeros(nb, np.int32), np.zeros((nb, 2), np.float64))
+    hist = np.zeros((w.R, 2, w.n_cv))
+    d_fs = torch.empty((w.R, w.n_cv), device="cuda")
+    d_f = dev(torch, w.forces0())
+    fb_ref = None
+    d_fb = None
+    for step in range(1, 5):
+        pos = w.positions(step % w.K)
+        # velocities with a strong common drift along the CV directions keep the samples same-sign dominated
+        vel = (rng.normal(scale=0.02, size=(w.R, w.N, 4)) + 0.3 * step).astype(np.float32)
+        ctx.abf_estimate(dev(torch, pos), dev(torch, vel), dev(torch, mass), dt, d_fb, d_fs)
+        ctx.step(dev(torch, pos), d_f, d_fs, step)
+        ctx.sync_check()
+        out = ctx.read_step_outputs()
+        fs_ref, _ = sysm.abf_estimate(pos, vel, mass, dt, fb_ref, hist, first=(step == 1))
+        fs_gpu = d_fs.cpu().numpy()
+        # the oracle's chain continues from the DEVICE's binary32 samples, so that a last-bit difference of a sample cannot
+        # move a walker across a bin edge of the comparison (the sample itself is compared above and here)
+        assert np.all(np.abs(fs_gpu - fs_ref) <= np.maximum(np.maximum(1e-5 * np.abs(fs_ref), 1e-6), 4e-7 * 50.0 / dt))
+        xi_ref = sysm.cv_eval(pos, want_jac=False)
+        b = oracle_bias(w, xi_ref.astype(np.float32), None, None, abf, fs_gpu)
+        assert np.array_equal(out["bin"].cpu().numpy(), b["bin"])
+        assert_close(out["dVdxi"].cpu().numpy(), b["dVdxi"], f"mean force, step {step}")
+        fb_ref = out["dVdxi"].cpu().numpy().astype(np.float64)
+        d_fb = out["dVdxi"]
+    hp, fp, nbins = ctx.abf_state()
+    from paper_2301_04835_b200.psg import _view
+    assert np.array_equal(_view(hp, (nbins,), torch.int32, 0).cpu().numpy(), abf[0])
+
+
 # ------------------------------------------------------------------------------------ error behaviour
 def test_argument_validation(torch, psg):
     ctx = psg.Context(0)
