@@ -28,7 +28,7 @@ struct EstSmem {
                                                            // shared memory (in registers they would be demoted to local memory)
 };
 
-__global__ void __launch_bounds__(128) k_abf_estimate(const __grid_constant__ SysParams P, const __grid_constant__ AbfEstArgs A) {
+__global__ void __launch_bounds__(128, 8) k_abf_estimate(const __grid_constant__ SysParams P, const __grid_constant__ AbfEstArgs A) {
     __shared__ EstSmem sm[4];
     const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
     EstSmem& S = sm[wid];
