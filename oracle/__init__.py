@@ -19,8 +19,8 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 _SRC = os.path.join(_HERE, "psg_oracle.c")
 _SO = os.path.join(_HERE, "libpsg_oracle.so")
 
-DISTANCE, ANGLE, DIHEDRAL, COMPONENT, RGYR = 1, 2, 3, 4, 5
-_NGROUPS = {DISTANCE: 2, ANGLE: 3, DIHEDRAL: 4, COMPONENT: 1, RGYR: 1}
+DISTANCE, ANGLE, DIHEDRAL, COMPONENT, RGYR, DISPLACEMENT = 1, 2, 3, 4, 5, 6
+_NGROUPS = {DISTANCE: 2, ANGLE: 3, DIHEDRAL: 4, COMPONENT: 1, RGYR: 1, DISPLACEMENT: 2}
 
 
 def build(force: bool = False) -> str:

@@ -42,7 +42,7 @@
 #include <omp.h>
 #endif
 
-enum { ORC_DISTANCE = 1, ORC_ANGLE = 2, ORC_DIHEDRAL = 3, ORC_COMPONENT = 4, ORC_RGYR = 5 };
+enum { ORC_DISTANCE = 1, ORC_ANGLE = 2, ORC_DIHEDRAL = 3, ORC_COMPONENT = 4, ORC_RGYR = 5, ORC_DISPLACEMENT = 6 };
 
 /* One collective variable: a function of 1..4 *groups* of atoms, each group
  * reduced to its (weighted) barycenter -- PAPER.md:L185-L189 (Sec. 2.2:
@@ -57,7 +57,7 @@ typedef struct {
     int slot_size[4];
     long long range_begin[4];
     long long range_size[4];
-    int axis;       /* ORC_COMPONENT: 0, 1 or 2 */
+    int axis;       /* ORC_COMPONENT, ORC_DISPLACEMENT: 0, 1 or 2 */
     double period;  /* 0 = not periodic */
 } orc_cv;
 
@@ -201,6 +201,11 @@ static double point_cv(const orc_cv *cv, double c[4][3], double dc[4][3], const 
             }
         }
         return phi;
+    }
+    case ORC_DISPLACEMENT: { /* PAPER.md:L185 Displacement (TwoPointCV): the vector c2 - c1; one CV per component (axis) */
+        double d[3]; v_sub(c[1], c[0], d); min_image(d, box);
+        dc[1][cv->axis] = 1.0; dc[0][cv->axis] = -1.0;
+        return d[cv->axis];
     }
     case ORC_COMPONENT: /* PAPER.md:L188 Component: barycenter coordinate along an axis */
         dc[0][cv->axis] = 1.0;

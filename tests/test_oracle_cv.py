@@ -310,3 +310,34 @@ def test_replica_layout_shared_vs_own_arrays():
     for r in range(R):
         x1, _ = orc.System(1, N, N, 4, cvs, idx2[r]).cv_eval(pos[0])
         assert np.array_equal(xi2[r], x1[0])
+
+
+# ---------------------------------------------------------------------------- Displacement
+def test_displacement_components_and_distance_agree():
+    """the three Displacement components of two weighted groups are the barycenter difference, their norm is the Distance
+    CV of the same groups, and each Jacobian row is +-(w_i / W) e_axis"""
+    rng = np.random.default_rng(21)
+    xyz = rng.normal(size=(5, 3))
+    w = np.array([1.0, 3.0, 2.0, 2.0, 4.0], np.float32)
+    groups = [[0, 1], [2, 3, 4]]
+    c1 = (w[:2, None] * xyz[:2]).sum(0) / w[:2].sum()
+    c2 = (w[2:, None] * xyz[2:]).sum(0) / w[2:].sum()
+    comps = []
+    for ax in range(3):
+        s = _sys(orc.DISPLACEMENT, 5, groups, weights=w, axis=ax)
+        xi, jac = s.cv_eval(_pos4(xyz)[None])
+        assert xi[0, 0] == pytest.approx((c2 - c1)[ax], abs=1e-6)
+        want = np.zeros((5, 3))
+        want[:2, ax] = -w[:2] / w[:2].sum()
+        want[2:, ax] = w[2:] / w[2:].sum()
+        assert np.allclose(jac[0], want, atol=1e-12)
+        comps.append(xi[0, 0])
+    d = _sys(orc.DISTANCE, 5, groups, weights=w).cv_eval(_pos4(xyz)[None], want_jac=False)[0, 0]
+    assert math.sqrt(sum(c * c for c in comps)) == pytest.approx(d, rel=1e-12)
+
+
+def test_displacement_minimum_image():
+    cv = {"type": orc.DISPLACEMENT, "groups": [("slots", 0, 1), ("slots", 1, 1)], "axis": 0, "period": 0.0}
+    s = orc.System(1, 2, 2, 4, [cv], np.array([0, 1], np.int32), box=(3.0, 0.0, 0.0))
+    xi = s.cv_eval(_pos4([[0.1, 0, 0], [2.9, 0, 0]])[None], want_jac=False)
+    assert xi[0, 0] == pytest.approx(-0.2, abs=1e-6)
