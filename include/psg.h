@@ -51,7 +51,8 @@ enum {
     PSG_CV_ANGLE = 2,         /* ThreePointCV Angle at the 2nd group, in [0, pi]        (L186) */
     PSG_CV_DIHEDRAL = 3,      /* FourPointCV DihedralAngle in (-pi, pi], IUPAC sign     (L187, L81) */
     PSG_CV_COM_COMPONENT = 4, /* AxisCV Component: barycenter coordinate along an axis  (L188) */
-    PSG_CV_RGYR = 5           /* RadiusofGyration: sqrt(sum w|r-c|^2 / sum w)           (L189) */
+    PSG_CV_RGYR = 5,          /* RadiusofGyration: sqrt(sum w|r-c|^2 / sum w)           (L189) */
+    PSG_CV_DISPLACEMENT = 6   /* TwoPointCV Displacement c2 - c1: one CV per component (axis) (L185) */
 };
 
 enum { PSG_METHOD_NONE = 0, PSG_METHOD_HARMONIC = 1, PSG_METHOD_METAD = 2, PSG_METHOD_ABF = 3 };
@@ -69,13 +70,13 @@ enum {
 
 typedef struct {
     int type;                            /* PSG_CV_* */
-    int n_groups;                        /* 2, 3, 4, 1, 1 for the five types */
+    int n_groups;                        /* 2, 3, 4, 1, 1, 2 for the six types */
     int group_is_range[PSG_MAX_GROUPS];  /* 0: explicit atoms (a slice of the slot list); 1: contiguous atom range */
     int group_begin[PSG_MAX_GROUPS];     /* explicit: slots [begin, begin + size) */
     int group_size[PSG_MAX_GROUPS];
     long long range_begin[PSG_MAX_GROUPS]; /* range: atoms [range_begin, range_begin + range_size) of the replica's array */
     long long range_size[PSG_MAX_GROUPS];
-    int axis;                            /* PSG_CV_COM_COMPONENT: 0, 1, 2 */
+    int axis;                            /* PSG_CV_COM_COMPONENT, PSG_CV_DISPLACEMENT: 0, 1, 2 */
     double period;                       /* 0 = not periodic; 2*pi for a dihedral (binary64: the wrap must not lose bits) */
 } psg_cv_desc;
 

@@ -81,6 +81,14 @@ __device__ __forceinline__ double cv_from_centers(int type, int axis, const D3* 
         }
         return phi;
     }
+    if (type == PSG_CV_DISPLACEMENT) {   // PAPER.md:L185 Displacement: component `axis` of c2 - c1
+        const D3 d = min_image(c[1] - c[0], box);
+        if (JAC) {
+            dc[1] = d3(axis == 0 ? 1.0 : 0.0, axis == 1 ? 1.0 : 0.0, axis == 2 ? 1.0 : 0.0);
+            dc[0] = (-1.0) * dc[1];
+        }
+        return axis == 0 ? d.x : (axis == 1 ? d.y : d.z);
+    }
     if (type == PSG_CV_COM_COMPONENT) {
         if (JAC) dc[0] = d3(axis == 0 ? 1.0 : 0.0, axis == 1 ? 1.0 : 0.0, axis == 2 ? 1.0 : 0.0);
         return axis == 0 ? c[0].x : (axis == 1 ? c[0].y : c[0].z);

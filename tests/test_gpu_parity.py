@@ -881,6 +881,46 @@ def test_abf_estimator_feeds_the_abf_step(torch, psg):
     assert np.array_equal(_view(hp, (nbins,), torch.int32, 0).cpu().numpy(), abf[0])
 
 
+def test_displacement_cv_harmonic_step(torch, psg):
+    """Displacement: the three components of the barycenter difference of two weighted
+    explicit groups as three CVs, harmonically restrained, through psg_cv_eval and the whole step, with and without a box"""
+    rng = np.random.default_rng(31)
+    R, N = 37, 60
+    xyz = rng.uniform(0.0, 3.0, size=(R, N, 3)).astype(np.float32)
+    pos = np.concatenate([xyz, rng.normal(size=(R, N, 1)).astype(np.float32)], axis=2)
+    slots = np.array([3, 7, 11, 20, 21], np.int32)
+    wts = np.array([1.0, 12.0, 16.0, 1.0, 14.0], np.float32)
+    grp = [("slots", 0, 3), ("slots", 3, 2)]
+    for box in (None, (3.0, 3.0, 3.0)):
+        ctx = psg.Context(0)
+        ctx.set_layout(R, N, N, 4, 4)
+        # every slot belongs to exactly one (CV, group): the three CVs list the five atoms three times
+        sl = np.concatenate([slots, slots, slots])
+        cvs = [{"type": psg.CV_DISPLACEMENT, "groups": [("slots", 5 * ax, 3), ("slots", 5 * ax + 3, 2)], "axis": ax, "period": 0.0}
+               for ax in range(3)]
+        ctx.set_cvs(cvs, sl, np.concatenate([wts, wts, wts]))
+        if box is not None:
+            ctx.set_box(box)
+        k = np.array([300.0, 500.0, 700.0], np.float32)
+        cen = rng.normal(scale=0.3, size=(R, 3)).astype(np.float32)
+        ctx.set_harmonic(k, cen)
+        o_cvs = [{"type": orc.DISPLACEMENT, "groups": c["groups"], "axis": c["axis"], "period": 0.0} for c in cvs]
+        sysm = orc.System(R, N, N, 4, o_cvs, sl, np.concatenate([wts, wts, wts]), None, box=box)
+        f0 = rng.normal(scale=100.0, size=(R, N, 4)).astype(np.float32)
+        d_f = dev(torch, f0)
+        ctx.step(dev(torch, pos), d_f, None, 1)
+        ctx.sync_check()
+        out = {kk: v.cpu().numpy() for kk, v in ctx.read_step_outputs().items()}
+        xi_ref = sysm.cv_eval(pos, want_jac=False)
+        V, dV = orc.harmonic(xi_ref.astype(np.float32).astype(np.float64), k, cen, np.zeros(3))
+        f_ref = sysm.apply_forces(pos, dV, f0[..., :3].astype(np.float64))
+        assert_close(out["xi"], xi_ref, "displacement xi")
+        assert_close(out["V"], V, "V")
+        assert_close(out["dVdxi"], dV, "dV/dxi")
+        assert_forces_close(d_f.cpu().numpy()[..., :3], f_ref, f0[..., :3], "forces")
+        ctx.close()
+
+
 # ------------------------------------------------------------------------------------ error behaviour
 def test_argument_validation(torch, psg):
     ctx = psg.Context(0)
