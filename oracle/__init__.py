@@ -218,3 +218,20 @@ def abf_update(xi_f32, fsample_f32, lower, upper, shape, periodic, n_threshold, 
                          _p(_i32(periodic), C.c_int), C.c_int(n_threshold), _p(hist, C.c_int),
                          _p(fsum, C.c_double), _p(b, C.c_int), _p(dV, C.c_double))
     return b, dV
+
+
+def dist_to_interface(pos, mobile_idx, mobile_w, ibegin, n_i, axis, sigma, scope, bins, coeff):
+    """DistanceToInterface of ONE replica (Sec. 2.2.1 / App. A): pos float32 [N][stride].
+    Returns (xi, jac_mobile [n_m][3], dxi_dx [n_i], mass [bins])."""
+    pos = _f32(pos)
+    idx = _i32(np.asarray(mobile_idx))
+    wm = _f32(mobile_w)
+    xi = C.c_double(0.0)
+    jm = np.zeros((len(idx), 3), np.float64)
+    dx = np.zeros(int(n_i), np.float64)
+    mass = np.zeros(int(bins), np.float64)
+    lib().orc_dist_to_interface(_p(pos, C.c_float), C.c_int(pos.shape[-1]), C.c_int(len(idx)), _p(idx, C.c_int), _p(wm, C.c_float),
+                                C.c_longlong(int(ibegin)), C.c_longlong(int(n_i)), C.c_int(int(axis)), C.c_double(float(sigma)),
+                                C.c_double(float(scope[0])), C.c_double(float(scope[1])), C.c_int(int(bins)), C.c_double(float(coeff)),
+                                C.byref(xi), _p(jm, C.c_double), _p(dx, C.c_double), _p(mass, C.c_double))
+    return xi.value, jm, dx, mass

@@ -534,3 +534,66 @@ void orc_abf_estimate(const orc_layout *L, const orc_cv *cvs, const int *slot_at
         for (int k = 0; k < n_cv; ++k) { free(jac[k]); free(atoms[k]); }
     }
 }
+
+/* DistanceToInterface, the paper's own worked CV: PAPER.md:L203-L290 (Sec. 2.2.1, Eq. 4-8) and the
+ * listing of Appendix A (L444-L475), followed line by line, for ONE replica:
+ *   mobile_axis   = barycenter(p1)[axis]                                   (weighted by wm, NULL = 1)
+ *   positions     = coordinate `axis` of every atom of p2                  (atoms [ibegin, ibegin + n_i) of the array)
+ *   centers_j     = linspace(scope0, scope1, bins)
+ *   mass_j        = sum_i exp(-1/2 ((x_i - centers_j) / sigma)^2)          (Eq. 6)
+ *   mass_diff_j   = |mass_{j+1} - mass_j|,  centers_mean_j = (centers_{j+1} + centers_j) / 2      (Eq. 7 up to 1/delta)
+ *   probability   = softmax(mass_diff * coeff);  interface = sum_j probability_j centers_mean_j   (Eq. 8)
+ *   xi            = mobile_axis - interface
+ * Derivatives (the paper takes them by autodiff; written out here): d xi/d r_m = (w_m / W) e_axis for mobile atoms;
+ * for interface atoms d xi/d x_i = -sum_j G_j d mass_j/d x_i with d mass_j/d x_i = -e_ij (x_i - centers_j)/sigma^2 and
+ * G_j = d interface/d mass_j = coeff [ s_{j-1} p_{j-1} (cm_{j-1} - I) - s_j p_j (cm_j - I) ], s_j = sign(mass_{j+1} - mass_j).
+ * Outputs: *xi; jac_mobile [n_m][3]; dxi_dx [n_i] (nullable); mass_out [bins] (nullable). */
+void orc_dist_to_interface(const float *pos, int ps, int n_m, const int *mobile_idx, const float *wm, long long ibegin,
+                           long long n_i, int axis, double sigma, double scope0, double scope1, int bins, double coeff,
+                           double *xi, double *jac_mobile, double *dxi_dx, double *mass_out) {
+    double W = 0, mob = 0;
+    for (int m = 0; m < n_m; ++m) {
+        double w = wm ? (double)wm[m] : 1.0;
+        mob += w * (double)pos[(long long)mobile_idx[m] * ps + axis];
+        W += w;
+    }
+    mob /= W;
+    double *c = (double *)malloc(sizeof(double) * (size_t)bins), *mass = (double *)calloc((size_t)bins, sizeof(double));
+    for (int j = 0; j < bins; ++j) c[j] = bins > 1 ? scope0 + (scope1 - scope0) * (double)j / (double)(bins - 1) : scope0;
+    for (int j = 0; j < bins; ++j)
+        for (long long i = 0; i < n_i; ++i) {
+            double d = ((double)pos[(ibegin + i) * ps + axis] - c[j]) / sigma;
+            mass[j] += exp(-0.5 * d * d);
+        }
+    int nb = bins - 1;
+    double *md = (double *)malloc(sizeof(double) * (size_t)nb), *p = (double *)malloc(sizeof(double) * (size_t)nb);
+    double mx = -INFINITY, Z = 0, I = 0;
+    for (int j = 0; j < nb; ++j) { md[j] = fabs(mass[j + 1] - mass[j]); if (md[j] * coeff > mx) mx = md[j] * coeff; }
+    for (int j = 0; j < nb; ++j) { p[j] = exp(md[j] * coeff - mx); Z += p[j]; }      /* softmax, shifted by its maximum */
+    for (int j = 0; j < nb; ++j) { p[j] /= Z; I += p[j] * 0.5 * (c[j + 1] + c[j]); }
+    *xi = mob - I;
+    if (jac_mobile)
+        for (int m = 0; m < n_m; ++m)
+            for (int x = 0; x < 3; ++x) jac_mobile[3 * m + x] = x == axis ? (wm ? (double)wm[m] : 1.0) / W : 0.0;
+    if (dxi_dx) {
+        double *G = (double *)calloc((size_t)bins, sizeof(double));
+        for (int j = 0; j < nb; ++j) {
+            double diff = mass[j + 1] - mass[j];
+            double s = diff > 0 ? 1.0 : (diff < 0 ? -1.0 : 0.0);
+            double t = coeff * s * p[j] * (0.5 * (c[j + 1] + c[j]) - I);   /* d I / d md_j times the sign of the difference */
+            G[j + 1] += t;
+            G[j] -= t;
+        }
+        for (long long i = 0; i < n_i; ++i) {
+            double x = (double)pos[(ibegin + i) * ps + axis], dI = 0;
+            for (int j = 0; j < bins; ++j) {
+                double d = x - c[j];
+                dI += G[j] * (-exp(-0.5 * (d / sigma) * (d / sigma)) * d / (sigma * sigma));
+            }
+            dxi_dx[i] = -dI;
+        }
+        free(G);
+    }
+    if (mass_out) memcpy(mass_out, mass, sizeof(double) * (size_t)bins);
+    free(c); free(mass); free(md); free(p);
+}
