@@ -199,6 +199,23 @@ int psg_step_host(psg_ctx* ctx, const float* h_pos, float* h_force, const float*
 /* The only other call that synchronises: waits for the ctx stream and returns sticky CUDA errors. */
 int psg_sync_check(psg_ctx* ctx);
 
+/* ------------------------------------------------------------- DistanceToInterface */
+/* The paper's own worked collective variable (Eq. 4-8; listing of Appendix A), for all
+ * replicas of the ctx layout (psg_set_layout), as a set of calls of its own (it is not a psg_cv_desc type yet):
+ *   xi = barycenter(mobile atoms)[axis] - sum_j softmax(coeff |mass_{j+1} - mass_j|)_j (c_{j+1} + c_j) / 2,
+ *   mass_j = sum_i exp(-(x_i - c_j)^2 / (2 sigma^2)) over the interface atoms, c = linspace(scope0, scope1, bins).
+ * psg_interface_cv_set (host arrays copied; allocates): mobile_idx [n_mobile <= PSG_MAX_SLOTS] 0-based, mobile_w nullable
+ *   (= 1); interface atoms = the contiguous range [iface_begin, iface_begin + iface_size) of every replica's array;
+ *   2 <= bins <= 1024.
+ * psg_interface_cv_eval: d_xi [R] out; also keeps d interface / d mass_j per replica for the apply call.
+ * psg_interface_cv_apply: force[i][axis] += -d_dVdxi[r] * d xi / d x_i for interface and mobile atoms of replica r, with
+ *   the derivatives written out analytically (the paper obtains them by autodiff); call after psg_interface_cv_eval on
+ *   the same positions.  Both enqueue on the ctx stream, no sync.  All arithmetic is binary64 (see interface_cv.cu). */
+int psg_interface_cv_set(psg_ctx* ctx, int n_mobile, const int* mobile_idx, const float* mobile_w, long long iface_begin,
+                         long long iface_size, int axis, double sigma, double scope0, double scope1, int bins, double coeff);
+int psg_interface_cv_eval(psg_ctx* ctx, const float* d_pos, float* d_xi);
+int psg_interface_cv_apply(psg_ctx* ctx, const float* d_pos, const float* d_dVdxi, float* d_force);
+
 /* ------------------------------------------------------------- measurement */
 /* Measured ALU throughput of this device (register-only loops, CUDA-event timed, synchronises):
  * which = 0: FP32 FFMA lane-ops/s; 1: packed FFMA2 (f32x2) lane-ops/s (2 per lane per instruction);

@@ -77,6 +77,7 @@ static void free_all(psg_ctx* c) {
     if (c->abf.own) { dfree(c->abf.hist); dfree(c->abf.fsum); }
     c->abf.hist = nullptr; c->abf.fsum = nullptr;
     dfree(c->d_pos_stage); dfree(c->d_frc_stage); dfree(c->d_fs_stage);
+    psg_interface_cv_free(c);
 }
 
 int psg_destroy(psg_ctx* c) {

@@ -116,7 +116,9 @@ struct psg_ctx {
     // host-engine staging (psg_step_host)
     float* d_pos_stage = nullptr; float* d_frc_stage = nullptr; float* d_fs_stage = nullptr;
     int sm_count = 148;
+    void* dti = nullptr;             // state of the DistanceToInterface CV (interface_cv.cu)
 };
+void psg_interface_cv_free(psg_ctx* c);
 
 // ---- launchers implemented in the .cu files (all enqueue on ctx->stream) ----
 cudaError_t psg_launch_cv_eval(psg_ctx* c, const float* d_pos, float* d_xi, float* d_jac);

@@ -23,7 +23,7 @@ EXPORTS = ["psg_create", "psg_destroy", "psg_set_stream", "psg_last_error", "psg
            "psg_set_box", "psg_set_harmonic", "psg_set_metad", "psg_set_hill_precision", "psg_load_hills", "psg_get_hills",
            "psg_set_abf", "psg_abf_state", "psg_cv_eval", "psg_bias_eval", "psg_deposit_hill", "psg_abf_update",
            "psg_abf_estimate", "psg_abf_estimate_reset", "psg_apply_bias_forces", "psg_step", "psg_step_outputs", "psg_step_host", "psg_sync_check",
-           "psg_measure_alu_peak", "psg_launch_count"]
+           "psg_interface_cv_set", "psg_interface_cv_eval", "psg_interface_cv_apply", "psg_measure_alu_peak", "psg_launch_count"]
 
 
 class PsgError(RuntimeError):
@@ -83,6 +83,10 @@ def load_library():
         L.psg_step_outputs.argtypes = [vp, C.POINTER(vp), C.POINTER(vp), C.POINTER(vp), C.POINTER(vp)]
         L.psg_step_host.argtypes = [vp, vp, vp, vp, ll]
         L.psg_sync_check.argtypes = [vp]
+        d = C.c_double
+        L.psg_interface_cv_set.argtypes = [vp, i, vp, vp, ll, ll, i, d, d, d, i, d]
+        L.psg_interface_cv_eval.argtypes = [vp, vp, vp]
+        L.psg_interface_cv_apply.argtypes = [vp, vp, vp, vp]
         L.psg_measure_alu_peak.argtypes = [i, i, C.POINTER(C.c_double)]
         _lib = L
     return _lib
@@ -290,6 +294,21 @@ class Context:
             assert (not x.is_cuda) and x.is_contiguous() and x.dtype == self._torch.float32
             return C.c_void_p(x.data_ptr())
         self._ck(self._L.psg_step_host(self._h, hp(h_pos), hp(h_force), hp(h_fsample), int(step)))
+
+    # ---- DistanceToInterface (Sec. 2.2.1, App. A)
+    def interface_cv_set(self, mobile_idx, mobile_w, iface_begin, iface_size, axis, sigma, scope, bins, coeff):
+        k1, p1 = _hp(np.asarray(mobile_idx), np.int32)
+        k2, p2 = _hp(None if mobile_w is None else np.asarray(mobile_w), np.float32)
+        self._ck(self._L.psg_interface_cv_set(self._h, len(k1), p1, p2, int(iface_begin), int(iface_size), int(axis), float(sigma),
+                                              float(scope[0]), float(scope[1]), int(bins), float(coeff)))
+
+    def interface_cv_eval(self, d_pos, d_xi):
+        t = self._torch
+        self._ck(self._L.psg_interface_cv_eval(self._h, _dp(d_pos, t.float32), _dp(d_xi, t.float32)))
+
+    def interface_cv_apply(self, d_pos, d_dVdxi, d_force):
+        t = self._torch
+        self._ck(self._L.psg_interface_cv_apply(self._h, _dp(d_pos, t.float32), _dp(d_dVdxi, t.float32), _dp(d_force, t.float32)))
 
     def sync_check(self):
         self._ck(self._L.psg_sync_check(self._h))

@@ -921,6 +921,54 @@ def test_displacement_cv_harmonic_step(torch, psg):
         ctx.close()
 
 
+# ------------------------------------------------------------------------------------ DistanceToInterface
+@pytest.mark.parametrize("R,n_i,bins,axis", [(3, 700, 40, 0), (9, 5000, 100, 2), (1, 1025, 2, 1)])
+def test_distance_to_interface_matches_oracle(torch, psg, R, n_i, bins, axis):
+    """the paper's worked CV (Eq. 4-8, App. A): liquid slabs with a diffuse edge, one per replica; value and the
+    force of a harmonic restraint on it (interface atoms through the softmax, mobile atoms through the barycenter) against
+    the oracle; chunks of 1,024 atoms with a ragged tail; bins = 2 is the one-entry softmax"""
+    rng = np.random.default_rng(50 + R)
+    n_m = 3
+    N = n_m + n_i + 5
+    pos = rng.normal(scale=2.0, size=(R, N, 4)).astype(np.float32)
+    for r in range(R):
+        edge = 0.3 + 0.2 * r
+        x = np.concatenate([rng.uniform(-4.0, edge, size=n_i - n_i // 8), edge + np.abs(rng.normal(scale=0.4, size=n_i // 8))])
+        pos[r, n_m:n_m + n_i, axis] = x.astype(np.float32)
+    mob, wm = np.array([0, 2, 1], np.int32), np.array([1.0, 4.0, 2.0], np.float32)
+    sigma, scope, coeff = 0.25, (-3.0, 3.5), 0.9
+    ctx = psg.Context(0)
+    ctx.set_layout(R, N, N, 4, 4)
+    ctx.interface_cv_set(mob, wm, n_m, n_i, axis, sigma, scope, bins, coeff)
+    d_pos = dev(torch, pos)
+    d_xi = torch.empty(R, device="cuda")
+    ctx.interface_cv_eval(d_pos, d_xi)
+    ctx.sync_check()
+    ref = [orc.dist_to_interface(pos[r], mob, wm, n_m, n_i, axis, sigma, scope, bins, coeff) for r in range(R)]
+    xi_ref = np.array([q[0] for q in ref])
+    assert_close(d_xi.cpu().numpy(), xi_ref, "distance to interface")
+    k, x0 = 800.0, 0.1
+    dV = (k * (xi_ref.astype(np.float32).astype(np.float64) - x0)).astype(np.float32)
+    f0 = rng.normal(scale=100.0, size=(R, N, 4)).astype(np.float32)
+    d_f = dev(torch, f0)
+    ctx.interface_cv_apply(d_pos, dev(torch, dV), d_f)
+    ctx.sync_check()
+    f = d_f.cpu().numpy()
+    f_ref = f0[..., :3].astype(np.float64)
+    for r in range(R):
+        _, jm, dx, _ = ref[r]
+        f_ref[r, n_m:n_m + n_i, axis] += -float(dV[r]) * dx
+        for m, a in enumerate(mob):
+            f_ref[r, a] += -float(dV[r]) * jm[m]
+    assert_forces_close(f[..., :3], f_ref, f0[..., :3], "interface CV forces")
+    untouched = np.ones(N, bool)
+    untouched[n_m:n_m + n_i] = False
+    untouched[mob] = False
+    assert np.array_equal(f[:, untouched].view(np.uint32), f0[:, untouched].view(np.uint32))
+    other = [x for x in range(4) if x != axis]
+    assert np.array_equal(f[:, n_m:n_m + n_i][..., other].view(np.uint32), f0[:, n_m:n_m + n_i][..., other].view(np.uint32))
+
+
 # ------------------------------------------------------------------------------------ error behaviour
 def test_argument_validation(torch, psg):
     ctx = psg.Context(0)
