@@ -890,7 +890,6 @@ def test_displacement_cv_harmonic_step(torch, psg):
     pos = np.concatenate([xyz, rng.normal(size=(R, N, 1)).astype(np.float32)], axis=2)
     slots = np.array([3, 7, 11, 20, 21], np.int32)
     wts = np.array([1.0, 12.0, 16.0, 1.0, 14.0], np.float32)
-    grp = [("slots", 0, 3), ("slots", 3, 2)]
     for box in (None, (3.0, 3.0, 3.0)):
         ctx = psg.Context(0)
         ctx.set_layout(R, N, N, 4, 4)
