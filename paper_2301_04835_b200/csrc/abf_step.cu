@@ -38,6 +38,9 @@ __global__ void __launch_bounds__(256, 4) k_abf_step(const __grid_constant__ Sys
             const D3 j = slot_jacobian(P, r, A.pos, S, s);
             const long long o = ((long long)r * P.n_slots + s) * 3;
             A.jac[o] = (float)j.x; A.jac[o + 1] = (float)j.y; A.jac[o + 2] = (float)j.z;
+            // the force record phase 2 will update, requested into L2 now (the arrays are GBs: a cold miss otherwise)
+            const int atom = P.slot_atom[(P.per_rep ? (long long)r * P.n_slots : 0) + s];
+            asm volatile("prefetch.global.L2 [%0];" ::"l"(A.force + ((long long)r * P.rstride + atom) * P.fs));
         }
         if (lane == 0) {
             float xi[PSG_MAX_CV];

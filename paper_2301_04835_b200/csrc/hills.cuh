@@ -273,6 +273,20 @@ __device__ __forceinline__ double thread_cv(const SysParams& P, int r, int k, co
     return xi;
 }
 
+// The force records the final scatter will update, requested into L2 while the hill loop runs: with a cold L2 the
+// atomics at the end of the step otherwise wait for DRAM.
+__device__ __forceinline__ void prefetch_force_lines(const SysParams& P, int r, int k, const float* force) {
+    const CvDev& C = P.cv[k];
+    const int* sa = P.slot_atom + (P.per_rep ? (long long)r * P.n_slots : 0);
+    for (int g = 0; g < C.n_groups; ++g) {
+        const GroupDev& G = P.grp[C.gid0 + g];
+        for (int i = 0; i < G.size; ++i) {
+            const long long atom = sa[G.begin + i];
+            asm volatile("prefetch.global.L2 [%0];" ::"l"(force + ((long long)r * P.rstride + atom) * P.fs));
+        }
+    }
+}
+
 struct HillKernelArgs {
     const float4* hills;     // packed records {s0, s1, s2, log2 W} (n_cv == 4: two float4)
     const float* heights;    // W, as exported
@@ -395,6 +409,7 @@ __global__ void __launch_bounds__(HWARPS * 32, 1) k_hills(const __grid_constant_
                     s_xi[k * TILE_R + rr] = v;
                 } else if (r < R) {
                     D3 dc[4];
+                    if (chunk == 0) prefetch_force_lines(P, r, k, A.force);
                     (void)thread_cv<true>(P, r, k, A.pos, dc);
                     const CvDev& C = P.cv[k];
 #pragma unroll
