@@ -15,7 +15,8 @@
 //              dihedral / component, radius of gyration) and the harmonic bias in binary64, publishes per-group
 //              force descriptors (16-byte records carrying a valid tag).
 //   PB warp  : positions (now an L2 hit) and forces of the B group's next items -> ring B.
-//   B group  (16 warps): waits for the window's descriptors, then
+//   B group  (16 warps): takes the window's descriptors (requested one item earlier with cp.async; polls only if the
+//              window is not finished), then
 //              F_i += -dV/dxi_k * w_i (v_g + coef_g (r_i - c_g))  out of shared memory, st.global.cs float4.
 //   HBM traffic: positions once (the second read is served by L2 while `lag` x grid x 32 KB fits), forces read
 //   once and written once = 48 B/atom, the algorithmic minimum; 64 B/atom if L2 keeps nothing.
@@ -131,9 +132,11 @@ struct RsShared {
     double gv[PSG_MAX_RANGE_GROUPS][3], gcoef[PSG_MAX_RANGE_GROUPS];   // d xi / d c_g / W_g,  Rg: 1/(W Rg)
     double dv[PSG_MAX_CV];                                        // -(dV/dxi_k), through binary32 like the unfused path
     double vk[PSG_MAX_CV];                                        // 1/2 k_k D_k^2
-    float4 desc[PSG_MAX_RANGE_GROUPS][RS_DESC];                   // B group: the window's force descriptors
-    int blo[PSG_MAX_RANGE_GROUPS], bhi[PSG_MAX_RANGE_GROUPS];     // B group: slice-local atom bounds of every group
-    int bfast;                                                    // B group: the item takes the straight-line path
+    // B group, three buffers indexed by item % 3: item it computes from [it % 3] while the descriptors of item it + 1 are
+    // already arriving in [(it + 1) % 3] (cp.async) and slow warps may still read item it - 1's in [(it - 1) % 3]
+    float4 desc[3][PSG_MAX_RANGE_GROUPS][RS_DESC];                // the window's force descriptors
+    int blo[3][PSG_MAX_RANGE_GROUPS], bhi[3][PSG_MAX_RANGE_GROUPS];   // slice-local atom bounds of every group
+    int bfast[3];                                                 // the item takes the straight-line path
     long long g_b[PSG_MAX_RANGE_GROUPS], g_e[PSG_MAX_RANGE_GROUPS];   // atom range of every range group (copied once from the
                                                                   // kernel parameters)
     uint64_t a_full[RS_ASTAGES], a_empty[RS_ASTAGES], b_full[RS_BSTAGES], b_empty[RS_BSTAGES];
@@ -364,21 +367,33 @@ __device__ __forceinline__ void rs_tail(const SysParams& P, const RangeStepArgs&
 
 // B group, one item: force update of the slice; positions and forces out of shared memory, result streamed to global
 __device__ __forceinline__ void rs_phase_b(const SysParams& P, const RangeStepArgs& A, RsShared& S, const float4* __restrict__ sp,
-                                           const float4* __restrict__ sf, const RsItem& I, int tid) {
+                                           const float4* __restrict__ sf, const RsItem& I, int tid, int db, int r_next) {
 #ifdef PSG_TRACE
     const long long rs_p0_ = clock64();
 #endif
     if (tid < P.n_ranges * RS_DESC) {
+        // this thread's record was requested one item ago (cp.async, no registers held): in steady state it is already
+        // here and the L2 round trip is off the critical path; poll only if the window was not finished yet
+        asm volatile("cp.async.wait_all;" ::: "memory");
+        float4* mine = &S.desc[db][tid / RS_DESC][tid % RS_DESC];
         const float4* src = A.desc + (long long)I.r * P.n_ranges * RS_DESC + tid;
-        float4 d = rs_ld_relaxed_f4(src);
-        while (d.w != RS_TAG) {   // window not finished yet: only at pipeline start-up or if `lag` is too short
-            __nanosleep(200);
+        float4 d = *mine;
+        while (d.w != RS_TAG) {
             d = rs_ld_relaxed_f4(src);
+            if (d.w != RS_TAG) __nanosleep(200);
 #ifdef PSG_TRACE
-            if (tid == 0 && A.trace) A.trace[blockIdx.x * 32 + 24] += 1;   // polls that found the window unfinished
+            if (tid == 0 && A.trace) A.trace[blockIdx.x * 64 + 24] += 1;   // polls
 #endif
         }
-        S.desc[tid / RS_DESC][tid % RS_DESC] = d;
+        *mine = d;
+        if (r_next >= 0) {
+            float4* nxt = &S.desc[(db + 1) % 3][tid / RS_DESC][tid % RS_DESC];
+            *nxt = make_float4(0.f, 0.f, 0.f, 0.f);   // (an unpublished or skipped copy must read as invalid)
+            asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(rs_smem_u32(nxt)),
+                         "l"(A.desc + (long long)r_next * P.n_ranges * RS_DESC + tid)
+                         : "memory");
+            asm volatile("cp.async.commit_group;" ::: "memory");
+        }
     }
     if (tid >= 32 && tid < 32 + P.n_ranges) {
         // slice-local bounds of every group: the atom loop compares 32-bit offsets held in shared memory
@@ -387,8 +402,8 @@ __device__ __forceinline__ void rs_phase_b(const SysParams& P, const RangeStepAr
         const long long cnt = (long long)(I.bytes >> 4);
         if (lo < 0) lo = 0;
         if (hi > cnt) hi = cnt;
-        S.blo[tid - 32] = (int)lo;
-        S.bhi[tid - 32] = hi > lo ? (int)hi : (int)lo;
+        S.blo[db][tid - 32] = (int)lo;
+        S.bhi[db][tid - 32] = hi > lo ? (int)hi : (int)lo;
     }
     if (tid == 64) {
         // fast path: a whole slice that every group either covers completely or does not touch, and is touched at all
@@ -401,7 +416,7 @@ __device__ __forceinline__ void rs_phase_b(const SysParams& P, const RangeStepAr
             if (touch && !cover) fast = false;
             any |= cover;
         }
-        S.bfast = fast && any;
+        S.bfast[db] = fast && any;
     }
     rs_b_sync();
 #ifdef PSG_TRACE
@@ -414,13 +429,13 @@ __device__ __forceinline__ void rs_phase_b(const SysParams& P, const RangeStepAr
     float ax[RS_PERB], ay[RS_PERB], az[RS_PERB];
 #pragma unroll
     for (int i = 0; i < RS_PERB; ++i) ax[i] = ay[i] = az[i] = 0.f;
-    if (S.bfast && !P.atom_weight) {
+    if (S.bfast[db] && !P.atom_weight) {
         // the common case, straight-line: a whole slice, every group either covers all of it or none of it, unit
         // weights (x * 1.0f is x: same bits as the general loop)
         for (int q = 0; q < P.n_ranges; ++q) {
-            if (S.blo[q] >= S.bhi[q]) continue;   // uniform
-            const float4 v = S.desc[q][0], hi = S.desc[q][1], lo = S.desc[q][2];
-            const float k = S.desc[q][3].x;
+            if (S.blo[db][q] >= S.bhi[db][q]) continue;   // uniform
+            const float4 v = S.desc[db][q][0], hi = S.desc[db][q][1], lo = S.desc[db][q][2];
+            const float k = S.desc[db][q][3].x;
 #pragma unroll
             for (int i = 0; i < RS_PERB; ++i) {
                 const float4 p = sp[tid + i * RS_GTB];   // re-read per group: registers are the scarce resource
@@ -440,10 +455,10 @@ __device__ __forceinline__ void rs_phase_b(const SysParams& P, const RangeStepAr
     }
     unsigned anym = 0u;
     for (int q = 0; q < P.n_ranges; ++q) {
-        const int lo_o = S.blo[q], hi_o = S.bhi[q];
+        const int lo_o = S.blo[db][q], hi_o = S.bhi[db][q];
         if (lo_o >= hi_o) continue;   // uniform: the slice does not touch this group
-        const float4 v = S.desc[q][0], hi = S.desc[q][1], lo = S.desc[q][2];
-        const float k = S.desc[q][3].x;
+        const float4 v = S.desc[db][q][0], hi = S.desc[db][q][1], lo = S.desc[db][q][2];
+        const float k = S.desc[db][q][3].x;
 #pragma unroll
         for (int i = 0; i < RS_PERB; ++i) {
             const int o = tid + i * RS_GTB;
@@ -484,6 +499,8 @@ __global__ void __launch_bounds__(RS_THREADS, 1) k_range_step(const __grid_const
         for (int st = 0; st < RS_BSTAGES; ++st) { rs_mbar_init(&S.b_full[st], 1); rs_mbar_init(&S.b_empty[st], RS_GTB / 32); }
         for (int b = 0; b < RS_RED; ++b) { rs_mbar_init(&S.red_full[b], RS_GT / 32); rs_mbar_init(&S.red_empty[b], 1); }
         S.b_prog = 0;
+        for (int q = 0; q < PSG_MAX_RANGE_GROUPS; ++q)
+            for (int i = 0; i < RS_DESC; ++i) S.desc[0][q][i] = make_float4(0.f, 0.f, 0.f, 0.f);
         for (int q = 0; q < P.n_ranges; ++q) {
             const GroupDev& G = P.grp[P.range_gid[q]];
             S.g_b[q] = G.rbegin; S.g_e[q] = G.rbegin + G.rsize;
@@ -582,10 +599,10 @@ __global__ void __launch_bounds__(RS_THREADS, 1) k_range_step(const __grid_const
             { RS_T0; rs_mbar_wait(&S.b_full[st], (uint32_t)((it / RS_BSTAGES) & 1)); RS_ACC(0); }
             RS_GSTAMP(t == 0 && it == 0, 27);
             RS_GSTAMP(t == 0 && it == n_mine / 2, 14);
-            { RS_T0; rs_phase_b(P, A, S, sp, sp + RS_SLICE, I, t); RS_ACC(1); }
+            const int r_next = it + 1 < n_mine ? rs_item(P, it + 1, G).r : -1;
+            { RS_T0; rs_phase_b(P, A, S, sp, sp + RS_SLICE, I, t, (int)(it % 3), r_next); RS_ACC(1); }
             __syncwarp();
             if ((t & 31) == 0) rs_mbar_arrive(&S.b_empty[st]);   // this warp is done reading the stage
-            rs_b_sync();                                    // S.desc may be overwritten by the next item
             if (t == 0) {
                 S.b_prog = it + 1;
                 // the last CTA to finish a window re-arms its counters and descriptor tags for the next launch
