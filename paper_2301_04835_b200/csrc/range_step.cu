@@ -382,7 +382,7 @@ __device__ __forceinline__ void rs_phase_b(const SysParams& P, const RangeStepAr
             d = rs_ld_relaxed_f4(src);
             if (d.w != RS_TAG) __nanosleep(200);
 #ifdef PSG_TRACE
-            if (tid == 0 && A.trace) A.trace[blockIdx.x * 64 + 24] += 1;   // polls
+            if (tid == 0 && A.trace) A.trace[blockIdx.x * 32 + 24] += 1;   // polls
 #endif
         }
         *mine = d;
