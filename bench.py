@@ -43,7 +43,7 @@ def hill_eval_instr(n_cv, n_periodic):
 
 # dram__bytes_read.sum + dram__bytes_write.sum of ONE launch of the dominant kernel, from the committed ncu --set full
 # captures (profiles/r1b_*_ncu_full.md); bytes
-NCU_TRAFFIC = {1: 1.15e6, 2: 6.98e6, 3: 1.2437e9, 4: 5.35e6}
+NCU_TRAFFIC = {1: 1.23e6, 2: 8.58e6, 3: 1.2412e9, 4: 5.87e6}
 
 
 def _peaks():
