@@ -20,7 +20,9 @@ _SRC = os.path.join(_HERE, "psg_oracle.c")
 _SO = os.path.join(_HERE, "libpsg_oracle.so")
 
 DISTANCE, ANGLE, DIHEDRAL, COMPONENT, RGYR, DISPLACEMENT = 1, 2, 3, 4, 5, 6
-_NGROUPS = {DISTANCE: 2, ANGLE: 3, DIHEDRAL: 4, COMPONENT: 1, RGYR: 1, DISPLACEMENT: 2}
+PRINCIPAL_MOMENT, ASPHERICITY, ACYLINDRICITY, SHAPE_ANISOTROPY = 7, 8, 9, 10     # gyration-tensor shape CVs (R-SHAPE)
+_NGROUPS = {DISTANCE: 2, ANGLE: 3, DIHEDRAL: 4, COMPONENT: 1, RGYR: 1, DISPLACEMENT: 2,
+            PRINCIPAL_MOMENT: 1, ASPHERICITY: 1, ACYLINDRICITY: 1, SHAPE_ANISOTROPY: 1}
 
 
 def build(force: bool = False) -> str:

@@ -34,6 +34,10 @@
  * (orc_abf_estimate, reading R-ABF-EST) is a reading as well -- the paper only
  * cites its reference [43] -- with its arithmetic pinned by closed-form
  * trajectories and numpy's least squares (tests/test_oracle_abf_estimator.py).
+ * The gyration-tensor shape CVs (shape_cv, reading R-SHAPE) are named by the
+ * paper without a formula; their arithmetic is pinned by hand-computed point
+ * sets, numpy.linalg.eigvalsh, the trace identity with the pinned Rg, rotation
+ * invariance and finite differences (tests/test_oracle_shape_cv.py).
  */
 #include <math.h>
 #include <stdlib.h>
@@ -42,7 +46,9 @@
 #include <omp.h>
 #endif
 
-enum { ORC_DISTANCE = 1, ORC_ANGLE = 2, ORC_DIHEDRAL = 3, ORC_COMPONENT = 4, ORC_RGYR = 5, ORC_DISPLACEMENT = 6 };
+enum { ORC_DISTANCE = 1, ORC_ANGLE = 2, ORC_DIHEDRAL = 3, ORC_COMPONENT = 4, ORC_RGYR = 5, ORC_DISPLACEMENT = 6,
+       /* gyration-tensor shape CVs, PAPER.md:L188-L189 (reading R-SHAPE) */
+       ORC_PRINCIPAL_MOMENT = 7, ORC_ASPHERICITY = 8, ORC_ACYLINDRICITY = 9, ORC_SHAPE_ANISOTROPY = 10 };
 
 /* One collective variable: a function of 1..4 *groups* of atoms, each group
  * reduced to its (weighted) barycenter -- PAPER.md:L185-L189 (Sec. 2.2:
@@ -57,7 +63,7 @@ typedef struct {
     int slot_size[4];
     long long range_begin[4];
     long long range_size[4];
-    int axis;       /* ORC_COMPONENT, ORC_DISPLACEMENT: 0, 1 or 2 */
+    int axis;       /* ORC_COMPONENT, ORC_DISPLACEMENT: 0, 1 or 2; ORC_PRINCIPAL_MOMENT: which eigenvalue, 0 = largest */
     double period;  /* 0 = not periodic */
 } orc_cv;
 
@@ -214,11 +220,106 @@ static double point_cv(const orc_cv *cv, double c[4][3], double dc[4][3], const 
     return NAN;
 }
 
+/* Eigenvalues and eigenvectors of a symmetric 3x3 matrix by cyclic Jacobi rotations (the textbook method: each rotation
+ * J zeroes one off-diagonal pair, A <- J^T A J, V <- V J, until the off-diagonal part has vanished).  Every product is
+ * written out as a plain triple loop.  On return lam[0] >= lam[1] >= lam[2] and column k of V is the unit eigenvector of
+ * lam[k].  Pinned against numpy.linalg.eigvalsh through the CVs below (tests/test_oracle_shape_cv.py). */
+static void sym3_eig(double S[3][3], double lam[3], double V[3][3]) {
+    double A[3][3], J[3][3], T[3][3];
+    static const int pairs[3][2] = {{0, 1}, {0, 2}, {1, 2}};
+    for (int i = 0; i < 3; ++i) for (int j = 0; j < 3; ++j) { A[i][j] = S[i][j]; V[i][j] = i == j ? 1.0 : 0.0; }
+    for (int sweep = 0; sweep < 64; ++sweep) {
+        double off = A[0][1] * A[0][1] + A[0][2] * A[0][2] + A[1][2] * A[1][2];
+        double dia = A[0][0] * A[0][0] + A[1][1] * A[1][1] + A[2][2] * A[2][2];
+        if (off <= 1e-60 * dia || off == 0.0) break;
+        for (int e = 0; e < 3; ++e) {
+            int p = pairs[e][0], q = pairs[e][1];
+            if (A[p][q] == 0.0) continue;
+            double theta = (A[q][q] - A[p][p]) / (2.0 * A[p][q]);
+            double t = (theta >= 0 ? 1.0 : -1.0) / (fabs(theta) + sqrt(theta * theta + 1.0));
+            double c = 1.0 / sqrt(t * t + 1.0), sn = t * c;
+            for (int i = 0; i < 3; ++i) for (int j = 0; j < 3; ++j) J[i][j] = i == j ? 1.0 : 0.0;
+            J[p][p] = c; J[q][q] = c; J[p][q] = sn; J[q][p] = -sn;
+            for (int i = 0; i < 3; ++i) for (int j = 0; j < 3; ++j) {         /* T = A J */
+                T[i][j] = 0; for (int k = 0; k < 3; ++k) T[i][j] += A[i][k] * J[k][j];
+            }
+            for (int i = 0; i < 3; ++i) for (int j = 0; j < 3; ++j) {         /* A = J^T T */
+                A[i][j] = 0; for (int k = 0; k < 3; ++k) A[i][j] += J[k][i] * T[k][j];
+            }
+            A[p][q] = A[q][p] = 0.0;                                          /* what the rotation is built to do */
+            for (int i = 0; i < 3; ++i) for (int j = 0; j < 3; ++j) {         /* T = V J */
+                T[i][j] = 0; for (int k = 0; k < 3; ++k) T[i][j] += V[i][k] * J[k][j];
+            }
+            memcpy(V, T, sizeof(T));
+        }
+    }
+    lam[0] = A[0][0]; lam[1] = A[1][1]; lam[2] = A[2][2];
+    for (int a = 0; a < 2; ++a) for (int b = 0; b < 2 - a; ++b) if (lam[b] < lam[b + 1]) {   /* bubble sort, descending */
+        double x = lam[b]; lam[b] = lam[b + 1]; lam[b + 1] = x;
+        for (int i = 0; i < 3; ++i) { x = V[i][b]; V[i][b] = V[i][b + 1]; V[i][b + 1] = x; }
+    }
+}
+
+/* Gyration-tensor shape CVs of one group, PAPER.md:L188 (PrincipalMoment) and L189 (Asphericity, Acylindricity,
+ * ShapeAnisotropy).  The paper only names them; reading R-SHAPE of DESIGN.md takes the polymer-physics definitions:
+ *   S = sum_i w_i (r_i - c)(r_i - c)^T / W   (the weights of the barycenter, so that tr S = Rg^2 of reading R-RG),
+ *   eigenvalues l1 >= l2 >= l3,
+ *   PrincipalMoment(axis k) = l_k,  Asphericity b = l1 - (l2 + l3)/2,  Acylindricity c = l2 - l3,
+ *   ShapeAnisotropy kappa^2 = (b^2 + 3/4 c^2) / (l1 + l2 + l3)^2   (0 for a point).
+ * First-order perturbation theory gives d l_k / d r_i = (2 w_i / W) (v_k . (r_i - c)) v_k  (the barycenter's own
+ * dependence on r_i drops out because sum_i w_i (r_i - c) = 0), and the chain rule through (l1, l2, l3) the rest.
+ * At a degenerate pair of eigenvalues the single eigenvalues are not differentiable; the formula then returns the
+ * derivative along the eigenvectors the Jacobi iteration happened to produce. */
+static double shape_cv(const orc_cv *cv, const float *pos, int ps, const int *slot_atom,
+                       const float *slot_weight, const float *atom_weight, const double *box, double *jac) {
+    double c[3], W, first[3], r[3], S[3][3] = {{0, 0, 0}, {0, 0, 0}, {0, 0, 0}}, lam[3], V[3][3], g[3] = {0, 0, 0}, xi = NAN;
+    group_center(cv, 0, pos, ps, slot_atom, slot_weight, atom_weight, box, c, &W);
+    long long n = group_count(cv, 0);
+    atom_image(pos, ps, group_atom(cv, 0, 0, slot_atom), NULL, NULL, first);
+    for (long long i = 0; i < n; ++i) {
+        double w = group_weight(cv, 0, i, slot_weight, atom_weight);
+        atom_image(pos, ps, group_atom(cv, 0, i, slot_atom), first, box, r);
+        double d[3] = {r[0] - c[0], r[1] - c[1], r[2] - c[2]};
+        for (int x = 0; x < 3; ++x) for (int y = 0; y < 3; ++y) S[x][y] += w * d[x] * d[y] / W;
+    }
+    sym3_eig(S, lam, V);
+    double tr = lam[0] + lam[1] + lam[2];
+    switch (cv->type) {
+    case ORC_PRINCIPAL_MOMENT: xi = lam[cv->axis]; g[cv->axis] = 1.0; break;
+    case ORC_ASPHERICITY: xi = lam[0] - 0.5 * (lam[1] + lam[2]); g[0] = 1.0; g[1] = -0.5; g[2] = -0.5; break;
+    case ORC_ACYLINDRICITY: xi = lam[1] - lam[2]; g[1] = 1.0; g[2] = -1.0; break;
+    case ORC_SHAPE_ANISOTROPY: {
+        double b = lam[0] - 0.5 * (lam[1] + lam[2]), a = lam[1] - lam[2];
+        double num = b * b + 0.75 * a * a;
+        xi = tr > 0 ? num / (tr * tr) : 0.0;
+        if (tr > 0) {
+            /* d num / d l = (2b, -b + 3a/2, -b - 3a/2);  d (num / tr^2) / d l_k = dnum_k / tr^2 - 2 num / tr^3 */
+            double dn[3] = {2.0 * b, -b + 1.5 * a, -b - 1.5 * a};
+            for (int k = 0; k < 3; ++k) g[k] = dn[k] / (tr * tr) - 2.0 * num / (tr * tr * tr);
+        }
+        break;
+    }
+    }
+    if (jac) for (long long i = 0; i < n; ++i) {
+        double w = group_weight(cv, 0, i, slot_weight, atom_weight);
+        atom_image(pos, ps, group_atom(cv, 0, i, slot_atom), first, box, r);
+        double d[3] = {r[0] - c[0], r[1] - c[1], r[2] - c[2]};
+        for (int x = 0; x < 3; ++x) jac[3 * i + x] = 0.0;
+        for (int k = 0; k < 3; ++k) {
+            double proj = V[0][k] * d[0] + V[1][k] * d[1] + V[2][k] * d[2];
+            for (int x = 0; x < 3; ++x) jac[3 * i + x] += (2.0 * w / W) * g[k] * proj * V[x][k];
+        }
+    }
+    return xi;
+}
+
 /* Evaluate one CV of one replica.  jac (nullable) receives d(xi)/d(r_i), three
  * doubles per atom, for the atoms of group 0, then group 1, ... in group order.
  * Returns xi. */
 static double cv_one(const orc_cv *cv, const float *pos, int ps, const int *slot_atom,
                      const float *slot_weight, const float *atom_weight, const double *box, double *jac) {
+    if (cv->type >= ORC_PRINCIPAL_MOMENT && cv->type <= ORC_SHAPE_ANISOTROPY)
+        return shape_cv(cv, pos, ps, slot_atom, slot_weight, atom_weight, box, jac);
     if (cv->type == ORC_RGYR) {
         /* PAPER.md:L189 RadiusofGyration. Reading R-RG: Rg^2 = sum w|r-c|^2 / sum w,
          * same weights as the barycenter; dRg/dr_i = w_i (r_i - c)/(W Rg). */
