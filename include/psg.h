@@ -52,7 +52,13 @@ enum {
     PSG_CV_DIHEDRAL = 3,      /* FourPointCV DihedralAngle in (-pi, pi], IUPAC sign     (L187, L81) */
     PSG_CV_COM_COMPONENT = 4, /* AxisCV Component: barycenter coordinate along an axis  (L188) */
     PSG_CV_RGYR = 5,          /* RadiusofGyration: sqrt(sum w|r-c|^2 / sum w)           (L189) */
-    PSG_CV_DISPLACEMENT = 6   /* TwoPointCV Displacement c2 - c1: one CV per component (axis) (L185) */
+    PSG_CV_DISPLACEMENT = 6,  /* TwoPointCV Displacement c2 - c1: one CV per component (axis) (L185) */
+    /* Gyration-tensor shape CVs of ONE explicit group (L188-L189; reading R-SHAPE):
+     * S = sum w (r - c)(r - c)^T / sum w, eigenvalues l1 >= l2 >= l3. */
+    PSG_CV_PRINCIPAL_MOMENT = 7, /* AxisCV PrincipalMoment: l_axis, axis 0 = the largest               (L188) */
+    PSG_CV_ASPHERICITY = 8,      /* l1 - (l2 + l3)/2                                                    (L189) */
+    PSG_CV_ACYLINDRICITY = 9,    /* l2 - l3                                                             (L189) */
+    PSG_CV_SHAPE_ANISOTROPY = 10 /* ((l1 - (l2+l3)/2)^2 + 3/4 (l2 - l3)^2) / (l1+l2+l3)^2; 0 for a point (L189) */
 };
 
 enum { PSG_METHOD_NONE = 0, PSG_METHOD_HARMONIC = 1, PSG_METHOD_METAD = 2, PSG_METHOD_ABF = 3 };
@@ -76,7 +82,7 @@ typedef struct {
     int group_size[PSG_MAX_GROUPS];
     long long range_begin[PSG_MAX_GROUPS]; /* range: atoms [range_begin, range_begin + range_size) of the replica's array */
     long long range_size[PSG_MAX_GROUPS];
-    int axis;                            /* PSG_CV_COM_COMPONENT, PSG_CV_DISPLACEMENT: 0, 1, 2 */
+    int axis;                            /* PSG_CV_COM_COMPONENT, PSG_CV_DISPLACEMENT: 0, 1, 2; PSG_CV_PRINCIPAL_MOMENT: which eigenvalue */
     double period;                       /* 0 = not periodic; 2*pi for a dihedral (binary64: the wrap must not lose bits) */
 } psg_cv_desc;
 

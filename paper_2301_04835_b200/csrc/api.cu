@@ -38,7 +38,7 @@ static cudaError_t dalloc(T*& p, size_t n) {
     return cudaMalloc((void**)&p, n * sizeof(T));
 }
 
-static const int kGroups[7] = {0, 2, 3, 4, 1, 1, 2};
+static const int kGroups[11] = {0, 2, 3, 4, 1, 1, 2, 1, 1, 1, 1};
 
 extern "C" {
 
@@ -129,13 +129,16 @@ int psg_set_cvs(psg_ctx* c, int n_cv, const psg_cv_desc* cvs, int n_slots, const
     std::vector<int> slot_gid(n_slots > 0 ? n_slots : 1, -1);
     for (int k = 0; k < n_cv; ++k) {
         const psg_cv_desc& d = cvs[k];
-        if (d.type < PSG_CV_DISTANCE || d.type > PSG_CV_DISPLACEMENT) return fail(c, PSG_EINVAL, "psg_set_cvs: unknown CV type");
+        if (d.type < PSG_CV_DISTANCE || d.type > PSG_CV_SHAPE_ANISOTROPY) return fail(c, PSG_EINVAL, "psg_set_cvs: unknown CV type");
         if (d.n_groups != kGroups[d.type]) return fail(c, PSG_EINVAL, "psg_set_cvs: wrong n_groups for this CV type");
-        if ((d.type == PSG_CV_COM_COMPONENT || d.type == PSG_CV_DISPLACEMENT) && (d.axis < 0 || d.axis > 2)) return fail(c, PSG_EINVAL, "psg_set_cvs: axis must be 0, 1 or 2");
+        if ((d.type == PSG_CV_COM_COMPONENT || d.type == PSG_CV_DISPLACEMENT || d.type == PSG_CV_PRINCIPAL_MOMENT) && (d.axis < 0 || d.axis > 2))
+            return fail(c, PSG_EINVAL, "psg_set_cvs: axis must be 0, 1 or 2");
+        const bool shape = d.type >= PSG_CV_PRINCIPAL_MOMENT && d.type <= PSG_CV_SHAPE_ANISOTROPY;
+        if (shape && d.group_is_range[0]) return fail(c, PSG_EINVAL, "psg_set_cvs: gyration-tensor CVs take an explicit group");
         if (!(d.period >= 0.0)) return fail(c, PSG_EINVAL, "psg_set_cvs: period must be >= 0");
         CvDev& C = P.cv[k];
         C.type = d.type; C.n_groups = d.n_groups; C.axis = d.axis; C.period = d.period; C.gid0 = P.n_groups;
-        if (d.type == PSG_CV_RGYR) P.any_rgyr = 1;
+        if (d.type == PSG_CV_RGYR || shape) P.any_rgyr = 1;   // per-atom Jacobian depends on r_i - c: the generic kernels
         for (int g = 0; g < d.n_groups; ++g) {
             GroupDev& G = P.grp[P.n_groups];
             memset(&G, 0, sizeof(G));

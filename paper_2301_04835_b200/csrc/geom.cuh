@@ -105,6 +105,58 @@ __device__ __forceinline__ D3 load_pos(const float* __restrict__ p, long long at
     return d3((double)__ldg(q), (double)__ldg(q + 1), (double)__ldg(q + 2));
 }
 
+// ---- gyration-tensor shape CVs (reading R-SHAPE) ---------------------------------------
+// A symmetric 3x3 matrix held as six scalars, diagonalised by cyclic Jacobi rotations in registers: each rotation acts on
+// the 2x2 block (app, aqq, apq), the two entries (arp, arq) that couple it to the third axis, and columns p, q of the
+// eigenvector matrix.  t = tan(theta) is the smaller root, so the iteration converges quadratically (<= 6 sweeps here).
+__device__ __forceinline__ void jacobi_rotate(double& app, double& aqq, double& apq, double& arp, double& arq,
+                                              D3& vp, D3& vq) {
+    if (apq == 0.0) return;
+    const double th = (aqq - app) / (2.0 * apq);
+    const double t = copysign(1.0, th) / (fabs(th) + sqrt(th * th + 1.0));
+    const double c = 1.0 / sqrt(t * t + 1.0), s = t * c;
+    app -= t * apq; aqq += t * apq; apq = 0.0;
+    const double rp = c * arp - s * arq, rq = s * arp + c * arq;
+    arp = rp; arq = rq;
+    const D3 np_ = c * vp - s * vq, nq = s * vp + c * vq;
+    vp = np_; vq = nq;
+}
+__device__ __forceinline__ void swap_desc(double& la, double& lb, D3& va, D3& vb) {
+    if (la < lb) { double t = la; la = lb; lb = t; D3 v = va; va = vb; vb = v; }
+}
+// eigenvalues l[0] >= l[1] >= l[2] of {xx, xy, xz, yy, yz, zz} and their unit eigenvectors
+__device__ __forceinline__ void sym3_eigen(const double* m, double* l, D3* v) {
+    double xx = m[0], xy = m[1], xz = m[2], yy = m[3], yz = m[4], zz = m[5];
+    D3 vx = d3(1, 0, 0), vy = d3(0, 1, 0), vz = d3(0, 0, 1);
+    for (int sweep = 0; sweep < 16; ++sweep) {
+        const double off = xy * xy + xz * xz + yz * yz;
+        if (off <= 1e-60 * (xx * xx + yy * yy + zz * zz)) break;
+        jacobi_rotate(xx, yy, xy, xz, yz, vx, vy);
+        jacobi_rotate(xx, zz, xz, xy, yz, vx, vz);
+        jacobi_rotate(yy, zz, yz, xy, xz, vy, vz);
+    }
+    swap_desc(xx, yy, vx, vy); swap_desc(yy, zz, vy, vz); swap_desc(xx, yy, vx, vy);
+    l[0] = xx; l[1] = yy; l[2] = zz; v[0] = vx; v[1] = vy; v[2] = vz;
+}
+__device__ __forceinline__ bool is_shape_cv(int type) { return type >= PSG_CV_PRINCIPAL_MOMENT && type <= PSG_CV_SHAPE_ANISOTROPY; }
+// value of the shape CV and g[k] = d xi / d l_k
+__device__ __forceinline__ double shape_from_eigenvalues(int type, int axis, const double* l, double* g) {
+    g[0] = g[1] = g[2] = 0.0;
+    if (type == PSG_CV_PRINCIPAL_MOMENT) {
+        g[0] = axis == 0 ? 1.0 : 0.0; g[1] = axis == 1 ? 1.0 : 0.0; g[2] = axis == 2 ? 1.0 : 0.0;
+        return axis == 0 ? l[0] : axis == 1 ? l[1] : l[2];
+    }
+    const double b = l[0] - 0.5 * (l[1] + l[2]), a = l[1] - l[2];
+    if (type == PSG_CV_ASPHERICITY) { g[0] = 1.0; g[1] = -0.5; g[2] = -0.5; return b; }
+    if (type == PSG_CV_ACYLINDRICITY) { g[1] = 1.0; g[2] = -1.0; return a; }
+    const double tr = l[0] + l[1] + l[2], num = b * b + 0.75 * a * a;   // PSG_CV_SHAPE_ANISOTROPY
+    if (!(tr > 0.0)) return 0.0;
+    const double i2 = 1.0 / (tr * tr), k = 2.0 * num * i2 / tr;
+    g[0] = 2.0 * b * i2 - k; g[1] = (1.5 * a - b) * i2 - k; g[2] = (-1.5 * a - b) * i2 - k;
+    return num * i2;
+}
+#define PSG_COEF_SHAPE (-1.0)   // WarpCvSmem::coef of a shape-CV group: sec[] holds (2/W) sum_k g_k v_k v_k^T
+
 __device__ __forceinline__ double warp_sum(double v) {
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
@@ -116,7 +168,8 @@ struct WarpCvSmem {
     double cen[PSG_MAX_GROUPS_TOTAL][4];   // cx cy cz W
     double m2[PSG_MAX_GROUPS_TOTAL];       // sum w |r|^2 (RGYR groups)
     double v[PSG_MAX_GROUPS_TOTAL][3];     // dxi/dc_g / W_g
-    double coef[PSG_MAX_GROUPS_TOTAL];     // RGYR: 1/(W Rg)
+    double coef[PSG_MAX_GROUPS_TOTAL];     // RGYR: 1/(W Rg); shape CVs: PSG_COEF_SHAPE; else 0
+    double sec[PSG_MAX_GROUPS_TOTAL][6];   // shape CVs: sum w x'x'^T (x' = r - first atom), then the matrix M of d xi/d r_i = w_i M (r_i - c)
     double xi[PSG_MAX_CV];
 };
 
@@ -151,6 +204,8 @@ __device__ __forceinline__ void warp_cv_eval(const SysParams& P, int r, const fl
         const GroupDev& G = P.grp[lane];
         const int* sa = P.slot_atom + (P.per_rep ? (long long)r * P.n_slots : 0);
         double sx = 0, sy = 0, sz = 0, sw = 0, s2 = 0;
+        double q[6] = {0, 0, 0, 0, 0, 0};
+        const bool shape = is_shape_cv(P.cv[G.cv].type);
         const double* box = sys_box(P);
         const D3 first = load_pos(p, sa[G.begin], P.ps);
         for (int i = 0; i < G.size; ++i) {
@@ -160,10 +215,20 @@ __device__ __forceinline__ void warp_cv_eval(const SysParams& P, int r, const fl
             double w = P.slot_weight ? (double)P.slot_weight[s] : 1.0;
             sx += w * x.x; sy += w * x.y; sz += w * x.z; sw += w;
             s2 += w * dot(x, x);
+            if (shape) {   // second moments about the first atom: no cancellation against |c|^2 far from the origin
+                const D3 e = x - first;
+                q[0] += w * e.x * e.x; q[1] += w * e.x * e.y; q[2] += w * e.x * e.z;
+                q[3] += w * e.y * e.y; q[4] += w * e.y * e.z; q[5] += w * e.z * e.z;
+            }
         }
         double iw = 1.0 / sw;
         sm.cen[lane][0] = sx * iw; sm.cen[lane][1] = sy * iw; sm.cen[lane][2] = sz * iw; sm.cen[lane][3] = sw;
         sm.m2[lane] = s2;
+        if (shape) {   // S = sum w x'x'^T / W - c'c'^T, c' = c - first
+            const D3 cp = d3(sx * iw - first.x, sy * iw - first.y, sz * iw - first.z);
+            sm.sec[lane][0] = q[0] * iw - cp.x * cp.x; sm.sec[lane][1] = q[1] * iw - cp.x * cp.y; sm.sec[lane][2] = q[2] * iw - cp.x * cp.z;
+            sm.sec[lane][3] = q[3] * iw - cp.y * cp.y; sm.sec[lane][4] = q[4] * iw - cp.y * cp.z; sm.sec[lane][5] = q[5] * iw - cp.z * cp.z;
+        }
     }
     __syncwarp();
     if (lane < P.n_cv) {
@@ -177,6 +242,24 @@ __device__ __forceinline__ void warp_cv_eval(const SysParams& P, int r, const fl
             double rg = rg2 > 0.0 ? sqrt(rg2) : 0.0;
             sm.xi[lane] = rg;
             sm.coef[g0] = rg > 0.0 ? 1.0 / (W * rg) : 0.0;
+            sm.v[g0][0] = sm.v[g0][1] = sm.v[g0][2] = 0.0;
+        } else if (is_shape_cv(C.type)) {
+            // eigenvalues of the gyration tensor; d l_k / d r_i = (2 w_i / W)(v_k . (r_i - c)) v_k, chained through g = d xi / d l
+            double l[3], g[3];
+            D3 v[3];
+            sym3_eigen(sm.sec[g0], l, v);
+            sm.xi[lane] = shape_from_eigenvalues(C.type, C.axis, l, g);
+            const double k = 2.0 / sm.cen[g0][3];
+            double M[6] = {0, 0, 0, 0, 0, 0};
+#pragma unroll
+            for (int e = 0; e < 3; ++e) {
+                const double ge = k * g[e];
+                M[0] += ge * v[e].x * v[e].x; M[1] += ge * v[e].x * v[e].y; M[2] += ge * v[e].x * v[e].z;
+                M[3] += ge * v[e].y * v[e].y; M[4] += ge * v[e].y * v[e].z; M[5] += ge * v[e].z * v[e].z;
+            }
+#pragma unroll
+            for (int e = 0; e < 6; ++e) sm.sec[g0][e] = M[e];
+            sm.coef[g0] = PSG_COEF_SHAPE;
             sm.v[g0][0] = sm.v[g0][1] = sm.v[g0][2] = 0.0;
         } else {
             D3 c[4], dc[4];
@@ -204,15 +287,22 @@ __device__ __forceinline__ D3 slot_jacobian(const SysParams& P, int r, const flo
     int gid = P.slot_gid[s];
     double w = P.slot_weight ? (double)P.slot_weight[s] : 1.0;
     D3 j = d3(w * sm.v[gid][0], w * sm.v[gid][1], w * sm.v[gid][2]);
-    if (sm.coef[gid] != 0.0) {   // explicit RGYR group: w (r - c) / (W Rg)
+    if (sm.coef[gid] != 0.0) {   // explicit RGYR group: w (r - c) / (W Rg); shape-CV group: w M (r - c)
         const int* sa = P.slot_atom + (P.per_rep ? (long long)r * P.n_slots : 0);
         D3 x = load_pos(pos + (long long)r * P.rstride * P.ps, sa[s], P.ps);
         if (P.has_box) {
             const D3 first = load_pos(pos + (long long)r * P.rstride * P.ps, sa[P.grp[gid].begin], P.ps);
             x = first + min_image(x - first, P.box);
         }
-        double k = w * sm.coef[gid];
-        j = d3(k * (x.x - sm.cen[gid][0]), k * (x.y - sm.cen[gid][1]), k * (x.z - sm.cen[gid][2]));
+        const D3 d = d3(x.x - sm.cen[gid][0], x.y - sm.cen[gid][1], x.z - sm.cen[gid][2]);
+        if (sm.coef[gid] == PSG_COEF_SHAPE) {   // w M (r - c), M symmetric
+            const double* M = sm.sec[gid];
+            j = d3(w * (M[0] * d.x + M[1] * d.y + M[2] * d.z), w * (M[1] * d.x + M[3] * d.y + M[4] * d.z),
+                   w * (M[2] * d.x + M[4] * d.y + M[5] * d.z));
+        } else {
+            const double k = w * sm.coef[gid];
+            j = d3(k * d.x, k * d.y, k * d.z);
+        }
     }
     return j;
 }

@@ -13,10 +13,12 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 _LIB_PATH = os.path.join(_HERE, "libpsg.so")
 
 CV_DISTANCE, CV_ANGLE, CV_DIHEDRAL, CV_COM_COMPONENT, CV_RGYR, CV_DISPLACEMENT = 1, 2, 3, 4, 5, 6
+CV_PRINCIPAL_MOMENT, CV_ASPHERICITY, CV_ACYLINDRICITY, CV_SHAPE_ANISOTROPY = 7, 8, 9, 10
 METHOD_NONE, METHOD_HARMONIC, METHOD_METAD, METHOD_ABF = 0, 1, 2, 3
 HILLS_F32, HILLS_F64 = 0, 1
 _KIND = {"distance": CV_DISTANCE, "angle": CV_ANGLE, "dihedral": CV_DIHEDRAL, "component": CV_COM_COMPONENT,
-         "rgyr": CV_RGYR, "displacement": CV_DISPLACEMENT}
+         "rgyr": CV_RGYR, "displacement": CV_DISPLACEMENT, "principal_moment": CV_PRINCIPAL_MOMENT,
+         "asphericity": CV_ASPHERICITY, "acylindricity": CV_ACYLINDRICITY, "shape_anisotropy": CV_SHAPE_ANISOTROPY}
 
 # every symbol include/psg.h declares
 EXPORTS = ["psg_create", "psg_destroy", "psg_set_stream", "psg_last_error", "psg_set_layout", "psg_set_cvs",

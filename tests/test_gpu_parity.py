@@ -993,3 +993,146 @@ def test_argument_validation(torch, psg):
     assert e.value.code == -1
     with pytest.raises(ValueError):
         ctx.cv_eval(x.double(), torch.zeros((2, 1), device="cuda"), None)
+
+
+# ------------------------------------------------------------------------------------ gyration-tensor shape CVs
+def _shape_molecules(rng, R, N, box=None):
+    """R replicas of N atoms: an anisotropic blob per replica (axes 2 : 1 : 0.5 after a random rotation, so that the three
+    eigenvalues are well separated), somewhere in a 6 nm region; wrapped into ``box`` when one is given"""
+    pos = np.empty((R, N, 3), np.float32)
+    for r in range(R):
+        q, _ = np.linalg.qr(rng.normal(size=(3, 3)))
+        pos[r] = (rng.normal(size=(N, 3)) * [0.5, 0.25, 0.12]) @ q.T + rng.uniform(0.0, 6.0, size=3)
+    if box is not None:
+        pos = np.mod(pos, np.asarray(box, np.float32)).astype(np.float32)
+    return pos
+
+
+@pytest.mark.parametrize("box", [None, (4.0, 4.5, 5.0)])
+@pytest.mark.parametrize("which", [0, 1])
+def test_shape_cvs_match_oracle(torch, psg, which, box):
+    """PrincipalMoment(0..2), Asphericity, Acylindricity, ShapeAnisotropy (reading R-SHAPE) of weighted
+    explicit groups with per-replica indices and stride-3 positions: values, the compact Jacobian, and the forces of a
+    harmonic restraint through the whole step; with a box the molecules are wrapped and most straddle a face"""
+    rng = np.random.default_rng(70 + which)
+    R, N = 41, 48
+    pos = _shape_molecules(rng, R, N, box)
+    sizes = [12, 9, 7, 5]
+    n_slots = sum(sizes)
+    slot = np.stack([rng.permutation(N)[:n_slots] for _ in range(R)]).astype(np.int32)
+    sw = rng.uniform(1, 16, size=n_slots).astype(np.float32)
+    begin = np.concatenate([[0], np.cumsum(sizes)[:-1]])
+    kinds = [[("PRINCIPAL_MOMENT", 0), ("PRINCIPAL_MOMENT", 1), ("PRINCIPAL_MOMENT", 2), ("ASPHERICITY", 0)],
+             [("ACYLINDRICITY", 0), ("SHAPE_ANISOTROPY", 0), ("RGYR", 0), ("PRINCIPAL_MOMENT", 1)]][which]
+    o_cvs = [{"type": getattr(orc, k), "groups": [("slots", int(begin[i]), sizes[i])], "axis": ax, "period": 0.0}
+             for i, (k, ax) in enumerate(kinds)]
+    g_cvs = [{"type": getattr(psg, "CV_" + k), "groups": [("slots", int(begin[i]), sizes[i])], "axis": ax, "period": 0.0}
+             for i, (k, ax) in enumerate(kinds)]
+    sysm = orc.System(R, N, N, 3, o_cvs, slot, sw, None, box=box)
+    xi_ref, jac_ref = sysm.cv_eval(pos)
+    ctx = psg.Context(0)
+    ctx.set_layout(R, N, N, 3, 3)
+    ctx.set_cvs(g_cvs, slot, sw, None)
+    if box is not None:
+        ctx.set_box(box)
+    d_xi = torch.empty((R, 4), device="cuda")
+    d_jac = torch.empty((R, n_slots, 3), device="cuda")
+    d_pos = dev(torch, pos)
+    ctx.cv_eval(d_pos, d_xi, d_jac)
+    ctx.sync_check()
+    assert_close(d_xi.cpu().numpy(), xi_ref, "shape xi")
+    assert_close(d_jac.cpu().numpy(), jac_ref, "shape jacobian")
+    if box is not None:   # the box is really in play: the open-boundary tensor of a split molecule is far larger
+        open_xi = orc.System(R, N, N, 3, o_cvs, slot, sw, None).cv_eval(pos, want_jac=False)
+        assert (np.abs(open_xi - xi_ref) > 1e-3 * np.abs(xi_ref)).any()
+    ks = np.array([400, 900, 2000, 700], np.float32)
+    cen = (xi_ref * rng.uniform(0.5, 1.5, size=xi_ref.shape)).astype(np.float32)
+    ctx.set_harmonic(ks, cen)
+    f0 = (rng.standard_normal((R, N, 3)) * 100).astype(np.float32)
+    d_f = dev(torch, f0)
+    ctx.step(d_pos, d_f, None, 1)
+    ctx.sync_check()
+    V, dV = orc.harmonic(xi_ref.astype(np.float32).astype(np.float64), ks, cen, np.zeros(4))
+    f_ref = sysm.apply_forces(pos, dV, f0.astype(np.float64))
+    assert_forces_close(d_f.cpu().numpy(), f_ref, f0, "shape forces")
+    out = ctx.read_step_outputs()
+    assert_close(out["V"].cpu().numpy(), V, "shape V")
+    assert_close(out["dVdxi"].cpu().numpy(), dV, "shape dV/dxi")
+    ctx.close()
+
+
+def test_shape_cv_metad_and_abf_steps(torch, psg):
+    """the shape CVs under the other two methods: a metadynamics step on (ShapeAnisotropy, Rg) -- the generic kernels, since
+    the per-atom Jacobian needs r_i - c -- and the one-launch ABF step on (PrincipalMoment 0, Acylindricity) with bit-exact
+    bins"""
+    rng = np.random.default_rng(81)
+    R, N = 300, 40
+    pos = np.concatenate([_shape_molecules(rng, R, N), np.zeros((R, N, 1), np.float32)], axis=2)
+    slot = np.concatenate([np.arange(0, 14), np.arange(10, 30)]).astype(np.int32)     # the two groups share atoms 10..13
+    groups = [[("slots", 0, 14)], [("slots", 14, 20)]]
+    f0 = (rng.standard_normal((R, N, 4)) * 100).astype(np.float32)
+    # -- metadynamics
+    o_cvs = [{"type": orc.SHAPE_ANISOTROPY, "groups": groups[0], "axis": 0, "period": 0.0},
+             {"type": orc.RGYR, "groups": groups[1], "axis": 0, "period": 0.0}]
+    g_cvs = [{"type": psg.CV_SHAPE_ANISOTROPY, "groups": groups[0], "axis": 0, "period": 0.0},
+             {"type": psg.CV_RGYR, "groups": groups[1], "axis": 0, "period": 0.0}]
+    sysm = orc.System(R, N, N, 4, o_cvs, slot, None, None)
+    xi_ref, _ = sysm.cv_eval(pos)
+    n_h = 500
+    sigma = np.array([0.05, 0.03], np.float32)
+    centers = (xi_ref[rng.integers(0, R, size=n_h)] + rng.normal(scale=0.04, size=(n_h, 2))).astype(np.float32)
+    heights = rng.uniform(0.2, 1.2, size=n_h).astype(np.float32)
+    ctx = psg.Context(0)
+    ctx.set_layout(R, N, N, 4, 4)
+    ctx.set_cvs(g_cvs, slot, None, None)
+    ctx.set_metad(sigma, 1.2, 0.0, n_h + 8, 0)
+    ctx.load_hills(dev(torch, centers), dev(torch, heights))
+    d_f = dev(torch, f0)
+    ctx.step(dev(torch, pos), d_f, None, 1)
+    ctx.sync_check()
+    out = {k: v.cpu().numpy() for k, v in ctx.read_step_outputs().items()}
+    assert_close(out["xi"], xi_ref, "metad shape xi")
+    V, dV, T = orc.metad(xi_ref.astype(np.float32).astype(np.float64), centers, heights, sigma, np.zeros(2))
+    assert (np.abs(out["V"] - V) <= 1e-5 * np.abs(V) + 1e-6 + 2e-7 * np.abs(heights).sum()).all()
+    assert (np.abs(out["dVdxi"] - dV) <= 1e-5 * np.abs(dV) + 1e-6 + 2e-7 * T).all()
+    f_ref = sysm.apply_forces(pos, out["dVdxi"].astype(np.float64), f0[..., :3].astype(np.float64))   # the scatter on its own
+    assert_forces_close(d_f.cpu().numpy()[..., :3], f_ref, f0[..., :3], "metad shape forces")
+    ctx.close()
+    # -- ABF
+    o_cvs = [{"type": orc.PRINCIPAL_MOMENT, "groups": groups[0], "axis": 0, "period": 0.0},
+             {"type": orc.ACYLINDRICITY, "groups": groups[1], "axis": 0, "period": 0.0}]
+    g_cvs = [{"type": psg.CV_PRINCIPAL_MOMENT, "groups": groups[0], "axis": 0, "period": 0.0},
+             {"type": psg.CV_ACYLINDRICITY, "groups": groups[1], "axis": 0, "period": 0.0}]
+    sysm = orc.System(R, N, N, 4, o_cvs, slot, None, None)
+    xi_ref, _ = sysm.cv_eval(pos)
+    lower, upper = xi_ref.min(axis=0).astype(np.float32) * 0.9, xi_ref.max(axis=0).astype(np.float32) * 1.1
+    shape, periodic, n_thr = np.array([7, 5], np.int32), np.array([0, 0], np.int32), 3
+    fs = rng.normal(scale=20.0, size=(R, 2)).astype(np.float32)
+    ctx = psg.Context(0)
+    ctx.set_layout(R, N, N, 4, 4)
+    ctx.set_cvs(g_cvs, slot, None, None)
+    ctx.set_abf(lower, upper, shape, periodic, n_thr)
+    d_f = dev(torch, f0)
+    n0 = ctx.launch_count()
+    ctx.step(dev(torch, pos), d_f, dev(torch, fs), 1)
+    assert ctx.launch_count() - n0 == 1
+    ctx.sync_check()
+    out = {k: v.cpu().numpy() for k, v in ctx.read_step_outputs().items()}
+    assert_close(out["xi"], xi_ref, "abf shape xi")
+    hist, fsum = np.zeros(35, np.int32), np.zeros((35, 2), np.float64)
+    b, dV = orc.abf_update(out["xi"], fs, lower, upper, shape, periodic, n_thr, hist, fsum)   # bins from the SAME binary32 xi
+    assert np.array_equal(out["bin"], b)
+    assert_close(out["dVdxi"], dV, "abf shape dV/dxi")
+    f_ref = sysm.apply_forces(pos, dV, f0[..., :3].astype(np.float64))
+    assert_forces_close(d_f.cpu().numpy()[..., :3], f_ref, f0[..., :3], "abf shape forces")
+    ctx.close()
+
+
+def test_shape_cv_argument_errors(torch, psg):
+    ctx = psg.Context(0)
+    ctx.set_layout(2, 30, 30, 4, 4)
+    with pytest.raises(psg.PsgError):      # a range group
+        ctx.set_cvs([{"type": psg.CV_ASPHERICITY, "groups": [("range", 0, 30)], "axis": 0, "period": 0.0}], np.zeros(0, np.int32))
+    with pytest.raises(psg.PsgError):      # which eigenvalue?
+        ctx.set_cvs([{"type": psg.CV_PRINCIPAL_MOMENT, "groups": [("slots", 0, 5)], "axis": 3, "period": 0.0}], np.arange(5, dtype=np.int32))
+    ctx.close()
