@@ -237,3 +237,41 @@ def dist_to_interface(pos, mobile_idx, mobile_w, ibegin, n_i, axis, sigma, scope
                                 C.c_double(float(scope[0])), C.c_double(float(scope[1])), C.c_int(int(bins)), C.c_double(float(coeff)),
                                 C.byref(xi), _p(jm, C.c_double), _p(dx, C.c_double), _p(mass, C.c_double))
     return xi.value, jm, dx, mass
+
+
+class _Grid(C.Structure):
+    _fields_ = [("n_cv", C.c_int), ("lower", C.c_double * 4), ("upper", C.c_double * 4), ("shape", C.c_int * 4),
+                ("periodic", C.c_int * 4)]
+
+
+class MetadGrid:
+    """Grid-stored metadynamics (reading R-GRID).  ``values`` is the node array
+    [nodes][1 + n_cv] (V, dV/dxi_1, ...), float64, row-major with the last CV fastest; tests may write it directly."""
+
+    def __init__(self, lower, upper, shape, periodic):
+        self.g = _Grid()
+        self.n_cv = self.g.n_cv = len(shape)
+        for k in range(self.n_cv):
+            self.g.lower[k], self.g.upper[k] = float(lower[k]), float(upper[k])
+            self.g.shape[k], self.g.periodic[k] = int(shape[k]), int(bool(periodic[k]))
+        lib().orc_grid_nodes.restype = C.c_longlong
+        self.nodes = int(lib().orc_grid_nodes(C.byref(self.g)))
+        self.values = np.zeros((self.nodes, 1 + self.n_cv), np.float64)
+
+    def eval(self, xi):
+        xi = _f64(xi).reshape(-1, self.n_cv)
+        V = np.empty(xi.shape[0], np.float64)
+        dV = np.empty((xi.shape[0], self.n_cv), np.float64)
+        lib().orc_grid_eval(C.byref(self.g), _p(self.values, C.c_double), C.c_int(xi.shape[0]), _p(xi, C.c_double),
+                            _p(V, C.c_double), _p(dV, C.c_double))
+        return V, dV
+
+    def deposit(self, xi_f32, sigma, w0, kB_deltaT=0.0, mask=None):
+        """one synchronous deposit event; returns the heights [R] (0 where masked out)"""
+        xi = _f32(xi_f32).reshape(-1, self.n_cv)
+        m = None if mask is None else np.ascontiguousarray(mask, dtype=np.uint8)
+        h = np.empty(xi.shape[0], np.float64)
+        lib().orc_grid_deposit(C.byref(self.g), _p(self.values, C.c_double), C.c_int(xi.shape[0]), _p(xi, C.c_float),
+                               _p(m, C.c_ubyte), C.c_double(w0), C.c_double(kB_deltaT), _p(_f64(sigma), C.c_double),
+                               _p(h, C.c_double))
+        return h

@@ -38,6 +38,10 @@
  * paper without a formula; their arithmetic is pinned by hand-computed point
  * sets, numpy.linalg.eigvalsh, the trace identity with the pinned Rg, rotation
  * invariance and finite differences (tests/test_oracle_shape_cv.py).
+ * Grid-stored metadynamics (orc_grid_*, reading R-GRID): the paper gives no
+ * layout or interpolation; pinned by the hill sum at the nodes, multilinear
+ * functions, scipy's interpolator and h^2 convergence
+ * (tests/test_oracle_grid_metad.py).
  */
 #include <math.h>
 #include <stdlib.h>
@@ -697,4 +701,113 @@ void orc_dist_to_interface(const float *pos, int ps, int n_m, const int *mobile_
     }
     if (mass_out) memcpy(mass_out, mass, sizeof(double) * (size_t)bins);
     free(c); free(mass); free(md); free(p);
+}
+
+/* ---------------------------------------------------------------------------------------------------------------
+ * Grid-stored metadynamics, PAPER.md:L151 ("optional support for storing the bias potentials ... on a pre-defined
+ * grid", trading accuracy for speed).  The paper gives neither the layout nor the interpolation, so
+ * this follows reading R-GRID of DESIGN.md:
+ *   - Grid(lower, upper, shape, periodic) as in PAPER.md:L82.  CV k has shape[k] NODES; a periodic CV spans exactly
+ *     one period upper - lower with spacing h = (upper - lower)/shape (node `shape` is node 0 again); an open CV has
+ *     its first and last nodes on lower and upper, h = (upper - lower)/(shape - 1).
+ *   - every node stores the hill sum of Eq. "sum of Gaussians" and its gradient, 1 + n_cv binary64
+ *     numbers, node index row-major with the last CV fastest.
+ *   - a deposit adds the new hill's value and gradient AT every node (orc_grid_deposit).
+ *   - the bias at xi is the multilinear interpolation of the 2^n_cv surrounding nodes, value and each gradient
+ *     component alike (orc_grid_eval); outside an open grid the CV is clamped to the nearest face first.
+ *   - well-tempered heights use the interpolated value before the event; several walkers deposit synchronously in
+ *     replica order (the readings R-WT and R-MW of the hill list).
+ * Pins (tests/test_oracle_grid_metad.py): node values against the separately pinned hill sum (orc_metad), exact
+ * reproduction of multilinear functions written straight into the grid, scipy's RegularGridInterpolator, the h^2
+ * convergence to the exact hill sum, periodic images, well-tempered heights by hand.
+ * --------------------------------------------------------------------------------------------------------------- */
+typedef struct {
+    int n_cv;
+    double lower[4], upper[4];
+    int shape[4];
+    int periodic[4];
+} orc_grid;
+
+long long orc_grid_nodes(const orc_grid *G) {
+    long long n = 1;
+    for (int k = 0; k < G->n_cv; ++k) n *= G->shape[k];
+    return n;
+}
+
+static double grid_spacing(const orc_grid *G, int k) {
+    return (G->upper[k] - G->lower[k]) / (double)(G->periodic[k] ? G->shape[k] : G->shape[k] - 1);
+}
+
+/* V [R] and dVdxi [R][n_cv] by multilinear interpolation of grid [nodes][1 + n_cv] */
+void orc_grid_eval(const orc_grid *G, const double *grid, int n_replicas, const double *xi, double *V, double *dVdxi) {
+    const int n = G->n_cv, rec = 1 + n;
+    for (int r = 0; r < n_replicas; ++r) {
+        int i0[4];
+        double f[4];
+        for (int k = 0; k < n; ++k) {
+            double t = (xi[r * n + k] - G->lower[k]) / grid_spacing(G, k);
+            if (G->periodic[k]) {
+                t -= (double)G->shape[k] * floor(t / (double)G->shape[k]);   /* into [0, shape) */
+                if (t >= (double)G->shape[k]) t = 0.0;                      /* rounding at the upper edge */
+                i0[k] = (int)floor(t);
+            } else {
+                if (t < 0.0) t = 0.0;
+                if (t > (double)(G->shape[k] - 1)) t = (double)(G->shape[k] - 1);
+                i0[k] = (int)floor(t);
+                if (i0[k] > G->shape[k] - 2) i0[k] = G->shape[k] - 2;       /* the last cell owns its upper node */
+                if (i0[k] < 0) i0[k] = 0;                                   /* a one-node dimension */
+            }
+            f[k] = t - (double)i0[k];
+        }
+        double out[5] = {0, 0, 0, 0, 0};
+        for (int corner = 0; corner < (1 << n); ++corner) {
+            double w = 1.0;
+            long long flat = 0;
+            for (int k = 0; k < n; ++k) {
+                int up = (corner >> k) & 1;
+                int i = i0[k] + up;
+                if (G->periodic[k]) i %= G->shape[k];
+                else if (i > G->shape[k] - 1) i = G->shape[k] - 1;
+                w *= up ? f[k] : 1.0 - f[k];
+                flat = flat * G->shape[k] + i;
+            }
+            for (int c = 0; c < rec; ++c) out[c] += w * grid[flat * rec + c];
+        }
+        if (V) V[r] = out[0];
+        if (dVdxi) for (int k = 0; k < n; ++k) dVdxi[r * n + k] = out[1 + k];
+    }
+}
+
+/* One synchronous deposit event of the walkers with mask[r] != 0 (NULL: all).  heights_out [R] (nullable) receives
+ * the height each walker deposited (0 where masked out). */
+void orc_grid_deposit(const orc_grid *G, double *grid, int n_replicas, const float *xi /*[R][n_cv]*/,
+                      const unsigned char *mask, double w0, double kB_deltaT, const double *sigma, double *heights_out) {
+    const int n = G->n_cv, rec = 1 + n;
+    const long long nodes = orc_grid_nodes(G);
+    double *xd = (double *)malloc(sizeof(double) * (size_t)n_replicas * n);
+    double *Vold = (double *)malloc(sizeof(double) * (size_t)n_replicas);
+    for (long long i = 0; i < (long long)n_replicas * n; ++i) xd[i] = (double)xi[i];
+    orc_grid_eval(G, grid, n_replicas, xd, Vold, NULL);       /* every height from the grid BEFORE this event */
+    for (int r = 0; r < n_replicas; ++r) {
+        double W = 0.0;
+        if (!mask || mask[r]) {
+            W = kB_deltaT > 0 ? w0 * exp(-Vold[r] / kB_deltaT) : w0;
+            for (long long node = 0; node < nodes; ++node) {
+                long long rem = node;
+                double d[4], e = 0;
+                for (int k = n - 1; k >= 0; --k) {
+                    int i = (int)(rem % G->shape[k]);
+                    rem /= G->shape[k];
+                    double x = G->lower[k] + (double)i * grid_spacing(G, k);
+                    d[k] = wrap_period(x - xd[r * n + k], G->periodic[k] ? G->upper[k] - G->lower[k] : 0.0);
+                    e += (d[k] / sigma[k]) * (d[k] / sigma[k]);
+                }
+                double g = W * exp(-0.5 * e);
+                grid[node * rec] += g;
+                for (int k = 0; k < n; ++k) grid[node * rec + 1 + k] += -g * d[k] / (sigma[k] * sigma[k]);
+            }
+        }
+        if (heights_out) heights_out[r] = W;
+    }
+    free(xd); free(Vold);
 }
