@@ -222,6 +222,29 @@ int psg_interface_cv_set(psg_ctx* ctx, int n_mobile, const int* mobile_idx, cons
 int psg_interface_cv_eval(psg_ctx* ctx, const float* d_pos, float* d_xi);
 int psg_interface_cv_apply(psg_ctx* ctx, const float* d_pos, const float* d_dVdxi, float* d_force);
 
+/* ------------------------------------------------------------- grid-stored metadynamics */
+/* "optional support for storing the bias potentials ... on a pre-defined grid".  The paper
+ * gives neither layout nor interpolation; reading R-GRID: Grid(lower, upper, shape, periodic) as in L82 with
+ * shape[k] NODES per CV (periodic: one period, h = (upper - lower)/shape; open: nodes on both ends, h = (upper - lower)/
+ * (shape - 1)); every node holds the hill sum and its gradient, [nodes][1 + n_cv] binary64, row-major, last CV fastest;
+ * the bias at xi is the multilinear interpolation of the 2^n_cv surrounding nodes (value and gradient alike; outside an
+ * open grid xi is clamped to the nearest face).  First version: calls of their own beside psg_cv_eval (which produces
+ * d_xi) and psg_apply_bias_forces (which consumes d_dVdxi); they do not touch the hill list of psg_set_metad.
+ * psg_metad_grid_set (host arrays copied; allocates and zeroes the grid; needs psg_set_layout for the walker count R):
+ *   lower, upper, sigma [n_cv]; shape >= 2; w0 > 0; kB_deltaT = 0: standard, > 0: well-tempered heights
+ *   w0 exp(-V_grid(xi) / kB_deltaT) from the grid BEFORE the event.  At most 2^27 nodes.
+ * psg_metad_grid_deposit: one synchronous event -- every walker r with d_mask[r] != 0 (NULL: all) adds its hill, centred on
+ *   d_xi[r] (device, [R][n_cv] binary32), to every node, in replica order.  Two launches on the ctx stream, no sync.
+ * psg_metad_grid_eval: d_V [R] and d_dVdxi [R][n_cv] (device, binary32; either may be NULL).  One launch, no sync.
+ * psg_metad_grid_state: device pointers of the node array and of the heights [R] (binary64) of the last event; owned by
+ *   the ctx, valid until the next psg_metad_grid_set or psg_destroy.
+ * Errors: PSG_EINVAL (arguments), PSG_ESTATE (call order), PSG_ENOMEM, PSG_ECUDA. */
+int psg_metad_grid_set(psg_ctx* ctx, int n_cv, const double* lower, const double* upper, const int* shape, const int* periodic,
+                       const double* sigma, double w0, double kB_deltaT);
+int psg_metad_grid_deposit(psg_ctx* ctx, const float* d_xi, const unsigned char* d_mask);
+int psg_metad_grid_eval(psg_ctx* ctx, const float* d_xi, float* d_V, float* d_dVdxi);
+int psg_metad_grid_state(psg_ctx* ctx, double** d_grid_out, long long* n_nodes_out, double** d_heights_out);
+
 /* ------------------------------------------------------------- measurement */
 /* Measured ALU throughput of this device (register-only loops, CUDA-event timed, synchronises):
  * which = 0: FP32 FFMA lane-ops/s; 1: packed FFMA2 (f32x2) lane-ops/s (2 per lane per instruction);

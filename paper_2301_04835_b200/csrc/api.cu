@@ -78,6 +78,7 @@ static void free_all(psg_ctx* c) {
     c->abf.hist = nullptr; c->abf.fsum = nullptr;
     dfree(c->d_pos_stage); dfree(c->d_frc_stage); dfree(c->d_fs_stage);
     psg_interface_cv_free(c);
+    psg_metad_grid_free(c);
 }
 
 int psg_destroy(psg_ctx* c) {

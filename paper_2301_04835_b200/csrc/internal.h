@@ -117,8 +117,10 @@ struct psg_ctx {
     float* d_pos_stage = nullptr; float* d_frc_stage = nullptr; float* d_fs_stage = nullptr;
     int sm_count = 148;
     void* dti = nullptr;             // state of the DistanceToInterface CV (interface_cv.cu)
+    void* mgrid = nullptr;           // state of grid-stored metadynamics (metad_grid.cu)
 };
 void psg_interface_cv_free(psg_ctx* c);
+void psg_metad_grid_free(psg_ctx* c);
 
 // ---- launchers implemented in the .cu files (all enqueue on ctx->stream) ----
 cudaError_t psg_launch_cv_eval(psg_ctx* c, const float* d_pos, float* d_xi, float* d_jac);

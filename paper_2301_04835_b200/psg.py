@@ -25,7 +25,8 @@ EXPORTS = ["psg_create", "psg_destroy", "psg_set_stream", "psg_last_error", "psg
            "psg_set_box", "psg_set_harmonic", "psg_set_metad", "psg_set_hill_precision", "psg_load_hills", "psg_get_hills",
            "psg_set_abf", "psg_abf_state", "psg_cv_eval", "psg_bias_eval", "psg_deposit_hill", "psg_abf_update",
            "psg_abf_estimate", "psg_abf_estimate_reset", "psg_apply_bias_forces", "psg_step", "psg_step_outputs", "psg_step_host", "psg_sync_check",
-           "psg_interface_cv_set", "psg_interface_cv_eval", "psg_interface_cv_apply", "psg_measure_alu_peak", "psg_launch_count"]
+           "psg_interface_cv_set", "psg_interface_cv_eval", "psg_interface_cv_apply", "psg_metad_grid_set",
+           "psg_metad_grid_deposit", "psg_metad_grid_eval", "psg_metad_grid_state", "psg_measure_alu_peak", "psg_launch_count"]
 
 
 class PsgError(RuntimeError):
@@ -89,6 +90,10 @@ def load_library():
         L.psg_interface_cv_set.argtypes = [vp, i, vp, vp, ll, ll, i, d, d, d, i, d]
         L.psg_interface_cv_eval.argtypes = [vp, vp, vp]
         L.psg_interface_cv_apply.argtypes = [vp, vp, vp, vp]
+        L.psg_metad_grid_set.argtypes = [vp, i, vp, vp, vp, vp, vp, d, d]
+        L.psg_metad_grid_deposit.argtypes = [vp, vp, vp]
+        L.psg_metad_grid_eval.argtypes = [vp, vp, vp, vp]
+        L.psg_metad_grid_state.argtypes = [vp, vp, vp, vp]
         L.psg_measure_alu_peak.argtypes = [i, i, C.POINTER(C.c_double)]
         _lib = L
     return _lib
@@ -311,6 +316,29 @@ class Context:
     def interface_cv_apply(self, d_pos, d_dVdxi, d_force):
         t = self._torch
         self._ck(self._L.psg_interface_cv_apply(self._h, _dp(d_pos, t.float32), _dp(d_dVdxi, t.float32), _dp(d_force, t.float32)))
+
+    # ---- grid-stored metadynamics
+    def metad_grid_set(self, lower, upper, shape, periodic, sigma, w0, kB_deltaT=0.0):
+        k1, p1 = _hp(np.asarray(lower), np.float64)
+        k2, p2 = _hp(np.asarray(upper), np.float64)
+        k3, p3 = _hp(np.asarray(shape), np.int32)
+        k4, p4 = _hp(np.asarray(periodic), np.int32)
+        k5, p5 = _hp(np.asarray(sigma), np.float64)
+        self._ck(self._L.psg_metad_grid_set(self._h, len(k3), p1, p2, p3, p4, p5, float(w0), float(kB_deltaT)))
+
+    def metad_grid_deposit(self, d_xi, d_mask=None):
+        t = self._torch
+        self._ck(self._L.psg_metad_grid_deposit(self._h, _dp(d_xi, t.float32), _dp(d_mask, t.uint8)))
+
+    def metad_grid_eval(self, d_xi, d_V, d_dVdxi):
+        t = self._torch
+        self._ck(self._L.psg_metad_grid_eval(self._h, _dp(d_xi, t.float32), _dp(d_V, t.float32), _dp(d_dVdxi, t.float32)))
+
+    def metad_grid_state(self):
+        """(grid_ptr, n_nodes, heights_ptr) raw device pointers (binary64)"""
+        g, n, h = C.c_void_p(), C.c_longlong(), C.c_void_p()
+        self._ck(self._L.psg_metad_grid_state(self._h, C.byref(g), C.byref(n), C.byref(h)))
+        return g.value, n.value, h.value
 
     def sync_check(self):
         self._ck(self._L.psg_sync_check(self._h))

@@ -1136,3 +1136,99 @@ def test_shape_cv_argument_errors(torch, psg):
     with pytest.raises(psg.PsgError):      # which eigenvalue?
         ctx.set_cvs([{"type": psg.CV_PRINCIPAL_MOMENT, "groups": [("slots", 0, 5)], "axis": 3, "period": 0.0}], np.arange(5, dtype=np.int32))
     ctx.close()
+
+
+# ------------------------------------------------------------------------------------ grid-stored metadynamics
+@pytest.mark.parametrize("case", ["2d_periodic_open", "1d_open", "3d_mixed"])
+def test_metad_grid_matches_oracle(torch, psg, case):
+    """PAPER.md:L151, reading R-GRID: several well-tempered deposit events of R walkers (some masked out) onto a node grid, the
+    node array compared with the oracle's after every event, then the interpolated bias and gradient at fresh points inside,
+    on the faces and outside the grid; shapes are not multiples of the 128-node tile"""
+    from paper_2301_04835_b200.psg import _view
+    rng = np.random.default_rng({"2d_periodic_open": 1, "1d_open": 2, "3d_mixed": 3}[case])
+    lower, upper, shape, periodic, sigma = {
+        "2d_periodic_open": ((-math.pi, 0.2), (math.pi, 2.4), (67, 45), (1, 0), (0.35, 0.2)),
+        "1d_open": ((-1.0,), (3.0,), (1001,), (0,), (0.15,)),
+        "3d_mixed": ((0.0, -math.pi, 1.0), (2.0, math.pi, 4.0), (19, 24, 13), (0, 1, 0), (0.3, 0.5, 0.4)),
+    }[case]
+    n, R = len(shape), 300
+    lo, up = np.array(lower), np.array(upper)
+    g = orc.MetadGrid(lower, upper, shape, periodic)
+    ctx = psg.Context(0)
+    ctx.set_layout(R, 8, 8, 4, 4)
+    w0, kT = 1.2, 2.5
+    ctx.metad_grid_set(lower, upper, shape, periodic, sigma, w0, kT)
+    gp, nodes, hp = ctx.metad_grid_state()
+    assert nodes == g.nodes
+    for event in range(4):
+        xi = (lo + (up - lo) * rng.uniform(-0.05, 1.05, size=(R, n))).astype(np.float32)   # some walkers just outside
+        mask = None if event == 0 else (rng.uniform(size=R) < 0.7).astype(np.uint8)
+        ctx.metad_grid_deposit(dev(torch, xi), None if mask is None else dev(torch, mask))
+        ctx.sync_check()
+        h_ref = g.deposit(xi, np.array(sigma), w0, kT, mask)
+        h_gpu = _view(hp, (R,), torch.float64, 0).cpu().numpy()
+        assert np.allclose(h_gpu, h_ref, rtol=1e-12, atol=0), f"heights, event {event}"
+        if mask is not None:
+            assert np.array_equal(h_gpu == 0.0, mask == 0)
+        grid = _view(gp, (nodes, 1 + n), torch.float64, 0).cpu().numpy()
+        scale = np.abs(g.values).max(axis=0)
+        assert np.all(np.abs(grid - g.values) <= 1e-12 * scale), f"node array, event {event}"
+    pts = (lo + (up - lo) * rng.uniform(-0.2, 1.2, size=(R, n))).astype(np.float32)
+    pts[:n] = lo.astype(np.float32)                    # on the lower faces / the first node
+    pts[n:2 * n] = up.astype(np.float32)               # on the upper faces (periodic: the first node again)
+    d_V, d_dV = torch.empty(R, device="cuda"), torch.empty((R, n), device="cuda")
+    ctx.metad_grid_eval(dev(torch, pts), d_V, d_dV)
+    ctx.sync_check()
+    V, dV = g.eval(pts.astype(np.float64))
+    assert_close(d_V.cpu().numpy(), V, "grid V")
+    assert_close(d_dV.cpu().numpy(), dV, "grid dV/dxi")
+    assert np.abs(V).max() > 1.0                        # the test is not comparing zeros
+    ctx.close()
+
+
+def test_metad_grid_drives_the_force_scatter(torch, psg):
+    """the grid bias in the per-step path: psg_cv_eval -> psg_metad_grid_eval -> psg_apply_bias_forces on dihedral CVs, forces
+    against the oracle's scatter of the oracle's interpolated gradient"""
+    w = small(1)
+    ctx = make_ctx(psg, w, with_method=False)
+    sysm = oracle_system(w)
+    P = 2 * math.pi
+    lower, upper, shape, periodic, sigma = (-math.pi, -math.pi), (math.pi, math.pi), (90, 90), (1, 1), (0.35, 0.35)
+    g = orc.MetadGrid(lower, upper, shape, periodic)
+    ctx.metad_grid_set(lower, upper, shape, periodic, sigma, 1.2, 0.0)
+    d_xi = torch.empty((w.R, 2), device="cuda")
+    for frame in range(3):                               # three events at the walkers' own CV values
+        ctx.cv_eval(dev(torch, w.positions(frame)), d_xi, None)
+        ctx.metad_grid_deposit(d_xi)
+        ctx.sync_check()
+        g.deposit(d_xi.cpu().numpy(), np.array(sigma), 1.2)
+    pos, f0 = w.positions(3 % w.K), w.forces0()
+    d_pos, d_f = dev(torch, pos), dev(torch, f0)
+    d_V, d_dV = torch.empty(w.R, device="cuda"), torch.empty((w.R, 2), device="cuda")
+    ctx.cv_eval(d_pos, d_xi, None)
+    ctx.metad_grid_eval(d_xi, d_V, d_dV)
+    ctx.apply_bias_forces(d_pos, d_dV, d_f)
+    ctx.sync_check()
+    xi32 = d_xi.cpu().numpy()
+    assert_close(xi32, sysm.cv_eval(pos, want_jac=False), "xi", period=w.period)
+    V, dV = g.eval(xi32.astype(np.float64))              # both sides interpolate at the SAME binary32 xi (reading R-XI32)
+    assert_close(d_V.cpu().numpy(), V, "grid V on the path")
+    assert_close(d_dV.cpu().numpy(), dV, "grid dV/dxi on the path")
+    f_ref = sysm.apply_forces(pos, dV, f0[..., :3].astype(np.float64))
+    assert_forces_close(d_f.cpu().numpy()[..., :3], f_ref, f0[..., :3], "grid metad forces")
+    ctx.close()
+
+
+def test_metad_grid_argument_errors(torch, psg):
+    ctx = psg.Context(0)
+    with pytest.raises(psg.PsgError):
+        ctx.metad_grid_set((0.0,), (1.0,), (8,), (0,), (0.1,), 1.0)          # no layout yet
+    ctx.set_layout(4, 8, 8, 4, 4)
+    with pytest.raises(psg.PsgError):
+        ctx.metad_grid_eval(torch.zeros((4, 1), device="cuda"), torch.zeros(4, device="cuda"), None)   # no grid yet
+    for bad in [dict(shape=(1,)), dict(upper=(-1.0,)), dict(sigma=(0.0,)), dict(w0=0.0)]:
+        kw = dict(lower=(0.0,), upper=(1.0,), shape=(8,), periodic=(0,), sigma=(0.1,), w0=1.0)
+        kw.update(bad)
+        with pytest.raises(psg.PsgError):
+            ctx.metad_grid_set(**kw)
+    ctx.close()
