@@ -14,7 +14,7 @@
 struct GridParams {
     int n_cv, R;
     int shape[PSG_MAX_CV], periodic[PSG_MAX_CV];
-    double lower[PSG_MAX_CV], h[PSG_MAX_CV], period[PSG_MAX_CV], inv_s2[PSG_MAX_CV];   // period = 0: open
+    double lower[PSG_MAX_CV], h[PSG_MAX_CV], period[PSG_MAX_CV], inv_period[PSG_MAX_CV], inv_s2[PSG_MAX_CV];   // period = 0: open
     double w0, kB_deltaT;
     long long nodes;
 };
@@ -127,7 +127,7 @@ __global__ void __launch_bounds__(GRID_TILE) k_grid_deposit(const __grid_constan
             for (int k = 0; k < PSG_MAX_CV; ++k)
                 if (k < n) {
                     d[k] = x[k] - s_x[j][k];
-                    if (G.period[k] > 0.0) d[k] -= G.period[k] * rint(d[k] / G.period[k]);
+                    d[k] -= G.period[k] * rint(d[k] * G.inv_period[k]);      // open: period = inv_period = 0, the identity
                     e += d[k] * d[k] * G.inv_s2[k];
                 }
             const double g = W * exp(-0.5 * e);
@@ -158,6 +158,7 @@ extern "C" int psg_metad_grid_set(psg_ctx* c, int n_cv, const double* lower, con
         G.shape[k] = shape[k]; G.periodic[k] = periodic[k] ? 1 : 0; G.lower[k] = lower[k];
         G.h[k] = (upper[k] - lower[k]) / (double)(periodic[k] ? shape[k] : shape[k] - 1);
         G.period[k] = periodic[k] ? upper[k] - lower[k] : 0.0;
+        G.inv_period[k] = periodic[k] ? 1.0 / G.period[k] : 0.0;
         G.inv_s2[k] = 1.0 / (sigma[k] * sigma[k]);
         G.nodes *= shape[k];
         if (G.nodes > (1ll << 27)) return bad("psg_metad_grid_set: more than 2^27 nodes");
