@@ -236,6 +236,10 @@ int psg_interface_cv_apply(psg_ctx* ctx, const float* d_pos, const float* d_dVdx
  * psg_metad_grid_deposit: one synchronous event -- every walker r with d_mask[r] != 0 (NULL: all) adds its hill, centred on
  *   d_xi[r] (device, [R][n_cv] binary32), to every node, in replica order.  Two launches on the ctx stream, no sync.
  * psg_metad_grid_eval: d_V [R] and d_dVdxi [R][n_cv] (device, binary32; either may be NULL).  One launch, no sync.
+ * psg_metad_grid_step: the per-step path with the bias on the grid in ONE launch: CVs and Jacobians of the configured CVs
+ *   (psg_set_cvs; n_cv and R must match the grid) -> interpolated bias at the binary32 CV values -> force[i] += -dV/dxi *
+ *   dxi/dr_i in place.  xi, V, dV/dxi are left in the buffers psg_step_outputs returns (feed that xi to
+ *   psg_metad_grid_deposit every `stride` steps).  CVs over atom ranges take three launches instead.  No sync.
  * psg_metad_grid_state: device pointers of the node array and of the heights [R] (binary64) of the last event; owned by
  *   the ctx, valid until the next psg_metad_grid_set or psg_destroy.
  * Errors: PSG_EINVAL (arguments), PSG_ESTATE (call order), PSG_ENOMEM, PSG_ECUDA. */
@@ -243,6 +247,7 @@ int psg_metad_grid_set(psg_ctx* ctx, int n_cv, const double* lower, const double
                        const double* sigma, double w0, double kB_deltaT);
 int psg_metad_grid_deposit(psg_ctx* ctx, const float* d_xi, const unsigned char* d_mask);
 int psg_metad_grid_eval(psg_ctx* ctx, const float* d_xi, float* d_V, float* d_dVdxi);
+int psg_metad_grid_step(psg_ctx* ctx, const float* d_pos, float* d_force);
 int psg_metad_grid_state(psg_ctx* ctx, double** d_grid_out, long long* n_nodes_out, double** d_heights_out);
 
 /* ------------------------------------------------------------- measurement */

@@ -7,7 +7,7 @@
 // The node array is [nodes][1 + n_cv] binary64, row-major with the last CV fastest; all arithmetic is binary64: a node sums
 // thousands of deposits over a run and every later bias value is a difference-free read of it, so the store is where
 // precision matters, and the deposit runs once per `stride` steps, not per step.  Shares nothing with oracle/.
-#include "internal.h"
+#include "geom.cuh"
 
 #define GRID_TILE 128
 
@@ -42,20 +42,16 @@ __device__ __forceinline__ void grid_cell(const GridParams& G, int k, double x, 
     f = t - (double)i0;
 }
 
-// V and dV/dxi of walker r by multilinear interpolation.  height == nullptr: write V / dVdxi (binary32, the bias arrays of
-// the rest of the path).  height != nullptr: write the height this walker deposits, w0 exp(-V / kB dT) or w0, 0 if masked.
-__global__ void __launch_bounds__(128) k_grid_eval(const __grid_constant__ GridParams G, const double* __restrict__ grid,
-                                                    const float* __restrict__ xi, float* __restrict__ V, float* __restrict__ dVdxi,
-                                                    double* __restrict__ height, const unsigned char* __restrict__ mask) {
-    const int r = blockIdx.x * blockDim.x + threadIdx.x;
-    if (r >= G.R) return;
+// out[0] = V, out[1 + k] = dV/dxi_k at the binary32 CV values xi[0..n_cv): multilinear interpolation of 2^n_cv nodes
+__device__ __forceinline__ void grid_interp(const GridParams& G, const double* __restrict__ grid, const float* xi, double* out) {
     const int n = G.n_cv, rec = 1 + n;
     int i0[PSG_MAX_CV];
     double f[PSG_MAX_CV];
 #pragma unroll
     for (int k = 0; k < PSG_MAX_CV; ++k)
-        if (k < n) grid_cell(G, k, (double)xi[(long long)r * n + k], i0[k], f[k]);
-    double out[1 + PSG_MAX_CV] = {0, 0, 0, 0, 0};
+        if (k < n) grid_cell(G, k, (double)xi[k], i0[k], f[k]);
+#pragma unroll
+    for (int c = 0; c < 1 + PSG_MAX_CV; ++c) out[c] = 0.0;
     for (int corner = 0; corner < (1 << n); ++corner) {
         double w = 1.0;
         long long flat = 0;
@@ -74,6 +70,21 @@ __global__ void __launch_bounds__(128) k_grid_eval(const __grid_constant__ GridP
         for (int c = 0; c < 1 + PSG_MAX_CV; ++c)
             if (c < rec) out[c] += w * node[c];
     }
+}
+
+// V and dV/dxi of walker r.  height == nullptr: write V / dVdxi (binary32, the bias arrays of the rest of the path).
+// height != nullptr: write the height this walker deposits, w0 exp(-V / kB dT) or w0, 0 if masked.
+__global__ void __launch_bounds__(128) k_grid_eval(const __grid_constant__ GridParams G, const double* __restrict__ grid,
+                                                    const float* __restrict__ xi, float* __restrict__ V, float* __restrict__ dVdxi,
+                                                    double* __restrict__ height, const unsigned char* __restrict__ mask) {
+    const int r = blockIdx.x * blockDim.x + threadIdx.x;
+    if (r >= G.R) return;
+    const int n = G.n_cv;
+    float x[PSG_MAX_CV];
+#pragma unroll
+    for (int k = 0; k < PSG_MAX_CV; ++k) x[k] = k < n ? xi[(long long)r * n + k] : 0.f;
+    double out[1 + PSG_MAX_CV];
+    grid_interp(G, grid, x, out);
     if (height) {
         double W = 0.0;
         if (!mask || mask[r]) W = G.kB_deltaT > 0.0 ? G.w0 * exp(-out[0] / G.kB_deltaT) : G.w0;
@@ -202,6 +213,68 @@ extern "C" int psg_metad_grid_eval(psg_ctx* c, const float* d_xi, float* d_V, fl
     k_grid_eval<<<(G.R + 127) / 128, 128, 0, c->stream>>>(G, S->grid, d_xi, d_V, d_dVdxi, nullptr, nullptr);
     c->launches += 1;
     if (cudaGetLastError() != cudaSuccess) { c->err = "psg_metad_grid_eval: launch failed"; return PSG_ECUDA; }
+    return PSG_OK;
+}
+
+// The per-step path with the bias on the grid, ONE launch (SURVEY rows A1, A2, A8 with the grid in place of the hill sum):
+// warp per walker -- gather the CV atoms in place, CVs and Jacobians in binary64 registers (geom.cuh), xi rounded to
+// binary32 (reading R-XI32: the bias is a function of the binary32 CV the caller sees), lane 0 interpolates the grid, every
+// lane scatters force[i] += -dV/dxi_k * dxi_k/dr_i for its slots (red.global.add.f32: atoms shared between CVs collide).
+// The grid is read-only here, so there is no barrier and the launch is an ordinary one.
+__global__ void __launch_bounds__(256) k_grid_step(const __grid_constant__ SysParams P, const __grid_constant__ GridParams G,
+                                                    const double* __restrict__ grid, const float* __restrict__ pos,
+                                                    float* __restrict__ force, float* __restrict__ xi_out,
+                                                    float* __restrict__ V_out, float* __restrict__ dV_out) {
+    __shared__ WarpCvSmem sm[8];
+    __shared__ float s_dv[8][PSG_MAX_CV];
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+    const int r = blockIdx.x * 8 + wid;
+    if (r >= P.R) return;
+    WarpCvSmem& S = sm[wid];
+    warp_cv_eval<true>(P, r, pos, nullptr, S, lane);
+    if (lane == 0) {
+        float x[PSG_MAX_CV];
+#pragma unroll
+        for (int k = 0; k < PSG_MAX_CV; ++k) x[k] = k < P.n_cv ? (float)S.xi[k] : 0.f;
+        double out[1 + PSG_MAX_CV];
+        grid_interp(G, grid, x, out);
+        V_out[r] = (float)out[0];
+#pragma unroll
+        for (int k = 0; k < PSG_MAX_CV; ++k)
+            if (k < P.n_cv) {
+                xi_out[(long long)r * P.n_cv + k] = x[k];
+                dV_out[(long long)r * P.n_cv + k] = s_dv[wid][k] = (float)out[1 + k];
+            }
+    }
+    __syncwarp();
+    for (int s = lane; s < P.n_slots; s += 32) {
+        const D3 j = slot_jacobian(P, r, pos, S, s);
+        const float dv = -s_dv[wid][P.grp[P.slot_gid[s]].cv];
+        const int atom = P.slot_atom[(P.per_rep ? (long long)r * P.n_slots : 0) + s];
+        float* f = force + ((long long)r * P.rstride + atom) * P.fs;
+        atomicAdd(f, dv * (float)j.x);
+        atomicAdd(f + 1, dv * (float)j.y);
+        atomicAdd(f + 2, dv * (float)j.z);
+    }
+}
+
+extern "C" int psg_metad_grid_step(psg_ctx* c, const float* d_pos, float* d_force) {
+    if (!c) return PSG_EINVAL;
+    GridState* S = gs(c);
+    if (!S) { c->err = "psg_metad_grid_step: call psg_metad_grid_set first"; return PSG_ESTATE; }
+    if (!c->have_cvs) { c->err = "psg_metad_grid_step: no CVs configured"; return PSG_ESTATE; }
+    if (!d_pos || !d_force) { c->err = "psg_metad_grid_step: NULL pointer"; return PSG_EINVAL; }
+    const SysParams& P = c->sys;
+    if (P.n_cv != S->G.n_cv || P.R != S->G.R) { c->err = "psg_metad_grid_step: the grid was set for another n_cv or walker count"; return PSG_ESTATE; }
+    if (P.n_ranges > 0) {   // range groups: their moments and forces live in the streaming kernels
+        int e = psg_cv_eval(c, d_pos, c->d_xi, nullptr);
+        if (e == PSG_OK) e = psg_metad_grid_eval(c, c->d_xi, c->d_V, c->d_dVdxi);
+        if (e == PSG_OK) e = psg_apply_bias_forces(c, d_pos, c->d_dVdxi, d_force);
+        return e;
+    }
+    k_grid_step<<<(P.R + 7) / 8, 256, 0, c->stream>>>(P, S->G, S->grid, d_pos, d_force, c->d_xi, c->d_V, c->d_dVdxi);
+    c->launches += 1;
+    if (cudaGetLastError() != cudaSuccess) { c->err = "psg_metad_grid_step: launch failed"; return PSG_ECUDA; }
     return PSG_OK;
 }
 

@@ -26,7 +26,7 @@ EXPORTS = ["psg_create", "psg_destroy", "psg_set_stream", "psg_last_error", "psg
            "psg_set_abf", "psg_abf_state", "psg_cv_eval", "psg_bias_eval", "psg_deposit_hill", "psg_abf_update",
            "psg_abf_estimate", "psg_abf_estimate_reset", "psg_apply_bias_forces", "psg_step", "psg_step_outputs", "psg_step_host", "psg_sync_check",
            "psg_interface_cv_set", "psg_interface_cv_eval", "psg_interface_cv_apply", "psg_metad_grid_set",
-           "psg_metad_grid_deposit", "psg_metad_grid_eval", "psg_metad_grid_state", "psg_measure_alu_peak", "psg_launch_count"]
+           "psg_metad_grid_deposit", "psg_metad_grid_eval", "psg_metad_grid_step", "psg_metad_grid_state", "psg_measure_alu_peak", "psg_launch_count"]
 
 
 class PsgError(RuntimeError):
@@ -94,6 +94,7 @@ def load_library():
         L.psg_metad_grid_deposit.argtypes = [vp, vp, vp]
         L.psg_metad_grid_eval.argtypes = [vp, vp, vp, vp]
         L.psg_metad_grid_state.argtypes = [vp, vp, vp, vp]
+        L.psg_metad_grid_step.argtypes = [vp, vp, vp]
         L.psg_measure_alu_peak.argtypes = [i, i, C.POINTER(C.c_double)]
         _lib = L
     return _lib
@@ -333,6 +334,10 @@ class Context:
     def metad_grid_eval(self, d_xi, d_V, d_dVdxi):
         t = self._torch
         self._ck(self._L.psg_metad_grid_eval(self._h, _dp(d_xi, t.float32), _dp(d_V, t.float32), _dp(d_dVdxi, t.float32)))
+
+    def metad_grid_step(self, d_pos, d_force):
+        t = self._torch
+        self._ck(self._L.psg_metad_grid_step(self._h, _dp(d_pos, t.float32), _dp(d_force, t.float32)))
 
     def metad_grid_state(self):
         """(grid_ptr, n_nodes, heights_ptr) raw device pointers (binary64)"""

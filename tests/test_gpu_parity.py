@@ -1216,6 +1216,80 @@ def test_metad_grid_drives_the_force_scatter(torch, psg):
     assert_close(d_dV.cpu().numpy(), dV, "grid dV/dxi on the path")
     f_ref = sysm.apply_forces(pos, dV, f0[..., :3].astype(np.float64))
     assert_forces_close(d_f.cpu().numpy()[..., :3], f_ref, f0[..., :3], "grid metad forces")
+    # the same step as ONE launch: identical xi, V, dV/dxi; forces differ only by the rounding of the Jacobian cache
+    d_f2 = dev(torch, f0)
+    n0 = ctx.launch_count()
+    ctx.metad_grid_step(d_pos, d_f2)
+    assert ctx.launch_count() - n0 == 1
+    ctx.sync_check()
+    out = ctx.read_step_outputs()
+    assert np.array_equal(out["xi"].cpu().numpy().view(np.uint32), xi32.view(np.uint32))
+    assert np.array_equal(out["V"].cpu().numpy().view(np.uint32), d_V.cpu().numpy().view(np.uint32))
+    assert np.array_equal(out["dVdxi"].cpu().numpy().view(np.uint32), d_dV.cpu().numpy().view(np.uint32))
+    assert_forces_close(d_f2.cpu().numpy()[..., :3], f_ref, f0[..., :3], "grid metad forces, one launch")
+    assert np.array_equal(d_f2.cpu().numpy()[..., 3].view(np.uint32), f0[..., 3].view(np.uint32))     # the pad is not touched
+    ctx.close()
+
+
+def test_metad_grid_step_other_cv_kinds(torch, psg):
+    """the one-launch grid step on CVs whose per-atom Jacobian needs r_i - c (Rg, shape anisotropy: the k_hills step cannot
+    take these) and, through the three-launch route, on CVs over atom ranges (config 3's windows)"""
+    rng = np.random.default_rng(91)
+    R, N = 130, 40
+    pos = np.concatenate([_shape_molecules(rng, R, N), np.zeros((R, N, 1), np.float32)], axis=2)
+    slot = np.concatenate([np.arange(0, 14), np.arange(10, 30)]).astype(np.int32)
+    groups = [[("slots", 0, 14)], [("slots", 14, 20)]]
+    o_cvs = [{"type": orc.SHAPE_ANISOTROPY, "groups": groups[0], "axis": 0, "period": 0.0},
+             {"type": orc.RGYR, "groups": groups[1], "axis": 0, "period": 0.0}]
+    g_cvs = [{"type": psg.CV_SHAPE_ANISOTROPY, "groups": groups[0], "axis": 0, "period": 0.0},
+             {"type": psg.CV_RGYR, "groups": groups[1], "axis": 0, "period": 0.0}]
+    sysm = orc.System(R, N, N, 4, o_cvs, slot, None, None)
+    xi_ref = sysm.cv_eval(pos, want_jac=False)
+    lower, upper = xi_ref.min(axis=0) - 0.02, xi_ref.max(axis=0) + 0.02
+    shape, periodic, sigma = (40, 33), (0, 0), (0.05, 0.03)
+    g = orc.MetadGrid(lower, upper, shape, periodic)
+    ctx = psg.Context(0)
+    ctx.set_layout(R, N, N, 4, 4)
+    ctx.set_cvs(g_cvs, slot, None, None)
+    ctx.metad_grid_set(lower, upper, shape, periodic, sigma, 1.2, 0.0)
+    seed_xi = (xi_ref[rng.integers(0, R, size=R)] + rng.normal(scale=0.03, size=(R, 2))).astype(np.float32)
+    ctx.metad_grid_deposit(dev(torch, seed_xi))
+    g.deposit(seed_xi, np.array(sigma), 1.2)
+    f0 = (rng.standard_normal((R, N, 4)) * 100).astype(np.float32)
+    d_f = dev(torch, f0)
+    ctx.metad_grid_step(dev(torch, pos), d_f)
+    ctx.sync_check()
+    out = {k: v.cpu().numpy() for k, v in ctx.read_step_outputs().items()}
+    assert_close(out["xi"], xi_ref, "xi")
+    V, dV = g.eval(out["xi"].astype(np.float64))
+    assert_close(out["V"], V, "V")
+    assert_close(out["dVdxi"], dV, "dV/dxi")
+    assert np.abs(dV).max() > 1.0
+    f_ref = sysm.apply_forces(pos, dV, f0[..., :3].astype(np.float64))
+    assert_forces_close(d_f.cpu().numpy()[..., :3], f_ref, f0[..., :3], "forces")
+    ctx.close()
+    # -- atom ranges
+    w = small(3)
+    ctx = make_ctx(psg, w, with_method=False)
+    sysm = oracle_system(w)
+    pos, f0 = w.positions(0), w.forces0()
+    xi_ref = sysm.cv_eval(pos, want_jac=False)
+    n = w.n_cv
+    lower, upper = xi_ref.min(axis=0) - 0.5, xi_ref.max(axis=0) + 0.5
+    g = orc.MetadGrid(lower, upper, (31,) * n, (0,) * n)
+    ctx.metad_grid_set(lower, upper, (31,) * n, (0,) * n, (0.4,) * n, 50.0, 0.0)
+    seed_xi = (xi_ref + rng.normal(scale=0.3, size=xi_ref.shape)).astype(np.float32)
+    ctx.metad_grid_deposit(dev(torch, seed_xi))
+    g.deposit(seed_xi, np.full(n, 0.4), 50.0)
+    d_f = dev(torch, f0)
+    ctx.metad_grid_step(dev(torch, pos), d_f)
+    ctx.sync_check()
+    out = {k: v.cpu().numpy() for k, v in ctx.read_step_outputs().items()}
+    assert_close(out["xi"], xi_ref, "range xi")
+    V, dV = g.eval(out["xi"].astype(np.float64))
+    assert_close(out["dVdxi"], dV, "range dV/dxi")
+    f_ref = sysm.apply_forces(pos, dV, f0[..., :3].astype(np.float64))
+    assert_forces_close(d_f.cpu().numpy()[..., :3], f_ref, f0[..., :3], "range forces")
     ctx.close()
 
 
