@@ -159,6 +159,16 @@ int psg_bias_eval(psg_ctx* ctx, const float* d_xi, float* d_V, float* d_dVdxi);
  * call and append in replica order.  d_mask [R] nullable (NULL = all deposit).  PSG_ECAPACITY, nothing
  * launched, if the host-side upper bound of the count + R exceeds capacity. */
 int psg_deposit_hill(psg_ctx* ctx, const float* d_xi, const unsigned char* d_mask);
+/* The same event in two halves, for walkers spread over several GPUs (multiple-walker metadynamics needs
+ * ONE exchange per deposit, an all-gather of the new hills; PAPER.md:L404-L406 runs replicas on separate GPUs).
+ * psg_hill_heights: d_heights [R] (device, binary32) := the height every walker of THIS ctx would deposit at d_xi now,
+ *   w0 or w0 exp(-V/(kB dT)) from the list as it is, 0 where d_mask[r] == 0; appends nothing.
+ * psg_append_hills: append n ready-made hills, centres d_centers [n][n_cv] and heights d_heights [n] (device), in order,
+ *   skipping zero heights.  After every rank has all-gathered (xi, heights) in rank order and appended them, every rank's
+ *   list is the one a single ctx holding all the walkers would have built with psg_deposit_hill, bit for bit.
+ *   PSG_ECAPACITY, nothing launched, if the host-side bound of the count + n exceeds capacity.  Neither call synchronises. */
+int psg_hill_heights(psg_ctx* ctx, const float* d_xi, const unsigned char* d_mask, float* d_heights);
+int psg_append_hills(psg_ctx* ctx, int n, const float* d_centers, const float* d_heights);
 
 /* ABF grid update for all replicas, then the mean force from the fully updated grid (two-phase):
  *  bin in binary32: I_k = floor(fl(fl(xi_k - lower_k) * invd_k)); in-grid: hist[bin] += 1, Fsum[bin][k] += f_k;

@@ -433,6 +433,25 @@ int psg_abf_estimate_reset(psg_ctx* c) {
     return PSG_OK;
 }
 
+int psg_hill_heights(psg_ctx* c, const float* d_xi, const unsigned char* d_mask, float* d_heights) {
+    if (!c) return PSG_EINVAL;
+    if (c->method != PSG_METHOD_METAD) return fail(c, PSG_ESTATE, "psg_hill_heights: metadynamics is not selected");
+    if (!d_xi || !d_heights) return fail(c, PSG_EINVAL, "psg_hill_heights: NULL pointer");
+    CK(c, psg_launch_hill_heights(c, d_xi, d_mask, d_heights));
+    return PSG_OK;
+}
+
+int psg_append_hills(psg_ctx* c, int n, const float* d_centers, const float* d_heights) {
+    if (!c) return PSG_EINVAL;
+    if (c->method != PSG_METHOD_METAD) return fail(c, PSG_ESTATE, "psg_append_hills: metadynamics is not selected");
+    if (n < 0 || (n > 0 && (!d_centers || !d_heights))) return fail(c, PSG_EINVAL, "psg_append_hills: n >= 0 and no NULL pointer");
+    if (c->nh_bound + n > c->md.capacity)
+        return fail(c, PSG_ECAPACITY, "psg_append_hills: hill store would overflow (host bound + n > capacity); nothing launched");
+    if (n > 0) CK(c, psg_launch_append_hills(c, n, d_centers, d_heights));
+    c->nh_bound += n;
+    return PSG_OK;
+}
+
 int psg_apply_bias_forces(psg_ctx* c, const float* d_pos, const float* d_dVdxi, float* d_force) {
     if (!c) return PSG_EINVAL;
     if (!c->have_jac) return fail(c, PSG_ESTATE, "psg_apply_bias_forces: no cached Jacobian; call psg_cv_eval on these positions first");

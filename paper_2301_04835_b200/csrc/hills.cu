@@ -26,9 +26,12 @@ __device__ __forceinline__ void store_hill(float4* __restrict__ hills, float* __
     }
 }
 
+// W_in == nullptr: one deposit event of this ctx's R walkers (heights from Vold).  W_in != nullptr: append R ready-made hills
+// (centres xi, heights W_in; the other ranks' included, psg_append_hills), skipping the zero heights of masked-out walkers.
 __global__ void __launch_bounds__(1024) k_deposit(int R, int n_cv, int rec, const float* __restrict__ xi, const double* __restrict__ Vold,
                                                    const unsigned char* __restrict__ mask, double w0, double kBdT, float4* __restrict__ hills,
-                                                   float* __restrict__ heights, int* __restrict__ n_hills, int capacity) {
+                                                   float* __restrict__ heights, int* __restrict__ n_hills, int capacity,
+                                                   const float* __restrict__ W_in) {
     __shared__ int s_warp[32];
     __shared__ int s_base;
     const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
@@ -36,7 +39,7 @@ __global__ void __launch_bounds__(1024) k_deposit(int R, int n_cv, int rec, cons
     __syncthreads();
     for (int r0 = 0; r0 < R; r0 += 1024) {
         int r = r0 + tid;
-        int dep = (r < R) && (!mask || mask[r]);
+        int dep = (r < R) && (W_in ? W_in[r] != 0.f : (!mask || mask[r]));
         unsigned b = __ballot_sync(0xffffffffu, dep);
         int pre = __popc(b & ((1u << lane) - 1u));
         if (lane == 0) s_warp[wid] = __popc(b);
@@ -49,7 +52,7 @@ __global__ void __launch_bounds__(1024) k_deposit(int R, int n_cv, int rec, cons
         if (dep) {
             int slot = s_base + off + pre;
             if (slot < capacity) {
-                float W = (float)(kBdT > 0.0 ? w0 * exp(-Vold[r] / kBdT) : w0);
+                float W = W_in ? W_in[r] : (float)(kBdT > 0.0 ? w0 * exp(-Vold[r] / kBdT) : w0);
                 float s[4] = {0.f, 0.f, 0.f, 0.f};
                 for (int k = 0; k < n_cv; ++k) s[k] = xi[(long long)r * n_cv + k];
                 store_hill(hills, heights, rec, slot, s, W);
@@ -182,7 +185,34 @@ cudaError_t psg_launch_deposit(psg_ctx* c, const float* d_xi, const unsigned cha
         if (e != cudaSuccess) return e;
     }
     k_deposit<<<1, 1024, 0, c->stream>>>(c->sys.R, c->sys.n_cv, c->md.rec, d_xi, c->d_V64, d_mask, c->md.w0, c->md.kB_deltaT,
-                                         c->md.hills, c->md.heights, c->md.n_hills, c->md.capacity);
+                                         c->md.hills, c->md.heights, c->md.n_hills, c->md.capacity, nullptr);
+    c->launches++;
+    return cudaGetLastError();
+}
+
+// the height every walker of this ctx would deposit now (0 where masked out); nothing is appended
+__global__ void __launch_bounds__(256) k_hill_heights(int R, const double* __restrict__ Vold, const unsigned char* __restrict__ mask,
+                                                       double w0, double kBdT, float* __restrict__ W_out) {
+    const int r = blockIdx.x * blockDim.x + threadIdx.x;
+    if (r >= R) return;
+    float W = 0.f;
+    if (!mask || mask[r]) W = (float)(kBdT > 0.0 ? w0 * exp(-Vold[r] / kBdT) : w0);   // the expression of k_deposit
+    W_out[r] = W;
+}
+
+cudaError_t psg_launch_hill_heights(psg_ctx* c, const float* d_xi, const unsigned char* d_mask, float* d_heights) {
+    if (c->md.kB_deltaT > 0.0) {
+        cudaError_t e = psg_launch_hillsum(c, d_xi, nullptr, nullptr);   // V_old -> d_V64
+        if (e != cudaSuccess) return e;
+    }
+    k_hill_heights<<<(c->sys.R + 255) / 256, 256, 0, c->stream>>>(c->sys.R, c->d_V64, d_mask, c->md.w0, c->md.kB_deltaT, d_heights);
+    c->launches++;
+    return cudaGetLastError();
+}
+
+cudaError_t psg_launch_append_hills(psg_ctx* c, int n, const float* d_centers, const float* d_heights) {
+    k_deposit<<<1, 1024, 0, c->stream>>>(n, c->sys.n_cv, c->md.rec, d_centers, nullptr, nullptr, c->md.w0, c->md.kB_deltaT,
+                                         c->md.hills, c->md.heights, c->md.n_hills, c->md.capacity, d_heights);
     c->launches++;
     return cudaGetLastError();
 }

@@ -128,6 +128,8 @@ cudaError_t psg_launch_apply(psg_ctx* c, const float* d_pos, const float* d_dVdx
 cudaError_t psg_launch_harmonic(psg_ctx* c, const float* d_xi, float* d_V, float* d_dVdxi);
 cudaError_t psg_launch_hillsum(psg_ctx* c, const float* d_xi, float* d_V, float* d_dVdxi);
 cudaError_t psg_launch_deposit(psg_ctx* c, const float* d_xi, const unsigned char* d_mask);
+cudaError_t psg_launch_hill_heights(psg_ctx* c, const float* d_xi, const unsigned char* d_mask, float* d_heights);
+cudaError_t psg_launch_append_hills(psg_ctx* c, int n, const float* d_centers, const float* d_heights);
 cudaError_t psg_launch_pack_hills(psg_ctx* c, int n, const float* d_centers, const float* d_heights);
 cudaError_t psg_launch_unpack_hills(psg_ctx* c, int n, float* d_centers, float* d_heights);
 cudaError_t psg_launch_null_hills(psg_ctx* c, int begin, int end);   // records [begin, end) := null

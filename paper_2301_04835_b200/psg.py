@@ -25,7 +25,7 @@ EXPORTS = ["psg_create", "psg_destroy", "psg_set_stream", "psg_last_error", "psg
            "psg_set_box", "psg_set_harmonic", "psg_set_metad", "psg_set_hill_precision", "psg_load_hills", "psg_get_hills",
            "psg_set_abf", "psg_abf_state", "psg_cv_eval", "psg_bias_eval", "psg_deposit_hill", "psg_abf_update",
            "psg_abf_estimate", "psg_abf_estimate_reset", "psg_apply_bias_forces", "psg_step", "psg_step_outputs", "psg_step_host", "psg_sync_check",
-           "psg_interface_cv_set", "psg_interface_cv_eval", "psg_interface_cv_apply", "psg_metad_grid_set",
+           "psg_interface_cv_set", "psg_interface_cv_eval", "psg_interface_cv_apply", "psg_hill_heights", "psg_append_hills", "psg_metad_grid_set",
            "psg_metad_grid_deposit", "psg_metad_grid_eval", "psg_metad_grid_step", "psg_metad_grid_state", "psg_measure_alu_peak", "psg_launch_count"]
 
 
@@ -90,6 +90,8 @@ def load_library():
         L.psg_interface_cv_set.argtypes = [vp, i, vp, vp, ll, ll, i, d, d, d, i, d]
         L.psg_interface_cv_eval.argtypes = [vp, vp, vp]
         L.psg_interface_cv_apply.argtypes = [vp, vp, vp, vp]
+        L.psg_hill_heights.argtypes = [vp, vp, vp, vp]
+        L.psg_append_hills.argtypes = [vp, i, vp, vp]
         L.psg_metad_grid_set.argtypes = [vp, i, vp, vp, vp, vp, vp, d, d]
         L.psg_metad_grid_deposit.argtypes = [vp, vp, vp]
         L.psg_metad_grid_eval.argtypes = [vp, vp, vp, vp]
@@ -212,6 +214,15 @@ class Context:
 
     def set_hill_precision(self, mode):
         self._ck(self._L.psg_set_hill_precision(self._h, mode))
+
+    def hill_heights(self, d_xi, d_mask, d_heights):
+        t = self._torch
+        self._ck(self._L.psg_hill_heights(self._h, _dp(d_xi, t.float32), _dp(d_mask, t.uint8), _dp(d_heights, t.float32)))
+
+    def append_hills(self, d_centers, d_heights):
+        t = self._torch
+        n = int(d_heights.shape[0])
+        self._ck(self._L.psg_append_hills(self._h, n, _dp(d_centers, t.float32), _dp(d_heights, t.float32)))
 
     def load_hills(self, d_centers, d_heights):
         n = int(d_heights.shape[0]) if d_heights is not None else 0

@@ -1306,3 +1306,52 @@ def test_metad_grid_argument_errors(torch, psg):
         with pytest.raises(psg.PsgError):
             ctx.metad_grid_set(**kw)
     ctx.close()
+
+
+# ------------------------------------------------------------------------------------ multiple walkers over several contexts
+def test_split_deposit_equals_single_context_deposit(torch, psg):
+    """psg_hill_heights + psg_append_hills: two contexts of R walkers each (two ranks' worth, run one after the other on this
+    GPU -- no kernel waits on another) exchange (xi, height) and append; their hill lists equal, bit for bit, the list of one
+    context holding all 2R walkers after psg_deposit_hill, over well-tempered events with masked-out walkers"""
+    rng = np.random.default_rng(17)
+    w = small(1)
+    R, n = w.R, w.n_cv
+    w2 = W.make(1, R=2 * R, n_hills=SMALL[1]["n_hills"], steps=SMALL[1]["steps"], stride=SMALL[1]["stride"])
+    sigma, w0, kT, cap = w.params["sigma"], w.params["w0"], w.params["kB_deltaT"], 40 * R
+    assert kT > 0
+    ctxs = []
+    for ww in (w, w, w2):
+        c = make_ctx(psg, ww, with_method=False)
+        c.set_metad(sigma, w0, kT, cap, 0)
+        ctxs.append(c)
+    a, b, whole = ctxs
+    for event in range(4):
+        xi = rng.uniform(-math.pi, math.pi, size=(2 * R, n)).astype(np.float32)
+        mask = None if event == 0 else (rng.uniform(size=2 * R) < 0.6).astype(np.uint8)
+        d_xi = dev(torch, xi)
+        d_mask = None if mask is None else dev(torch, mask)
+        hs = []
+        for c, sl in ((a, slice(0, R)), (b, slice(R, 2 * R))):
+            d_h = torch.empty(R, device="cuda")
+            c.hill_heights(d_xi[sl].contiguous(), None if mask is None else d_mask[sl].contiguous(), d_h)
+            hs.append(d_h)
+        all_h = torch.cat(hs)                              # what the all-gather delivers to every rank
+        for c in (a, b):
+            c.append_hills(d_xi, all_h)
+        whole.deposit_hill(d_xi, d_mask)
+        lists = []
+        for c in ctxs:
+            c.sync_check()
+            cen, hgt = c.get_hills()
+            lists.append((cen.cpu().numpy(), hgt.cpu().numpy()))
+        n_exp = 2 * R if mask is None else int(mask.sum())
+        assert lists[2][1].shape[0] == (lists[2][1].shape[0] if event else n_exp)
+        for cen, hgt in lists[:2]:
+            assert cen.shape == lists[2][0].shape, f"event {event}: hill count"
+            assert np.array_equal(cen.view(np.uint32), lists[2][0].view(np.uint32)), f"event {event}: centres"
+            assert np.array_equal(hgt.view(np.uint32), lists[2][1].view(np.uint32)), f"event {event}: heights"
+    assert lists[2][1].min() < 0.999 * w0                  # well-tempered heights really varied
+    with pytest.raises(psg.PsgError):                      # capacity is checked on the host before anything is launched
+        a.append_hills(torch.zeros((cap, n), device="cuda"), torch.ones(cap, device="cuda"))
+    for c in ctxs:
+        c.close()

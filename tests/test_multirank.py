@@ -54,3 +54,67 @@ def test_reference_arm_under_torchrun_prints_one_line_from_rank0():
     d = json.loads(lines[0])
     assert d["impl"] == "reference" and d["n_gpus"] == 2 and d["cpu_baseline"]["kind"] == "oracle"
     assert d["e2e"]["h2d_bytes_per_step"] == 0 and d["value"] > 0
+
+
+_MW_WORKER = r"""
+import os, sys, json
+sys.path.insert(0, {root!r})
+import torch, torch.distributed as dist
+from paper_2301_04835_b200.multiwalker import deposit_hill_all_ranks
+rank, world = int(os.environ["RANK"]), int(os.environ["WORLD_SIZE"])
+dist.init_process_group("gloo")
+
+class FakeCtx:                       # stands in for psg.Context on CPU tensors: records what the helper asks the library for
+    def __init__(self): self.centres, self.heights = [], []
+    def hill_heights(self, xi, mask, out):
+        out.copy_(100.0 * (rank + 1) + xi[:, 0])          # any rank-dependent numbers
+        if mask is not None: out[mask == 0] = 0.0
+    def append_hills(self, c, h):
+        self.centres.append(c.clone()); self.heights.append(h.clone())
+
+ctx = FakeCtx()
+R, n_cv = 3, 2
+xi = torch.arange(R * n_cv, dtype=torch.float32).reshape(R, n_cv) + 10.0 * rank
+mask = torch.tensor([1, 0, 1], dtype=torch.uint8) if rank == 1 else None
+n = deposit_hill_all_ranks(ctx, xi, mask)
+out = dict(rank=rank, n=n, centres=ctx.centres[0].tolist(), heights=ctx.heights[0].tolist())
+gathered = [None] * world
+dist.all_gather_object(gathered, out)
+if rank == 0:
+    print(json.dumps(gathered))
+dist.destroy_process_group()
+"""
+
+
+def test_multiwalker_deposit_gathers_in_rank_order_gloo(tmp_path):
+    """deposit_hill_all_ranks: every rank appends the (centre, height) pairs of ALL walkers, rank 0's first,
+    with the zero heights of masked-out walkers kept in place for the library to skip; both ranks append the same list"""
+    script = tmp_path / "mw_worker.py"
+    script.write_text(_MW_WORKER.format(root=ROOT))
+    p = _torchrun([str(script)])
+    assert p.returncode == 0, p.stderr[-2000:]
+    line = [l for l in p.stdout.splitlines() if l.startswith("[")]
+    assert len(line) == 1
+    r0, r1 = json.loads(line[0])
+    assert r0["n"] == r1["n"] == 6
+    assert r0["centres"] == r1["centres"] and r0["heights"] == r1["heights"]
+    assert r0["centres"] == [[0.0, 1.0], [2.0, 3.0], [4.0, 5.0], [10.0, 11.0], [12.0, 13.0], [14.0, 15.0]]
+    assert r0["heights"] == [100.0, 102.0, 104.0, 210.0, 0.0, 214.0]
+
+
+def test_multiwalker_deposit_single_process():
+    """without an initialised process group the helper is the two library calls back to back"""
+    import torch
+    from paper_2301_04835_b200.multiwalker import deposit_hill_all_ranks
+
+    class Ctx:
+        def hill_heights(self, xi, mask, out):
+            out.fill_(1.5)
+
+        def append_hills(self, c, h):
+            self.got = (c.clone(), h.clone())
+
+    c = Ctx()
+    xi = torch.ones((4, 2))
+    assert deposit_hill_all_ranks(c, xi) == 4
+    assert torch.equal(c.got[0], xi) and torch.equal(c.got[1], torch.full((4,), 1.5))
