@@ -132,7 +132,8 @@ int psg_set_hill_precision(psg_ctx* ctx, int mode /* PSG_HILLS_* */);
 /* Replace the store's contents by n hills: centers [n][n_cv], heights [n], DEVICE pointers (copied). */
 int psg_load_hills(psg_ctx* ctx, int n, const float* d_centers, const float* d_heights);
 /* Synchronises. *n_out (host) = exact hill count; if d_centers/d_heights are non-NULL (device) and
- * max_n >= count they receive the store's contents as [n][n_cv] / [n]. */
+ * max_n >= count they receive the store's contents as [n][n_cv] / [n].  PSG_ECAPACITY (after filling *n_out) if an
+ * earlier deposit was clamped at capacity. */
 int psg_get_hills(psg_ctx* ctx, int* n_out, float* d_centers, float* d_heights, int max_n);
 
 /* ABF, PAPER.md:L143 (Sec. 2.1.4), Grid(lower, upper, shape, periodic) of L82, N of L501/L507.
@@ -156,8 +157,15 @@ int psg_cv_eval(psg_ctx* ctx, const float* d_pos, float* d_xi, float* d_jac);
 int psg_bias_eval(psg_ctx* ctx, const float* d_xi, float* d_V, float* d_dVdxi);
 
 /* Append one hill per replica at xi: all walkers see the list as it was BEFORE this
- * call and append in replica order.  d_mask [R] nullable (NULL = all deposit).  PSG_ECAPACITY, nothing
- * launched, if the host-side upper bound of the count + R exceeds capacity. */
+ * call and append in replica order.  d_mask [R] nullable (NULL = all deposit).
+ * Capacity: the exact count lives on the device; the host tracks a lower and an upper bound of it, equal as long as no
+ * mask was used.  PSG_ECAPACITY, nothing launched, when the overflow is certain (exact for d_mask == NULL: count + R >
+ * capacity).  A MASKED call whose overflow the host cannot rule out is launched; the kernel never writes beyond
+ * capacity, drops the excess hills and raises a sticky flag that the next psg_sync_check / psg_get_hills returns as
+ * PSG_ECAPACITY (cleared by psg_load_hills / psg_set_metad).  No padding of `capacity` is needed.
+ * CUDA graphs: a deposit (this call, psg_append_hills, or a psg_step on a deposit step) may be captured; replays then
+ * append behind the host's back, so from that moment every launch of this ctx takes the hill count from the device
+ * counter and capacity is enforced by the device clamp alone, until psg_get_hills or psg_load_hills re-synchronises. */
 int psg_deposit_hill(psg_ctx* ctx, const float* d_xi, const unsigned char* d_mask);
 /* The same event in two halves, for walkers spread over several GPUs (multiple-walker metadynamics needs
  * ONE exchange per deposit, an all-gather of the new hills; PAPER.md:L404-L406 runs replicas on separate GPUs).
@@ -165,8 +173,9 @@ int psg_deposit_hill(psg_ctx* ctx, const float* d_xi, const unsigned char* d_mas
  *   w0 or w0 exp(-V/(kB dT)) from the list as it is, 0 where d_mask[r] == 0; appends nothing.
  * psg_append_hills: append n ready-made hills, centres d_centers [n][n_cv] and heights d_heights [n] (device), in order,
  *   skipping zero heights.  After every rank has all-gathered (xi, heights) in rank order and appended them, every rank's
- *   list is the one a single ctx holding all the walkers would have built with psg_deposit_hill, bit for bit.
- *   PSG_ECAPACITY, nothing launched, if the host-side bound of the count + n exceeds capacity.  Neither call synchronises. */
+ *   list is IDENTICAL: the centres a single ctx holding all the walkers would have appended with psg_deposit_hill, with
+ *   heights equal to that ctx's up to the binary32 rounding of V_old (the hill sum's chunk length depends on the walkers
+ *   per ctx).  Capacity as for a masked psg_deposit_hill (zero heights are skipped on the device).  Neither call synchronises. */
 int psg_hill_heights(psg_ctx* ctx, const float* d_xi, const unsigned char* d_mask, float* d_heights);
 int psg_append_hills(psg_ctx* ctx, int n, const float* d_centers, const float* d_heights);
 
@@ -175,6 +184,20 @@ int psg_append_hills(psg_ctx* ctx, int n, const float* d_centers, const float* d
  *  d_dVdxi[r][k] := Fsum[bin][k] / max(hist[bin], N);  outside: bin = -1, 0.
  *  d_fsample [R][n_cv] in;  d_bin [R] out nullable;  d_dVdxi [R][n_cv] out. */
 int psg_abf_update(psg_ctx* ctx, const float* d_xi, const float* d_fsample, int* d_bin, float* d_dVdxi);
+
+/* The same update in two halves, for replicas spread over several GPUs that share ONE grid (shared-grid ABF
+ * needs one exchange per step, an all-reduce of the step's histogram and force-sum contributions; the paper runs replicas on
+ * separate GPUs).  Reading R-ABF-2 (two-phase) then spans the ranks: ALL replicas of ALL ranks
+ * accumulate before anyone reads a mean force.
+ * psg_abf_accumulate_delta: gather -> CVs (+ Jacobians, cached) -> bin; the contributions of THIS ctx's replicas go to
+ *   d_hist_delta int32 [n_bins] and d_fsum_delta float32 [n_bins][n_cv] (device, caller-owned, overwritten: zeroed first);
+ *   the ctx grid is not touched.  Bins stay in the ctx (psg_step_outputs).
+ * psg_abf_apply_grid_delta: grid += the (all-reduced) deltas, then every replica reads its mean force from the updated grid
+ *   and force[i] += -Fbar_k dxi_k/dr_i, as psg_step does.  PSG_ESTATE without a pending psg_abf_accumulate_delta.
+ * With one rank the two calls build the grid psg_step builds (histogram bit for bit; force sums up to the order of the
+ * binary32 additions).  Neither call synchronises; both are graph-capturable. */
+int psg_abf_accumulate_delta(psg_ctx* ctx, const float* d_pos, const float* d_fsample, int* d_hist_delta, float* d_fsum_delta);
+int psg_abf_apply_grid_delta(psg_ctx* ctx, const int* d_hist_delta, const float* d_fsum_delta, const float* d_pos, float* d_force);
 
 /* ABF instantaneous generalized-force estimator.  The paper says only "based on the algorithm
  * described in [43]"; this is DESIGN.md reading R-ABF-EST: with J[k][i] = d xi_k/d r_i and momenta
@@ -212,7 +235,8 @@ int psg_step_outputs(psg_ctx* ctx, float** d_xi, float** d_V, float** d_dVdxi, i
  * h_pos (and h_force) to ctx-owned device buffers, runs psg_step, copies the forces back and waits. */
 int psg_step_host(psg_ctx* ctx, const float* h_pos, float* h_force, const float* h_fsample, long long step);
 
-/* The only other call that synchronises: waits for the ctx stream and returns sticky CUDA errors. */
+/* The only other call that synchronises: waits for the ctx stream and returns sticky CUDA errors, and PSG_ECAPACITY if a
+ * masked or graph-captured deposit was clamped at the hill store's capacity. */
 int psg_sync_check(psg_ctx* ctx);
 
 /* ------------------------------------------------------------- DistanceToInterface */
@@ -259,18 +283,6 @@ int psg_metad_grid_deposit(psg_ctx* ctx, const float* d_xi, const unsigned char*
 int psg_metad_grid_eval(psg_ctx* ctx, const float* d_xi, float* d_V, float* d_dVdxi);
 int psg_metad_grid_step(psg_ctx* ctx, const float* d_pos, float* d_force);
 int psg_metad_grid_state(psg_ctx* ctx, double** d_grid_out, long long* n_nodes_out, double** d_heights_out);
-
-/* ------------------------------------------------------------- measurement */
-/* Measured ALU throughput of this device (register-only loops, CUDA-event timed, synchronises):
- * which = 0: FP32 FFMA lane-ops/s; 1: packed FFMA2 (f32x2) lane-ops/s (2 per lane per instruction);
- * 2: MUFU.EX2/s; 3: FP64 DFMA lane-ops/s; 4: F2F f32->f64->f32 round trips/s; 5: I2F.F32.S32/s;
- * 6: packed FADD2 lane-ops/s.  Denominators for the hill-sum roofline.
- * 7 / 8: hill evaluations/s of the BARE hill loop (k_hills' own inner loop on a shared-memory table, nothing
- * else; 2-D periodic / 3-D with 2 periodic CVs): the ceiling of the kernel's instruction mix.
- * 100 + n: the same as 7 with only n passes of 1,024 hills (short-run behaviour). */
-int psg_measure_alu_peak(int device, int which, double* ops_per_second_out);
-/* Launch counter: number of kernels this ctx has enqueued since creation (for bench.py's gpu_launches). */
-long long psg_launch_count(const psg_ctx* ctx);
 
 #ifdef __cplusplus
 }

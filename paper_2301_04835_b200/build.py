@@ -19,7 +19,7 @@ NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", 
 
 
 def _newest_source() -> float:
-    t = os.path.getmtime(os.path.join(ROOT, "include", "psg.h"))
+    t = max(os.path.getmtime(os.path.join(ROOT, "include", f)) for f in os.listdir(os.path.join(ROOT, "include")))
     for f in os.listdir(CSRC):
         t = max(t, os.path.getmtime(os.path.join(CSRC, f)))
     return t

@@ -22,6 +22,8 @@ struct AbfStepArgs {
     float* dV_out;          // [R][n_cv]
     float* jac;             // [R][n_slots][3] (the ctx cache, as after psg_cv_eval)
     unsigned* bar;          // [2] arrive / depart counters, zero between launches
+    int phase;              // 0: the whole step; 1: phase 1 only (G then points at per-step DELTA arrays, psg_abf_accumulate_delta);
+                            // 2: phase 2 only (bins and Jacobians of an earlier phase-1 launch, psg_abf_apply_grid_delta)
 };
 
 __global__ void __launch_bounds__(256, 4) k_abf_step(const __grid_constant__ SysParams P, const __grid_constant__ AbfState G,
@@ -31,7 +33,7 @@ __global__ void __launch_bounds__(256, 4) k_abf_step(const __grid_constant__ Sys
     const int warps = gridDim.x * 8, gw = blockIdx.x * 8 + wid;
     WarpCvSmem& S = sm[wid];
 
-    for (int r = gw; r < P.R; r += warps) {
+    for (int r = gw; A.phase != 2 && r < P.R; r += warps) {
         warp_cv_eval<true>(P, r, A.pos, nullptr, S, lane);
         if (lane < P.n_cv) A.xi_out[(long long)r * P.n_cv + lane] = (float)S.xi[lane];
         for (int s = lane; s < P.n_slots; s += 32) {
@@ -51,9 +53,10 @@ __global__ void __launch_bounds__(256, 4) k_abf_step(const __grid_constant__ Sys
         __syncwarp();
     }
 
+    if (A.phase == 1) return;
     // ---- grid barrier: every replica's atomics are performed before anyone reads the grid
     __syncthreads();
-    if (tid == 0) {
+    if (A.phase == 0 && tid == 0) {
         __threadfence();
         atomicAdd(A.bar, 1u);
         unsigned n;
@@ -73,15 +76,13 @@ __global__ void __launch_bounds__(256, 4) k_abf_step(const __grid_constant__ Sys
             const int atom = P.slot_atom[(P.per_rep ? (long long)r * P.n_slots : 0) + s];
             float* f = A.force + ((long long)r * P.rstride + atom) * P.fs;
             const float* j = A.jac + ((long long)r * P.n_slots + s) * 3;
-            atomicAdd(f, dv * j[0]);
-            atomicAdd(f + 1, dv * j[1]);
-            atomicAdd(f + 2, dv * j[2]);
+            force_add(f, dv * j[0], dv * j[1], dv * j[2], P.fs);
         }
     }
 
     // ---- the last CTA to leave re-arms the barrier for the next launch
     __syncthreads();
-    if (tid == 0) {
+    if (A.phase == 0 && tid == 0) {
         const unsigned old = atomicAdd(A.bar + 1, 1u);
         if (old == gridDim.x - 1) { A.bar[0] = 0u; A.bar[1] = 0u; }
     }
@@ -100,11 +101,46 @@ bool psg_abf_step_supported(const psg_ctx* c) {
     return c->method == PSG_METHOD_ABF && c->sys.n_ranges == 0 && c->d_gbar != nullptr && abf_blocks_per_sm() >= 1;
 }
 
+// grid[b] += delta[b] for every bin (the all-reduced contribution of one step, psg_abf_apply_grid_delta)
+__global__ void __launch_bounds__(256) k_abf_add_delta(long long n_bins, int n_cv, int* __restrict__ hist, float* __restrict__ fsum,
+                                                        const int* __restrict__ dh, const float* __restrict__ df) {
+    const long long b = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (b >= n_bins) return;
+    hist[b] += dh[b];
+    for (int k = 0; k < n_cv; ++k) fsum[b * n_cv + k] += df[b * n_cv + k];
+}
+
+cudaError_t psg_launch_abf_add_delta(psg_ctx* c, const int* d_hist_delta, const float* d_fsum_delta) {
+    const long long nb = c->abf.n_bins;
+    k_abf_add_delta<<<(unsigned)((nb + 255) / 256), 256, 0, c->stream>>>(nb, c->sys.n_cv, c->abf.hist, c->abf.fsum, d_hist_delta,
+                                                                         d_fsum_delta);
+    c->launches++;
+    return cudaGetLastError();
+}
+
+// one half of the step on its own (phase 1 into `hist` / `fsum`, which may be per-step delta arrays; phase 2 from the ctx grid):
+// no inter-CTA wait, so an ordinary launch
+cudaError_t psg_launch_abf_phase(psg_ctx* c, int phase, const float* d_pos, const float* d_fsample, float* d_force, int* hist,
+                                 float* fsum) {
+    const SysParams& P = c->sys;
+    AbfStepArgs A{};
+    A.pos = d_pos; A.fsample = d_fsample; A.force = d_force;
+    A.xi_out = c->d_xi; A.bin_out = c->d_bin; A.dV_out = c->d_dVdxi; A.jac = c->d_jac; A.bar = c->d_gbar; A.phase = phase;
+    AbfState G = c->abf;
+    G.hist = hist; G.fsum = fsum;
+    long long grid = (P.R + 7) / 8;
+    const long long cap = (long long)c->sm_count * 8;
+    if (grid > cap) grid = cap;
+    k_abf_step<<<(unsigned)grid, 256, 0, c->stream>>>(P, G, A);
+    c->launches++;
+    return cudaGetLastError();
+}
+
 cudaError_t psg_launch_abf_step(psg_ctx* c, const float* d_pos, const float* d_fsample, float* d_force) {
     const SysParams& P = c->sys;
     AbfStepArgs A{};
     A.pos = d_pos; A.fsample = d_fsample; A.force = d_force;
-    A.xi_out = c->d_xi; A.bin_out = c->d_bin; A.dV_out = c->d_dVdxi; A.jac = c->d_jac; A.bar = c->d_gbar;
+    A.xi_out = c->d_xi; A.bin_out = c->d_bin; A.dV_out = c->d_dVdxi; A.jac = c->d_jac; A.bar = c->d_gbar; A.phase = 0;
     long long grid = (P.R + 7) / 8;
     const long long cap = (long long)c->sm_count * abf_blocks_per_sm();
     if (grid > cap) grid = cap;

@@ -38,6 +38,28 @@ static cudaError_t dalloc(T*& p, size_t n) {
     return cudaMalloc((void**)&p, n * sizeof(T));
 }
 
+// Host-side admission of a deposit of up to n hills: the exact count lives on the device; the host keeps a
+// lower and an upper bound (equal while no mask was used).  Refused, nothing launched, when overflow is CERTAIN (lower bound
+// + the hills this call surely adds > capacity; exact for unmasked calls).  A masked call that might overflow is launched:
+// the kernel clamps at capacity and raises the sticky flag psg_sync_check / psg_get_hills report.  After a deposit captured
+// in a CUDA graph the host knows nothing (replays append behind its back): admission is left to the device clamp.
+static int deposit_admit(psg_ctx* c, long long n, bool masked, const char* msg) {
+    if (c->count_unknown) return PSG_OK;
+    const long long sure = masked ? 0 : n;
+    if (c->nh_lo + sure > c->md.capacity) {
+        c->err = msg;
+        return PSG_ECAPACITY;
+    }
+    return PSG_OK;
+}
+static void deposit_account(psg_ctx* c, long long n, bool masked) {
+    const long long cap = c->md.capacity;
+    if (c->nh_bound + n > cap || c->count_unknown) c->overflow_possible = true;   // launched although the host could not rule it out
+    c->nh_bound = std::min(c->nh_bound + n, cap);
+    if (!masked) c->nh_lo = std::min(c->nh_lo + n, cap);
+    if (psg_stream_capturing(c)) { c->count_unknown = true; c->overflow_possible = true; }
+}
+
 static const int kGroups[11] = {0, 2, 3, 4, 1, 1, 2, 1, 1, 1, 1};
 
 extern "C" {
@@ -284,13 +306,13 @@ int psg_set_metad(psg_ctx* c, const float* sigma, float w0, float kB_deltaT, int
     size_t part = psg_hill_part_doubles(c, &M.max_chunks, &n_rt);
     CK(c, dalloc(M.hills, (size_t)capacity * M.rec + 2));
     CK(c, dalloc(M.heights, (size_t)capacity + 2));
-    CK(c, dalloc(M.n_hills, 1));
+    CK(c, dalloc(M.n_hills, 2));
     CK(c, dalloc(M.part, part));
     CK(c, dalloc(M.ticket, (size_t)n_rt));
-    CK(c, cudaMemset(M.n_hills, 0, sizeof(int)));
+    CK(c, cudaMemset(M.n_hills, 0, 2 * sizeof(int)));
     CK(c, cudaMemset(M.ticket, 0, n_rt * sizeof(unsigned)));
     CK(c, psg_launch_null_hills(c, 0, capacity));   // invariant: records beyond the count are null (contribute 0)
-    c->nh_bound = 0;
+    c->nh_bound = c->nh_lo = 0; c->count_unknown = false; c->overflow_possible = false;
     c->method = PSG_METHOD_METAD;
     return PSG_OK;
 }
@@ -310,10 +332,12 @@ int psg_load_hills(psg_ctx* c, int n, const float* d_centers, const float* d_hei
     if (n > c->md.capacity) return fail(c, PSG_ECAPACITY, "psg_load_hills: more hills than capacity");
     cudaSetDevice(c->device);
     CK(c, psg_launch_pack_hills(c, n, d_centers, d_heights));
-    if (c->nh_bound > n) CK(c, psg_launch_null_hills(c, n, (int)c->nh_bound));
-    CK(c, cudaMemcpyAsync(c->md.n_hills, &n, sizeof(int), cudaMemcpyHostToDevice, c->stream));
-    CK(c, cudaStreamSynchronize(c->stream));   // n is a stack variable
-    c->nh_bound = n;
+    const long long old_bound = c->count_unknown ? c->md.capacity : c->nh_bound;
+    if (old_bound > n) CK(c, psg_launch_null_hills(c, n, (int)old_bound));
+    const int cnt[2] = {n, 0};                  // exact count, overflow flag cleared
+    CK(c, cudaMemcpyAsync(c->md.n_hills, cnt, 2 * sizeof(int), cudaMemcpyHostToDevice, c->stream));
+    CK(c, cudaStreamSynchronize(c->stream));   // cnt is a stack variable
+    c->nh_bound = c->nh_lo = n; c->count_unknown = false; c->overflow_possible = false;
     return PSG_OK;
 }
 
@@ -321,11 +345,13 @@ int psg_get_hills(psg_ctx* c, int* n_out, float* d_centers, float* d_heights, in
     if (!c) return PSG_EINVAL;
     if (c->method != PSG_METHOD_METAD) return fail(c, PSG_ESTATE, "psg_get_hills: metadynamics is not selected");
     cudaSetDevice(c->device);
-    int n = 0;
-    CK(c, cudaMemcpyAsync(&n, c->md.n_hills, sizeof(int), cudaMemcpyDeviceToHost, c->stream));
+    int cnt[2] = {0, 0};
+    CK(c, cudaMemcpyAsync(cnt, c->md.n_hills, 2 * sizeof(int), cudaMemcpyDeviceToHost, c->stream));
     CK(c, cudaStreamSynchronize(c->stream));
+    const int n = cnt[0];
     if (n_out) *n_out = n;
-    c->nh_bound = n;   // exact now
+    c->nh_bound = c->nh_lo = n; c->count_unknown = false;   // exact now
+    if (cnt[1]) return fail(c, PSG_ECAPACITY, "psg_get_hills: an earlier deposit overflowed the hill store; hills were dropped");
     if (d_centers && d_heights) {
         if (max_n < n) return fail(c, PSG_ECAPACITY, "psg_get_hills: output arrays too small");
         CK(c, psg_launch_unpack_hills(c, n, d_centers, d_heights));
@@ -366,6 +392,7 @@ int psg_set_abf(psg_ctx* c, const float* lower, const float* upper, const int* s
         CK(c, cudaMemset(G.fsum, 0, nb * n_cv * sizeof(float)));
     }
     c->method = PSG_METHOD_ABF;
+    c->abf_delta_pending = false;
     return PSG_OK;
 }
 
@@ -401,10 +428,10 @@ int psg_deposit_hill(psg_ctx* c, const float* d_xi, const unsigned char* d_mask)
     if (!c) return PSG_EINVAL;
     if (c->method != PSG_METHOD_METAD) return fail(c, PSG_ESTATE, "psg_deposit_hill: metadynamics is not selected");
     if (!d_xi) return fail(c, PSG_EINVAL, "psg_deposit_hill: NULL pointer");
-    if (c->nh_bound + c->sys.R > c->md.capacity)
-        return fail(c, PSG_ECAPACITY, "psg_deposit_hill: hill store would overflow (host bound + R > capacity); nothing launched");
+    int rc = deposit_admit(c, c->sys.R, d_mask != nullptr, "psg_deposit_hill: hill store would overflow (count + R > capacity); nothing launched");
+    if (rc != PSG_OK) return rc;
     CK(c, psg_launch_deposit(c, d_xi, d_mask));
-    c->nh_bound += c->sys.R;
+    deposit_account(c, c->sys.R, d_mask != nullptr);
     return PSG_OK;
 }
 
@@ -413,6 +440,43 @@ int psg_abf_update(psg_ctx* c, const float* d_xi, const float* d_fsample, int* d
     if (c->method != PSG_METHOD_ABF) return fail(c, PSG_ESTATE, "psg_abf_update: ABF is not selected");
     if (!d_xi || !d_fsample || !d_dVdxi) return fail(c, PSG_EINVAL, "psg_abf_update: NULL pointer");
     CK(c, psg_launch_abf(c, d_xi, d_fsample, d_bin, d_dVdxi));
+    return PSG_OK;
+}
+
+// Shared-grid ABF with the replicas spread over several GPUs: phase 1 into per-step delta arrays ...
+int psg_abf_accumulate_delta(psg_ctx* c, const float* d_pos, const float* d_fsample, int* d_hist_delta, float* d_fsum_delta) {
+    if (!c) return PSG_EINVAL;
+    if (c->method != PSG_METHOD_ABF) return fail(c, PSG_ESTATE, "psg_abf_accumulate_delta: ABF is not selected");
+    if (!d_pos || !d_fsample || !d_hist_delta || !d_fsum_delta) return fail(c, PSG_EINVAL, "psg_abf_accumulate_delta: NULL pointer");
+    const size_t nb = (size_t)c->abf.n_bins;
+    CK(c, cudaMemsetAsync(d_hist_delta, 0, nb * sizeof(int), c->stream));
+    CK(c, cudaMemsetAsync(d_fsum_delta, 0, nb * c->sys.n_cv * sizeof(float), c->stream));
+    if (psg_abf_step_supported(c)) {
+        CK(c, psg_launch_abf_phase(c, 1, d_pos, d_fsample, nullptr, d_hist_delta, d_fsum_delta));
+    } else {
+        CK(c, psg_launch_cv_eval(c, d_pos, c->d_xi, nullptr));
+        CK(c, psg_launch_abf_accumulate(c, c->d_xi, d_fsample, d_hist_delta, d_fsum_delta));
+    }
+    c->have_jac = true;
+    c->abf_delta_pending = true;
+    return PSG_OK;
+}
+
+// ... and, after the all-reduce over ranks, grid += delta and phase 2 (mean force from the updated grid, force scatter)
+int psg_abf_apply_grid_delta(psg_ctx* c, const int* d_hist_delta, const float* d_fsum_delta, const float* d_pos, float* d_force) {
+    if (!c) return PSG_EINVAL;
+    if (c->method != PSG_METHOD_ABF) return fail(c, PSG_ESTATE, "psg_abf_apply_grid_delta: ABF is not selected");
+    if (!d_hist_delta || !d_fsum_delta || !d_pos || !d_force) return fail(c, PSG_EINVAL, "psg_abf_apply_grid_delta: NULL pointer");
+    if (!c->abf_delta_pending)
+        return fail(c, PSG_ESTATE, "psg_abf_apply_grid_delta: no pending psg_abf_accumulate_delta on this ctx");
+    CK(c, psg_launch_abf_add_delta(c, d_hist_delta, d_fsum_delta));
+    if (psg_abf_step_supported(c)) {
+        CK(c, psg_launch_abf_phase(c, 2, d_pos, nullptr, d_force, c->abf.hist, c->abf.fsum));
+    } else {
+        CK(c, psg_launch_abf_mean(c, nullptr, c->d_dVdxi));
+        CK(c, psg_launch_apply(c, d_pos, c->d_dVdxi, d_force));
+    }
+    c->abf_delta_pending = false;
     return PSG_OK;
 }
 
@@ -445,10 +509,11 @@ int psg_append_hills(psg_ctx* c, int n, const float* d_centers, const float* d_h
     if (!c) return PSG_EINVAL;
     if (c->method != PSG_METHOD_METAD) return fail(c, PSG_ESTATE, "psg_append_hills: metadynamics is not selected");
     if (n < 0 || (n > 0 && (!d_centers || !d_heights))) return fail(c, PSG_EINVAL, "psg_append_hills: n >= 0 and no NULL pointer");
-    if (c->nh_bound + n > c->md.capacity)
-        return fail(c, PSG_ECAPACITY, "psg_append_hills: hill store would overflow (host bound + n > capacity); nothing launched");
+    // (zero heights are skipped on the device: like a masked deposit, the host only knows bounds)
+    int rc = deposit_admit(c, n, true, "psg_append_hills: hill store would overflow (count + n > capacity); nothing launched");
+    if (rc != PSG_OK) return rc;
     if (n > 0) CK(c, psg_launch_append_hills(c, n, d_centers, d_heights));
-    c->nh_bound += n;
+    deposit_account(c, n, true);
     return PSG_OK;
 }
 
@@ -469,10 +534,11 @@ int psg_step(psg_ctx* c, const float* d_pos, float* d_force, const float* d_fsam
         const MetadState& M = c->md;
         if (M.stride > 0 && step > 0 && step % M.stride == 0) {
             // xi -> deposit (heights from the OLD list) -> bias with the NEW list
-            if (c->nh_bound + c->sys.R > M.capacity) return fail(c, PSG_ECAPACITY, "psg_step: hill store would overflow; nothing launched");
+            int rc = deposit_admit(c, c->sys.R, false, "psg_step: hill store would overflow; nothing launched");
+            if (rc != PSG_OK) return rc;
             CK(c, psg_launch_cv_eval(c, d_pos, c->d_xi, nullptr));
             CK(c, psg_launch_deposit(c, c->d_xi, nullptr));
-            c->nh_bound += c->sys.R;
+            deposit_account(c, c->sys.R, false);
         }
         if (psg_metad_step_supported(c)) {
             CK(c, psg_launch_metad_step(c, d_pos, d_force));
@@ -546,6 +612,12 @@ int psg_sync_check(psg_ctx* c) {
     cudaSetDevice(c->device);
     CK(c, cudaStreamSynchronize(c->stream));
     CK(c, cudaGetLastError());
+    if (c->method == PSG_METHOD_METAD && c->md.n_hills && c->overflow_possible) {
+        // the host could not rule an overflow out (masked or captured deposits): ask the device
+        int cnt[2] = {0, 0};
+        CK(c, cudaMemcpy(cnt, c->md.n_hills, 2 * sizeof(int), cudaMemcpyDeviceToHost));
+        if (cnt[1]) return fail(c, PSG_ECAPACITY, "psg_sync_check: a deposit overflowed the hill store; hills were dropped");
+    }
     return PSG_OK;
 }
 

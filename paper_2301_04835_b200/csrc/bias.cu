@@ -46,10 +46,22 @@ cudaError_t psg_launch_harmonic(psg_ctx* c, const float* d_xi, float* d_V, float
     return cudaGetLastError();
 }
 
-cudaError_t psg_launch_abf(psg_ctx* c, const float* d_xi, const float* d_fsample, int* d_bin, float* d_dVdxi) {
-    int R = c->sys.R, g = (R + 255) / 256;
-    k_abf_accumulate<<<g, 256, 0, c->stream>>>(c->abf, R, c->sys.n_cv, d_xi, d_fsample, c->d_bin);
-    k_abf_mean<<<g, 256, 0, c->stream>>>(c->abf, R, c->sys.n_cv, c->d_bin, d_bin, d_dVdxi);
-    c->launches += 2;
+cudaError_t psg_launch_abf_accumulate(psg_ctx* c, const float* d_xi, const float* d_fsample, int* hist, float* fsum) {
+    AbfState G = c->abf;
+    G.hist = hist; G.fsum = fsum;
+    k_abf_accumulate<<<(c->sys.R + 255) / 256, 256, 0, c->stream>>>(G, c->sys.R, c->sys.n_cv, d_xi, d_fsample, c->d_bin);
+    c->launches++;
     return cudaGetLastError();
+}
+
+cudaError_t psg_launch_abf_mean(psg_ctx* c, int* d_bin, float* d_dVdxi) {
+    k_abf_mean<<<(c->sys.R + 255) / 256, 256, 0, c->stream>>>(c->abf, c->sys.R, c->sys.n_cv, c->d_bin, d_bin, d_dVdxi);
+    c->launches++;
+    return cudaGetLastError();
+}
+
+cudaError_t psg_launch_abf(psg_ctx* c, const float* d_xi, const float* d_fsample, int* d_bin, float* d_dVdxi) {
+    cudaError_t e = psg_launch_abf_accumulate(c, d_xi, d_fsample, c->abf.hist, c->abf.fsum);
+    if (e != cudaSuccess) return e;
+    return psg_launch_abf_mean(c, d_bin, d_dVdxi);
 }

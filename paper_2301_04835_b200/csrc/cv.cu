@@ -111,7 +111,7 @@ __global__ void __launch_bounds__(256) k_cv_eval(const __grid_constant__ SysPara
 
 // --------------------------------------------------------------------------------------------
 // Sparse scatter: thread per (replica, slot). Atoms shared between CVs (6, 8, 14 of phi/psi) or between
-// walkers of a shared array collide, hence red.global.add.f32 (fire-and-forget L2 atomics).
+// walkers of a shared array collide, hence L2 reductions (force_add: red.global.add.v2.f32 + one scalar per float4 record).
 __global__ void __launch_bounds__(256) k_apply_sparse(const __grid_constant__ SysParams P, const float* __restrict__ jac,
                                                        const float* __restrict__ dVdxi, float* __restrict__ force) {
     long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
@@ -122,9 +122,7 @@ __global__ void __launch_bounds__(256) k_apply_sparse(const __grid_constant__ Sy
     int atom = P.slot_atom[(P.per_rep ? (long long)r * P.n_slots : 0) + s];
     float* f = force + ((long long)r * P.rstride + atom) * P.fs;
     const float* j = jac + t * 3;
-    atomicAdd(f, dv * j[0]);
-    atomicAdd(f + 1, dv * j[1]);
-    atomicAdd(f + 2, dv * j[2]);
+    force_add(f, dv * j[0], dv * j[1], dv * j[2], P.fs);
 }
 
 // --------------------------------------------------------------------------------------------
@@ -189,7 +187,7 @@ __global__ void __launch_bounds__(256) k_apply_dense(const __grid_constant__ Sys
         float w = P.atom_weight ? __ldg(P.atom_weight + a) : 1.f;
         ax *= w; ay *= w; az *= w;
         if (shared_arr) {
-            atomicAdd(f + a * P.fs, ax); atomicAdd(f + a * P.fs + 1, ay); atomicAdd(f + a * P.fs + 2, az);
+            force_add(f + a * P.fs, ax, ay, az, P.fs);
         } else if (P.fs == 4) {
             float4* fp = reinterpret_cast<float4*>(f) + a;
             float4 v = *fp;

@@ -96,6 +96,20 @@ __device__ __forceinline__ double cv_from_centers(int type, int axis, const D3* 
     return 0.0;
 }
 
+// force[i] += (fx, fy, fz) where several CVs / walkers may hit the same atom (A8): fire-and-forget L2 atomics.  A float4
+// force record is 16-byte aligned, so x and y go as ONE vector reduction (red.global.add.v2.f32) and z as a scalar one; w is
+// never touched.  Records of 3 floats are only 4-byte aligned: three scalar reductions.
+__device__ __forceinline__ void force_add(float* __restrict__ fa, float fx, float fy, float fz, int fs) {
+    if (fs == 4) {
+        atomicAdd(reinterpret_cast<float2*>(fa), make_float2(fx, fy));
+        atomicAdd(fa + 2, fz);
+    } else {
+        atomicAdd(fa, fx);
+        atomicAdd(fa + 1, fy);
+        atomicAdd(fa + 2, fz);
+    }
+}
+
 __device__ __forceinline__ D3 load_pos(const float* __restrict__ p, long long atom, int ps) {
     if (ps == 4) {
         float4 v = __ldg(reinterpret_cast<const float4*>(p) + atom);

@@ -59,7 +59,10 @@ __global__ void __launch_bounds__(1024) k_deposit(int R, int n_cv, int rec, cons
             }
         }
         __syncthreads();
-        if (tid == 0) s_base = min(s_base + tot, capacity);
+        if (tid == 0) {
+            if (s_base + tot > capacity) n_hills[1] = 1;   // sticky: hills were dropped (reported by psg_sync_check / psg_get_hills)
+            s_base = min(s_base + tot, capacity);
+        }
         __syncthreads();
     }
     if (tid == 0) *n_hills = s_base;
@@ -110,6 +113,11 @@ extern "C" int psg_debug_trace(long long* host_out, int n_ctas) {
     return (int)cudaMemcpy(host_out, psg_trace_buffer(), (size_t)n_ctas * 8 * sizeof(long long), cudaMemcpyDeviceToHost);
 }
 #endif
+bool psg_stream_capturing(const psg_ctx* c) {
+    cudaStreamCaptureStatus st = cudaStreamCaptureStatusNone;
+    if (cudaStreamIsCapturing(c->stream, &st) != cudaSuccess) { st = cudaStreamCaptureStatusNone; (void)cudaGetLastError(); }
+    return st != cudaStreamCaptureStatusNone;
+}
 static int hills_grid(const psg_ctx* c) { return c->sm_count; }   // one 16-warp CTA per SM
 
 size_t psg_hill_part_doubles(const psg_ctx* c, int* max_chunks_out, int* n_rtiles_out) {
@@ -146,10 +154,9 @@ static HillKernelArgs base_args(psg_ctx* c) {
     A.hills = c->md.hills; A.heights = c->md.heights; A.n_hills = c->md.n_hills; A.part = c->md.part; A.ticket = c->md.ticket;
     A.R = c->sys.R;
     // The host's upper bound of the hill count saves the kernel a dependent global load. Under stream capture the
-    // launch may be replayed with a longer list than the one seen now, so the kernel reads the device counter.
-    cudaStreamCaptureStatus st = cudaStreamCaptureStatusNone;
-    if (cudaStreamIsCapturing(c->stream, &st) != cudaSuccess) { st = cudaStreamCaptureStatusNone; (void)cudaGetLastError(); }
-    A.n_h_host = st == cudaStreamCaptureStatusNone ? (int)c->nh_bound : -1;
+    // launch may be replayed with a longer list than the one seen now, and after a CAPTURED deposit the replays grow the
+    // list behind the host's back: in both cases the kernel reads the device counter.
+    A.n_h_host = (psg_stream_capturing(c) || c->count_unknown) ? -1 : (int)c->nh_bound;
 #ifdef PSG_TRACE
     A.trace = psg_trace_buffer();
 #endif

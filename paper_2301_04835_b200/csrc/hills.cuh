@@ -578,9 +578,7 @@ __global__ void __launch_bounds__(HWARPS * 32, 1) k_hills(const __grid_constant_
                     const float* j = s_jv + (rr * P.n_groups + gid) * 3;
                     int atom = P.slot_atom[(P.per_rep ? (long long)r * P.n_slots : 0) + s];
                     float* fa = A.force + ((long long)r * P.rstride + atom) * P.fs;
-                    atomicAdd(fa, fdv * (w * j[0]));
-                    atomicAdd(fa + 1, fdv * (w * j[1]));
-                    atomicAdd(fa + 2, fdv * (w * j[2]));
+                    force_add(fa, fdv * (w * j[0]), fdv * (w * j[1]), fdv * (w * j[2]), P.fs);
                 }
             }
         }

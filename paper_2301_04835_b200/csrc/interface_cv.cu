@@ -99,7 +99,6 @@ __global__ void __launch_bounds__(256) k_dti_apply(const __grid_constant__ DtiPa
     const float* p = pos + (long long)r * D.rstride * D.ps;
     float* f = force + (long long)r * D.rstride * D.fs;
     const double dv = (double)dVdxi[r], is2 = 1.0 / (D.sigma * D.sigma);
-    const bool shared_arr = D.rstride == 0;
     const long long a0 = D.ibegin + (long long)ch * DTI_CHUNK;
     for (int i = tid; i < DTI_CHUNK; i += 256) {
         const long long a = a0 + i;
@@ -112,8 +111,9 @@ __global__ void __launch_bounds__(256) k_dti_apply(const __grid_constant__ DtiPa
         }
         // d xi / d x_i = -dI;  F_i = -dV/dxi * d xi / d x_i
         const float add = (float)(dv * dI);
-        if (shared_arr) atomicAdd(f + a * D.fs + D.axis, add);
-        else f[a * D.fs + D.axis] += add;
+        // always a reduction: block 0 adds the mobile atoms' term in this same launch and a mobile atom may lie inside the
+        // interface range (a plain += racing that atomic could lose one of the two); free next to the exp loop above
+        atomicAdd(f + a * D.fs + D.axis, add);
     }
     if (ch == 0 && tid < D.n_mobile) {   // mobile atoms: d xi / d r_m = (w_m / W) e_axis; they may coincide with interface atoms
         double W = 0.0;

@@ -65,7 +65,7 @@ struct HillConsts {
 struct MetadState {
     float4* hills;          // kernel-side records: n_cv<=3: {s0,s1,s2,log2 W}; n_cv==4: {s0..s3},{log2 W,0,0,0}
     float* heights;         // W as deposited / loaded (exported by psg_get_hills; read by the binary64 path)
-    int* n_hills;           // device counter (exact)
+    int* n_hills;           // device: [0] the exact count, [1] sticky overflow flag (a deposit was clamped at capacity)
     int capacity;
     double* part;           // [max_chunks][n_rtiles][TILE_R][1+n_cv]
     unsigned* ticket;       // [n_rtiles]
@@ -111,8 +111,13 @@ struct psg_ctx {
     // harmonic
     float* d_kspring = nullptr; float* d_centers = nullptr;
     MetadState md{};
-    long long nh_bound = 0;          // host upper bound of the hill count
+    long long nh_bound = 0;          // host UPPER bound of the hill count (+R per deposit call; exact while no mask was used)
+    long long nh_lo = 0;             // host LOWER bound (+0 for a masked call): a deposit is refused only when overflow is certain
+    bool overflow_possible = false;  // a deposit was launched that the host could not prove to fit: psg_sync_check asks the device
+    bool count_unknown = false;      // a deposit was enqueued under stream capture: replays move the device counter behind the
+                                     // host's back, so kernels read the device counter until psg_get_hills / psg_load_hills
     AbfState abf{};
+    bool abf_delta_pending = false;  // psg_abf_accumulate_delta has run, psg_abf_apply_grid_delta has not
     // host-engine staging (psg_step_host)
     float* d_pos_stage = nullptr; float* d_frc_stage = nullptr; float* d_fs_stage = nullptr;
     int sm_count = 148;
@@ -140,8 +145,14 @@ cudaError_t psg_launch_abf_estimate(psg_ctx* c, const float* d_pos, const float*
                                     const float* d_fbias_prev, float* d_fsample);
 bool psg_abf_step_supported(const psg_ctx* c);
 cudaError_t psg_launch_abf_step(psg_ctx* c, const float* d_pos, const float* d_fsample, float* d_force);   // fused ABF step
+cudaError_t psg_launch_abf_phase(psg_ctx* c, int phase, const float* d_pos, const float* d_fsample, float* d_force, int* hist,
+                                 float* fsum);   // one half of the fused ABF step (phase 1 or 2)
+cudaError_t psg_launch_abf_add_delta(psg_ctx* c, const int* d_hist_delta, const float* d_fsum_delta);
+cudaError_t psg_launch_abf_accumulate(psg_ctx* c, const float* d_xi, const float* d_fsample, int* hist, float* fsum);   // k_abf_accumulate
+cudaError_t psg_launch_abf_mean(psg_ctx* c, int* d_bin, float* d_dVdxi);                                             // k_abf_mean
 bool psg_range_step_supported(const psg_ctx* c, const float* d_pos, const float* d_force);
 cudaError_t psg_launch_range_step(psg_ctx* c, const float* d_pos, float* d_force);   // fused harmonic step over range groups
+bool psg_stream_capturing(const psg_ctx* c);
 size_t psg_hill_part_doubles(const psg_ctx* c, int* max_chunks_out, int* n_rtiles_out);
 
 #ifdef PSG_TRACE

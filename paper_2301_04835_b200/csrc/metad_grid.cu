@@ -252,9 +252,7 @@ __global__ void __launch_bounds__(256) k_grid_step(const __grid_constant__ SysPa
         const float dv = -s_dv[wid][P.grp[P.slot_gid[s]].cv];
         const int atom = P.slot_atom[(P.per_rep ? (long long)r * P.n_slots : 0) + s];
         float* f = force + ((long long)r * P.rstride + atom) * P.fs;
-        atomicAdd(f, dv * (float)j.x);
-        atomicAdd(f + 1, dv * (float)j.y);
-        atomicAdd(f + 2, dv * (float)j.z);
+        force_add(f, dv * (float)j.x, dv * (float)j.y, dv * (float)j.z, P.fs);
     }
 }
 

@@ -4,6 +4,7 @@
 #include <stdint.h>
 
 #include "hills.cuh"
+#include "psg_bench.h"
 
 #define ITERS 4096
 #define CHAINS 8
@@ -155,6 +156,45 @@ static cudaError_t time_one(int sms, double ops_per_thread_iter, double* out) {
     return e == cudaSuccess ? cudaGetLastError() : e;
 }
 
+// The launch floor: an empty kernel as a node of a replayed CUDA graph (what bounds a step that moves a few
+// MB).  64 nodes per graph, best of 5 replays; returns nodes per second.
+__global__ void k_empty() {}
+static cudaError_t time_launch_floor(double* out) {
+    cudaStream_t s;
+    cudaError_t e = cudaStreamCreateWithFlags(&s, cudaStreamNonBlocking);
+    if (e != cudaSuccess) return e;
+    cudaGraph_t g = nullptr;
+    cudaGraphExec_t ge = nullptr;
+    cudaEvent_t t0, t1;
+    cudaEventCreate(&t0);
+    cudaEventCreate(&t1);
+    const int n = 64;
+    e = cudaStreamBeginCapture(s, cudaStreamCaptureModeThreadLocal);
+    if (e == cudaSuccess) {
+        for (int i = 0; i < n; ++i) k_empty<<<1, 32, 0, s>>>();
+        e = cudaStreamEndCapture(s, &g);
+    }
+    if (e == cudaSuccess) e = cudaGraphInstantiate(&ge, g, 0);
+    double best = 0.0;
+    for (int rep = 0; rep < 6 && e == cudaSuccess; ++rep) {
+        cudaEventRecord(t0, s);
+        cudaGraphLaunch(ge, s);
+        cudaEventRecord(t1, s);
+        e = cudaEventSynchronize(t1);
+        float ms = 0.f;
+        cudaEventElapsedTime(&ms, t0, t1);
+        const double rate = n / (ms * 1e-3);
+        if (rep > 0 && rate > best) best = rate;
+    }
+    if (ge) cudaGraphExecDestroy(ge);
+    if (g) cudaGraphDestroy(g);
+    cudaEventDestroy(t0);
+    cudaEventDestroy(t1);
+    cudaStreamDestroy(s);
+    *out = best;
+    return e;
+}
+
 extern "C" int psg_measure_alu_peak(int device, int which, double* out) {
     if (!out) return PSG_EINVAL;
     if (cudaSetDevice(device) != cudaSuccess) return PSG_ECUDA;
@@ -172,6 +212,7 @@ extern "C" int psg_measure_alu_peak(int device, int which, double* out) {
     case 6: e = time_one<6>(sms, CHAINS, out); break;          // FADD2
     case 7: e = time_hill_loop<2, 3, 2>(sms, out); break;      // hill evaluations/s of the bare loop, 2-D periodic (C = 16)
     case 8: e = time_hill_loop<3, 3, 2>(sms, out); break;      // hill evaluations/s of the bare loop, 3-D, 2 periodic (C = 20)
+    case 9: e = time_launch_floor(out); break;                 // empty graph nodes/s
     default:
         if (which >= 100 && which < 200) { e = time_hill_loop<2, 3, 2>(sms, out, which - 100); break; }   // short runs: which - 100 passes
         return PSG_EINVAL;

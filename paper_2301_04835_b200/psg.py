@@ -24,7 +24,7 @@ _KIND = {"distance": CV_DISTANCE, "angle": CV_ANGLE, "dihedral": CV_DIHEDRAL, "c
 EXPORTS = ["psg_create", "psg_destroy", "psg_set_stream", "psg_last_error", "psg_set_layout", "psg_set_cvs",
            "psg_set_box", "psg_set_harmonic", "psg_set_metad", "psg_set_hill_precision", "psg_load_hills", "psg_get_hills",
            "psg_set_abf", "psg_abf_state", "psg_cv_eval", "psg_bias_eval", "psg_deposit_hill", "psg_abf_update",
-           "psg_abf_estimate", "psg_abf_estimate_reset", "psg_apply_bias_forces", "psg_step", "psg_step_outputs", "psg_step_host", "psg_sync_check",
+           "psg_abf_accumulate_delta", "psg_abf_apply_grid_delta", "psg_abf_estimate", "psg_abf_estimate_reset", "psg_apply_bias_forces", "psg_step", "psg_step_outputs", "psg_step_host", "psg_sync_check",
            "psg_interface_cv_set", "psg_interface_cv_eval", "psg_interface_cv_apply", "psg_hill_heights", "psg_append_hills", "psg_metad_grid_set",
            "psg_metad_grid_deposit", "psg_metad_grid_eval", "psg_metad_grid_step", "psg_metad_grid_state", "psg_measure_alu_peak", "psg_launch_count"]
 
@@ -79,6 +79,8 @@ def load_library():
         L.psg_bias_eval.argtypes = [vp, vp, vp, vp]
         L.psg_deposit_hill.argtypes = [vp, vp, vp]
         L.psg_abf_update.argtypes = [vp, vp, vp, vp, vp]
+        L.psg_abf_accumulate_delta.argtypes = [vp, vp, vp, vp, vp]
+        L.psg_abf_apply_grid_delta.argtypes = [vp, vp, vp, vp, vp]
         L.psg_abf_estimate.argtypes = [vp, vp, vp, vp, C.c_double, vp, vp]
         L.psg_abf_estimate_reset.argtypes = [vp]
         L.psg_apply_bias_forces.argtypes = [vp, vp, vp, vp]
@@ -145,6 +147,7 @@ class Context:
         rc = self._L.psg_create(C.byref(self._h), device, C.c_void_p(stream))
         if rc != 0:
             raise PsgError(rc, self._L.psg_last_error(None).decode())
+        self.stream_handle = int(stream or 0)      # the cudaStream_t the ctx enqueues on (multiwalker orders collectives against it)
         self.R = self.n_cv = self.n_slots = 0
 
     def _ck(self, rc):
@@ -167,6 +170,7 @@ class Context:
         if hasattr(stream, "cuda_stream"):
             stream = stream.cuda_stream
         self._ck(self._L.psg_set_stream(self._h, C.c_void_p(stream)))
+        self.stream_handle = int(stream or 0)
 
     def set_layout(self, n_replicas, n_atoms, replica_stride_atoms, pos_stride_floats=4, frc_stride_floats=4):
         self._ck(self._L.psg_set_layout(self._h, n_replicas, n_atoms, replica_stride_atoms, pos_stride_floats,
@@ -277,6 +281,19 @@ class Context:
         t = self._torch
         self._ck(self._L.psg_abf_update(self._h, _dp(d_xi, t.float32), _dp(d_fsample, t.float32), _dp(d_bin, t.int32),
                                         _dp(d_dVdxi, t.float32)))
+
+    def abf_accumulate_delta(self, d_pos, d_fsample, d_hist_delta, d_fsum_delta):
+        t = self._torch
+        self._ck(self._L.psg_abf_accumulate_delta(self._h, _dp(d_pos, t.float32), _dp(d_fsample, t.float32),
+                                                  _dp(d_hist_delta, t.int32), _dp(d_fsum_delta, t.float32)))
+
+    def abf_apply_grid_delta(self, d_hist_delta, d_fsum_delta, d_pos, d_force):
+        t = self._torch
+        self._ck(self._L.psg_abf_apply_grid_delta(self._h, _dp(d_hist_delta, t.int32), _dp(d_fsum_delta, t.float32),
+                                                  _dp(d_pos, t.float32), _dp(d_force, t.float32)))
+
+    def abf_n_bins(self):
+        return int(self.abf_state()[2])
 
     def abf_estimate(self, d_pos, d_vel, d_mass, dt, d_fbias_prev, d_fsample):
         t = self._torch

@@ -231,8 +231,7 @@ def test_hill_sum_periodic_image(torch, psg):
 def test_well_tempered_hill_store_matches_oracle(torch, psg, cfg):
     """build the whole pre-filled hill list by psg_deposit_hill in the workload's rounds (ragged last round
     through the mask) and compare centres (bit-exact) and heights with the oracle's list"""
-    w = small(cfg)
-    w.params["capacity"] += w.R          # the host-side capacity bound counts +R per call, masked or not
+    w = small(cfg)                       # capacity = exactly the number of hills: a masked (ragged) round needs no padding
     ctx = make_ctx(psg, w)
     c = w.params["hill_centers"]
     for b, e in w.hill_rounds():
@@ -567,6 +566,67 @@ def test_fused_abf_step_equals_unfused_calls(torch, psg, R, N):
     assert np.allclose(a[2], c[2], rtol=2e-6, atol=1e-6), "dV/dxi"
     assert np.allclose(a[3], c[3], rtol=1e-5, atol=1e-4), "forces"
     assert np.array_equal(a[3][..., 3].view(np.uint32), f0[..., 3].view(np.uint32))
+
+
+def test_abf_shared_grid_split_over_two_contexts(torch, psg):
+    """SURVEY 8(e), shared-grid ABF over several GPUs, on one: two contexts hold half of the replicas each, run
+    psg_abf_accumulate_delta, exchange by summing the two delta grids (what the all-reduce does), and run
+    psg_abf_apply_grid_delta; one context holds all replicas and runs psg_step.  Histograms and bins must agree bit for
+    bit (and with the oracle); force sums, mean forces and forces up to the order of the binary32 additions."""
+    from paper_2301_04835_b200.psg import _view
+    R, N, steps = 600, 90, 4
+    w = W.make(2, R=R, N=N, steps=steps)
+    h = R // 2
+    p = w.params
+    f0 = w.forces0()
+    nb = int(np.prod(p["shape"]))
+
+    def ctx_for(n):
+        c = psg.Context(0)
+        c.set_layout(n, N, N, 4, 4)
+        cvs = [{"type": psg.CV_DISTANCE, "groups": cv["groups"], "axis": 0, "period": 0.0} for cv in w.cvs]
+        c.set_cvs(cvs, w.slot_atom, None, None)
+        c.set_abf(p["lower"], p["upper"], p["shape"], p["periodic"], p["n_threshold"])
+        return c
+
+    halves, whole = [ctx_for(h), ctx_for(R - h)], ctx_for(R)
+    with pytest.raises(psg.PsgError):     # apply without a pending accumulate
+        halves[0].abf_apply_grid_delta(torch.zeros(nb, dtype=torch.int32, device="cuda"), torch.zeros(nb * 2, device="cuda"),
+                                       dev(torch, w.positions(0)[:h]), dev(torch, f0[:h]))
+    d_fw = dev(torch, f0)
+    d_fh = [dev(torch, f0[:h]), dev(torch, f0[h:])]
+    hist_ref, fsum_ref = np.zeros(nb, np.int32), np.zeros((nb, 2), np.float64)
+    for step in range(1, steps + 1):
+        pos, fs = w.positions(step % w.K), w.fsample(step % w.K)
+        whole.step(dev(torch, pos), d_fw, dev(torch, fs), step)
+        parts = [(dev(torch, pos[:h]), dev(torch, fs[:h])), (dev(torch, pos[h:]), dev(torch, fs[h:]))]
+        deltas = []
+        for c, (dp, dfs) in zip(halves, parts):
+            dh = torch.full((nb,), 77, dtype=torch.int32, device="cuda")       # the call must overwrite, not add
+            dfm = torch.full((nb * 2,), 7.0, device="cuda")
+            c.abf_accumulate_delta(dp, dfs, dh, dfm)
+            deltas.append((dh, dfm))
+        tot_h, tot_f = deltas[0][0] + deltas[1][0], deltas[0][1] + deltas[1][1]      # the all-reduce
+        for c, (dp, _), df in zip(halves, parts, d_fh):
+            c.abf_apply_grid_delta(tot_h, tot_f, dp, df)
+        for c in halves + [whole]:
+            c.sync_check()
+        xi = whole.read_step_outputs()["xi"].cpu().numpy()
+        b_ref, _ = orc.abf_update(xi, fs, p["lower"], p["upper"], p["shape"], p["periodic"], p["n_threshold"], hist_ref, fsum_ref)
+        ow = whole.read_step_outputs()
+        oh = [c.read_step_outputs() for c in halves]
+        assert np.array_equal(np.concatenate([o["bin"].cpu().numpy() for o in oh]), ow["bin"].cpu().numpy())
+        assert np.array_equal(ow["bin"].cpu().numpy(), b_ref)
+        assert np.allclose(np.concatenate([o["dVdxi"].cpu().numpy() for o in oh]), ow["dVdxi"].cpu().numpy(), rtol=2e-6, atol=1e-6)
+    grids = []
+    for c in halves + [whole]:
+        hp, fp, n = c.abf_state()
+        grids.append((_view(hp, (n,), torch.int32, 0).cpu().numpy().copy(), _view(fp, (n, 2), torch.float32, 0).cpu().numpy().copy()))
+    assert np.array_equal(grids[0][0], grids[2][0]) and np.array_equal(grids[1][0], grids[2][0]), "histogram, bit for bit"
+    assert np.array_equal(grids[2][0], hist_ref) and hist_ref.sum() > R
+    assert np.array_equal(grids[0][1].view(np.uint32), grids[1][1].view(np.uint32)), "both ranks hold the identical grid"
+    assert_close(grids[0][1], fsum_ref, "Fsum of the split update")
+    assert np.allclose(np.concatenate([d_fh[0].cpu().numpy(), d_fh[1].cpu().numpy()]), d_fw.cpu().numpy(), rtol=1e-5, atol=1e-4)
 
 
 def test_fused_abf_step_is_cuda_graph_capturable(torch, psg):
@@ -1082,22 +1142,33 @@ def test_shape_cv_metad_and_abf_steps(torch, psg):
     sigma = np.array([0.05, 0.03], np.float32)
     centers = (xi_ref[rng.integers(0, R, size=n_h)] + rng.normal(scale=0.04, size=(n_h, 2))).astype(np.float32)
     heights = rng.uniform(0.2, 1.2, size=n_h).astype(np.float32)
-    ctx = psg.Context(0)
-    ctx.set_layout(R, N, N, 4, 4)
-    ctx.set_cvs(g_cvs, slot, None, None)
-    ctx.set_metad(sigma, 1.2, 0.0, n_h + 8, 0)
-    ctx.load_hills(dev(torch, centers), dev(torch, heights))
-    d_f = dev(torch, f0)
-    ctx.step(dev(torch, pos), d_f, None, 1)
-    ctx.sync_check()
-    out = {k: v.cpu().numpy() for k, v in ctx.read_step_outputs().items()}
-    assert_close(out["xi"], xi_ref, "metad shape xi")
     V, dV, T = orc.metad(xi_ref.astype(np.float32).astype(np.float64), centers, heights, sigma, np.zeros(2))
-    assert (np.abs(out["V"] - V) <= 1e-5 * np.abs(V) + 1e-6 + 2e-7 * np.abs(heights).sum()).all()
-    assert (np.abs(out["dVdxi"] - dV) <= 1e-5 * np.abs(dV) + 1e-6 + 2e-7 * T).all()
-    f_ref = sysm.apply_forces(pos, out["dVdxi"].astype(np.float64), f0[..., :3].astype(np.float64))   # the scatter on its own
-    assert_forces_close(d_f.cpu().numpy()[..., :3], f_ref, f0[..., :3], "metad shape forces")
-    ctx.close()
+    f_ref = sysm.apply_forces(pos, dV, f0[..., :3].astype(np.float64))     # the ORACLE's gradient through the oracle's Jacobian
+    _, jac = sysm.cv_eval(pos)                                             # rows in slot order here (CV 0: 14 slots, CV 1: 20)
+    slot_cv = np.array([0] * 14 + [1] * 20)
+    extra = np.zeros((R, N, 3))
+    for r in range(R):
+        np.add.at(extra[r], slot, 2e-7 * T[r, slot_cv][:, None] * np.abs(jac[r]))
+    for mode in (psg.HILLS_F32, psg.HILLS_F64):
+        ctx = psg.Context(0)
+        ctx.set_layout(R, N, N, 4, 4)
+        ctx.set_cvs(g_cvs, slot, None, None)
+        ctx.set_metad(sigma, 1.2, 0.0, n_h + 8, 0)
+        ctx.set_hill_precision(mode)
+        ctx.load_hills(dev(torch, centers), dev(torch, heights))
+        d_f = dev(torch, f0)
+        ctx.step(dev(torch, pos), d_f, None, 1)
+        ctx.sync_check()
+        out = {k: v.cpu().numpy() for k, v in ctx.read_step_outputs().items()}
+        assert_close(out["xi"], xi_ref, "metad shape xi")
+        assert_close(out["V"], V, "metad shape V")
+        if mode == psg.HILLS_F64:      # binary64 terms: the literal rule, and forces with the binary32 += rounding only
+            assert_close(out["dVdxi"], dV, "metad shape dV/dxi (binary64 terms)")
+            assert_forces_close(d_f.cpu().numpy()[..., :3], f_ref, f0[..., :3], "metad shape forces (binary64 terms)")
+        else:                          # binary32 terms: the conditioning bound of DESIGN.md "Hill sum precision"
+            assert (np.abs(out["dVdxi"] - dV) <= np.maximum(np.maximum(1e-5 * np.abs(dV), 1e-6), 2e-7 * T)).all()
+            assert_forces_close(d_f.cpu().numpy()[..., :3], f_ref, f0[..., :3], "metad shape forces", extra)
+        ctx.close()
     # -- ABF
     o_cvs = [{"type": orc.PRINCIPAL_MOMENT, "groups": groups[0], "axis": 0, "period": 0.0},
              {"type": orc.ACYLINDRICITY, "groups": groups[1], "axis": 0, "period": 0.0}]
@@ -1351,7 +1422,90 @@ def test_split_deposit_equals_single_context_deposit(torch, psg):
             assert np.array_equal(cen.view(np.uint32), lists[2][0].view(np.uint32)), f"event {event}: centres"
             assert np.array_equal(hgt.view(np.uint32), lists[2][1].view(np.uint32)), f"event {event}: heights"
     assert lists[2][1].min() < 0.999 * w0                  # well-tempered heights really varied
-    with pytest.raises(psg.PsgError):                      # capacity is checked on the host before anything is launched
-        a.append_hills(torch.zeros((cap, n), device="cuda"), torch.ones(cap, device="cuda"))
+    # (the lists are bit-identical here because every context's hill sum uses the same chunk length at <= 560 hills; in
+    # general a rank's V_old equals the single context's up to binary32 rounding -- include/psg.h, psg_append_hills)
+    # zero heights are skipped on the device, so the host cannot rule this overflow out: the kernel clamps at capacity and
+    # the next synchronising call reports it
+    n_before = a.n_hills()
+    a.append_hills(torch.zeros((cap, n), device="cuda"), torch.ones(cap, device="cuda"))
+    with pytest.raises(psg.PsgError) as ei:
+        a.sync_check()
+    assert ei.value.code == -4
+    with pytest.raises(psg.PsgError):
+        a.n_hills()
+    assert n_before < cap
     for c in ctxs:
         c.close()
+
+
+def test_masked_deposit_needs_no_capacity_padding_and_overflow_is_reported(torch, psg):
+    """capacity is exact: masked rounds fill the store to the last slot without PSG_ECAPACITY; one hill too many is dropped
+    by the kernel (never written beyond capacity) and reported by psg_sync_check; an unmasked overflow is refused on the host"""
+    w = small(1, stride=0)
+    R, cap = w.R, 2 * w.R + 5
+    ctx = make_ctx(psg, w, with_method=False)
+    ctx.set_metad(w.params["sigma"], 1.2, 0.0, cap, 0)
+    xi = dev(torch, W.random_xi(w, 3))
+    ctx.deposit_hill(xi)
+    ctx.deposit_hill(xi)
+    mask = np.zeros(R, np.uint8); mask[:5] = 1
+    ctx.deposit_hill(xi, dev(torch, mask))            # exactly full now
+    ctx.sync_check()
+    assert ctx.n_hills() == cap
+    V = torch.empty(R, device="cuda"); dV = torch.empty((R, 2), device="cuda")
+    ctx.bias_eval(xi, V, dV); ctx.sync_check()
+    V_full = V.cpu().numpy().copy()
+    with pytest.raises(psg.PsgError) as ei:            # unmasked: the host knows the count exactly -> refused, nothing launched
+        ctx.deposit_hill(xi)
+    assert ei.value.code == -4
+    one = np.zeros(R, np.uint8); one[7] = 1
+    ctx.deposit_hill(xi, dev(torch, one))              # masked: launched, clamped on the device
+    with pytest.raises(psg.PsgError) as ei:
+        ctx.sync_check()
+    assert ei.value.code == -4
+    ctx.bias_eval(xi, V, dV)
+    torch.cuda.synchronize()
+    assert np.array_equal(V.cpu().numpy(), V_full), "a clamped deposit must not change the stored list"
+    ctx.close()
+
+
+def test_graph_captured_deposit_step_replays_and_later_launches_see_the_new_hills(torch, psg):
+    """a deposit-phase psg_step captured in a CUDA graph appends R hills per REPLAY; launches issued outside the
+    capture afterwards must sum over all of them (the ctx switches to the device counter until psg_get_hills)"""
+    w = small(1, stride=5)
+    R = w.R
+    s = torch.cuda.Stream()
+    ctx = psg.Context(0, s)
+    psg.configure_from_workload(ctx, w, with_method=False)
+    ctx.set_metad(w.params["sigma"], 1.2, w.params["kB_deltaT"], 10 * R, 5)
+    ref = make_ctx(psg, w, with_method=False)
+    ref.set_metad(w.params["sigma"], 1.2, w.params["kB_deltaT"], 10 * R, 5)
+    d_pos = dev(torch, w.positions(0))
+    d_f, d_fr = dev(torch, w.forces0()), dev(torch, w.forces0())
+    torch.cuda.synchronize()
+    g = torch.cuda.CUDAGraph()
+    with torch.cuda.graph(g, stream=s):
+        ctx.step(d_pos, d_f, None, 5)                 # a deposit step
+    d_f.copy_(d_fr)
+    torch.cuda.synchronize()
+    for _ in range(3):
+        g.replay()
+    torch.cuda.synchronize()
+    for _ in range(3):
+        ref.step(d_pos, d_fr, None, 5)
+    ref.sync_check()
+    xi = dev(torch, W.random_xi(w, 9))
+    out = []
+    for c in (ctx, ref):
+        V = torch.empty(R, device="cuda"); dV = torch.empty((R, 2), device="cuda")
+        if c is ctx:
+            with torch.cuda.stream(s):
+                c.bias_eval(xi, V, dV)                # NOT captured: must still see the 3 R hills of the replays
+        else:
+            c.bias_eval(xi, V, dV)
+        torch.cuda.synchronize()
+        out.append((V.cpu().numpy(), dV.cpu().numpy()))
+    assert np.array_equal(out[0][0], out[1][0]) and np.array_equal(out[0][1], out[1][1])
+    assert ctx.n_hills() == ref.n_hills() == 3 * R
+    assert np.allclose(d_f.cpu().numpy(), d_fr.cpu().numpy(), rtol=1e-5, atol=1e-4)
+    ctx.close(); ref.close()

@@ -118,3 +118,57 @@ def test_multiwalker_deposit_single_process():
     xi = torch.ones((4, 2))
     assert deposit_hill_all_ranks(c, xi) == 4
     assert torch.equal(c.got[0], xi) and torch.equal(c.got[1], torch.full((4,), 1.5))
+
+
+_ABF_WORKER = r"""
+import os, sys, json
+sys.path.insert(0, {root!r})
+import torch, torch.distributed as dist
+from paper_2301_04835_b200.multiwalker import abf_step_all_ranks
+rank, world = int(os.environ["RANK"]), int(os.environ["WORLD_SIZE"])
+dist.init_process_group("gloo")
+
+class FakeCtx:                       # stands in for psg.Context on CPU tensors: a 6-bin grid, one CV
+    n_cv = 1
+    def __init__(self): self.hist = torch.zeros(6, dtype=torch.int32); self.fsum = torch.zeros(6); self.calls = []
+    def abf_n_bins(self): return 6
+    def abf_accumulate_delta(self, pos, fs, dh, df):
+        dh.zero_(); df.zero_()
+        for b, f in zip(pos.tolist(), fs.tolist()):      # "positions" are the bins here
+            dh[int(b)] += 1; df[int(b)] += f
+        self.calls.append("acc")
+    def abf_apply_grid_delta(self, dh, df, pos, force):
+        self.hist += dh; self.fsum += df
+        force += self.fsum[pos.long()] / self.hist[pos.long()].clamp(min=1)
+        self.calls.append("apply")
+
+ctx = FakeCtx()
+pos = torch.tensor([0.0, 2.0, 2.0]) if rank == 0 else torch.tensor([2.0, 5.0, 0.0])
+fs = torch.tensor([1.0, 2.0, 3.0]) * (rank + 1)
+force = torch.zeros(3)
+for _ in range(2):
+    abf_step_all_ranks(ctx, pos, force, fs)
+out = dict(rank=rank, hist=ctx.hist.tolist(), fsum=ctx.fsum.tolist(), force=force.tolist(), calls=ctx.calls)
+gathered = [None] * world
+dist.all_gather_object(gathered, out)
+if rank == 0:
+    print(json.dumps(gathered))
+dist.destroy_process_group()
+"""
+
+
+def test_multiwalker_abf_all_reduces_the_grid_deltas_gloo(tmp_path):
+    """abf_step_all_ranks: both ranks end with the grid ONE context holding all six replicas would build --
+    the all-reduce sums the per-step histogram / force-sum contributions before anyone reads a mean force"""
+    script = tmp_path / "abf_worker.py"
+    script.write_text(_ABF_WORKER.format(root=ROOT))
+    p = _torchrun([str(script)])
+    assert p.returncode == 0, p.stderr[-2000:]
+    line = [l for l in p.stdout.splitlines() if l.startswith("[")]
+    assert len(line) == 1
+    r0, r1 = json.loads(line[0])
+    assert r0["hist"] == r1["hist"] == [4, 0, 6, 0, 0, 2]                  # two steps of {0: 2, 2: 3, 5: 1}
+    assert r0["fsum"] == r1["fsum"] == [2 * (1.0 + 6.0), 0.0, 2 * (2.0 + 3.0 + 2.0), 0.0, 0.0, 2 * 4.0]
+    assert r0["calls"] == ["acc", "apply", "acc", "apply"]
+    # step 1 means: bin 0 -> 7/2, bin 2 -> 7/3, bin 5 -> 4; step 2: 14/4, 14/6, 8/2: the same numbers
+    assert r0["force"] == pytest.approx([7.0, 14 / 3, 14 / 3]) and r1["force"] == pytest.approx([14 / 3, 8.0, 7.0])
