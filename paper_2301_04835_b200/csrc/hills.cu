@@ -105,12 +105,12 @@ __global__ void k_null_hills(int begin, int end, int rec, float4* __restrict__ h
 #ifdef PSG_TRACE
 static long long* g_trace = nullptr;
 long long* psg_trace_buffer() {
-    if (!g_trace) { cudaMalloc(&g_trace, 4096 * 8 * sizeof(long long)); cudaMemset(g_trace, 0, 4096 * 8 * sizeof(long long)); }
+    if (!g_trace) { cudaMalloc(&g_trace, 4096 * 16 * sizeof(long long)); cudaMemset(g_trace, 0, 4096 * 16 * sizeof(long long)); }
     return g_trace;
 }
-extern "C" int psg_debug_trace_clear() { return (int)cudaMemset(psg_trace_buffer(), 0, 4096 * 8 * sizeof(long long)); }
+extern "C" int psg_debug_trace_clear() { return (int)cudaMemset(psg_trace_buffer(), 0, 4096 * 16 * sizeof(long long)); }
 extern "C" int psg_debug_trace(long long* host_out, int n_ctas) {
-    return (int)cudaMemcpy(host_out, psg_trace_buffer(), (size_t)n_ctas * 8 * sizeof(long long), cudaMemcpyDeviceToHost);
+    return (int)cudaMemcpy(host_out, psg_trace_buffer(), (size_t)n_ctas * 16 * sizeof(long long), cudaMemcpyDeviceToHost);
 }
 #endif
 bool psg_stream_capturing(const psg_ctx* c) {
@@ -132,9 +132,9 @@ size_t psg_hill_part_doubles(const psg_ctx* c, int* max_chunks_out, int* n_rtile
 static cudaError_t launch_hills(psg_ctx* c, HillKernelArgs& A) {
     const int n_cv = c->sys.n_cv;
     const bool fused = A.fused != 0;
-    // stages: up to 3, as many as fit the SM's 227 KB (1 KB reserved per CTA) beside the binary64 accumulators
-    int stages = 3;
-    for (; stages > 1; --stages)
+    // stages of 32 KB: as many as fit the SM's 227 KB (1 KB reserved per CTA), at most 6 (the binary64 accumulators are registers)
+    int stages = PSG_HILL_MAX_STAGES;
+    for (; stages > 3; --stages)
         if (hills_smem_bytes(n_cv, stages, c->sys.n_groups, fused) + 1024 <= 227 * 1024) break;
     A.stages = stages;
     const size_t smem = hills_smem_bytes(n_cv, stages, c->sys.n_groups, fused);

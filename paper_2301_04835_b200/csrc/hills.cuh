@@ -14,9 +14,11 @@
 //     per periodic dim  d = xi - s; t = d/P + M; k = t - M; d -= k P_hi; d -= k P_lo   (5)
 //     exponent          q = d0^2 (+ d1^2 ...);  x = log2(W) - c q                        (NCV + 1 if the sigmas agree)
 //     MUFU.EX2 (one per replica), V += e, g_k += e d_k                                   (1 + NCV)
-// Binary32 partial sums are flushed into binary64 accumulators (shared memory, thread-private slots) after every
-// sub-tile (<= 32 hills per lane); lanes, then chunks, are combined in binary64 in FIXED order (the last CTA of
-// a tile, found with a ticket counter, sums the chunk partials), so results are bitwise reproducible.
+// Binary32 partial sums (<= 64 hills per lane) are flushed into binary64 by a warp-wide transpose-reduction (31 shuffle +
+// add steps turn 32 per-lane values into one warp total per lane): the binary64 accumulators are ONE register per lane, not
+// shared memory, which leaves the SM's shared memory to the hill stages (up to 6 x 32 KB in flight).  Lanes (butterfly),
+// warps, then chunks are combined in binary64 in FIXED order (the last CTA of a tile, found with a ticket counter, sums the
+// chunk partials), so results are bitwise reproducible.
 // FUSED: the CTA first evaluates the CVs (and Jacobians, kept in shared memory) of its tile from the engine's
 // positions; the last CTA of the tile scatters -dV/dxi * J into the engine's forces: one launch per MD step.
 #pragma once
@@ -24,6 +26,7 @@
 
 #define RT PSG_HILL_RT
 #define HWARPS PSG_HILL_WARPS
+#define HHALF PSG_HILL_HALF
 #define TILE_R PSG_HILL_TILE_R
 #define SUB PSG_HILL_SUB
 #ifndef PSG_FLUSH_EVERY
@@ -59,6 +62,21 @@ __device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
         "}" ::"r"(smem_u32(bar)),
         "r"(parity)
         : "memory");
+}
+
+// non-blocking poll (acquire): true if the phase with this parity has completed
+__device__ __forceinline__ bool mbar_test(uint64_t* bar, uint32_t parity) {
+    uint32_t ok;
+    asm volatile(
+        "{\n"
+        ".reg .pred P1;\n"
+        "mbarrier.test_wait.parity.shared::cta.b64 P1, [%1], %2;\n"
+        "selp.u32 %0, 1, 0, P1;\n"
+        "}"
+        : "=r"(ok)
+        : "r"(smem_u32(bar)), "r"(parity)
+        : "memory");
+    return ok != 0;
 }
 
 // ---------------------------------------------------------------- packed binary32 (two replicas per instruction)
@@ -175,12 +193,64 @@ __device__ __forceinline__ void accumulate_f32(const float4* __restrict__ sm, in
     if (off + 64 * n_full < n_sub) body(sm, off + 64 * n_full, X, a32);
 }
 
+#ifndef PSG_ACC_IN_REGS
+#define PSG_ACC_IN_REGS(NCV) ((NCV) >= 3)
+#endif
+#ifndef PSG_PEND_VARS
+#define PSG_PEND_VARS(NCV) ((NCV) >= 3)
+#endif
+// Warp-wide transpose-reduction of the thread's binary32 partial sums into binary64: value i = (2 p + h) NV + v of the
+// thread's RT replicas (padded with zeros to 32 per pass); after the steps xor 16, 8, 4, 2, 1 lane l holds the sum over the
+// warp's 32 lanes of value 32 pass + l, which it adds to its own slot of the warp's binary64 accumulators wacc[32 pass + l] (shared
+// memory; a register would be taken from the hill loop, which needs all 128).  Every addition is binary64, in an order fixed
+// by the lane numbers.  a32 is cleared.
+template <int NCV>
+__device__ __forceinline__ void butterfly_flush(u64 (&a32)[RT / 2][1 + NCV], double (&accd)[(RT * (1 + NCV) + 31) / 32],
+                                                double* __restrict__ wacc, int lane) {
+    constexpr int NV = 1 + NCV, NVAL = RT * NV, PASSES = (NVAL + 31) / 32;
+    float f[32 * PASSES];
+#pragma unroll
+    for (int i = 0; i < 32 * PASSES; ++i) f[i] = 0.f;
+#pragma unroll
+    for (int p = 0; p < RT / 2; ++p)
+#pragma unroll
+        for (int v = 0; v < NV; ++v) {
+            upk(a32[p][v], f[(2 * p) * NV + v], f[(2 * p + 1) * NV + v]);
+            a32[p][v] = 0ull;
+        }
+#pragma unroll
+    for (int ps = 0; ps < PASSES; ++ps) {
+        double w[16];
+        const bool up16 = (lane & 16) != 0;
+#pragma unroll
+        for (int i = 0; i < 16; ++i) {
+            // the first step exchanges binary32 (one shuffle) and converts after: the sum itself is binary64
+            const float a = f[32 * ps + i], b = f[32 * ps + i + 16];
+            const float keep = up16 ? b : a, send = up16 ? a : b;
+            w[i] = (double)keep + (double)__shfl_xor_sync(0xffffffffu, send, 16);
+        }
+#pragma unroll
+        for (int m = 8; m >= 1; m >>= 1) {
+            const bool up = (lane & m) != 0;
+#pragma unroll
+            for (int i = 0; i < m; ++i) {
+                const double keep = up ? w[i + m] : w[i], send = up ? w[i] : w[i + m];
+                w[i] = keep + __shfl_xor_sync(0xffffffffu, send, m);
+            }
+        }
+        // the lane's running total: a register where the hill loop can spare one (measured per NCV: the loop's schedule is
+        // sensitive to a single register at the 128-register limit), else its own slot of the warp's shared-memory accumulators
+        if (PSG_ACC_IN_REGS(NCV)) accd[ps] += w[0];
+        else wacc[32 * ps + lane] += w[0];
+    }
+}
+
 // binary64 terms (PSG_HILLS_F64): the definition, evaluated in double on the FP64 pipe; heights read from the
-// exported height array (global). Accumulates straight into the thread's binary64 slots.
+// exported height array (global).  Two replicas at a time over the sub-tile; their sums are reduced over the warp by
+// shuffles (binary64, fixed order) and lane 0 adds them to the warp's accumulators wacc[RT * NV] in shared memory.
 template <int NCV>
 __device__ __forceinline__ void accumulate_f64(const float4* __restrict__ sm, const float* __restrict__ W, int n_sub, int off,
-                                               const float (&xi)[RT][NCV], const HillConsts& hc, double* __restrict__ acc,
-                                               int acc_stride) {
+                                               const float (&xi)[RT][NCV], const HillConsts& hc, double* __restrict__ wacc, int lane) {
     constexpr int NV = 1 + NCV;
     for (int j0 = 0; j0 < RT; j0 += 2) {
         double a[2][NV];
@@ -211,8 +281,12 @@ __device__ __forceinline__ void accumulate_f64(const float4* __restrict__ sm, co
 #pragma unroll
         for (int jj = 0; jj < 2; ++jj)
 #pragma unroll
-            for (int v = 0; v < NV; ++v) acc[((j0 + jj) * NV + v) * acc_stride] += a[jj][v];
+            for (int v = 0; v < NV; ++v) {
+                const double t = warp_sum(a[jj][v]);
+                if (lane == 0) wacc[(j0 + jj) * NV + v] += t;
+            }
     }
+    __syncwarp();
 }
 
 // lane-local CV of (replica r, CV k) for systems with explicit groups only; dc[g] = d xi / d c_g / W_g.
@@ -309,22 +383,27 @@ struct HillKernelArgs {
 #endif
 };
 #ifdef PSG_TRACE
-#define PSG_STAMP(i) do { if (threadIdx.x == 0 && item == (int)blockIdx.x && A.trace) { long long t_; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t_)); A.trace[blockIdx.x * 8 + (i)] = t_; } } while (0)
+#define PSG_TS 16
+#define PSG_STAMP(i) do { if (threadIdx.x == 0 && item == (int)blockIdx.x && A.trace) { long long t_; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t_)); A.trace[blockIdx.x * PSG_TS + (i)] = t_; } } while (0)
+#define PSG_STAMP_T(tidx, i) do { if (threadIdx.x == (tidx) && item == (int)blockIdx.x && A.trace) { long long t_; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t_)); A.trace[blockIdx.x * PSG_TS + (i)] = t_; } } while (0)
 #else
 #define PSG_STAMP(i) do { } while (0)
+#define PSG_STAMP_T(tidx, i) do { } while (0)
 #endif
 
+__host__ __device__ inline size_t hills_wacc_doubles(int n_cv) { return (size_t)((RT * (1 + n_cv) + 31) / 32) * 32; }
 __host__ __device__ inline size_t hills_smem_bytes(int n_cv, int stages, int n_groups, bool fused) {
-    int rec = n_cv <= 3 ? 1 : 2;
-    (void)rec;
     size_t b = (size_t)stages * SUB * 16;                          // hill stages (SUB / rec hills each)
-    b += (size_t)RT * (1 + n_cv) * HWARPS * 32 * 8;                // binary64 accumulators [RT*NV][256]
+    b += (size_t)HWARPS * hills_wacc_doubles(n_cv) * 8;            // per-warp binary64 totals
     b += (size_t)3 * TILE_R * (1 + n_cv) * 8;                      // s_out, s_half[2]
     b += (size_t)TILE_R * n_cv * 4;                                // s_xi
     b += fused ? (size_t)TILE_R * n_groups * 3 * 4 : 0;            // s_jv
     b += 8 * 8 + 64;                                               // barriers, pad
     return b;
 }
+#ifndef PSG_HILL_MAX_STAGES
+#define PSG_HILL_MAX_STAGES 6
+#endif
 
 // One kernel for psg_bias_eval and the whole metadynamics step (A.fused).
 template <int NCV, int PM, int NEQ, bool F64>
@@ -335,11 +414,13 @@ __global__ void __launch_bounds__(HWARPS * 32, 1) k_hills(const __grid_constant_
     constexpr int NV = 1 + NCV;
     constexpr int NT = HWARPS * 32;
     extern __shared__ __align__(128) unsigned char smem_raw[];
+    constexpr int WACC = ((RT * NV + 31) / 32) * 32;   // per-warp binary64 totals (padded to whole butterfly passes)
+    constexpr int PASSES = WACC / 32;
     const int STG = A.stages;
     float4* stage = reinterpret_cast<float4*>(smem_raw);                          // STG * SUBH * REC float4
-    double* s_acc = reinterpret_cast<double*>(stage + STG * SUBH * REC);           // [RT*NV][NT]
-    double* s_out = s_acc + RT * NV * NT;                                         // [TILE_R][NV]
-    double* s_half = s_out + TILE_R * NV;                                         // [2][TILE_R][NV]: per-half / per-part sums
+    double* s_wacc = reinterpret_cast<double*>(stage + STG * SUBH * REC);          // [HWARPS][WACC]
+    double* s_out = s_wacc + HWARPS * WACC;                                       // [TILE_R][NV]
+    double* s_half = s_out + TILE_R * NV;                                         // [2][TILE_R][NV]: per-part sums of the last CTA
     uint64_t* full = reinterpret_cast<uint64_t*>(s_half + 2 * TILE_R * NV);       // 8 barriers
     float* s_xi = reinterpret_cast<float*>(full + 8);                             // [NCV][TILE_R] (pairs of replicas adjacent)
     float* s_jv = s_xi + TILE_R * NCV;                                            // fused: [TILE_R][n_groups][3]
@@ -347,7 +428,7 @@ __global__ void __launch_bounds__(HWARPS * 32, 1) k_hills(const __grid_constant_
     __shared__ int s_cnt[8];   // warps that have left a stage
 
     const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
-    const int half = wid >> 3, w8 = wid & 7;   // warps w8 and w8 + 8 own the same replicas; half picks the hills
+    const int half = wid / HHALF, w8 = wid % HHALF;   // warps w8 and w8 + HHALF own the same replicas; half picks the hills
     const int R = A.R;
     const int n_rt = (R + TILE_R - 1) / TILE_R;
     const int n_h = A.n_h_host >= 0 ? A.n_h_host : *A.n_hills;
@@ -388,9 +469,7 @@ __global__ void __launch_bounds__(HWARPS * 32, 1) k_hills(const __grid_constant_
                 tma_load_1d(stage + s * SUBH * REC, A.hills + (size_t)(h0 + t * SUBH) * REC, (uint32_t)cnt * REC * 16u, &full[s]);
             }
         }
-        // binary64 accumulators of this item
-#pragma unroll
-        for (int i = 0; i < RT * NV; ++i) s_acc[i * NT + tid] = 0.0;
+        PSG_STAMP(8);
         // CV values (and per-group Jacobian vectors) of this tile's replicas; overlaps the first TMA loads
         if (A.fused) {
             // the value (gather, cross products, atan2) and the Jacobian (gather, cross products, divisions) of one CV are
@@ -407,6 +486,7 @@ __global__ void __launch_bounds__(HWARPS * 32, 1) k_hills(const __grid_constant_
                         if (chunk == 0 && A.xi_out) A.xi_out[(long long)r * NCV + k] = v;
                     }
                     s_xi[k * TILE_R + rr] = v;
+                    PSG_STAMP(10);
                 } else if (r < R) {
                     D3 dc[4];
                     if (chunk == 0) prefetch_force_lines(P, r, k, A.force);
@@ -418,6 +498,7 @@ __global__ void __launch_bounds__(HWARPS * 32, 1) k_hills(const __grid_constant_
                             float* j = s_jv + (rr * P.n_groups + C.gid0 + g) * 3;
                             j[0] = (float)dc[g].x; j[1] = (float)dc[g].y; j[2] = (float)dc[g].z;
                         }
+                    PSG_STAMP_T(TILE_R * NCV, 11);
                 }
             }
         } else {
@@ -429,8 +510,41 @@ __global__ void __launch_bounds__(HWARPS * 32, 1) k_hills(const __grid_constant_
         __syncthreads();
         PSG_STAMP(1);
         const bool warp_active = r0 + w8 * RT < R;
+        // Stage hand-back without a CTA-wide barrier (measured: the bare loop reaches 0.95 of the FFMA peak, the loop with a
+        // barrier per 1,024 hills 0.80): warps drift freely; lane 0 counts its warp out of the stage with a shared-memory
+        // atomic, and the warp that left LAST refills it.  The atomic's result is only looked at one sub-tile LATER, so
+        // nobody waits for its round trip (STG >= 3 keeps the refill two sub-tiles ahead of its use); likewise the barrier
+        // of the NEXT stage is polled (test_wait) before the bookkeeping, and the blocking wait is skipped when it was ready.
+        // (whether the previous sub-tile's stage and index are kept in registers or re-derived from seq and t changes the
+        // register allocation of the hill loop, hence PSG_PEND_VARS, chosen per NCV like PSG_ACC_IN_REGS)
+        int pend_old = -1;      // lane 0: the count-out of the previous sub-tile (stage (seq - 1) % STG, sub-tile t - 1)
+        int pend_s = 0, pend_t = 0;
+        bool ready = false;
+        auto hand_back = [&](int s, int t) {
+            if (lane == 0) {
+                if (pend_old == HWARPS - 1) {
+                    const int ps = PSG_PEND_VARS(NCV) ? pend_s : (int)((seq + STG - 1) % STG), pt = PSG_PEND_VARS(NCV) ? pend_t : t - 1;
+                    s_cnt[ps] = 0;
+                    if (pt + STG < n_st) {
+                        const int cn = min(SUBH, len - (pt + STG) * SUBH);
+                        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+                        mbar_expect_tx(&full[ps], (uint32_t)cn * REC * 16u);
+                        tma_load_1d(stage + ps * SUBH * REC, A.hills + (size_t)(h0 + (pt + STG) * SUBH) * REC, (uint32_t)cn * REC * 16u,
+                                    &full[ps]);
+                    }
+                }
+                pend_old = atomicAdd(&s_cnt[s], 1);
+                if (PSG_PEND_VARS(NCV)) { pend_s = s; pend_t = t; }
+            }
+        };
         if (!F64) {
             u64 X[RT / 2][NCV], a32[RT / 2][NV];
+            double accd[PASSES];
+#pragma unroll
+            for (int ps = 0; ps < PASSES; ++ps) {
+                accd[ps] = 0.0;
+                s_wacc[wid * WACC + 32 * ps + lane] = 0.0;
+            }
 #pragma unroll
             for (int p = 0; p < RT / 2; ++p) {
 #pragma unroll
@@ -440,43 +554,33 @@ __global__ void __launch_bounds__(HWARPS * 32, 1) k_hills(const __grid_constant_
                 for (int v = 0; v < NV; ++v) a32[p][v] = 0ull;
             }
             for (int t = 0; t < n_st; ++t) {
-                int s = seq % STG;
-                mbar_wait(&full[s], (seq / STG) & 1);
-                int cnt = min(SUBH, len - t * SUBH);
+                const int s = seq % STG;
+                if (!ready) mbar_wait(&full[s], (seq / STG) & 1);
+                if (t == 0) PSG_STAMP(12);
+                const int cnt = min(SUBH, len - t * SUBH);
                 if (warp_active) {
                     // a full sub-tile gets a compile-time trip count (the compiler then schedules across iterations)
                     if (cnt == SUBH) accumulate_f32<NCV, PM, NEQ>(stage + s * SUBH * REC, SUBH, lane + 32 * half, X, hc, a32);
                     else accumulate_f32<NCV, PM, NEQ>(stage + s * SUBH * REC, cnt, lane + 32 * half, X, hc, a32);
                 }
-                if (warp_active && ((t % PSG_FLUSH_EVERY) == PSG_FLUSH_EVERY - 1 || t == n_st - 1)) {
-                    // flush the binary32 partial sums (<= 64 hills per lane: 4 sub-tiles of 16) into the binary64 slots
-#pragma unroll
-                    for (int p = 0; p < RT / 2; ++p)
-#pragma unroll
-                        for (int v = 0; v < NV; ++v) {
-                            float lo, hi;
-                            upk(a32[p][v], lo, hi);
-                            s_acc[((2 * p) * NV + v) * NT + tid] += (double)lo;
-                            s_acc[((2 * p + 1) * NV + v) * NT + tid] += (double)hi;
-                            a32[p][v] = 0ull;
-                        }
-                }
-                // No CTA-wide barrier per sub-tile (measured: the bare loop reaches 0.95 of the FFMA peak, the loop with a
-                // barrier per 1,024 hills 0.80): warps drift freely, and the warp that leaves a stage LAST refills it.
+#ifndef PSG_NO_EARLY_POLL
+                ready = t + 1 < n_st && mbar_test(&full[(seq + 1) % STG], ((seq + 1) / STG) & 1);
+#endif
+                // flush the binary32 partial sums (<= 64 hills per lane) into the lanes' binary64 registers; the four warps
+                // of a scheduler (wid mod 4) flush at different sub-tiles, so that the FMA pipe keeps work while one reduces
+#ifdef PSG_NO_STAGGER
+                const int ph = 0;
+#else
+                const int ph = (wid >> 2) % PSG_FLUSH_EVERY;
+#endif
+                if (warp_active && (((t + ph) % PSG_FLUSH_EVERY) == PSG_FLUSH_EVERY - 1 || t == n_st - 1)) butterfly_flush<NCV>(a32, accd, s_wacc + wid * WACC, lane);
                 __syncwarp();
-                if (lane == 0) {
-                    if (atomicAdd(&s_cnt[s], 1) == HWARPS - 1) {
-                        s_cnt[s] = 0;
-                        if (t + STG < n_st) {
-                            int cn = min(SUBH, len - (t + STG) * SUBH);
-                            asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
-                            mbar_expect_tx(&full[s], (uint32_t)cn * REC * 16u);
-                            tma_load_1d(stage + s * SUBH * REC, A.hills + (size_t)(h0 + (t + STG) * SUBH) * REC,
-                                        (uint32_t)cn * REC * 16u, &full[s]);
-                        }
-                    }
-                }
+                hand_back(s, t);
                 ++seq;
+            }
+            if (PSG_ACC_IN_REGS(NCV)) {
+#pragma unroll
+                for (int ps = 0; ps < PASSES; ++ps) s_wacc[wid * WACC + 32 * ps + lane] = accd[ps];
             }
         } else {
             float xi[RT][NCV];
@@ -484,44 +588,30 @@ __global__ void __launch_bounds__(HWARPS * 32, 1) k_hills(const __grid_constant_
             for (int j = 0; j < RT; ++j)
 #pragma unroll
                 for (int k = 0; k < NCV; ++k) xi[j][k] = s_xi[k * TILE_R + w8 * RT + j];
+#pragma unroll
+            for (int ps = 0; ps < PASSES; ++ps) s_wacc[wid * WACC + 32 * ps + lane] = 0.0;
+            __syncwarp();
             for (int t = 0; t < n_st; ++t) {
-                int s = seq % STG;
+                const int s = seq % STG;
                 mbar_wait(&full[s], (seq / STG) & 1);
-                int cnt = min(SUBH, len - t * SUBH);
+                const int cnt = min(SUBH, len - t * SUBH);
                 if (warp_active)
-                    accumulate_f64<NCV>(stage + s * SUBH * REC, A.heights + h0 + t * SUBH, cnt, lane + 32 * half, xi, hc, s_acc + tid, NT);
+                    accumulate_f64<NCV>(stage + s * SUBH * REC, A.heights + h0 + t * SUBH, cnt, lane + 32 * half, xi, hc, s_wacc + wid * WACC, lane);
                 __syncwarp();
-                if (lane == 0) {
-                    if (atomicAdd(&s_cnt[s], 1) == HWARPS - 1) {
-                        s_cnt[s] = 0;
-                        if (t + STG < n_st) {
-                            int cn = min(SUBH, len - (t + STG) * SUBH);
-                            asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
-                            mbar_expect_tx(&full[s], (uint32_t)cn * REC * 16u);
-                            tma_load_1d(stage + s * SUBH * REC, A.hills + (size_t)(h0 + (t + STG) * SUBH) * REC,
-                                        (uint32_t)cn * REC * 16u, &full[s]);
-                        }
-                    }
-                }
+                hand_back(s, t);
                 ++seq;
             }
         }
+        if (lane == 0 && pend_old == HWARPS - 1) s_cnt[PSG_PEND_VARS(NCV) ? pend_s : (int)((seq + STG - 1) % STG)] = 0;   // the item's last count-out (nothing left to refill)
         PSG_STAMP(2);
-        // lanes -> warp totals through the shared accumulators: lane v (< RT*NV) sums value v over the 32 lanes
-        // (rotated start => no bank conflicts; the order is fixed per lane => deterministic)
-        __syncwarp();
         constexpr int TV = TILE_R * NV;
-        double* dst = s_half + half * TV + w8 * RT * NV;
-        for (int v = lane; v < RT * NV; v += 32) {
-            const double* src = s_acc + v * NT + wid * 32;
-            double sum = 0.0;
-#pragma unroll 8
-            for (int i = 0; i < 32; ++i) sum += src[(i + lane) & 31];
-            dst[v] = sum;
-        }
         __syncthreads();
-        // the two warp halves in fixed order -> this chunk's partial of the tile
-        for (int t = tid; t < TV; t += NT) A.part[(size_t)(chunk * n_rt + tile) * TV + t] = s_half[t] + s_half[TV + t];
+        PSG_STAMP(14);
+        // warps w8 and w8 + HHALF (the two halves of the chunk's hills) in fixed order -> this chunk's partial of the tile
+        for (int t = tid; t < TV; t += NT) {
+            const int rr = t / NV, v = t - rr * NV, ww = rr / RT, j = rr - ww * RT;
+            A.part[(size_t)(chunk * n_rt + tile) * TV + t] = s_wacc[ww * WACC + j * NV + v] + s_wacc[(ww + HHALF) * WACC + j * NV + v];
+        }
         __syncthreads();
         PSG_STAMP(3);
         if (tid == 0) {
@@ -587,7 +677,7 @@ __global__ void __launch_bounds__(HWARPS * 32, 1) k_hills(const __grid_constant_
 #ifdef PSG_TRACE
         if (threadIdx.x == 0 && item == (int)blockIdx.x && A.trace) {
             unsigned smid; asm volatile("mov.u32 %0, %%smid;" : "=r"(smid));
-            A.trace[blockIdx.x * 8 + 7] = smid;
+            A.trace[blockIdx.x * PSG_TS + 7] = smid;
         }
 #endif
     }

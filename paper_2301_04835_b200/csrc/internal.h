@@ -13,8 +13,11 @@
 #define PSG_RANGE_TILE 2048      // atoms per block / slice in the range-moment, dense-apply and fused range-step kernels
 #define PSG_RANGE_THREADS 256    // threads that reduce one slice's moments (k_range_moments block = A group of k_range_step: same thread -> atom map, same bits)
 #define PSG_HILL_RT 8            // replicas per thread in the hill sum
-#define PSG_HILL_WARPS 16        // warps per CTA in the hill sum: two halves of 8 warps share the tile's replicas and split its hills
-#define PSG_HILL_TILE_R (PSG_HILL_RT * 8)   // replicas per CTA tile (64): warp w and warp w + 8 own the same 8 replicas
+#ifndef PSG_HILL_WARPS
+#define PSG_HILL_WARPS 16        // warps per CTA in the hill sum: two halves share the tile's replicas and split its hills
+#endif
+#define PSG_HILL_HALF (PSG_HILL_WARPS / 2)
+#define PSG_HILL_TILE_R (PSG_HILL_RT * PSG_HILL_HALF)   // replicas per CTA tile (64): warp w and warp w + HALF own the same 8 replicas
 #define PSG_HILL_SUB 2048        // hills per shared-memory stage
 
 struct CvDev {
