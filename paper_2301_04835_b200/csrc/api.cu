@@ -214,6 +214,18 @@ int psg_set_cvs(psg_ctx* c, int n_cv, const psg_cv_desc* cvs, int n_slots, const
         CK(c, cudaMemcpy(c->d_atom_weight, atom_weight, (size_t)P.N * sizeof(float), cudaMemcpyHostToDevice));
     }
     for (int i = 0; i < PSG_MAX_SLOTS; ++i) P.slot_atom_c[i] = (!per_rep && i < n_slots) ? slot_atom[i] : 0;
+    P.simple_groups = (P.n_ranges == 0 && !P.any_rgyr) ? 1 : 0;
+    for (int k = 0; k < PSG_MAX_CV; ++k)
+        for (int g = 0; g < PSG_MAX_GROUPS; ++g) {
+            int slot = 0;
+            if (k < n_cv) {
+                const GroupDev& G = P.grp[P.cv[k].gid0 + (g < P.cv[k].n_groups ? g : 0)];
+                if (G.is_range || G.size != 1) P.simple_groups = 0;
+                else slot = G.begin;
+            }
+            P.cv_slot[k * PSG_MAX_GROUPS + g] = slot;
+            P.cv_atom[k * PSG_MAX_GROUPS + g] = (!per_rep && n_slots > 0) ? slot_atom[slot] : 0;
+        }
     P.slot_atom = c->d_slot_atom; P.slot_gid = c->d_slot_gid; P.slot_weight = c->d_slot_weight; P.atom_weight = c->d_atom_weight;
     // scratch
     size_t R = (size_t)P.R;

@@ -110,6 +110,74 @@ __device__ __forceinline__ void force_add(float* __restrict__ fa, float fx, floa
     }
 }
 
+// Reciprocal and reciprocal square root in binary64 without the library's subroutine calls: the hardware seed (MUFU.RCP64H /
+// RSQ64H, ~20 bits) refined by two Newton steps (~1 ulp).  Several of them overlap in one thread (no call boundary), which is
+// what shortens the Jacobian chain of the fused step's prologue.  x must be finite and > 0.
+__device__ __forceinline__ double fast_rcp(double x) {
+    double r;
+    asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(r) : "d"(x));
+    r = fma(fma(-x, r, 1.0), r, r);
+    r = fma(fma(-x, r, 1.0), r, r);
+    return r;
+}
+__device__ __forceinline__ double fast_rsqrt(double x) {
+    double r;
+    asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(r) : "d"(x));
+    r = fma(0.5 * r, fma(-x * r, r, 1.0), r);
+    r = fma(0.5 * r, fma(-x * r, r, 1.0), r);
+    return r;
+}
+
+// dxi/dc_g alone (no value, no box), same formulas as cv_from_centers<true> with fast_rcp / fast_rsqrt in place of divisions
+// and square roots; zero where undefined.  Used by the fused metadynamics step, whose value threads take the atan2 chain.
+__device__ __forceinline__ void cv_jacobian_only(int type, int axis, const D3* c, D3* dc) {
+#pragma unroll
+    for (int g = 0; g < 4; ++g) dc[g] = d3(0, 0, 0);
+    if (type == PSG_CV_DISTANCE) {
+        const D3 d = c[1] - c[0];
+        const double r2 = dot(d, d);
+        if (r2 > 0.0) {
+            const double ir = fast_rsqrt(r2);
+            dc[1] = ir * d;
+            dc[0] = (-ir) * d;
+        }
+    } else if (type == PSG_CV_ANGLE) {
+        const D3 u = c[0] - c[1], v = c[2] - c[1];
+        const D3 n = cross(u, v);
+        const double n2 = dot(n, n);
+        if (n2 > 0.0) {
+            const double inn = fast_rsqrt(n2);
+            dc[0] = (fast_rcp(dot(u, u)) * inn) * cross(u, n);
+            dc[2] = (-fast_rcp(dot(v, v)) * inn) * cross(v, n);
+            dc[1] = (-1.0) * (dc[0] + dc[2]);
+        }
+    } else if (type == PSG_CV_DIHEDRAL) {
+        const D3 b1 = c[1] - c[0], b2 = c[2] - c[1], b3 = c[3] - c[2];
+        const D3 m = cross(b1, b2), n = cross(b2, b3);
+        const double l2 = dot(b2, b2), mm = dot(m, m), nn = dot(n, n);
+        if (mm > 0.0 && nn > 0.0) {
+            const double il2 = fast_rcp(l2), l = l2 * fast_rsqrt(l2);
+            const D3 f0 = (-l * fast_rcp(mm)) * m, f3 = (l * fast_rcp(nn)) * n;
+            const double p = dot(b1, b2) * il2, q = dot(b3, b2) * il2;
+            dc[0] = f0;
+            dc[3] = f3;
+            dc[1] = (-(1.0 + p)) * f0 + q * f3;
+            dc[2] = (-(1.0 + q)) * f3 + p * f0;
+        }
+    } else if (type == PSG_CV_DISPLACEMENT) {
+        dc[1] = d3(axis == 0 ? 1.0 : 0.0, axis == 1 ? 1.0 : 0.0, axis == 2 ? 1.0 : 0.0);
+        dc[0] = (-1.0) * dc[1];
+    } else if (type == PSG_CV_COM_COMPONENT) {
+        dc[0] = d3(axis == 0 ? 1.0 : 0.0, axis == 1 ? 1.0 : 0.0, axis == 2 ? 1.0 : 0.0);
+    }
+}
+
+// the raw binary32 record of an atom (w of a 3-float record reads as 0): lets a load be issued long before its use
+__device__ __forceinline__ float4 load_pos_raw(const float* __restrict__ p, long long atom, int ps) {
+    if (ps == 4) return __ldg(reinterpret_cast<const float4*>(p) + atom);
+    const float* q = p + atom * 3;
+    return make_float4(__ldg(q), __ldg(q + 1), __ldg(q + 2), 0.f);
+}
 __device__ __forceinline__ D3 load_pos(const float* __restrict__ p, long long atom, int ps) {
     if (ps == 4) {
         float4 v = __ldg(reinterpret_cast<const float4*>(p) + atom);

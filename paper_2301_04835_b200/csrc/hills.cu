@@ -105,12 +105,12 @@ __global__ void k_null_hills(int begin, int end, int rec, float4* __restrict__ h
 #ifdef PSG_TRACE
 static long long* g_trace = nullptr;
 long long* psg_trace_buffer() {
-    if (!g_trace) { cudaMalloc(&g_trace, 4096 * 16 * sizeof(long long)); cudaMemset(g_trace, 0, 4096 * 16 * sizeof(long long)); }
+    if (!g_trace) { cudaMalloc(&g_trace, 4096 * 32 * sizeof(long long)); cudaMemset(g_trace, 0, 4096 * 32 * sizeof(long long)); }
     return g_trace;
 }
-extern "C" int psg_debug_trace_clear() { return (int)cudaMemset(psg_trace_buffer(), 0, 4096 * 16 * sizeof(long long)); }
+extern "C" int psg_debug_trace_clear() { return (int)cudaMemset(psg_trace_buffer(), 0, 4096 * 32 * sizeof(long long)); }
 extern "C" int psg_debug_trace(long long* host_out, int n_ctas) {
-    return (int)cudaMemcpy(host_out, psg_trace_buffer(), (size_t)n_ctas * 16 * sizeof(long long), cudaMemcpyDeviceToHost);
+    return (int)cudaMemcpy(host_out, psg_trace_buffer(), (size_t)n_ctas * 32 * sizeof(long long), cudaMemcpyDeviceToHost);
 }
 #endif
 bool psg_stream_capturing(const psg_ctx* c) {
@@ -139,6 +139,11 @@ static cudaError_t launch_hills(psg_ctx* c, HillKernelArgs& A) {
     A.stages = stages;
     const size_t smem = hills_smem_bytes(n_cv, stages, c->sys.n_groups, fused);
     const int grid = hills_grid(c);
+    const int n_rt = (c->sys.R + TILE_R - 1) / TILE_R;
+    A.inv_n_rt = 1.0f / (float)n_rt;
+    A.Lc_host = A.n_chunks_host = 0;
+    if (A.n_h_host >= 0) hills_chunking(A.n_h_host, grid, n_rt, A.Lc_host, A.n_chunks_host);
+    A.simple = fused && c->sys.simple_groups && !c->sys.slot_weight && !c->sys.has_box;
     if (c->md.precision == PSG_HILLS_F64) return psg_hills_dispatch_f64(c, A, smem, grid);
     switch (n_cv) {
     case 1:

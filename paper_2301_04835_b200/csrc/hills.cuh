@@ -85,6 +85,12 @@ __device__ __forceinline__ u64 pk(float lo, float hi) {
     asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(lo), "f"(hi));
     return r;
 }
+// the same, opaque to common-subexpression elimination: every call is its own mov.b64 in the PTX (see HillBody)
+__device__ __forceinline__ u64 pk_once(float lo, float hi) {
+    u64 r;
+    asm volatile("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(lo), "f"(hi));
+    return r;
+}
 __device__ __forceinline__ void upk(u64 v, float& lo, float& hi) { asm("mov.b64 {%0, %1}, %2;" : "=f"(lo), "=f"(hi) : "l"(v)); }
 __device__ __forceinline__ u64 fma2(u64 a, u64 b, u64 c) {
     u64 d;
@@ -106,6 +112,10 @@ __device__ __forceinline__ u64 mul2(u64 a, u64 b) {
     asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b));
     return d;
 }
+// accumulate in place (read-write operand): biases the register allocator towards updating the accumulator's own pair
+// instead of rotating it through a copy at the loop's back edge
+__device__ __forceinline__ void acc_add2(u64& a, u64 b) { asm("add.rn.f32x2 %0, %0, %1;" : "+l"(a) : "l"(b)); }
+__device__ __forceinline__ void acc_fma2(u64& a, u64 b, u64 c) { asm("fma.rn.f32x2 %0, %1, %2, %0;" : "+l"(a) : "l"(b), "l"(c)); }
 __device__ __forceinline__ float ex2_approx(float x) {
     float y;
     asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
@@ -146,16 +156,15 @@ struct HillBody {
         const u64 MG = pk(MAGIC_RN, MAGIC_RN), NMG = pk(-MAGIC_RN, -MAGIC_RN);
         float s[NCV], lw;
         load_rec<NCV>(sm, h, s, lw);
-        u64 S[NCV];
-#pragma unroll
-        for (int k = 0; k < NCV; ++k) S[k] = pk(s[k], s[k]);
-        const u64 LW = pk(lw, lw);
+        // (the {s, s} pairs are formed at every use, not once per hill: a single-use pair is what ptxas reliably folds
+        // into the scalar-broadcast operand form of the packed instruction; a shared one it sometimes materialises with
+        // two MOVs per value -- +10 % instructions in the loop)
 #pragma unroll
         for (int p = 0; p < RT / 2; ++p) {
             u64 D[NCV];
 #pragma unroll
             for (int k = 0; k < NCV; ++k) {
-                u64 d = sub2(X[p][k], S[k]);
+                u64 d = sub2(X[p][k], pk_once(s[k], s[k]));
                 if (PM & (1 << k)) {
                     // nearest image: d -= P rint(d / P), -P = np_hi + np_lo (two constants: the wrap adds no bias)
                     u64 t = fma2(d, INVP[k], MG);
@@ -168,15 +177,15 @@ struct HillBody {
             u64 q = mul2(D[0], D[0]);
 #pragma unroll
             for (int k = 1; k < NEQ; ++k) q = fma2(D[k], D[k], q);
-            u64 x = fma2(q, NC[0], LW);   // base-2 exponent: log2(W) - sum_k d_k^2 log2(e) / (2 sigma_k^2)
+            u64 x = fma2(q, NC[0], pk_once(lw, lw));   // base-2 exponent: log2(W) - sum_k d_k^2 log2(e) / (2 sigma_k^2)
 #pragma unroll
             for (int k = NEQ; k < NCV; ++k) x = fma2(mul2(D[k], D[k]), NC[k], x);
             float x0, x1;
             upk(x, x0, x1);
             const u64 E = pk(ex2_approx(x0), ex2_approx(x1));
-            a32[p][0] = add2(a32[p][0], E);
+            acc_add2(a32[p][0], E);
 #pragma unroll
-            for (int k = 0; k < NCV; ++k) a32[p][1 + k] = fma2(E, D[k], a32[p][1 + k]);
+            for (int k = 0; k < NCV; ++k) acc_fma2(a32[p][1 + k], E, D[k]);
         }
     }
 };
@@ -194,7 +203,7 @@ __device__ __forceinline__ void accumulate_f32(const float4* __restrict__ sm, in
 }
 
 #ifndef PSG_ACC_IN_REGS
-#define PSG_ACC_IN_REGS(NCV) ((NCV) >= 3)
+#define PSG_ACC_IN_REGS(NCV) 0
 #endif
 #ifndef PSG_PEND_VARS
 #define PSG_PEND_VARS(NCV) ((NCV) >= 3)
@@ -289,6 +298,13 @@ __device__ __forceinline__ void accumulate_f64(const float4* __restrict__ sm, co
     __syncwarp();
 }
 
+#ifdef PSG_TRACE
+#define PSG_CLK_EARLY(i) do { if (threadIdx.x == 0 && blockIdx.x == 0 && g_trace_slot) g_trace_slot[16 + (i)] = clock64() - g_clk0; } while (0)
+__device__ long long* g_trace_slot = nullptr;   // debug builds: the CTA's stamp row, set by thread 0
+__device__ long long g_clk0 = 0;
+#else
+#define PSG_CLK_EARLY(i) do { } while (0)
+#endif
 // lane-local CV of (replica r, CV k) for systems with explicit groups only; dc[g] = d xi / d c_g / W_g.
 template <bool JAC>
 __device__ __forceinline__ double thread_cv(const SysParams& P, int r, int k, const float* __restrict__ pos, D3* dc) {
@@ -300,6 +316,7 @@ __device__ __forceinline__ double thread_cv(const SysParams& P, int r, int k, co
     // Fast path (measured: the gather, not the arithmetic, was half of the prologue): every group a single unweighted
     // atom -- a single atom is its own barycenter -- so all indices are formed first and the four position loads are in
     // flight together instead of one dependent (index -> position) chain per group.
+    PSG_CLK_EARLY(3);
     bool single = !P.slot_weight;
 #pragma unroll
     for (int g = 0; g < 4; ++g)
@@ -311,11 +328,22 @@ __device__ __forceinline__ double thread_cv(const SysParams& P, int r, int k, co
             const int s = P.grp[C.gid0 + (g < C.n_groups ? g : 0)].begin;   // unused groups re-read group 0 (no branch)
             a[g] = P.per_rep ? sa[s] : P.slot_atom_c[s];                    // shared index lists come from kernel parameters
         }
+#ifdef PSG_TRACE
+        if (threadIdx.x == 0 && blockIdx.x == 0 && g_trace_slot) { long long t_ = clock64() - g_clk0 + (a[0] + a[1] + a[2] + a[3] == -12345 ? 1 : 0); g_trace_slot[16 + 4] = t_; }
+#endif
 #pragma unroll
         for (int g = 0; g < 4; ++g) {
             c[g] = load_pos(p, a[g], P.ps);
             W[g] = 1.0;
         }
+#ifdef PSG_TRACE
+        if (threadIdx.x == 0 && blockIdx.x == 0 && g_trace_slot) {   // thread 0: all four positions have arrived
+            long long t_;
+            asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t_) : "d"(c[0].x + c[1].x + c[2].x + c[3].x));
+            g_trace_slot[9] = t_;
+            g_trace_slot[16 + 5] = clock64() - g_clk0;
+        }
+#endif
     } else {
 #pragma unroll
         for (int g = 0; g < 4; ++g) {
@@ -378,32 +406,66 @@ struct HillKernelArgs {
     int R;
     int fused;
     int stages;              // shared-memory stages of SUB x 16 bytes
+    int Lc_host, n_chunks_host;   // the chunking for n_h_host (computed on the host: three integer divisions off the kernel's entry path)
+    float inv_n_rt;          // 1 / (number of replica tiles), for the item -> (tile, chunk) split
+    int simple;              // fused: every group one unweighted atom, no box: the lean gather (SysParams::cv_slot / cv_atom)
 #ifdef PSG_TRACE
     long long* trace;        // [grid][8] clock64 stamps of the first item of every CTA (debug builds only)
 #endif
 };
 #ifdef PSG_TRACE
-#define PSG_TS 16
+#define PSG_TS 32
+#define PSG_CLK(i) do { if (threadIdx.x == 0 && blockIdx.x == 0 && g_trace_slot) g_trace_slot[16 + (i)] = clock64() - g_clk0; } while (0)
 #define PSG_STAMP(i) do { if (threadIdx.x == 0 && item == (int)blockIdx.x && A.trace) { long long t_; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t_)); A.trace[blockIdx.x * PSG_TS + (i)] = t_; } } while (0)
 #define PSG_STAMP_T(tidx, i) do { if (threadIdx.x == (tidx) && item == (int)blockIdx.x && A.trace) { long long t_; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t_)); A.trace[blockIdx.x * PSG_TS + (i)] = t_; } } while (0)
 #else
 #define PSG_STAMP(i) do { } while (0)
 #define PSG_STAMP_T(tidx, i) do { } while (0)
+#define PSG_CLK(i) do { } while (0)
 #endif
 
+// chunk length (a multiple of 32, at least 32) and number of chunks per replica tile for n_h hills on `grid` CTAs
+__host__ __device__ inline void hills_chunking(int n_h, int grid, int n_rt, int& Lc, int& n_chunks) {
+    int cpt = grid / n_rt;
+    if (cpt < 1) cpt = 1;
+    Lc = (n_h + cpt - 1) / cpt;
+    Lc = ((Lc + 31) / 32) * 32;
+    if (Lc < 32) Lc = 32;
+    n_chunks = (n_h + Lc - 1) / Lc;
+    if (n_chunks < 1) n_chunks = 1;
+}
 __host__ __device__ inline size_t hills_wacc_doubles(int n_cv) { return (size_t)((RT * (1 + n_cv) + 31) / 32) * 32; }
 __host__ __device__ inline size_t hills_smem_bytes(int n_cv, int stages, int n_groups, bool fused) {
     size_t b = (size_t)stages * SUB * 16;                          // hill stages (SUB / rec hills each)
     b += (size_t)HWARPS * hills_wacc_doubles(n_cv) * 8;            // per-warp binary64 totals
     b += (size_t)3 * TILE_R * (1 + n_cv) * 8;                      // s_out, s_half[2]
     b += (size_t)TILE_R * n_cv * 4;                                // s_xi
-    b += fused ? (size_t)TILE_R * n_groups * 3 * 4 : 0;            // s_jv
+    b += fused ? (size_t)TILE_R * n_groups * 4 * 4 : 0;            // s_jv, s_ja
     b += 8 * 8 + 64;                                               // barriers, pad
     return b;
 }
 #ifndef PSG_HILL_MAX_STAGES
 #define PSG_HILL_MAX_STAGES 6
 #endif
+
+// item -> (tile, chunk) without an integer division: a binary32 quotient, corrected by one (item < 2^24)
+__device__ __forceinline__ void hills_item(int item, int n_rt, float inv_n_rt, int& tile, int& chunk) {
+    chunk = (int)((float)item * inv_n_rt);
+    if (chunk * n_rt > item) --chunk;
+    else if ((chunk + 1) * n_rt <= item) ++chunk;
+    tile = item - chunk * n_rt;
+}
+// the atoms of CV k of replica r in the lean gather (every group one atom): one table look-up per group
+__device__ __forceinline__ void hills_cv_atoms(const SysParams& P, int r, int k, int (&a)[4]) {
+    if (P.per_rep) {
+        const int* sa = P.slot_atom + (long long)r * P.n_slots;
+#pragma unroll
+        for (int g = 0; g < 4; ++g) a[g] = __ldg(sa + P.cv_slot[k * PSG_MAX_GROUPS + g]);
+    } else {
+#pragma unroll
+        for (int g = 0; g < 4; ++g) a[g] = P.cv_atom[k * PSG_MAX_GROUPS + g];
+    }
+}
 
 // One kernel for psg_bias_eval and the whole metadynamics step (A.fused).
 template <int NCV, int PM, int NEQ, bool F64>
@@ -413,6 +475,9 @@ __global__ void __launch_bounds__(HWARPS * 32, 1) k_hills(const __grid_constant_
     constexpr int SUBH = SUB / REC;   // hills per stage: a stage is always SUB x 16 bytes
     constexpr int NV = 1 + NCV;
     constexpr int NT = HWARPS * 32;
+#ifdef PSG_TRACE
+    if (threadIdx.x == 0 && blockIdx.x == 0) { g_clk0 = clock64(); g_trace_slot = A.trace; }
+#endif
     extern __shared__ __align__(128) unsigned char smem_raw[];
     constexpr int WACC = ((RT * NV + 31) / 32) * 32;   // per-warp binary64 totals (padded to whole butterfly passes)
     constexpr int PASSES = WACC / 32;
@@ -424,6 +489,7 @@ __global__ void __launch_bounds__(HWARPS * 32, 1) k_hills(const __grid_constant_
     uint64_t* full = reinterpret_cast<uint64_t*>(s_half + 2 * TILE_R * NV);       // 8 barriers
     float* s_xi = reinterpret_cast<float*>(full + 8);                             // [NCV][TILE_R] (pairs of replicas adjacent)
     float* s_jv = s_xi + TILE_R * NCV;                                            // fused: [TILE_R][n_groups][3]
+    int* s_ja = reinterpret_cast<int*>(s_jv + TILE_R * P.n_groups * 3);           // fused, lean gather: [TILE_R][n_groups] atom of the group
     __shared__ int s_last;
     __shared__ int s_cnt[8];   // warps that have left a stage
 
@@ -431,28 +497,97 @@ __global__ void __launch_bounds__(HWARPS * 32, 1) k_hills(const __grid_constant_
     const int half = wid / HHALF, w8 = wid % HHALF;   // warps w8 and w8 + HHALF own the same replicas; half picks the hills
     const int R = A.R;
     const int n_rt = (R + TILE_R - 1) / TILE_R;
-    const int n_h = A.n_h_host >= 0 ? A.n_h_host : *A.n_hills;
-    // chunking: as many chunks per tile as the grid allows, chunk length a multiple of 32
-    int cpt = (int)gridDim.x / n_rt;
-    if (cpt < 1) cpt = 1;
-    int Lc = (n_h + cpt - 1) / cpt;
-    Lc = ((Lc + 31) / 32) * 32;
-    if (Lc < 32) Lc = 32;
-    int n_chunks = (n_h + Lc - 1) / Lc;
-    if (n_chunks < 1) n_chunks = 1;
+    // Lean gather, FIRST thing in the kernel: the position loads of this CTA's first item are on the critical path of
+    // the launch (measured: ~250 set-up instructions at a cold instruction cache otherwise precede them), so they are
+    // issued before anything else.  They are consumed BEFORE the item loop (lean_finish below): registers that stayed live
+    // into the loop would be taken from the hill loop.
+    static_assert(2 * TILE_R * NCV <= NT, "one pass of the CV prologue covers a tile");
+    const bool early = A.fused && A.simple && A.n_h_host >= 0 && (int)blockIdx.x < n_rt * A.n_chunks_host;   // CTA-uniform
+    float4 pre[4];
+    int pre_a[4];
+    int tile0 = 0, chunk0 = 0;
+    if (early) {
+        hills_item((int)blockIdx.x, n_rt, A.inv_n_rt, tile0, chunk0);
+        const int t = tid >= TILE_R * NCV ? tid - TILE_R * NCV : tid;
+        const int r = tile0 * TILE_R + t / NCV;
+        if (tid < 2 * TILE_R * NCV && r < R) {
+            hills_cv_atoms(P, r, t % NCV, pre_a);
+            const float* p = A.pos + (long long)r * P.rstride * P.ps;
+#pragma unroll
+            for (int g = 0; g < 4; ++g) pre[g] = load_pos_raw(p, pre_a[g], P.ps);
+        }
+    }
+    // chunking: as many chunks per tile as the grid allows, chunk length a multiple of 32 (hills_chunking: the host did
+    // these divisions when it knows the hill count; under stream capture the count is the device counter's)
+    int n_h, Lc, n_chunks;
+    if (A.n_h_host >= 0) {
+        n_h = A.n_h_host; Lc = A.Lc_host; n_chunks = A.n_chunks_host;
+    } else {
+        n_h = *A.n_hills;
+        hills_chunking(n_h, (int)gridDim.x, n_rt, Lc, n_chunks);
+    }
     const int items = n_rt * n_chunks;
-
-    if (tid < 8) s_cnt[tid] = 0;
-    if (tid == 0) {
+    PSG_CLK(8);
+    // One thread with no CV work of its own (lane 0 of the last warp) owns the barriers and the first TMA loads of an item;
+    // nobody else touches them before the __syncthreads that follows the CV prologue.
+    const bool producer = tid == NT - 32;
+    if (producer) {
+        for (int i = 0; i < 8; ++i) s_cnt[i] = 0;
         for (int s = 0; s < STG; ++s) mbar_init(&full[s], 1);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
-    // no CTA-wide sync here: thread 0 issues the first TMA loads itself; everybody else first meets the barriers
-    // after the __syncthreads that follows the CV prologue
+    PSG_CLK(9);
     unsigned seq = 0;   // sub-tiles consumed so far by this CTA (stage = seq % STG, parity = (seq / STG) & 1)
 
+    // Lean gather (every group a single unweighted atom, no box: the ADP dihedrals of PAPER.md:L81 and every BASELINE.json
+    // metadynamics config): a single atom is its own barycenter, so a thread forms its four atom indices from one table
+    // look-up each and has all four position loads in flight at once.  The value (cross products, atan2) and the Jacobian
+    // (cross products, reciprocals without subroutine calls) of a CV are taken by different threads; both chains are a few
+    // hundred cycles once the loads are back.  lean_finish: positions -> xi (shared memory, step output) or Jacobian
+    // vectors + atoms (shared memory, for the scatter).
+    auto lean_finish = [&](bool want_j, int rr, int k, int r, bool first_chunk, const int (&a)[4], const float4 (&raw)[4]) {
+        if (r < R) {
+            D3 c[4], dc[4];
+#pragma unroll
+            for (int g = 0; g < 4; ++g) c[g] = d3((double)raw[g].x, (double)raw[g].y, (double)raw[g].z);
+            const CvDev& C = P.cv[k];
+            if (!want_j) {
+                const float v = (float)cv_from_centers<false>(C.type, C.axis, c, dc, nullptr);
+                if (first_chunk && A.xi_out) A.xi_out[(long long)r * NCV + k] = v;
+                s_xi[k * TILE_R + rr] = v;
+            } else {
+                if (first_chunk) {   // the force records the final scatter will update, requested into L2 now
+#pragma unroll
+                    for (int g = 0; g < 4; ++g)
+                        if (g < C.n_groups)
+                            asm volatile("prefetch.global.L2 [%0];" ::"l"(A.force + ((long long)r * P.rstride + a[g]) * P.fs));
+                }
+                cv_jacobian_only(C.type, C.axis, c, dc);
+#pragma unroll
+                for (int g = 0; g < 4; ++g)
+                    if (g < C.n_groups) {
+                        float* j = s_jv + (rr * P.n_groups + C.gid0 + g) * 3;
+                        j[0] = (float)dc[g].x; j[1] = (float)dc[g].y; j[2] = (float)dc[g].z;
+                        s_ja[rr * P.n_groups + C.gid0 + g] = a[g];   // the scatter needs no index load of its own
+                    }
+            }
+        } else if (!want_j) {
+            s_xi[k * TILE_R + rr] = 0.f;
+        }
+    };
+    bool lean_done = false;
+    if (early) {   // the first item's prologue, from the loads issued at the top of the kernel
+        if (tid < 2 * TILE_R * NCV) {
+            const bool want_j = tid >= TILE_R * NCV;
+            const int t = want_j ? tid - TILE_R * NCV : tid;
+            lean_finish(want_j, t / NCV, t % NCV, tile0 * TILE_R + t / NCV, chunk0 == 0, pre_a, pre);
+        }
+        lean_done = true;
+    }
+
     for (int item = blockIdx.x; item < items; item += gridDim.x) {
-        const int tile = item % n_rt, chunk = item / n_rt;
+        int tile, chunk;
+        hills_item(item, n_rt, A.inv_n_rt, tile, chunk);
         const int r0 = tile * TILE_R;
         const int h0 = chunk * Lc;
         int len = n_h - h0;
@@ -460,8 +595,8 @@ __global__ void __launch_bounds__(HWARPS * 32, 1) k_hills(const __grid_constant_
         if (len < 0) len = 0;
         const int n_st = (len + SUBH - 1) / SUBH;
         PSG_STAMP(0);
-        // producer prologue
-        if (tid == 0) {
+        PSG_CLK(0);
+        if (producer) {
             for (int t = 0; t < n_st && t < STG; ++t) {
                 int s = (seq + t) % STG;
                 int cnt = min(SUBH, len - t * SUBH);
@@ -470,10 +605,28 @@ __global__ void __launch_bounds__(HWARPS * 32, 1) k_hills(const __grid_constant_
             }
         }
         PSG_STAMP(8);
+        PSG_CLK(1);
         // CV values (and per-group Jacobian vectors) of this tile's replicas; overlaps the first TMA loads
-        if (A.fused) {
-            // the value (gather, cross products, atan2) and the Jacobian (gather, cross products, divisions) of one CV are
-            // two serial binary64 chains: different threads (different warps) take them, which shortens the prologue
+        if (A.fused && A.simple) {
+            if (!lean_done) {
+                for (int t2 = tid; t2 < 2 * TILE_R * NCV; t2 += NT) {
+                    const bool want_j = t2 >= TILE_R * NCV;
+                    const int t = want_j ? t2 - TILE_R * NCV : t2;
+                    const int rr = t / NCV, k = t % NCV, r = r0 + rr;
+                    int a[4];
+                    float4 raw[4];
+                    if (r < R) {
+                        hills_cv_atoms(P, r, k, a);
+                        const float* p = A.pos + (long long)r * P.rstride * P.ps;
+#pragma unroll
+                        for (int g = 0; g < 4; ++g) raw[g] = load_pos_raw(p, a[g], P.ps);
+                    }
+                    lean_finish(want_j, rr, k, r, chunk == 0, a, raw);
+                }
+            }
+            lean_done = false;
+        } else if (A.fused) {
+            // the general gather (groups of several atoms, weights, minimum image): value and Jacobian again in different threads
             for (int t2 = tid; t2 < 2 * TILE_R * NCV; t2 += NT) {
                 const bool want_j = t2 >= TILE_R * NCV;
                 const int t = want_j ? t2 - TILE_R * NCV : t2;
@@ -487,6 +640,7 @@ __global__ void __launch_bounds__(HWARPS * 32, 1) k_hills(const __grid_constant_
                     }
                     s_xi[k * TILE_R + rr] = v;
                     PSG_STAMP(10);
+                    PSG_CLK(6);
                 } else if (r < R) {
                     D3 dc[4];
                     if (chunk == 0) prefetch_force_lines(P, r, k, A.force);
@@ -509,6 +663,7 @@ __global__ void __launch_bounds__(HWARPS * 32, 1) k_hills(const __grid_constant_
         }
         __syncthreads();
         PSG_STAMP(1);
+        PSG_CLK(7);
         const bool warp_active = r0 + w8 * RT < R;
         // Stage hand-back without a CTA-wide barrier (measured: the bare loop reaches 0.95 of the FFMA peak, the loop with a
         // barrier per 1,024 hills 0.80): warps drift freely; lane 0 counts its warp out of the stage with a shared-memory
@@ -657,7 +812,19 @@ __global__ void __launch_bounds__(HWARPS * 32, 1) k_hills(const __grid_constant_
             if (A.fused) {
                 __syncthreads();
                 PSG_STAMP(5);
-                // forces: one thread per (replica, slot); red.global.add (atoms shared by CVs / walkers collide)
+                // forces: L2 reductions (atoms shared by CVs / walkers collide).  Lean gather: one thread per (replica, group),
+                // atom and Jacobian out of shared memory -- no global load between the last sum and the reductions
+                if (A.simple) {
+                    for (int t = tid; t < TILE_R * P.n_groups; t += NT) {
+                        const int rr = t / P.n_groups, gid = t - rr * P.n_groups, r = r0 + rr;
+                        if (r >= R) continue;
+                        const float fdv = -(float)s_out[rr * NV + 1 + P.grp[gid].cv];   // dV/dxi and J pass through binary32, as unfused
+                        const float* j = s_jv + t * 3;
+                        float* fa = A.force + ((long long)r * P.rstride + s_ja[t]) * P.fs;
+                        force_add(fa, fdv * j[0], fdv * j[1], fdv * j[2], P.fs);
+                    }
+                } else
+                // general gather: one thread per (replica, slot)
                 for (int t = tid; t < TILE_R * P.n_slots; t += NT) {
                     int rr = t / P.n_slots, s = t % P.n_slots, r = r0 + rr;
                     if (r >= R) continue;

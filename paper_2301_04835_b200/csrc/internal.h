@@ -48,6 +48,11 @@ struct SysParams {
     long long span_begin, span_end;          // union span of all range groups
     int range_blocks;                        // blocks per replica over the span
     int slot_atom_c[PSG_MAX_SLOTS];          // shared index list (per_rep == 0): read from kernel parameters
+    // fast gather of the fused metadynamics step: when every group is ONE explicit atom (simple_groups), group g of CV k
+    // is slot cv_slot[4 k + g] and, with a shared index list, atom cv_atom[4 k + g]; unused groups repeat group 0
+    int simple_groups;
+    int cv_slot[PSG_MAX_CV * PSG_MAX_GROUPS];
+    int cv_atom[PSG_MAX_CV * PSG_MAX_GROUPS];
     const int* slot_atom;        // device [n_slots] or [R][n_slots]
     const int* slot_gid;         // device [n_slots]: global group id of a slot
     const float* slot_weight;    // device [n_slots] or nullptr
