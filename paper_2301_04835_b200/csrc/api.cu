@@ -95,7 +95,7 @@ static void free_all(psg_ctx* c) {
     dfree(c->d_xi); dfree(c->d_V); dfree(c->d_dVdxi); dfree(c->d_bin); dfree(c->d_V64);
     dfree(c->d_jac); dfree(c->d_gdesc); dfree(c->d_rpart); dfree(c->d_arrive); dfree(c->d_rdesc); dfree(c->d_gbar); dfree(c->d_whist);
     dfree(c->d_kspring); dfree(c->d_centers);
-    dfree(c->md.hills); dfree(c->md.heights); dfree(c->md.n_hills); dfree(c->md.part); dfree(c->md.ticket);
+    dfree(c->md.hills); dfree(c->md.heights); dfree(c->md.n_hills); dfree(c->md.part);
     if (c->abf.own) { dfree(c->abf.hist); dfree(c->abf.fsum); }
     c->abf.hist = nullptr; c->abf.fsum = nullptr;
     dfree(c->d_pos_stage); dfree(c->d_frc_stage); dfree(c->d_fs_stage);
@@ -320,9 +320,8 @@ int psg_set_metad(psg_ctx* c, const float* sigma, float w0, float kB_deltaT, int
     CK(c, dalloc(M.heights, (size_t)capacity + 2));
     CK(c, dalloc(M.n_hills, 2));
     CK(c, dalloc(M.part, part));
-    CK(c, dalloc(M.ticket, (size_t)n_rt));
     CK(c, cudaMemset(M.n_hills, 0, 2 * sizeof(int)));
-    CK(c, cudaMemset(M.ticket, 0, n_rt * sizeof(unsigned)));
+    CK(c, cudaMemset(M.part, 0, part * sizeof(double)));   // a cleared word = "not published yet" (hills.cuh)
     CK(c, psg_launch_null_hills(c, 0, capacity));   // invariant: records beyond the count are null (contribute 0)
     c->nh_bound = c->nh_lo = 0; c->count_unknown = false; c->overflow_possible = false;
     c->method = PSG_METHOD_METAD;

@@ -156,7 +156,7 @@ static cudaError_t launch_hills(psg_ctx* c, HillKernelArgs& A) {
 
 static HillKernelArgs base_args(psg_ctx* c) {
     HillKernelArgs A{};
-    A.hills = c->md.hills; A.heights = c->md.heights; A.n_hills = c->md.n_hills; A.part = c->md.part; A.ticket = c->md.ticket;
+    A.hills = c->md.hills; A.heights = c->md.heights; A.n_hills = c->md.n_hills; A.part = c->md.part;
     A.R = c->sys.R;
     // The host's upper bound of the hill count saves the kernel a dependent global load. Under stream capture the
     // launch may be replayed with a longer list than the one seen now, and after a CAPTURED deposit the replays grow the

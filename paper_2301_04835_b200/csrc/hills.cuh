@@ -15,12 +15,12 @@
 //     exponent          q = d0^2 (+ d1^2 ...);  x = log2(W) - c q                        (NCV + 1 if the sigmas agree)
 //     MUFU.EX2 (one per replica), V += e, g_k += e d_k                                   (1 + NCV)
 // Binary32 partial sums (<= 64 hills per lane) are flushed into binary64 by a warp-wide transpose-reduction (31 shuffle +
-// add steps turn 32 per-lane values into one warp total per lane): the binary64 accumulators are ONE register per lane, not
-// shared memory, which leaves the SM's shared memory to the hill stages (up to 6 x 32 KB in flight).  Lanes (butterfly),
-// warps, then chunks are combined in binary64 in FIXED order (the last CTA of a tile, found with a ticket counter, sums the
-// chunk partials), so results are bitwise reproducible.
+// add steps turn 32 per-lane values into one warp total per lane): the binary64 accumulators are ONE slot per lane (4 KB per CTA), not
+// 98-131 KB of shared memory, which leaves the SM's shared memory to the hill stages (up to 6 x 32 KB in flight).  Lanes (butterfly),
+// warps, then chunks are combined in binary64 in FIXED order (the CTA of a tile's chunk 0 collects the other chunks'
+// published partials, each word carrying its own valid flag), so results are bitwise reproducible.
 // FUSED: the CTA first evaluates the CVs (and Jacobians, kept in shared memory) of its tile from the engine's
-// positions; the last CTA of the tile scatters -dV/dxi * J into the engine's forces: one launch per MD step.
+// positions; the finishing CTA of the tile scatters -dV/dxi * J into the engine's forces: one launch per MD step.
 #pragma once
 #include "geom.cuh"
 
@@ -395,7 +395,6 @@ struct HillKernelArgs {
     const int* n_hills;      // device counter (exact), read only when n_h_host < 0 (stream capture)
     int n_h_host;            // host upper bound of the count; records beyond the exact count are null (contribute 0)
     double* part;
-    unsigned* ticket;
     const float* xi_in;      // not fused: [R][n_cv]
     float* V_out;            // nullable
     double* V64_out;         // nullable
@@ -490,7 +489,6 @@ __global__ void __launch_bounds__(HWARPS * 32, 1) k_hills(const __grid_constant_
     float* s_xi = reinterpret_cast<float*>(full + 8);                             // [NCV][TILE_R] (pairs of replicas adjacent)
     float* s_jv = s_xi + TILE_R * NCV;                                            // fused: [TILE_R][n_groups][3]
     int* s_ja = reinterpret_cast<int*>(s_jv + TILE_R * P.n_groups * 3);           // fused, lean gather: [TILE_R][n_groups] atom of the group
-    __shared__ int s_last;
     __shared__ int s_cnt[8];   // warps that have left a stage
 
     const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
@@ -762,33 +760,53 @@ __global__ void __launch_bounds__(HWARPS * 32, 1) k_hills(const __grid_constant_
         constexpr int TV = TILE_R * NV;
         __syncthreads();
         PSG_STAMP(14);
-        // warps w8 and w8 + HHALF (the two halves of the chunk's hills) in fixed order -> this chunk's partial of the tile
+        // Warps w8 and w8 + HHALF (the two halves of the chunk's hills) in fixed order -> this chunk's partial of the tile.
+        // The CTA of chunk 0 FINISHES the tile: the others publish their partials and are done; it keeps its own on chip
+        // and collects theirs.  A published value is ONE 64-bit word that carries its own valid flag -- the lowest mantissa
+        // bit, forced to 1 (a deterministic perturbation of at most 1 ulp of binary64; a cleared word is 0) -- so a single
+        // relaxed 8-byte load either sees the new value or knows it is not there yet: no ticket, no fence, one L2 round trip
+        // between the end of the hill loop and the sums.  The finisher clears what it consumed for the next launch.  (A
+        // launch runs one item per CTA whenever a tile has several chunks, and only finishers wait, so nothing can deadlock.)
+        const bool finisher = chunk == 0;   // block-uniform
+        u64* const part_bits = reinterpret_cast<u64*>(A.part);
         for (int t = tid; t < TV; t += NT) {
             const int rr = t / NV, v = t - rr * NV, ww = rr / RT, j = rr - ww * RT;
-            A.part[(size_t)(chunk * n_rt + tile) * TV + t] = s_wacc[ww * WACC + j * NV + v] + s_wacc[(ww + HHALF) * WACC + j * NV + v];
+            const double val = s_wacc[ww * WACC + j * NV + v] + s_wacc[(ww + HHALF) * WACC + j * NV + v];
+            if (finisher) s_out[t] = val;
+            else __stcg(part_bits + (size_t)(chunk * n_rt + tile) * TV + t, (u64)__double_as_longlong(val) | 1ull);
         }
-        __syncthreads();
         PSG_STAMP(3);
-        if (tid == 0) {
-            // release: the CTA's partials (ordered before this by the barrier) are visible to whoever acquires the ticket
-            unsigned old;
-            asm volatile("atom.acq_rel.gpu.global.add.u32 %0, [%1], 1;" : "=r"(old) : "l"(A.ticket + tile) : "memory");
-            s_last = (old == (unsigned)(n_chunks - 1));
-        }
-        __syncthreads();
-        PSG_STAMP(4);
-        if (s_last) {   // block-uniform: this CTA finishes the tile
+        if (finisher) {
+            __syncthreads();
+            PSG_STAMP(4);
             // chunk partials in fixed order; two thread groups split the chunks so that more loads are in flight
             constexpr int PARTS = NT >= 2 * TV ? 2 : 1;
+            constexpr int BATCH = 9;   // words in flight per thread (config 1: 18 chunks per tile = 2 groups x 9: one round trip)
             const size_t cstride = (size_t)n_rt * TV;
             const int cn = (n_chunks + PARTS - 1) / PARTS;
             for (int t = tid; t < PARTS * TV; t += NT) {
                 const int pt = t / TV, v = t - pt * TV;
-                const double* src = A.part + (size_t)tile * TV + v;
+                u64* src = part_bits + (size_t)tile * TV + v;
                 const int c1 = min(n_chunks, (pt + 1) * cn);
                 double sum = 0.0;
-#pragma unroll 9
-                for (int c = pt * cn; c < c1; ++c) sum += __ldcg(src + c * cstride);
+                for (int c = pt * cn; c < c1; c += BATCH) {
+                    u64 w[BATCH];
+#pragma unroll
+                    for (int i = 0; i < BATCH; ++i)
+                        if (c + i < c1 && c + i > 0) w[i] = __ldcg(src + (size_t)(c + i) * cstride);
+#pragma unroll
+                    for (int i = 0; i < BATCH; ++i) {
+                        if (c + i >= c1) break;
+                        if (c + i == 0) {
+                            sum += s_out[v];   // this CTA's own chunk
+                        } else {
+                            u64* q = src + (size_t)(c + i) * cstride;
+                            while (!(w[i] & 1ull)) asm volatile("ld.relaxed.gpu.global.u64 %0, [%1];" : "=l"(w[i]) : "l"(q) : "memory");
+                            sum += __longlong_as_double((long long)w[i]);
+                            __stcg(q, 0ull);
+                        }
+                    }
+                }
                 s_half[pt * TV + v] = sum;
             }
             __syncthreads();
@@ -808,7 +826,6 @@ __global__ void __launch_bounds__(HWARPS * 32, 1) k_hills(const __grid_constant_
                     }
                 }
             }
-            if (tid == 0) A.ticket[tile] = 0u;   // ready for the next launch
             if (A.fused) {
                 __syncthreads();
                 PSG_STAMP(5);
@@ -839,7 +856,7 @@ __global__ void __launch_bounds__(HWARPS * 32, 1) k_hills(const __grid_constant_
                 }
             }
         }
-        __syncthreads();   // s_xi / s_out / s_acc / s_last are reused by the next item
+        __syncthreads();   // s_xi / s_out / s_wacc are reused by the next item
         PSG_STAMP(6);
 #ifdef PSG_TRACE
         if (threadIdx.x == 0 && item == (int)blockIdx.x && A.trace) {

@@ -75,8 +75,7 @@ struct MetadState {
     float* heights;         // W as deposited / loaded (exported by psg_get_hills; read by the binary64 path)
     int* n_hills;           // device: [0] the exact count, [1] sticky overflow flag (a deposit was clamped at capacity)
     int capacity;
-    double* part;           // [max_chunks][n_rtiles][TILE_R][1+n_cv]
-    unsigned* ticket;       // [n_rtiles]
+    double* part;           // [max_chunks][n_rtiles][TILE_R][1+n_cv]: published chunk partials, a cleared word = not there yet
     int max_chunks;
     double w0, kB_deltaT;
     int stride;
