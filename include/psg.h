@@ -61,7 +61,7 @@ enum {
     PSG_CV_SHAPE_ANISOTROPY = 10 /* ((l1 - (l2+l3)/2)^2 + 3/4 (l2 - l3)^2) / (l1+l2+l3)^2; 0 for a point (L189) */
 };
 
-enum { PSG_METHOD_NONE = 0, PSG_METHOD_HARMONIC = 1, PSG_METHOD_METAD = 2, PSG_METHOD_ABF = 3 };
+enum { PSG_METHOD_NONE = 0, PSG_METHOD_HARMONIC = 1, PSG_METHOD_METAD = 2, PSG_METHOD_ABF = 3, PSG_METHOD_METAD_GRID = 4 };
 
 /* precision of the metadynamics hill sum */
 enum {
@@ -224,8 +224,7 @@ int psg_apply_bias_forces(psg_ctx* ctx, const float* d_pos, const float* d_dVdxi
  * array per window, at most (SM count) slices of 2,048 atoms per window (k_range_step).  Anything else runs the
  * kernels of the separate calls in sequence.  k_abf_step and k_range_step contain inter-CTA waits and are
  * launched cooperatively: the launch fails (PSG_ECUDA) rather than hangs if the grid cannot be co-resident.
- * Environment (read once, for experiments): PSG_RANGE_LAG = items the position producer of k_range_step may
- * run ahead of the force group (default 10); PSG_DISABLE_RANGE_STEP = take the separate kernels instead. */
+ * Every hot-path call is wrapped in an NVTX range of its own name. */
 int psg_step(psg_ctx* ctx, const float* d_pos, float* d_force, const float* d_fsample, long long step);
 /* Device pointers (ctx-owned, valid until destroy/reconfigure) of the last step's per-replica results:
  * xi [R][n_cv], V [R] (0 for ABF), dVdxi [R][n_cv], bin [R] (ABF only, else NULL). Any out may be NULL. */
@@ -276,7 +275,16 @@ int psg_interface_cv_apply(psg_ctx* ctx, const float* d_pos, const float* d_dVdx
  *   psg_metad_grid_deposit every `stride` steps).  CVs over atom ranges take three launches instead.  No sync.
  * psg_metad_grid_state: device pointers of the node array and of the heights [R] (binary64) of the last event; owned by
  *   the ctx, valid until the next psg_metad_grid_set or psg_destroy.
+ * All of this state is dropped by psg_set_layout (it is sized by the layout).
  * Errors: PSG_EINVAL (arguments), PSG_ESTATE (call order), PSG_ENOMEM, PSG_ECUDA. */
+/* psg_set_metad_grid: the grid-stored bias as the METHOD of the ctx (PAPER.md:L151 with the deposit interval of L147):
+ *   psg_metad_grid_set with the same arguments, then psg_step / psg_step_host run CVs -> (one deposit event onto the grid
+ *   when step % stride == 0, step >= 1; stride = 0: never) -> interpolated bias -> forces, psg_bias_eval is
+ *   psg_metad_grid_eval and psg_deposit_hill is psg_metad_grid_deposit.  Call after psg_set_cvs (n_cv must match).  A
+ *   periodic CV needs a periodic grid spanning exactly its period and an open CV an open grid: PSG_EINVAL otherwise (a
+ *   dihedral on an open grid would be clamped at +-pi instead of wrapped). */
+int psg_set_metad_grid(psg_ctx* ctx, const double* lower, const double* upper, const int* shape, const int* periodic,
+                       const double* sigma, double w0, double kB_deltaT, int stride);
 int psg_metad_grid_set(psg_ctx* ctx, int n_cv, const double* lower, const double* upper, const int* shape, const int* periodic,
                        const double* sigma, double w0, double kB_deltaT);
 int psg_metad_grid_deposit(psg_ctx* ctx, const float* d_xi, const unsigned char* d_mask);

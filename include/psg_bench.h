@@ -22,6 +22,10 @@ extern "C" {
  *    latency-bound configs 0 and 2).
  * 100 + n: the same as 7 with only n passes of 1,024 hills (short-run behaviour). */
 int psg_measure_alu_peak(int device, int which, double* ops_per_second_out);
+/* Tuning knobs of the fused large-group step, for measurements: range_step_lag = items the position
+ * producer of k_range_step may run ahead of the force group (0 = the default, 10); disable_range_step != 0 makes psg_step
+ * take the separate kernels (k_range_moments, k_cv_eval, k_harmonic, k_apply_dense) instead. */
+int psg_set_tuning(psg_ctx* ctx, int range_step_lag, int disable_range_step);
 /* Launch counter: number of kernels this ctx has enqueued since creation (for bench.py's gpu_launches). */
 long long psg_launch_count(const psg_ctx* ctx);
 

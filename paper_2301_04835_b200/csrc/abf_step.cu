@@ -88,9 +88,12 @@ __global__ void __launch_bounds__(256, 4) k_abf_step(const __grid_constant__ Sys
     }
 }
 
-static int abf_blocks_per_sm() {
-    static int n = -1;
-    if (n < 0) {
+static int abf_blocks_per_sm(int device) {
+    static int cache[PSG_MAX_DEVICES];
+    static bool have[PSG_MAX_DEVICES] = {};
+    int& n = cache[device % PSG_MAX_DEVICES];
+    if (!have[device % PSG_MAX_DEVICES]) {
+        have[device % PSG_MAX_DEVICES] = true;
         if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n, k_abf_step, 256, 0) != cudaSuccess) n = 0;
         (void)cudaGetLastError();
     }
@@ -98,7 +101,7 @@ static int abf_blocks_per_sm() {
 }
 
 bool psg_abf_step_supported(const psg_ctx* c) {
-    return c->method == PSG_METHOD_ABF && c->sys.n_ranges == 0 && c->d_gbar != nullptr && abf_blocks_per_sm() >= 1;
+    return c->method == PSG_METHOD_ABF && c->sys.n_ranges == 0 && c->d_gbar != nullptr && abf_blocks_per_sm(c->device) >= 1;
 }
 
 // grid[b] += delta[b] for every bin (the all-reduced contribution of one step, psg_abf_apply_grid_delta)
@@ -142,7 +145,7 @@ cudaError_t psg_launch_abf_step(psg_ctx* c, const float* d_pos, const float* d_f
     A.pos = d_pos; A.fsample = d_fsample; A.force = d_force;
     A.xi_out = c->d_xi; A.bin_out = c->d_bin; A.dV_out = c->d_dVdxi; A.jac = c->d_jac; A.bar = c->d_gbar; A.phase = 0;
     long long grid = (P.R + 7) / 8;
-    const long long cap = (long long)c->sm_count * abf_blocks_per_sm();
+    const long long cap = (long long)c->sm_count * abf_blocks_per_sm(c->device);
     if (grid > cap) grid = cap;
     cudaLaunchConfig_t cfg{};
     cfg.gridDim = dim3((unsigned)grid); cfg.blockDim = dim3(256); cfg.dynamicSmemBytes = 0; cfg.stream = c->stream;

@@ -7,9 +7,17 @@
 #include <new>
 #include <vector>
 
+#include <nvtx3/nvToolsExt.h>
+
 #include "internal.h"
 
 static thread_local std::string g_create_err;
+
+// NVTX range around a hot-path call: visible in Nsight Systems timelines, a few ns when no tool listens
+struct NvtxRange {
+    explicit NvtxRange(const char* name) { nvtxRangePushA(name); }
+    ~NvtxRange() { nvtxRangePop(); }
+};
 
 #define CK(ctx, expr)                                                                  \
     do {                                                                               \
@@ -112,6 +120,14 @@ int psg_destroy(psg_ctx* c) {
     return PSG_OK;
 }
 
+int psg_set_tuning(psg_ctx* c, int range_step_lag, int disable_range_step) {
+    if (!c) return PSG_EINVAL;
+    if (range_step_lag < 0 || range_step_lag > 1024) return fail(c, PSG_EINVAL, "psg_set_tuning: 0 <= range_step_lag <= 1024");
+    c->range_lag = range_step_lag > 0 ? range_step_lag : 10;
+    c->range_step_off = disable_range_step != 0;
+    return PSG_OK;
+}
+
 int psg_set_stream(psg_ctx* c, void* s) {
     if (!c) return PSG_EINVAL;
     c->stream = (cudaStream_t)s;
@@ -133,6 +149,10 @@ int psg_set_layout(psg_ctx* c, int R, long long N, long long rstride, int ps, in
     memset(&P, 0, sizeof(P));
     P.R = R; P.N = N; P.rstride = rstride; P.ps = ps; P.fs = fs;
     c->have_layout = true; c->have_cvs = false; c->have_jac = false; c->method = PSG_METHOD_NONE;
+    // state sized by the old layout must not survive it: the grid-stored bias and the interface CV hold R, strides and
+    // per-replica buffers (their *_set calls come after psg_set_layout); the host-engine staging buffers are re-sized on demand
+    psg_interface_cv_free(c);
+    psg_metad_grid_free(c);
     return PSG_OK;
 }
 
@@ -419,6 +439,7 @@ int psg_abf_state(psg_ctx* c, int** h, float** f, long long* nb) {
 // ---------------------------------------------------------------------------- hot path
 int psg_cv_eval(psg_ctx* c, const float* d_pos, float* d_xi, float* d_jac) {
     if (!c) return PSG_EINVAL;
+    NvtxRange nvtx_("psg_cv_eval");
     if (!c->have_cvs) return fail(c, PSG_ESTATE, "psg_cv_eval: no CVs configured");
     if (!d_pos || !d_xi) return fail(c, PSG_EINVAL, "psg_cv_eval: NULL pointer");
     CK(c, psg_launch_cv_eval(c, d_pos, d_xi, d_jac));
@@ -428,15 +449,19 @@ int psg_cv_eval(psg_ctx* c, const float* d_pos, float* d_xi, float* d_jac) {
 
 int psg_bias_eval(psg_ctx* c, const float* d_xi, float* d_V, float* d_dVdxi) {
     if (!c) return PSG_EINVAL;
+    NvtxRange nvtx_("psg_bias_eval");
     if (!d_xi || !d_dVdxi) return fail(c, PSG_EINVAL, "psg_bias_eval: NULL pointer");
     if (c->method == PSG_METHOD_HARMONIC) CK(c, psg_launch_harmonic(c, d_xi, d_V, d_dVdxi));
     else if (c->method == PSG_METHOD_METAD) CK(c, psg_launch_hillsum(c, d_xi, d_V, d_dVdxi));
+    else if (c->method == PSG_METHOD_METAD_GRID) return psg_metad_grid_eval(c, d_xi, d_V, d_dVdxi);
     else return fail(c, PSG_ESTATE, "psg_bias_eval: select harmonic or metadynamics first (ABF uses psg_abf_update)");
     return PSG_OK;
 }
 
 int psg_deposit_hill(psg_ctx* c, const float* d_xi, const unsigned char* d_mask) {
     if (!c) return PSG_EINVAL;
+    NvtxRange nvtx_("psg_deposit_hill");
+    if (c->method == PSG_METHOD_METAD_GRID) return psg_metad_grid_deposit(c, d_xi, d_mask);
     if (c->method != PSG_METHOD_METAD) return fail(c, PSG_ESTATE, "psg_deposit_hill: metadynamics is not selected");
     if (!d_xi) return fail(c, PSG_EINVAL, "psg_deposit_hill: NULL pointer");
     int rc = deposit_admit(c, c->sys.R, d_mask != nullptr, "psg_deposit_hill: hill store would overflow (count + R > capacity); nothing launched");
@@ -448,6 +473,7 @@ int psg_deposit_hill(psg_ctx* c, const float* d_xi, const unsigned char* d_mask)
 
 int psg_abf_update(psg_ctx* c, const float* d_xi, const float* d_fsample, int* d_bin, float* d_dVdxi) {
     if (!c) return PSG_EINVAL;
+    NvtxRange nvtx_("psg_abf_update");
     if (c->method != PSG_METHOD_ABF) return fail(c, PSG_ESTATE, "psg_abf_update: ABF is not selected");
     if (!d_xi || !d_fsample || !d_dVdxi) return fail(c, PSG_EINVAL, "psg_abf_update: NULL pointer");
     CK(c, psg_launch_abf(c, d_xi, d_fsample, d_bin, d_dVdxi));
@@ -530,6 +556,7 @@ int psg_append_hills(psg_ctx* c, int n, const float* d_centers, const float* d_h
 
 int psg_apply_bias_forces(psg_ctx* c, const float* d_pos, const float* d_dVdxi, float* d_force) {
     if (!c) return PSG_EINVAL;
+    NvtxRange nvtx_("psg_apply_bias_forces");
     if (!c->have_jac) return fail(c, PSG_ESTATE, "psg_apply_bias_forces: no cached Jacobian; call psg_cv_eval on these positions first");
     if (!d_pos || !d_dVdxi || !d_force) return fail(c, PSG_EINVAL, "psg_apply_bias_forces: NULL pointer");
     CK(c, psg_launch_apply(c, d_pos, d_dVdxi, d_force));
@@ -538,6 +565,7 @@ int psg_apply_bias_forces(psg_ctx* c, const float* d_pos, const float* d_dVdxi, 
 
 int psg_step(psg_ctx* c, const float* d_pos, float* d_force, const float* d_fsample, long long step) {
     if (!c) return PSG_EINVAL;
+    NvtxRange nvtx_("psg_step");
     if (!c->have_cvs || c->method == PSG_METHOD_NONE) return fail(c, PSG_ESTATE, "psg_step: configure CVs and a method first");
     if (!d_pos || !d_force) return fail(c, PSG_EINVAL, "psg_step: NULL pointer");
     if (c->method == PSG_METHOD_ABF && !d_fsample) return fail(c, PSG_EINVAL, "psg_step: ABF needs d_fsample");
@@ -558,6 +586,15 @@ int psg_step(psg_ctx* c, const float* d_pos, float* d_force, const float* d_fsam
         }
         CK(c, psg_launch_cv_eval(c, d_pos, c->d_xi, nullptr));
         CK(c, psg_launch_hillsum(c, c->d_xi, c->d_V, c->d_dVdxi));
+    } else if (c->method == PSG_METHOD_METAD_GRID) {
+        // xi -> deposit onto the grid (heights from the grid BEFORE the event) -> interpolated bias of the new grid -> forces
+        if (c->mgrid_stride > 0 && step > 0 && step % c->mgrid_stride == 0) {
+            CK(c, psg_launch_cv_eval(c, d_pos, c->d_xi, nullptr));
+            int rc = psg_metad_grid_deposit(c, c->d_xi, nullptr);
+            if (rc != PSG_OK) return rc;
+        }
+        c->have_jac = false;
+        return psg_metad_grid_step(c, d_pos, d_force);
     } else if (c->method == PSG_METHOD_HARMONIC) {
         if (psg_range_step_supported(c, d_pos, d_force)) {
             CK(c, psg_launch_range_step(c, d_pos, d_force));   // large contiguous groups: one persistent launch
@@ -592,6 +629,7 @@ int psg_step_outputs(psg_ctx* c, float** xi, float** V, float** dV, int** bin) {
 
 int psg_step_host(psg_ctx* c, const float* h_pos, float* h_force, const float* h_fsample, long long step) {
     if (!c) return PSG_EINVAL;
+    NvtxRange nvtx_("psg_step_host");
     if (!c->have_cvs || c->method == PSG_METHOD_NONE) return fail(c, PSG_ESTATE, "psg_step_host: configure CVs and a method first");
     if (!h_pos || !h_force) return fail(c, PSG_EINVAL, "psg_step_host: NULL pointer");
     if (c->method == PSG_METHOD_ABF && !h_fsample) return fail(c, PSG_EINVAL, "psg_step_host: ABF needs h_fsample");
@@ -601,13 +639,13 @@ int psg_step_host(psg_ctx* c, const float* h_pos, float* h_force, const float* h
     size_t atoms = P.rstride == 0 ? (size_t)P.N : (size_t)(P.R - 1) * P.rstride + P.N;
     (void)n_arr;
     size_t pb = atoms * P.ps * sizeof(float), fb = atoms * P.fs * sizeof(float);
-    if (!c->d_pos_stage) CK(c, dalloc(c->d_pos_stage, atoms * P.ps));
-    if (!c->d_frc_stage) CK(c, dalloc(c->d_frc_stage, atoms * P.fs));
+    if (c->n_pos_stage < atoms * P.ps) { CK(c, dalloc(c->d_pos_stage, atoms * P.ps)); c->n_pos_stage = atoms * P.ps; }
+    if (c->n_frc_stage < atoms * P.fs) { CK(c, dalloc(c->d_frc_stage, atoms * P.fs)); c->n_frc_stage = atoms * P.fs; }
     CK(c, cudaMemcpyAsync(c->d_pos_stage, h_pos, pb, cudaMemcpyHostToDevice, c->stream));
     CK(c, cudaMemcpyAsync(c->d_frc_stage, h_force, fb, cudaMemcpyHostToDevice, c->stream));
     const float* fsd = nullptr;
     if (c->method == PSG_METHOD_ABF) {
-        if (!c->d_fs_stage) CK(c, dalloc(c->d_fs_stage, (size_t)P.R * P.n_cv));
+        if (c->n_fs_stage < (size_t)P.R * P.n_cv) { CK(c, dalloc(c->d_fs_stage, (size_t)P.R * P.n_cv)); c->n_fs_stage = (size_t)P.R * P.n_cv; }
         CK(c, cudaMemcpyAsync(c->d_fs_stage, h_fsample, (size_t)P.R * P.n_cv * sizeof(float), cudaMemcpyHostToDevice, c->stream));
         fsd = c->d_fs_stage;
     }

@@ -5,11 +5,12 @@
 template <int NCV, int PM, int NEQ, bool F64>
 static cudaError_t launch_k(psg_ctx* c, const HillKernelArgs& A, size_t smem, int grid) {
     auto kern = k_hills<NCV, PM, NEQ, F64>;
-    static size_t attr_bytes = 0;
-    if (smem > attr_bytes) {
+    static size_t attr_bytes[PSG_MAX_DEVICES] = {};   // function attributes are per device: one process may hold ctxs on several
+    size_t& have = attr_bytes[c->device % PSG_MAX_DEVICES];
+    if (smem > have) {
         cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
         if (e != cudaSuccess) return e;
-        attr_bytes = smem;
+        have = smem;
     }
     kern<<<grid, HWARPS * 32, smem, c->stream>>>(c->sys, c->md.hc, A);
     c->launches++;

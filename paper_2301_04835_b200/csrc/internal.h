@@ -8,6 +8,7 @@
 #include "psg.h"
 
 #define PSG_MAX_GROUPS_TOTAL (PSG_MAX_CV * PSG_MAX_GROUPS)
+#define PSG_MAX_DEVICES 64        // per-device caches of function attributes / occupancy (device ordinal modulo this)
 #define PSG_GDESC_DOUBLES 8      // per (replica, group): vx vy vz | cx cy cz | coef | W
 #define PSG_MOM 5                // moments per range group: W, sum w x, sum w y, sum w z, sum w |r|^2
 #define PSG_RANGE_TILE 2048      // atoms per block / slice in the range-moment, dense-apply and fused range-step kernels
@@ -127,9 +128,13 @@ struct psg_ctx {
     bool abf_delta_pending = false;  // psg_abf_accumulate_delta has run, psg_abf_apply_grid_delta has not
     // host-engine staging (psg_step_host)
     float* d_pos_stage = nullptr; float* d_frc_stage = nullptr; float* d_fs_stage = nullptr;
+    size_t n_pos_stage = 0, n_frc_stage = 0, n_fs_stage = 0;   // their sizes in floats (grown on demand: the layout may change)
+    int range_lag = 10;              // items the position producer of k_range_step may run ahead of the force group
+    bool range_step_off = false;     // psg_set_tuning: take the separate kernels instead of k_range_step
     int sm_count = 148;
     void* dti = nullptr;             // state of the DistanceToInterface CV (interface_cv.cu)
     void* mgrid = nullptr;           // state of grid-stored metadynamics (metad_grid.cu)
+    int mgrid_stride = 0;            // PSG_METHOD_METAD_GRID: psg_step deposits when step % stride == 0
 };
 void psg_interface_cv_free(psg_ctx* c);
 void psg_metad_grid_free(psg_ctx* c);

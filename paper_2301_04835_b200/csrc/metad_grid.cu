@@ -7,6 +7,8 @@
 // The node array is [nodes][1 + n_cv] binary64, row-major with the last CV fastest; all arithmetic is binary64: a node sums
 // thousands of deposits over a run and every later bias value is a difference-free read of it, so the store is where
 // precision matters, and the deposit runs once per `stride` steps, not per step.  Shares nothing with oracle/.
+#include <math.h>
+
 #include "geom.cuh"
 
 #define GRID_TILE 128
@@ -273,6 +275,30 @@ extern "C" int psg_metad_grid_step(psg_ctx* c, const float* d_pos, float* d_forc
     k_grid_step<<<(P.R + 7) / 8, 256, 0, c->stream>>>(P, S->G, S->grid, d_pos, d_force, c->d_xi, c->d_V, c->d_dVdxi);
     c->launches += 1;
     if (cudaGetLastError() != cudaSuccess) { c->err = "psg_metad_grid_step: launch failed"; return PSG_ECUDA; }
+    return PSG_OK;
+}
+
+extern "C" int psg_set_metad_grid(psg_ctx* c, const double* lower, const double* upper, const int* shape, const int* periodic,
+                                  const double* sigma, double w0, double kB_deltaT, int stride) {
+    if (!c) return PSG_EINVAL;
+    if (!c->have_cvs) { c->err = "psg_set_metad_grid: call psg_set_cvs first"; return PSG_ESTATE; }
+    if (!lower || !upper || !shape || !periodic || !sigma || stride < 0) { c->err = "psg_set_metad_grid: bad argument"; return PSG_EINVAL; }
+    for (int k = 0; k < c->sys.n_cv; ++k) {
+        const double per = c->sys.cv[k].period;
+        if (per > 0.0) {
+            if (!periodic[k] || fabs((upper[k] - lower[k]) - per) > 1e-9 * per) {
+                c->err = "psg_set_metad_grid: a periodic CV needs a periodic grid spanning exactly its period";
+                return PSG_EINVAL;
+            }
+        } else if (periodic[k]) {
+            c->err = "psg_set_metad_grid: a periodic grid on a CV that is not periodic";
+            return PSG_EINVAL;
+        }
+    }
+    int rc = psg_metad_grid_set(c, c->sys.n_cv, lower, upper, shape, periodic, sigma, w0, kB_deltaT);
+    if (rc != PSG_OK) return rc;
+    c->mgrid_stride = stride;
+    c->method = PSG_METHOD_METAD_GRID;
     return PSG_OK;
 }
 

@@ -26,8 +26,6 @@
 // grid is co-resident and a window has at most `grid` slices: the kernel is launched cooperatively (the launch
 // fails instead of hanging).  Results are bitwise reproducible and equal to the unfused calls: fixed
 // thread -> atom map, fixed reduction order, one writer per atom.
-#include <stdlib.h>
-
 #include "geom.cuh"
 
 #define RS_SLICE PSG_RANGE_TILE   // atoms per slice (2048): 32 KB of float4 per array and stage
@@ -622,9 +620,12 @@ __global__ void __launch_bounds__(RS_THREADS, 1) k_range_step(const __grid_const
 static const size_t kRsSmem = (size_t)(RS_ASTAGES + 2 * RS_BSTAGES) * RS_SLICE * 16 + sizeof(RsShared);
 
 // co-resident CTAs per SM (0 if the kernel cannot be configured)
-static int rs_blocks_per_sm() {
-    static int n = -1;
-    if (n < 0) {
+static int rs_blocks_per_sm(int device) {
+    static int cache[PSG_MAX_DEVICES];
+    static bool have[PSG_MAX_DEVICES] = {};
+    int& n = cache[device % PSG_MAX_DEVICES];
+    if (!have[device % PSG_MAX_DEVICES]) {
+        have[device % PSG_MAX_DEVICES] = true;
         n = 0;
         if (cudaFuncSetAttribute(k_range_step, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kRsSmem) == cudaSuccess) {
             if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n, k_range_step, RS_THREADS, kRsSmem) != cudaSuccess) n = 0;
@@ -640,18 +641,17 @@ static int rs_blocks_per_sm() {
 // separate kernels of cv.cu / bias.cu.
 bool psg_range_step_supported(const psg_ctx* c, const float* d_pos, const float* d_force) {
     const SysParams& P = c->sys;
-    static const bool disabled = getenv("PSG_DISABLE_RANGE_STEP") != nullptr;   // profiling aid: take the separate kernels
-    if (disabled) return false;
+    if (c->range_step_off) return false;   // psg_set_tuning: take the separate kernels
     if (!(c->method == PSG_METHOD_HARMONIC && P.n_ranges > 0 && P.n_slots == 0 && P.ps == 4 && P.fs == 4 && P.rstride > 0 &&
           ((reinterpret_cast<uintptr_t>(d_pos) | reinterpret_cast<uintptr_t>(d_force)) & 15u) == 0 &&
           c->d_arrive != nullptr))
         return false;
-    const long long grid = (long long)c->sm_count * rs_blocks_per_sm();
+    const long long grid = (long long)c->sm_count * rs_blocks_per_sm(c->device);
     return grid >= 1 && P.range_blocks <= grid;
 }
 
 cudaError_t psg_launch_range_step(psg_ctx* c, const float* d_pos, float* d_force) {
-    const int max_blocks_per_sm = rs_blocks_per_sm();
+    const int max_blocks_per_sm = rs_blocks_per_sm(c->device);
     if (max_blocks_per_sm < 1) return cudaErrorLaunchOutOfResources;
     const SysParams& P = c->sys;
     RangeStepArgs A{};
@@ -660,8 +660,7 @@ cudaError_t psg_launch_range_step(psg_ctx* c, const float* d_pos, float* d_force
     A.rpart = c->d_rpart; A.arrive = c->d_arrive; A.done = c->d_arrive + P.R; A.desc = c->d_rdesc;
     // B runs `lag` items behind A: long enough to cover the window dependency (several L2 round trips), short
     // enough that lag x grid x 32 KB of positions stays in L2 (10 x 148 x 32 KB = 47 MB of 126 MB; measured optimum)
-    static const int lag_env = getenv("PSG_RANGE_LAG") ? atoi(getenv("PSG_RANGE_LAG")) : 0;
-    A.lag = lag_env > 0 ? lag_env : 10;
+    A.lag = c->range_lag > 0 ? c->range_lag : 10;
 #ifdef PSG_TRACE
     A.trace = psg_trace_buffer();
 #endif

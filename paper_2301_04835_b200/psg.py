@@ -14,7 +14,7 @@ _LIB_PATH = os.path.join(_HERE, "libpsg.so")
 
 CV_DISTANCE, CV_ANGLE, CV_DIHEDRAL, CV_COM_COMPONENT, CV_RGYR, CV_DISPLACEMENT = 1, 2, 3, 4, 5, 6
 CV_PRINCIPAL_MOMENT, CV_ASPHERICITY, CV_ACYLINDRICITY, CV_SHAPE_ANISOTROPY = 7, 8, 9, 10
-METHOD_NONE, METHOD_HARMONIC, METHOD_METAD, METHOD_ABF = 0, 1, 2, 3
+METHOD_NONE, METHOD_HARMONIC, METHOD_METAD, METHOD_ABF, METHOD_METAD_GRID = 0, 1, 2, 3, 4
 HILLS_F32, HILLS_F64 = 0, 1
 _KIND = {"distance": CV_DISTANCE, "angle": CV_ANGLE, "dihedral": CV_DIHEDRAL, "component": CV_COM_COMPONENT,
          "rgyr": CV_RGYR, "displacement": CV_DISPLACEMENT, "principal_moment": CV_PRINCIPAL_MOMENT,
@@ -25,8 +25,8 @@ EXPORTS = ["psg_create", "psg_destroy", "psg_set_stream", "psg_last_error", "psg
            "psg_set_box", "psg_set_harmonic", "psg_set_metad", "psg_set_hill_precision", "psg_load_hills", "psg_get_hills",
            "psg_set_abf", "psg_abf_state", "psg_cv_eval", "psg_bias_eval", "psg_deposit_hill", "psg_abf_update",
            "psg_abf_accumulate_delta", "psg_abf_apply_grid_delta", "psg_abf_estimate", "psg_abf_estimate_reset", "psg_apply_bias_forces", "psg_step", "psg_step_outputs", "psg_step_host", "psg_sync_check",
-           "psg_interface_cv_set", "psg_interface_cv_eval", "psg_interface_cv_apply", "psg_hill_heights", "psg_append_hills", "psg_metad_grid_set",
-           "psg_metad_grid_deposit", "psg_metad_grid_eval", "psg_metad_grid_step", "psg_metad_grid_state", "psg_measure_alu_peak", "psg_launch_count"]
+           "psg_interface_cv_set", "psg_interface_cv_eval", "psg_interface_cv_apply", "psg_hill_heights", "psg_append_hills", "psg_set_metad_grid", "psg_metad_grid_set",
+           "psg_metad_grid_deposit", "psg_metad_grid_eval", "psg_metad_grid_step", "psg_metad_grid_state", "psg_measure_alu_peak", "psg_launch_count", "psg_set_tuning"]
 
 
 class PsgError(RuntimeError):
@@ -95,11 +95,13 @@ def load_library():
         L.psg_hill_heights.argtypes = [vp, vp, vp, vp]
         L.psg_append_hills.argtypes = [vp, i, vp, vp]
         L.psg_metad_grid_set.argtypes = [vp, i, vp, vp, vp, vp, vp, d, d]
+        L.psg_set_metad_grid.argtypes = [vp, vp, vp, vp, vp, vp, d, d, i]
         L.psg_metad_grid_deposit.argtypes = [vp, vp, vp]
         L.psg_metad_grid_eval.argtypes = [vp, vp, vp, vp]
         L.psg_metad_grid_state.argtypes = [vp, vp, vp, vp]
         L.psg_metad_grid_step.argtypes = [vp, vp, vp]
         L.psg_measure_alu_peak.argtypes = [i, i, C.POINTER(C.c_double)]
+        L.psg_set_tuning.argtypes = [vp, i, i]
         _lib = L
     return _lib
 
@@ -355,6 +357,15 @@ class Context:
         k5, p5 = _hp(np.asarray(sigma), np.float64)
         self._ck(self._L.psg_metad_grid_set(self._h, len(k3), p1, p2, p3, p4, p5, float(w0), float(kB_deltaT)))
 
+    def set_metad_grid(self, lower, upper, shape, periodic, sigma, w0, kB_deltaT=0.0, stride=0):
+        """the grid-stored bias as the ctx's method: psg_step then deposits every `stride` steps and interpolates"""
+        k1, p1 = _hp(np.asarray(lower), np.float64)
+        k2, p2 = _hp(np.asarray(upper), np.float64)
+        k3, p3 = _hp(np.asarray(shape), np.int32)
+        k4, p4 = _hp(np.asarray(periodic), np.int32)
+        k5, p5 = _hp(np.asarray(sigma), np.float64)
+        self._ck(self._L.psg_set_metad_grid(self._h, p1, p2, p3, p4, p5, float(w0), float(kB_deltaT), int(stride)))
+
     def metad_grid_deposit(self, d_xi, d_mask=None):
         t = self._torch
         self._ck(self._L.psg_metad_grid_deposit(self._h, _dp(d_xi, t.float32), _dp(d_mask, t.uint8)))
@@ -372,6 +383,9 @@ class Context:
         g, n, h = C.c_void_p(), C.c_longlong(), C.c_void_p()
         self._ck(self._L.psg_metad_grid_state(self._h, C.byref(g), C.byref(n), C.byref(h)))
         return g.value, n.value, h.value
+
+    def set_tuning(self, range_step_lag=0, disable_range_step=False):
+        self._ck(self._L.psg_set_tuning(self._h, int(range_step_lag), int(bool(disable_range_step))))
 
     def sync_check(self):
         self._ck(self._L.psg_sync_check(self._h))

@@ -1302,6 +1302,99 @@ def test_metad_grid_drives_the_force_scatter(torch, psg):
     ctx.close()
 
 
+def test_metad_grid_as_the_method_of_psg_step(torch, psg):
+    """PSG_METHOD_METAD_GRID (PAPER.md:L151 + the deposit interval of L147): psg_step deposits onto the grid every `stride`
+    steps (well-tempered heights from the grid BEFORE the event) and interpolates; every step against the oracle's grid,
+    the node array after the last event, psg_step_host, psg_bias_eval / psg_deposit_hill routed to the grid, and the
+    refusal of a grid whose periodicity does not match the CVs"""
+    from paper_2301_04835_b200.psg import _view
+    w = small(1, stride=0)
+    sysm = oracle_system(w)
+    lower, upper, shape, periodic, sigma = (-math.pi, -math.pi), (math.pi, math.pi), (72, 60), (1, 1), (0.35, 0.35)
+    w0, kT, stride = 1.2, w.params["kB_deltaT"], 3
+    ctx = make_ctx(psg, w, with_method=False)
+    with pytest.raises(psg.PsgError):          # dihedrals on an open grid
+        ctx.set_metad_grid(lower, upper, shape, (0, 1), sigma, w0, kT, stride)
+    with pytest.raises(psg.PsgError):          # a periodic grid that does not span the period
+        ctx.set_metad_grid((-3.0, -math.pi), upper, shape, periodic, sigma, w0, kT, stride)
+    ctx.set_metad_grid(lower, upper, shape, periodic, sigma, w0, kT, stride)
+    g = orc.MetadGrid(lower, upper, shape, periodic)
+    f0 = w.forces0()
+    d_f = dev(torch, f0)
+    n_events = 0
+    for step in range(1, 8):
+        pos = w.positions(step % w.K)
+        f_before = d_f.cpu().numpy()
+        n0 = ctx.launch_count()
+        ctx.step(dev(torch, pos), d_f, None, step)
+        ctx.sync_check()
+        xi_ref = sysm.cv_eval(pos, want_jac=False)
+        out = {k: v.cpu().numpy() for k, v in ctx.read_step_outputs().items()}
+        assert_close(out["xi"], xi_ref, "xi", period=w.period)
+        if step % stride == 0:
+            h = g.deposit(out["xi"], np.array(sigma), w0, kT)      # at the SAME binary32 xi (reading R-XI32)
+            n_events += 1
+            assert ctx.launch_count() - n0 == 4                   # k_cv_eval, heights + node update, the one-launch step
+            assert h.min() < w0 or n_events == 1
+        else:
+            assert ctx.launch_count() - n0 == 1
+        V, dV = g.eval(out["xi"].astype(np.float64))
+        assert_close(out["V"], V, f"grid V, step {step}")
+        assert_close(out["dVdxi"], dV, f"grid dV/dxi, step {step}")
+        f_ref = sysm.apply_forces(pos, dV, f_before[..., :3].astype(np.float64))
+        assert_forces_close(d_f.cpu().numpy()[..., :3], f_ref, f_before[..., :3], f"grid forces, step {step}")
+    assert n_events == 2
+    gp, nodes, _ = ctx.metad_grid_state()
+    vals = _view(gp, (nodes, 3), torch.float64, 0).cpu().numpy()
+    assert nodes == g.nodes and np.abs(vals - g.values).max() <= 1e-12 * max(1.0, np.abs(g.values).max())
+    # the calls of the boundary follow the method
+    xi = dev(torch, W.random_xi(w, 5))
+    d_V, d_dV = torch.empty(w.R, device="cuda"), torch.empty((w.R, 2), device="cuda")
+    ctx.bias_eval(xi, d_V, d_dV)
+    ctx.sync_check()
+    V, dV = g.eval(xi.cpu().numpy().astype(np.float64))
+    assert_close(d_V.cpu().numpy(), V, "psg_bias_eval on the grid")
+    ctx.deposit_hill(xi)
+    ctx.sync_check()
+    g.deposit(xi.cpu().numpy(), np.array(sigma), w0, kT)
+    vals = _view(gp, (nodes, 3), torch.float64, 0).cpu().numpy()
+    assert np.abs(vals - g.values).max() <= 1e-12 * max(1.0, np.abs(g.values).max())
+    # host-array step (a non-deposit step)
+    pos = w.positions(0)
+    h_f = f0.copy()
+    ctx.step_host(torch.from_numpy(pos), torch.from_numpy(h_f), None, 1)
+    _, dV = g.eval(sysm.cv_eval(pos, want_jac=False).astype(np.float32).astype(np.float64))
+    f_ref = sysm.apply_forces(pos, dV, f0[..., :3].astype(np.float64))
+    assert_forces_close(h_f[..., :3], f_ref, f0[..., :3], "grid forces through psg_step_host")
+    # a new layout drops the grid (it is sized by the old one)
+    ctx.set_layout(w.R + 1, w.N, w.N, 4, 4)
+    with pytest.raises(psg.PsgError):
+        ctx.metad_grid_state()
+    ctx.close()
+
+
+def test_relayout_grows_the_host_staging_buffers(torch, psg):
+    """psg_step_host after psg_set_layout to a LARGER system must not reuse staging buffers sized for the old one"""
+    outs = []
+    for R in (3, 40):
+        w = W.make(1, R=R, n_hills=90, steps=2, stride=0)
+        if not outs:
+            ctx = make_ctx(psg, w)
+        else:
+            psg.configure_from_workload(ctx, w)          # the same ctx, re-laid out
+        heights = oracle_heights(w)
+        ctx.load_hills(dev(torch, w.params["hill_centers"]), dev(torch, heights))
+        pos, f0 = w.positions(0), w.forces0()
+        h_f = f0.copy()
+        ctx.step_host(torch.from_numpy(pos), torch.from_numpy(h_f), None, 1)
+        d_f = dev(torch, f0)
+        ctx.step(dev(torch, pos), d_f, None, 1)
+        ctx.sync_check()
+        assert np.array_equal(h_f.view(np.uint32), d_f.cpu().numpy().view(np.uint32))
+        outs.append(R)
+    ctx.close()
+
+
 def test_metad_grid_step_other_cv_kinds(torch, psg):
     """the one-launch grid step on CVs whose per-atom Jacobian needs r_i - c (Rg, shape anisotropy: the k_hills step cannot
     take these) and, through the three-launch route, on CVs over atom ranges (config 3's windows)"""
