@@ -112,11 +112,12 @@ int psg_set_cvs(psg_ctx* ctx, int n_cv, const psg_cv_desc* cvs, int n_slots, con
 /* Minimum-image convention for periodic POSITIONS (the paper is silent: Fig. 3 and App. A subtract raw coordinates,
  * PAPER.md:L230, L466, reading R-MI).  box [3] (host): orthorhombic box lengths, 0 = open
  * in that direction; NULL or all zeros switches it off (the default after psg_set_layout).  With a box, (i) the atoms of
- * an explicit group are taken as the images nearest to the group's FIRST atom before the barycenter / radius of gyration
+ * a group are taken as the images nearest to the group's FIRST atom before the barycenter / radius of gyration
  * is formed (a molecule split by wrapping is made whole; the group must be smaller than half the box), and (ii) the
  * displacement vectors between group centres in Distance, Angle and Dihedral are nearest images.  Component reads the
- * centre as is.  Explicit groups only: PSG_EINVAL if a CV has a contiguous-range group (large groups are taken as
- * given); call after psg_set_cvs. */
+ * centre as is.  Contiguous-range groups follow the same rule, the first atom being the range's first (a chain wrapped
+ * atom by atom into the box is made whole; psg_step then takes the separate streaming kernels, not k_range_step).
+ * Call after psg_set_cvs. */
 int psg_set_box(psg_ctx* ctx, const double* box);
 
 /* Harmonic bias, PAPER.md:L125 (Sec. 2.1.1): V = 1/2 sum_k k_k (xi_k - xi0_k)^2, differences of periodic

@@ -279,8 +279,6 @@ int psg_set_box(psg_ctx* c, const double* box) {
             if (!(box[x] >= 0.0)) return fail(c, PSG_EINVAL, "psg_set_box: box lengths must be >= 0");
             on |= box[x] > 0.0;
         }
-    if (on && c->sys.n_ranges > 0)
-        return fail(c, PSG_EINVAL, "psg_set_box: the minimum-image convention covers explicit groups only; this ctx has range groups");
     c->sys.has_box = on ? 1 : 0;
     for (int x = 0; x < 3; ++x) c->sys.box[x] = on ? box[x] : 0.0;
     c->have_jac = false;

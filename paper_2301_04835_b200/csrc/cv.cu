@@ -40,7 +40,11 @@ __global__ void __launch_bounds__(PSG_RANGE_THREADS, 4) k_range_moments(const __
         const long long gb = G.rbegin, ge = G.rbegin + G.rsize;
         double m[PSG_MOM] = {0, 0, 0, 0, 0};
         if (t0 < ge && t1 > gb) {   // block-uniform
-            const bool inside = gb <= t0 && t1 <= ge;
+            // minimum image (psg_set_box, reading R-MI): the group's atoms are the images nearest to its FIRST atom, so
+            // the moments depend on the group and a block's sums cannot be shared between groups
+            const bool inside = gb <= t0 && t1 <= ge && !P.has_box;
+            D3 first = d3(0, 0, 0);
+            if (P.has_box) first = load_pos(p, gb, P.ps);
             if (inside && have_full) {
 #pragma unroll
                 for (int i = 0; i < PSG_MOM; ++i) m[i] = mf[i];
@@ -52,8 +56,12 @@ __global__ void __launch_bounds__(PSG_RANGE_THREADS, 4) k_range_moments(const __
                     const bool in = a >= gb && a < ge && a < t1;
                     float wf = 0.f;
                     if (in) wf = P.atom_weight ? __ldg(P.atom_weight + a) : 1.f;   // (weights are re-read per group pass: L1/L2 hits)
-                    const double wd = (double)wf, xd = in ? (double)x[i] : 0.0, yd = in ? (double)y[i] : 0.0,
-                                 zd = in ? (double)z[i] : 0.0;
+                    double xd = in ? (double)x[i] : 0.0, yd = in ? (double)y[i] : 0.0, zd = in ? (double)z[i] : 0.0;
+                    if (P.has_box && in) {
+                        const D3 d = min_image(d3(xd - first.x, yd - first.y, zd - first.z), P.box);
+                        xd = first.x + d.x; yd = first.y + d.y; zd = first.z + d.z;
+                    }
+                    const double wd = (double)wf;
                     m[0] += wd; m[1] += wd * xd; m[2] += wd * yd; m[3] += wd * zd;
                     m[4] += wd * (xd * xd + yd * yd + zd * zd);
                 }
@@ -140,6 +148,7 @@ __global__ void __launch_bounds__(256) k_apply_dense(const __grid_constant__ Sys
     __shared__ float s_v[PSG_MAX_RANGE_GROUPS][3], s_chi[PSG_MAX_RANGE_GROUPS][3], s_clo[PSG_MAX_RANGE_GROUPS][3],
         s_k[PSG_MAX_RANGE_GROUPS];
     __shared__ long long s_b[PSG_MAX_RANGE_GROUPS], s_e[PSG_MAX_RANGE_GROUPS];
+    __shared__ double s_first[PSG_MAX_RANGE_GROUPS][3], s_cd[PSG_MAX_RANGE_GROUPS][3];   // minimum image: first atom, centre
     if (tid < P.n_ranges) {
         int gid = P.range_gid[tid];
         const GroupDev& G = P.grp[gid];
@@ -154,6 +163,11 @@ __global__ void __launch_bounds__(256) k_apply_dense(const __grid_constant__ Sys
         }
         s_k[tid] = (float)(dv * d[6]);
         s_b[tid] = G.rbegin; s_e[tid] = G.rbegin + G.rsize;
+        if (P.has_box) {
+            const D3 f0 = load_pos(pos + (long long)r * P.rstride * P.ps, G.rbegin, P.ps);
+            s_first[tid][0] = f0.x; s_first[tid][1] = f0.y; s_first[tid][2] = f0.z;
+            s_cd[tid][0] = d[3]; s_cd[tid][1] = d[4]; s_cd[tid][2] = d[5];
+        }
     }
     __syncthreads();
     const float* p = pos + (long long)r * P.rstride * P.ps;
@@ -178,6 +192,13 @@ __global__ void __launch_bounds__(256) k_apply_dense(const __grid_constant__ Sys
             if (a >= s_b[q] && a < s_e[q]) {
                 any = true;
                 float k = s_k[q];
+                if (P.has_box) {   // r_i = the image nearest to the group's first atom, as in the moments
+                    const D3 d = min_image(d3((double)px - s_first[q][0], (double)py - s_first[q][1], (double)pz - s_first[q][2]), P.box);
+                    ax += s_v[q][0] + k * (float)((s_first[q][0] + d.x) - s_cd[q][0]);
+                    ay += s_v[q][1] + k * (float)((s_first[q][1] + d.y) - s_cd[q][1]);
+                    az += s_v[q][2] + k * (float)((s_first[q][2] + d.z) - s_cd[q][2]);
+                    continue;
+                }
                 ax += s_v[q][0] + k * ((px - s_chi[q][0]) - s_clo[q][0]);
                 ay += s_v[q][1] + k * ((py - s_chi[q][1]) - s_clo[q][1]);
                 az += s_v[q][2] + k * ((pz - s_chi[q][2]) - s_clo[q][2]);

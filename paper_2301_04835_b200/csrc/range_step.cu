@@ -636,13 +636,13 @@ static int rs_blocks_per_sm(int device) {
 }
 
 // The fused step covers: harmonic bias; every group a contiguous range; float4 positions and forces, 16-byte
-// aligned (the position slices are TMA bulk copies); one array per window; windows of at most `grid` slices (so
+// aligned (the position slices are TMA bulk copies); no minimum-image box; one array per window; windows of at most `grid` slices (so
 // that every A a waiting B depends on belongs to the same or the next round of items). Anything else takes the
 // separate kernels of cv.cu / bias.cu.
 bool psg_range_step_supported(const psg_ctx* c, const float* d_pos, const float* d_force) {
     const SysParams& P = c->sys;
     if (c->range_step_off) return false;   // psg_set_tuning: take the separate kernels
-    if (!(c->method == PSG_METHOD_HARMONIC && P.n_ranges > 0 && P.n_slots == 0 && P.ps == 4 && P.fs == 4 && P.rstride > 0 &&
+    if (!(c->method == PSG_METHOD_HARMONIC && !P.has_box && P.n_ranges > 0 && P.n_slots == 0 && P.ps == 4 && P.fs == 4 && P.rstride > 0 &&
           ((reinterpret_cast<uintptr_t>(d_pos) | reinterpret_cast<uintptr_t>(d_force)) & 15u) == 0 &&
           c->d_arrive != nullptr))
         return false;

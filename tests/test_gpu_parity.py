@@ -855,14 +855,53 @@ def test_minimum_image_step_matches_oracle(torch, psg, cfg):
 def test_set_box_validation(torch, psg):
     w = small(3)
     ctx = make_ctx(psg, w)
-    with pytest.raises(psg.PsgError):
-        ctx.set_box((3.0, 3.0, 3.0))          # range groups are taken as given
+    ctx.set_box((30.0, 30.0, 30.0))           # range groups follow the rule of explicit groups (first atom of the range)
     ctx.set_box(None)                          # switching it off is always fine
     w1 = small(1)
     c1 = make_ctx(psg, w1)
     with pytest.raises(psg.PsgError):
         c1.set_box((3.0, -1.0, 3.0))
     c1.set_box((0.0, 0.0, 0.0))
+
+
+def test_minimum_image_range_groups_match_oracle(torch, psg):
+    """SURVEY NEXT-4 "unwrapping large groups": umbrella windows over contiguous-range groups (Rg of the chain, distance of
+    the two halves' centers of mass, mass-weighted) whose atoms were wrapped one by one into a periodic box; the step takes
+    the streaming kernels (k_range_step is for open boundaries) and must match the oracle with the same box"""
+    w = small(3, R=4, N=6007, weighted=True)
+    ext = float(np.ptp(w.positions(0)[..., :3], axis=1).max())
+    L = np.ceil(np.array([2.6, 2.3, 3.0]) * ext)             # every chain spans less than half of the box
+    sysm = orc.System(w.R, w.N, w.N, 4, [{"type": {"rgyr": orc.RGYR, "distance": orc.DISTANCE}[cv["kind"]], "groups": cv["groups"],
+                                          "axis": 0, "period": 0.0} for cv in w.cvs], None, atom_weight=w.atom_weight, box=L)
+    pos = w.positions(0).copy()
+    assert np.ptp(pos[..., :3], axis=1).max() < 0.45 * L.min()
+    unwrapped = pos[..., :3].astype(np.float64) + 0.93 * L          # the chains straddle the upper faces
+    pos[..., :3] = np.mod(unwrapped, L).astype(np.float32)
+    assert (np.abs(pos[..., :3] - unwrapped) > 1).mean() > 0.2        # a good part of every chain is wrapped
+    pos[..., :3] = np.where(pos[..., :3] >= L.astype(np.float32), 0.0, pos[..., :3])
+    f0 = w.forces0()
+    ctx = make_ctx(psg, w)
+    ctx.set_box(L)
+    d_f = dev(torch, f0)
+    n0 = ctx.launch_count()
+    ctx.step(dev(torch, pos), d_f, None, 1)
+    ctx.sync_check()
+    assert ctx.launch_count() - n0 == 4                      # moments, CVs, bias, dense apply
+    out = {k: v.cpu().numpy() for k, v in ctx.read_step_outputs().items()}
+    xi_ref = sysm.cv_eval(pos, want_jac=False)
+    assert_close(out["xi"], xi_ref, "wrapped range groups: xi")
+    b = oracle_bias(w, xi_ref.astype(np.float32))
+    assert_close(out["V"], b["V"], "V")
+    assert_close(out["dVdxi"], b["dVdxi"], "dV/dxi")
+    f_ref = sysm.apply_forces(pos, b["dVdxi"], f0[..., :3].astype(np.float64))
+    assert_forces_close(d_f.cpu().numpy()[..., :3], f_ref, f0[..., :3], "wrapped range groups: forces")
+    assert np.array_equal(d_f.cpu().numpy()[..., 3].view(np.uint32), f0[..., 3].view(np.uint32))
+    # and the torn chain without the box is something else
+    ctx.set_box(None)
+    ctx.step(dev(torch, pos), dev(torch, f0), None, 1)
+    ctx.sync_check()
+    assert np.abs(ctx.read_step_outputs()["xi"].cpu().numpy() - xi_ref).max() > 0.5
+    ctx.close()
 
 
 # ------------------------------------------------------------------------------------ ABF force estimator (SURVEY NEXT-1)

@@ -105,3 +105,33 @@ def test_forces_of_a_wrapped_molecule_have_no_net_force():
     s = _sys(orc.DIHEDRAL, 4, [[0], [1], [2], [3]], BOX)
     f = s.apply_forces(_pos4(xyz)[None], np.array([[7.0]]), np.zeros((1, 4, 3)))
     assert np.abs(f.sum(axis=1)).max() < 1e-9 * np.abs(f).sum()
+
+
+def test_contiguous_range_groups_wrapped_atom_by_atom_are_made_whole():
+    """range groups follow the same rule (images nearest to the range's FIRST atom): a chain whose atoms an engine has
+    wrapped one by one into the box gives the CVs, Jacobians and forces of the unwrapped chain (extent < half the box).
+    Dyadic coordinates and box lengths make every wrap exact in binary32, so the comparison is to rounding error."""
+    rng = np.random.default_rng(12)
+    n, L = 600, (16.0, 32.0, 16.0)
+    steps = rng.integers(-64, 65, size=(n, 3)) / 1024.0                      # a random walk on a dyadic lattice
+    xyz = np.array([15.5, 0.25, 8.0]) + np.cumsum(steps, axis=0)             # starts next to two faces, extent ~ 1.5
+    assert np.ptp(xyz, axis=0).max() < 0.4 * min(L)
+    wrapped = np.mod(xyz, np.array(L))
+    assert (np.abs(wrapped - xyz) > 1).any()                                  # it really crosses faces
+    h = n // 2
+    cvs = [{"type": orc.RGYR, "groups": [("range", 0, n)], "axis": 0, "period": 0.0},
+           {"type": orc.DISTANCE, "groups": [("range", 0, h), ("range", h, n - h)], "axis": 0, "period": 0.0}]
+    aw = rng.uniform(1.0, 4.0, size=n).astype(np.float32)
+    s_box = orc.System(1, n, n, 4, cvs, None, atom_weight=aw, box=L)
+    s_open = orc.System(1, n, n, 4, cvs, None, atom_weight=aw, box=None)
+    xi_w = s_box.cv_eval(_pos4(wrapped)[None], want_jac=False)
+    xi_o = s_open.cv_eval(_pos4(xyz)[None], want_jac=False)
+    assert np.allclose(xi_w, xi_o, rtol=1e-12, atol=1e-12)
+    dV = np.array([[3.0, -2.0]])
+    f_w = s_box.apply_forces(_pos4(wrapped)[None], dV, np.zeros((1, n, 3)))
+    f_o = s_open.apply_forces(_pos4(xyz)[None], dV, np.zeros((1, n, 3)))
+    assert np.allclose(f_w, f_o, rtol=1e-10, atol=1e-12)
+    assert np.abs(f_w.sum(axis=1)).max() < 1e-9 * np.abs(f_w).sum()
+    # without the box the wrapped chain is a different (torn) object
+    xi_torn = s_open.cv_eval(_pos4(wrapped)[None], want_jac=False)
+    assert abs(xi_torn[0, 0] - xi_o[0, 0]) > 1.0
