@@ -20,6 +20,11 @@ extern "C" {
  * else; 2-D periodic / 3-D with 2 periodic CVs): the ceiling of the kernel's instruction mix.
  * 9: empty-kernel nodes/s of a replayed CUDA graph (1 / the launch floor t_floor of SURVEY.md 8(d), the bound of the
  *    latency-bound configs 0 and 2).
+ * 10: binary64 exp() evaluations/s (the library routine on the FP64 pipe): the bound of the grid deposit (k_grid_deposit),
+ *     of the interface CV (k_dti_mass, k_dti_apply) and of the binary64 hill terms (PSG_HILLS_F64).
+ * 11: 1 / t where t = the time two event records bracket when the kernel between them is EMPTY and the stream has just
+ *     flushed L2 with a 256 MiB memset -- the floor of bench.py's per-step timing protocol (about 6 us on B200; an event
+ *     record drains the pipeline on both sides).
  * 100 + n: the same as 7 with only n passes of 1,024 hills (short-run behaviour). */
 int psg_measure_alu_peak(int device, int which, double* ops_per_second_out);
 /* Tuning knobs of the fused large-group step, for measurements: range_step_lag = items the position

@@ -9,6 +9,7 @@
 // Moments of range groups. grid = (range_blocks, R); block b covers atoms [span_begin + b*TILE, +TILE).
 // Every atom is loaded once (coalesced float4) and contributes to each range group that contains it.
 // Output: rpart[r][q][b][5] in binary64 (products of binary32 inputs are exact in binary64).
+template <bool BOX>   // BOX: minimum image on (psg_set_box); a separate instantiation keeps the open-boundary kernel as lean as it was
 __global__ void __launch_bounds__(PSG_RANGE_THREADS, 4) k_range_moments(const __grid_constant__ SysParams P, const float* __restrict__ pos,
                                                         double* __restrict__ rpart) {
     constexpr int NT = PSG_RANGE_THREADS, PER = PSG_RANGE_TILE / NT;
@@ -42,9 +43,9 @@ __global__ void __launch_bounds__(PSG_RANGE_THREADS, 4) k_range_moments(const __
         if (t0 < ge && t1 > gb) {   // block-uniform
             // minimum image (psg_set_box, reading R-MI): the group's atoms are the images nearest to its FIRST atom, so
             // the moments depend on the group and a block's sums cannot be shared between groups
-            const bool inside = gb <= t0 && t1 <= ge && !P.has_box;
+            const bool inside = gb <= t0 && t1 <= ge && !BOX;
             D3 first = d3(0, 0, 0);
-            if (P.has_box) first = load_pos(p, gb, P.ps);
+            if (BOX) first = load_pos(p, gb, P.ps);
             if (inside && have_full) {
 #pragma unroll
                 for (int i = 0; i < PSG_MOM; ++i) m[i] = mf[i];
@@ -57,7 +58,7 @@ __global__ void __launch_bounds__(PSG_RANGE_THREADS, 4) k_range_moments(const __
                     float wf = 0.f;
                     if (in) wf = P.atom_weight ? __ldg(P.atom_weight + a) : 1.f;   // (weights are re-read per group pass: L1/L2 hits)
                     double xd = in ? (double)x[i] : 0.0, yd = in ? (double)y[i] : 0.0, zd = in ? (double)z[i] : 0.0;
-                    if (P.has_box && in) {
+                    if (BOX && in) {
                         const D3 d = min_image(d3(xd - first.x, yd - first.y, zd - first.z), P.box);
                         xd = first.x + d.x; yd = first.y + d.y; zd = first.z + d.z;
                     }
@@ -139,6 +140,7 @@ __global__ void __launch_bounds__(256) k_apply_sparse(const __grid_constant__ Sy
 // Force is read and written once (float4, w preserved bit for bit); positions are read only when an Rg
 // CV needs r_i. Each replica owns its atoms here (no atomics); with a shared array (rstride = 0) several
 // replicas would hit the same atoms, so that case uses atomics.
+template <bool BOX>
 __global__ void __launch_bounds__(256) k_apply_dense(const __grid_constant__ SysParams P, const float* __restrict__ pos,
                                                       const double* __restrict__ gdesc, const float* __restrict__ dVdxi,
                                                       float* __restrict__ force) {
@@ -163,7 +165,7 @@ __global__ void __launch_bounds__(256) k_apply_dense(const __grid_constant__ Sys
         }
         s_k[tid] = (float)(dv * d[6]);
         s_b[tid] = G.rbegin; s_e[tid] = G.rbegin + G.rsize;
-        if (P.has_box) {
+        if (BOX) {
             const D3 f0 = load_pos(pos + (long long)r * P.rstride * P.ps, G.rbegin, P.ps);
             s_first[tid][0] = f0.x; s_first[tid][1] = f0.y; s_first[tid][2] = f0.z;
             s_cd[tid][0] = d[3]; s_cd[tid][1] = d[4]; s_cd[tid][2] = d[5];
@@ -192,7 +194,7 @@ __global__ void __launch_bounds__(256) k_apply_dense(const __grid_constant__ Sys
             if (a >= s_b[q] && a < s_e[q]) {
                 any = true;
                 float k = s_k[q];
-                if (P.has_box) {   // r_i = the image nearest to the group's first atom, as in the moments
+                if (BOX) {   // r_i = the image nearest to the group's first atom, as in the moments
                     const D3 d = min_image(d3((double)px - s_first[q][0], (double)py - s_first[q][1], (double)pz - s_first[q][2]), P.box);
                     ax += s_v[q][0] + k * (float)((s_first[q][0] + d.x) - s_cd[q][0]);
                     ay += s_v[q][1] + k * (float)((s_first[q][1] + d.y) - s_cd[q][1]);
@@ -224,7 +226,8 @@ cudaError_t psg_launch_cv_eval(psg_ctx* c, const float* d_pos, float* d_xi, floa
     const SysParams& P = c->sys;
     if (P.n_ranges > 0) {
         dim3 g(P.range_blocks, P.R);
-        k_range_moments<<<g, PSG_RANGE_THREADS, 0, c->stream>>>(P, d_pos, c->d_rpart);
+        if (P.has_box) k_range_moments<true><<<g, PSG_RANGE_THREADS, 0, c->stream>>>(P, d_pos, c->d_rpart);
+        else k_range_moments<false><<<g, PSG_RANGE_THREADS, 0, c->stream>>>(P, d_pos, c->d_rpart);
         c->launches++;
     }
     k_cv_eval<<<(P.R + 7) / 8, 256, 0, c->stream>>>(P, d_pos, c->d_rpart, d_xi, d_jac, c->d_jac, c->d_gdesc);
@@ -241,7 +244,8 @@ cudaError_t psg_launch_apply(psg_ctx* c, const float* d_pos, const float* d_dVdx
     }
     if (P.n_ranges > 0) {
         dim3 g(P.range_blocks, P.R);
-        k_apply_dense<<<g, 256, 0, c->stream>>>(P, d_pos, c->d_gdesc, d_dVdxi, d_force);
+        if (P.has_box) k_apply_dense<true><<<g, 256, 0, c->stream>>>(P, d_pos, c->d_gdesc, d_dVdxi, d_force);
+        else k_apply_dense<false><<<g, 256, 0, c->stream>>>(P, d_pos, c->d_gdesc, d_dVdxi, d_force);
         c->launches++;
     }
     return cudaGetLastError();

@@ -5,7 +5,8 @@
 // Three kernels, all binary64 (the softmax of DIFFERENCES of nearly equal masses amplifies rounding: binary32 masses
 // put the interface off by ~1e-4 nm, far outside the parity bar; the paper's JAX code runs in binary32):
 //   k_dti_mass   grid (chunks of 1,024 atoms, R): coordinates of the chunk -> shared memory; thread j sums bin j
-//   k_dti_finish block per replica: chunk partials in fixed order, softmax, interface, G_j = d interface / d mass_j, xi
+//   k_dti_finish block per replica: chunk partials in fixed order; softmax, interface and G_j = d interface / d mass_j by the
+//                whole block (fixed-order block reductions); xi
 //   k_dti_apply  grid (chunks, R): thread per atom, F_i[axis] += dV/dxi * sum_j G_j d mass_j / d x_i; mobile atoms too
 // A first version: exp-bound (bins x atoms binary64 exponentials per pass), not tuned.
 #include "internal.h"
@@ -59,25 +60,53 @@ __global__ void __launch_bounds__(128) k_dti_finish(const __grid_constant__ DtiP
         mass[j] = m;
     }
     __syncthreads();
+    // softmax over the nb = bins - 1 bin boundaries, the interface position and its derivative with respect to every bin
+    // mass, by the whole block: maximum, partition sum and interface are block reductions in a fixed order (lanes by an
+    // xor tree, the four warps in sequence), everything else is one bin boundary per thread
+    __shared__ double red[4];
+    __shared__ double bc[3];   // mx, Z, I
+    const int nb = D.bins - 1, lane = tid & 31, wid = tid >> 5;
+    auto block_reduce = [&](double v, bool is_max, int slot) {
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) {
+            const double u = __shfl_xor_sync(0xffffffffu, v, o);
+            v = is_max ? fmax(v, u) : v + u;
+        }
+        if (lane == 0) red[wid] = v;
+        __syncthreads();
+        if (tid == 0) {
+            double t = red[0];
+            for (int w = 1; w < 4; ++w) t = is_max ? fmax(t, red[w]) : t + red[w];
+            bc[slot] = t;
+        }
+        __syncthreads();
+    };
+    double mx = -1e300;
+    for (int j = tid; j < nb; j += 128) {
+        const double v = fabs(mass[j + 1] - mass[j]) * D.coeff;
+        prob[j] = v;
+        mx = fmax(mx, v);
+    }
+    block_reduce(mx, true, 0);
+    double z = 0.0;
+    for (int j = tid; j < nb; j += 128) { prob[j] = exp(prob[j] - bc[0]); z += prob[j]; }
+    block_reduce(z, false, 1);
+    double it = 0.0;
+    for (int j = tid; j < nb; j += 128) {
+        prob[j] /= bc[1];
+        it += prob[j] * 0.5 * (dti_center(D, j + 1) + dti_center(D, j));
+    }
+    block_reduce(it, false, 2);
+    const double I = bc[2];
+    // d interface / d mass_j: boundary j - 1 pulls bin j one way, boundary j the other
+    auto pull = [&](int j) {   // boundary j in [0, nb)
+        const double diff = mass[j + 1] - mass[j];
+        const double sg = diff > 0.0 ? 1.0 : (diff < 0.0 ? -1.0 : 0.0);
+        return D.coeff * sg * prob[j] * (0.5 * (dti_center(D, j + 1) + dti_center(D, j)) - I);
+    };
+    double* g = G + (long long)r * D.bins;
+    for (int j = tid; j < D.bins; j += 128) g[j] = (j >= 1 ? pull(j - 1) : 0.0) - (j < nb ? pull(j) : 0.0);
     if (tid == 0) {
-        const int nb = D.bins - 1;
-        double mx = -1e300, Z = 0.0, I = 0.0;
-        for (int j = 0; j < nb; ++j) {
-            const double v = fabs(mass[j + 1] - mass[j]) * D.coeff;
-            prob[j] = v;
-            if (v > mx) mx = v;
-        }
-        for (int j = 0; j < nb; ++j) { prob[j] = exp(prob[j] - mx); Z += prob[j]; }
-        for (int j = 0; j < nb; ++j) { prob[j] /= Z; I += prob[j] * 0.5 * (dti_center(D, j + 1) + dti_center(D, j)); }
-        double* g = G + (long long)r * D.bins;
-        for (int j = 0; j < D.bins; ++j) g[j] = 0.0;
-        for (int j = 0; j < nb; ++j) {
-            const double diff = mass[j + 1] - mass[j];
-            const double s = diff > 0.0 ? 1.0 : (diff < 0.0 ? -1.0 : 0.0);
-            const double t = D.coeff * s * prob[j] * (0.5 * (dti_center(D, j + 1) + dti_center(D, j)) - I);
-            g[j + 1] += t;
-            g[j] -= t;
-        }
         const float* p = pos + (long long)r * D.rstride * D.ps;
         double W = 0.0, mob = 0.0;
         for (int m = 0; m < D.n_mobile; ++m) {

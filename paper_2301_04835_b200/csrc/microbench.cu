@@ -49,6 +49,9 @@ __global__ void __launch_bounds__(1024) k_peak(float* out, float seed) {
                 asm volatile("cvt.rn.f32.s32 %0, %1;" : "=f"(a[i]) : "r"(q[i]));
                 q[i] = __float_as_int(a[i]);
             }
+        } else if (WHICH == 7) {
+#pragma unroll
+            for (int i = 0; i < CHAINS / 2; ++i) d[i] = exp(d[i] * -0.25);   // the library's binary64 exp, value stays in (0, 1]
         } else if (WHICH == 6) {
 #pragma unroll
             for (int i = 0; i < CHAINS; i += 2)
@@ -195,6 +198,41 @@ static cudaError_t time_launch_floor(double* out) {
     return e;
 }
 
+// The floor of bench.py's own timing protocol: an EMPTY kernel between two event records on a stream, after a 256 MiB
+// memset (the L2 flush): what a per-step event pair measures when the step does nothing.  Median of 30; returns 1 / seconds.
+static cudaError_t time_event_pair_floor(double* out) {
+    cudaStream_t s;
+    cudaError_t e = cudaStreamCreateWithFlags(&s, cudaStreamNonBlocking);
+    if (e != cudaSuccess) return e;
+    void* buf = nullptr;
+    const size_t nbytes = (size_t)256 << 20;
+    e = cudaMalloc(&buf, nbytes);
+    if (e != cudaSuccess) { cudaStreamDestroy(s); return e; }
+    cudaEvent_t t0, t1;
+    cudaEventCreate(&t0);
+    cudaEventCreate(&t1);
+    float ms[30];
+    int n = 0;
+    for (int rep = 0; rep < 33 && e == cudaSuccess; ++rep) {
+        cudaMemsetAsync(buf, rep, nbytes, s);
+        cudaEventRecord(t0, s);
+        k_empty<<<1, 32, 0, s>>>();
+        cudaEventRecord(t1, s);
+        e = cudaStreamSynchronize(s);
+        float t = 0.f;
+        cudaEventElapsedTime(&t, t0, t1);
+        if (rep >= 3) ms[n++] = t;
+    }
+    for (int i = 1; i < n; ++i)
+        for (int j = i; j > 0 && ms[j] < ms[j - 1]; --j) { float t = ms[j]; ms[j] = ms[j - 1]; ms[j - 1] = t; }
+    *out = n > 0 ? 1.0 / (ms[n / 2] * 1e-3) : 0.0;
+    cudaEventDestroy(t0);
+    cudaEventDestroy(t1);
+    cudaFree(buf);
+    cudaStreamDestroy(s);
+    return e;
+}
+
 extern "C" int psg_measure_alu_peak(int device, int which, double* out) {
     if (!out) return PSG_EINVAL;
     if (cudaSetDevice(device) != cudaSuccess) return PSG_ECUDA;
@@ -213,6 +251,8 @@ extern "C" int psg_measure_alu_peak(int device, int which, double* out) {
     case 7: e = time_hill_loop<2, 3, 2>(sms, out); break;      // hill evaluations/s of the bare loop, 2-D periodic (C = 16)
     case 8: e = time_hill_loop<3, 3, 2>(sms, out); break;      // hill evaluations/s of the bare loop, 3-D, 2 periodic (C = 20)
     case 9: e = time_launch_floor(out); break;                 // empty graph nodes/s
+    case 10: e = time_one<7>(sms, CHAINS / 2, out); break;     // binary64 exp() per second
+    case 11: e = time_event_pair_floor(out); break;            // 1 / (event pair around an empty kernel after an L2 flush)
     default:
         if (which >= 100 && which < 200) { e = time_hill_loop<2, 3, 2>(sms, out, which - 100); break; }   // short runs: which - 100 passes
         return PSG_EINVAL;
