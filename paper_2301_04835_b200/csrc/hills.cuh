@@ -261,6 +261,7 @@ template <int NCV>
 __device__ __forceinline__ void accumulate_f64(const float4* __restrict__ sm, const float* __restrict__ W, int n_sub, int off,
                                                const float (&xi)[RT][NCV], const HillConsts& hc, double* __restrict__ wacc, int lane) {
     constexpr int NV = 1 + NCV;
+#pragma unroll   // (static replica indices keep xi in registers; a rolled loop puts it in local memory)
     for (int j0 = 0; j0 < RT; j0 += 2) {
         double a[2][NV];
 #pragma unroll
