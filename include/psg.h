@@ -58,7 +58,14 @@ enum {
     PSG_CV_PRINCIPAL_MOMENT = 7, /* AxisCV PrincipalMoment: l_axis, axis 0 = the largest               (L188) */
     PSG_CV_ASPHERICITY = 8,      /* l1 - (l2 + l3)/2                                                    (L189) */
     PSG_CV_ACYLINDRICITY = 9,    /* l2 - l3                                                             (L189) */
-    PSG_CV_SHAPE_ANISOTROPY = 10 /* ((l1 - (l2+l3)/2)^2 + 3/4 (l2 - l3)^2) / (l1+l2+l3)^2; 0 for a point (L189) */
+    PSG_CV_SHAPE_ANISOTROPY = 10, /* ((l1 - (l2+l3)/2)^2 + 3/4 (l2 - l3)^2) / (l1+l2+l3)^2; 0 for a point (L189) */
+    /* The paper's worked CV (L203-L290, Eq. 4-8; listing of Appendix A): group 0 = the mobile atoms (explicit,
+     * weights = slot_weight), group 1 = the interface atoms (a contiguous range); parameters in psg_cv_desc::dti_*.
+     *   xi = barycenter(group 0)[axis] - sum_j softmax(coeff |mass_{j+1} - mass_j|)_j (c_{j+1} + c_j) / 2,
+     *   mass_j = sum_{i in group 1} exp(-(x_i - c_j)^2 / (2 sigma^2)),  c = linspace(scope[0], scope[1], bins).
+     * At most one per ctx, shared index list; psg_step then runs the separate kernels in sequence (CVs, bias, forces) and
+     * every method (harmonic, metadynamics, grid metadynamics, ABF) applies to it like to any other CV. */
+    PSG_CV_DIST_TO_INTERFACE = 11
 };
 
 enum { PSG_METHOD_NONE = 0, PSG_METHOD_HARMONIC = 1, PSG_METHOD_METAD = 2, PSG_METHOD_ABF = 3, PSG_METHOD_METAD_GRID = 4 };
@@ -76,7 +83,7 @@ enum {
 
 typedef struct {
     int type;                            /* PSG_CV_* */
-    int n_groups;                        /* 2, 3, 4, 1, 1, 2 for the six types */
+    int n_groups;                        /* 2, 3, 4, 1, 1, 2 for the first six types, 1 for the shape CVs, 2 for DistanceToInterface */
     int group_is_range[PSG_MAX_GROUPS];  /* 0: explicit atoms (a slice of the slot list); 1: contiguous atom range */
     int group_begin[PSG_MAX_GROUPS];     /* explicit: slots [begin, begin + size) */
     int group_size[PSG_MAX_GROUPS];
@@ -84,6 +91,9 @@ typedef struct {
     long long range_size[PSG_MAX_GROUPS];
     int axis;                            /* PSG_CV_COM_COMPONENT, PSG_CV_DISPLACEMENT: 0, 1, 2; PSG_CV_PRINCIPAL_MOMENT: which eigenvalue */
     double period;                       /* 0 = not periodic; 2*pi for a dihedral (binary64: the wrap must not lose bits) */
+    /* PSG_CV_DIST_TO_INTERFACE only (Eq. 6-8): kernel width, bin-centre range, number of bins (2..1024), softmax sharpness */
+    double dti_sigma, dti_scope[2], dti_coeff;
+    int dti_bins;
 } psg_cv_desc;
 
 /* ------------------------------------------------------------------ lifetime */
@@ -241,7 +251,8 @@ int psg_sync_check(psg_ctx* ctx);
 
 /* ------------------------------------------------------------- DistanceToInterface */
 /* The paper's own worked collective variable (Eq. 4-8; listing of Appendix A), for all
- * replicas of the ctx layout (psg_set_layout), as a set of calls of its own (it is not a psg_cv_desc type yet):
+ * replicas of the ctx layout (psg_set_layout), as calls of its own (PSG_CV_DIST_TO_INTERFACE configures the same kernels
+ * through psg_set_cvs and puts the CV on the psg_step path; use one or the other on a ctx):
  *   xi = barycenter(mobile atoms)[axis] - sum_j softmax(coeff |mass_{j+1} - mass_j|)_j (c_{j+1} + c_j) / 2,
  *   mass_j = sum_i exp(-(x_i - c_j)^2 / (2 sigma^2)) over the interface atoms, c = linspace(scope0, scope1, bins).
  * psg_interface_cv_set (host arrays copied; allocates): mobile_idx [n_mobile <= PSG_MAX_SLOTS] 0-based, mobile_w nullable

@@ -8,10 +8,10 @@ CUDA device is present, calls raise.
 """
 from .psg import (Context, PsgError, load_library, lib_path, measure_alu_peak, configure_from_workload,
                   CV_DISTANCE, CV_ANGLE, CV_DIHEDRAL, CV_COM_COMPONENT, CV_RGYR, CV_DISPLACEMENT,
-                  CV_PRINCIPAL_MOMENT, CV_ASPHERICITY, CV_ACYLINDRICITY, CV_SHAPE_ANISOTROPY,
+                  CV_PRINCIPAL_MOMENT, CV_ASPHERICITY, CV_ACYLINDRICITY, CV_SHAPE_ANISOTROPY, CV_DIST_TO_INTERFACE,
                   HILLS_F32, HILLS_F64, METHOD_NONE, METHOD_HARMONIC, METHOD_METAD, METHOD_ABF, METHOD_METAD_GRID, EXPORTS)
 
 __all__ = ["Context", "PsgError", "load_library", "lib_path", "measure_alu_peak", "configure_from_workload",
            "CV_DISTANCE", "CV_ANGLE", "CV_DIHEDRAL", "CV_COM_COMPONENT", "CV_RGYR", "CV_DISPLACEMENT", "CV_PRINCIPAL_MOMENT",
-           "CV_ASPHERICITY", "CV_ACYLINDRICITY", "CV_SHAPE_ANISOTROPY", "HILLS_F32", "HILLS_F64",
+           "CV_ASPHERICITY", "CV_ACYLINDRICITY", "CV_SHAPE_ANISOTROPY", "CV_DIST_TO_INTERFACE", "HILLS_F32", "HILLS_F64",
            "METHOD_NONE", "METHOD_HARMONIC", "METHOD_METAD", "METHOD_ABF", "METHOD_METAD_GRID", "EXPORTS"]

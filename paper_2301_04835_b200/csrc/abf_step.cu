@@ -101,7 +101,7 @@ static int abf_blocks_per_sm(int device) {
 }
 
 bool psg_abf_step_supported(const psg_ctx* c) {
-    return c->method == PSG_METHOD_ABF && c->sys.n_ranges == 0 && c->d_gbar != nullptr && abf_blocks_per_sm(c->device) >= 1;
+    return c->method == PSG_METHOD_ABF && c->sys.n_ranges == 0 && c->dti_cv < 0 && c->d_gbar != nullptr && abf_blocks_per_sm(c->device) >= 1;
 }
 
 // grid[b] += delta[b] for every bin (the all-reduced contribution of one step, psg_abf_apply_grid_delta)

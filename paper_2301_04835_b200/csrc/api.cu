@@ -68,7 +68,7 @@ static void deposit_account(psg_ctx* c, long long n, bool masked) {
     if (psg_stream_capturing(c)) { c->count_unknown = true; c->overflow_possible = true; }
 }
 
-static const int kGroups[11] = {0, 2, 3, 4, 1, 1, 2, 1, 1, 1, 1};
+static const int kGroups[12] = {0, 2, 3, 4, 1, 1, 2, 1, 1, 1, 1, 2};
 
 extern "C" {
 
@@ -152,6 +152,7 @@ int psg_set_layout(psg_ctx* c, int R, long long N, long long rstride, int ps, in
     // state sized by the old layout must not survive it: the grid-stored bias and the interface CV hold R, strides and
     // per-replica buffers (their *_set calls come after psg_set_layout); the host-engine staging buffers are re-sized on demand
     psg_interface_cv_free(c);
+    c->dti_cv = -1;
     psg_metad_grid_free(c);
     return PSG_OK;
 }
@@ -170,11 +171,13 @@ int psg_set_cvs(psg_ctx* c, int n_cv, const psg_cv_desc* cvs, int n_slots, const
     P.has_box = 0; P.box[0] = P.box[1] = P.box[2] = 0.0;   // psg_set_box comes after psg_set_cvs
     P.span_begin = P.N; P.span_end = 0;
     std::vector<int> slot_gid(n_slots > 0 ? n_slots : 1, -1);
+    int dti_k = -1;
     for (int k = 0; k < n_cv; ++k) {
         const psg_cv_desc& d = cvs[k];
-        if (d.type < PSG_CV_DISTANCE || d.type > PSG_CV_SHAPE_ANISOTROPY) return fail(c, PSG_EINVAL, "psg_set_cvs: unknown CV type");
+        if (d.type < PSG_CV_DISTANCE || d.type > PSG_CV_DIST_TO_INTERFACE) return fail(c, PSG_EINVAL, "psg_set_cvs: unknown CV type");
         if (d.n_groups != kGroups[d.type]) return fail(c, PSG_EINVAL, "psg_set_cvs: wrong n_groups for this CV type");
-        if ((d.type == PSG_CV_COM_COMPONENT || d.type == PSG_CV_DISPLACEMENT || d.type == PSG_CV_PRINCIPAL_MOMENT) && (d.axis < 0 || d.axis > 2))
+        if ((d.type == PSG_CV_COM_COMPONENT || d.type == PSG_CV_DISPLACEMENT || d.type == PSG_CV_PRINCIPAL_MOMENT || d.type == PSG_CV_DIST_TO_INTERFACE) &&
+            (d.axis < 0 || d.axis > 2))
             return fail(c, PSG_EINVAL, "psg_set_cvs: axis must be 0, 1 or 2");
         const bool shape = d.type >= PSG_CV_PRINCIPAL_MOMENT && d.type <= PSG_CV_SHAPE_ANISOTROPY;
         if (shape && d.group_is_range[0]) return fail(c, PSG_EINVAL, "psg_set_cvs: gyration-tensor CVs take an explicit group");
@@ -182,11 +185,25 @@ int psg_set_cvs(psg_ctx* c, int n_cv, const psg_cv_desc* cvs, int n_slots, const
         CvDev& C = P.cv[k];
         C.type = d.type; C.n_groups = d.n_groups; C.axis = d.axis; C.period = d.period; C.gid0 = P.n_groups;
         if (d.type == PSG_CV_RGYR || shape) P.any_rgyr = 1;   // per-atom Jacobian depends on r_i - c: the generic kernels
+        const bool is_dti = d.type == PSG_CV_DIST_TO_INTERFACE;
+        if (is_dti) {
+            if (dti_k >= 0) return fail(c, PSG_EINVAL, "psg_set_cvs: at most one DistanceToInterface CV per ctx");
+            if (per_rep) return fail(c, PSG_EINVAL, "psg_set_cvs: DistanceToInterface needs a shared index list");
+            if (d.group_is_range[0] || !d.group_is_range[1])
+                return fail(c, PSG_EINVAL, "psg_set_cvs: DistanceToInterface takes explicit mobile atoms (group 0) and a contiguous interface range (group 1)");
+            dti_k = k;
+            P.any_rgyr = 1;   // (keeps every fused one-launch step off: this CV has kernels of its own)
+        }
         for (int g = 0; g < d.n_groups; ++g) {
             GroupDev& G = P.grp[P.n_groups];
             memset(&G, 0, sizeof(G));
             G.cv = k; G.g = g; G.range_id = -1;
-            if (d.group_is_range[g]) {
+            if (d.group_is_range[g] && is_dti) {
+                // the interface atoms: a range that only interface_cv.cu walks (not in the table of the moment kernels)
+                if (d.range_size[g] <= 0 || d.range_begin[g] < 0 || d.range_begin[g] + d.range_size[g] > P.N)
+                    return fail(c, PSG_EINVAL, "psg_set_cvs: atom range outside [0, n_atoms)");
+                G.is_range = 1; G.rbegin = d.range_begin[g]; G.rsize = d.range_size[g];
+            } else if (d.group_is_range[g]) {
                 if (P.n_ranges >= PSG_MAX_RANGE_GROUPS) return fail(c, PSG_EINVAL, "psg_set_cvs: too many range groups");
                 if (d.range_size[g] <= 0 || d.range_begin[g] < 0 || d.range_begin[g] + d.range_size[g] > P.N)
                     return fail(c, PSG_EINVAL, "psg_set_cvs: atom range outside [0, n_atoms)");
@@ -267,6 +284,16 @@ int psg_set_cvs(psg_ctx* c, int n_cv, const psg_cv_desc* cvs, int n_slots, const
     CK(c, cudaMemset(c->d_bin, 0xff, R * sizeof(int)));
     c->sys = P;
     c->have_cvs = true; c->have_jac = false; c->method = PSG_METHOD_NONE;
+    c->dti_cv = -1;
+    if (dti_k >= 0) {
+        // DistanceToInterface as a CV of the path: the same state psg_interface_cv_set builds, from the descriptor
+        const psg_cv_desc& d = cvs[dti_k];
+        const GroupDev& G0 = P.grp[P.cv[dti_k].gid0];
+        int rc = psg_interface_cv_set(c, G0.size, slot_atom + G0.begin, slot_weight ? slot_weight + G0.begin : nullptr, d.range_begin[1],
+                                      d.range_size[1], d.axis, d.dti_sigma, d.dti_scope[0], d.dti_scope[1], d.dti_bins, d.dti_coeff);
+        if (rc != PSG_OK) { c->have_cvs = false; return rc; }
+        c->dti_cv = dti_k;
+    }
     return PSG_OK;
 }
 
@@ -521,7 +548,7 @@ int psg_abf_estimate(psg_ctx* c, const float* d_pos, const float* d_vel, const f
     if (!c->have_cvs) return fail(c, PSG_ESTATE, "psg_abf_estimate: no CVs configured");
     if (!d_pos || !d_vel || !d_mass || !d_fsample) return fail(c, PSG_EINVAL, "psg_abf_estimate: NULL pointer");
     if (!(dt > 0.0)) return fail(c, PSG_EINVAL, "psg_abf_estimate: dt must be > 0");
-    if (c->sys.n_ranges > 0) return fail(c, PSG_EINVAL, "psg_abf_estimate: explicit groups only (this ctx has range groups)");
+    if (c->sys.n_ranges > 0 || c->dti_cv >= 0) return fail(c, PSG_EINVAL, "psg_abf_estimate: explicit groups only (this ctx has range groups)");
     CK(c, psg_launch_abf_estimate(c, d_pos, d_vel, d_mass, dt, d_fbias_prev, d_fsample));
     return PSG_OK;
 }

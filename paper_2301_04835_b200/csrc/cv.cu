@@ -232,7 +232,10 @@ cudaError_t psg_launch_cv_eval(psg_ctx* c, const float* d_pos, float* d_xi, floa
     }
     k_cv_eval<<<(P.R + 7) / 8, 256, 0, c->stream>>>(P, d_pos, c->d_rpart, d_xi, d_jac, c->d_jac, c->d_gdesc);
     c->launches++;
-    return cudaGetLastError();
+    cudaError_t e = cudaGetLastError();
+    // DistanceToInterface: k_cv_eval left 0 in its column and zero Jacobians for its mobile slots; its own kernels fill the column
+    if (e == cudaSuccess && c->dti_cv >= 0) e = psg_launch_dti_eval(c, d_pos, d_xi, P.n_cv, c->dti_cv);
+    return e;
 }
 
 cudaError_t psg_launch_apply(psg_ctx* c, const float* d_pos, const float* d_dVdxi, float* d_force) {
@@ -248,5 +251,7 @@ cudaError_t psg_launch_apply(psg_ctx* c, const float* d_pos, const float* d_dVdx
         else k_apply_dense<false><<<g, 256, 0, c->stream>>>(P, d_pos, c->d_gdesc, d_dVdxi, d_force);
         c->launches++;
     }
-    return cudaGetLastError();
+    cudaError_t e = cudaGetLastError();
+    if (e == cudaSuccess && c->dti_cv >= 0) e = psg_launch_dti_apply(c, d_pos, d_dVdxi, P.n_cv, c->dti_cv, d_force);
+    return e;
 }

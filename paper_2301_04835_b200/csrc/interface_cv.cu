@@ -51,7 +51,7 @@ __global__ void __launch_bounds__(128) k_dti_mass(const __grid_constant__ DtiPar
 
 __global__ void __launch_bounds__(128) k_dti_finish(const __grid_constant__ DtiParams D, const float* __restrict__ pos,
                                                     const double* __restrict__ part, double* __restrict__ G /*[R][bins]*/,
-                                                    float* __restrict__ xi_out) {
+                                                    float* __restrict__ xi_out, int xi_stride, int xi_col) {
     __shared__ double mass[DTI_MAX_BINS], prob[DTI_MAX_BINS];
     const int r = blockIdx.x, tid = threadIdx.x;
     for (int j = tid; j < D.bins; j += 128) {
@@ -114,20 +114,20 @@ __global__ void __launch_bounds__(128) k_dti_finish(const __grid_constant__ DtiP
             mob += w * (double)p[(long long)D.mobile_idx[m] * D.ps + D.axis];
             W += w;
         }
-        xi_out[r] = (float)(mob / W - I);
+        xi_out[(long long)r * xi_stride + xi_col] = (float)(mob / W - I);
     }
 }
 
 __global__ void __launch_bounds__(256) k_dti_apply(const __grid_constant__ DtiParams D, const float* __restrict__ pos,
-                                                   const double* __restrict__ G, const float* __restrict__ dVdxi,
-                                                   float* __restrict__ force) {
+                                                   const double* __restrict__ G, const float* __restrict__ dVdxi, int dv_stride,
+                                                   int dv_col, float* __restrict__ force) {
     __shared__ double g[DTI_MAX_BINS];
     const int r = blockIdx.y, ch = blockIdx.x, tid = threadIdx.x;
     for (int j = tid; j < D.bins; j += 256) g[j] = G[(long long)r * D.bins + j];
     __syncthreads();
     const float* p = pos + (long long)r * D.rstride * D.ps;
     float* f = force + (long long)r * D.rstride * D.fs;
-    const double dv = (double)dVdxi[r], is2 = 1.0 / (D.sigma * D.sigma);
+    const double dv = (double)dVdxi[(long long)r * dv_stride + dv_col], is2 = 1.0 / (D.sigma * D.sigma);
     const long long a0 = D.ibegin + (long long)ch * DTI_CHUNK;
     for (int i = tid; i < DTI_CHUNK; i += 256) {
         const long long a = a0 + i;
@@ -195,11 +195,7 @@ extern "C" int psg_interface_cv_eval(psg_ctx* c, const float* d_pos, float* d_xi
     DtiState* S = dti(c);
     if (!S) { c->err = "psg_interface_cv_eval: call psg_interface_cv_set first"; return PSG_ESTATE; }
     if (!d_pos || !d_xi) { c->err = "psg_interface_cv_eval: NULL pointer"; return PSG_EINVAL; }
-    const DtiParams& D = S->D;
-    k_dti_mass<<<dim3(D.n_chunks, D.R), 128, 0, c->stream>>>(D, d_pos, S->part);
-    k_dti_finish<<<D.R, 128, 0, c->stream>>>(D, d_pos, S->part, S->G, d_xi);
-    c->launches += 2;
-    if (cudaGetLastError() != cudaSuccess) { c->err = "psg_interface_cv_eval: launch failed"; return PSG_ECUDA; }
+    if (psg_launch_dti_eval(c, d_pos, d_xi, 1, 0) != cudaSuccess) { c->err = "psg_interface_cv_eval: launch failed"; return PSG_ECUDA; }
     return PSG_OK;
 }
 
@@ -208,11 +204,26 @@ extern "C" int psg_interface_cv_apply(psg_ctx* c, const float* d_pos, const floa
     DtiState* S = dti(c);
     if (!S) { c->err = "psg_interface_cv_apply: call psg_interface_cv_set and psg_interface_cv_eval first"; return PSG_ESTATE; }
     if (!d_pos || !d_dVdxi || !d_force) { c->err = "psg_interface_cv_apply: NULL pointer"; return PSG_EINVAL; }
-    const DtiParams& D = S->D;
-    k_dti_apply<<<dim3(D.n_chunks, D.R), 256, 0, c->stream>>>(D, d_pos, S->G, d_dVdxi, d_force);
-    c->launches += 1;
-    if (cudaGetLastError() != cudaSuccess) { c->err = "psg_interface_cv_apply: launch failed"; return PSG_ECUDA; }
+    if (psg_launch_dti_apply(c, d_pos, d_dVdxi, 1, 0, d_force) != cudaSuccess) { c->err = "psg_interface_cv_apply: launch failed"; return PSG_ECUDA; }
     return PSG_OK;
+}
+
+// value into column xi_col of a [R][xi_stride] array (psg_cv_eval: the CV's own column of xi) ...
+cudaError_t psg_launch_dti_eval(psg_ctx* c, const float* d_pos, float* d_xi, int xi_stride, int xi_col) {
+    DtiState* S = dti(c);
+    const DtiParams& D = S->D;
+    k_dti_mass<<<dim3(D.n_chunks, D.R), 128, 0, c->stream>>>(D, d_pos, S->part);
+    k_dti_finish<<<D.R, 128, 0, c->stream>>>(D, d_pos, S->part, S->G, d_xi, xi_stride, xi_col);
+    c->launches += 2;
+    return cudaGetLastError();
+}
+// ... and the forces of that CV from column dv_col of dV/dxi (psg_apply_bias_forces)
+cudaError_t psg_launch_dti_apply(psg_ctx* c, const float* d_pos, const float* d_dVdxi, int dv_stride, int dv_col, float* d_force) {
+    DtiState* S = dti(c);
+    const DtiParams& D = S->D;
+    k_dti_apply<<<dim3(D.n_chunks, D.R), 256, 0, c->stream>>>(D, d_pos, S->G, d_dVdxi, dv_stride, dv_col, d_force);
+    c->launches += 1;
+    return cudaGetLastError();
 }
 
 void psg_interface_cv_free(psg_ctx* c) {

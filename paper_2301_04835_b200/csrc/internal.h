@@ -134,9 +134,12 @@ struct psg_ctx {
     int sm_count = 148;
     void* dti = nullptr;             // state of the DistanceToInterface CV (interface_cv.cu)
     void* mgrid = nullptr;           // state of grid-stored metadynamics (metad_grid.cu)
+    int dti_cv = -1;                 // index of the PSG_CV_DIST_TO_INTERFACE CV (its value and forces come from interface_cv.cu), else -1
     int mgrid_stride = 0;            // PSG_METHOD_METAD_GRID: psg_step deposits when step % stride == 0
 };
 void psg_interface_cv_free(psg_ctx* c);
+cudaError_t psg_launch_dti_eval(psg_ctx* c, const float* d_pos, float* d_xi, int xi_stride, int xi_col);
+cudaError_t psg_launch_dti_apply(psg_ctx* c, const float* d_pos, const float* d_dVdxi, int dv_stride, int dv_col, float* d_force);
 void psg_metad_grid_free(psg_ctx* c);
 
 // ---- launchers implemented in the .cu files (all enqueue on ctx->stream) ----

@@ -266,7 +266,7 @@ extern "C" int psg_metad_grid_step(psg_ctx* c, const float* d_pos, float* d_forc
     if (!d_pos || !d_force) { c->err = "psg_metad_grid_step: NULL pointer"; return PSG_EINVAL; }
     const SysParams& P = c->sys;
     if (P.n_cv != S->G.n_cv || P.R != S->G.R) { c->err = "psg_metad_grid_step: the grid was set for another n_cv or walker count"; return PSG_ESTATE; }
-    if (P.n_ranges > 0) {   // range groups: their moments and forces live in the streaming kernels
+    if (P.n_ranges > 0 || c->dti_cv >= 0) {   // range groups / the interface CV: their values and forces live in kernels of their own
         int e = psg_cv_eval(c, d_pos, c->d_xi, nullptr);
         if (e == PSG_OK) e = psg_metad_grid_eval(c, c->d_xi, c->d_V, c->d_dVdxi);
         if (e == PSG_OK) e = psg_apply_bias_forces(c, d_pos, c->d_dVdxi, d_force);

@@ -13,12 +13,13 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 _LIB_PATH = os.path.join(_HERE, "libpsg.so")
 
 CV_DISTANCE, CV_ANGLE, CV_DIHEDRAL, CV_COM_COMPONENT, CV_RGYR, CV_DISPLACEMENT = 1, 2, 3, 4, 5, 6
-CV_PRINCIPAL_MOMENT, CV_ASPHERICITY, CV_ACYLINDRICITY, CV_SHAPE_ANISOTROPY = 7, 8, 9, 10
+CV_PRINCIPAL_MOMENT, CV_ASPHERICITY, CV_ACYLINDRICITY, CV_SHAPE_ANISOTROPY, CV_DIST_TO_INTERFACE = 7, 8, 9, 10, 11
 METHOD_NONE, METHOD_HARMONIC, METHOD_METAD, METHOD_ABF, METHOD_METAD_GRID = 0, 1, 2, 3, 4
 HILLS_F32, HILLS_F64 = 0, 1
 _KIND = {"distance": CV_DISTANCE, "angle": CV_ANGLE, "dihedral": CV_DIHEDRAL, "component": CV_COM_COMPONENT,
          "rgyr": CV_RGYR, "displacement": CV_DISPLACEMENT, "principal_moment": CV_PRINCIPAL_MOMENT,
-         "asphericity": CV_ASPHERICITY, "acylindricity": CV_ACYLINDRICITY, "shape_anisotropy": CV_SHAPE_ANISOTROPY}
+         "asphericity": CV_ASPHERICITY, "acylindricity": CV_ACYLINDRICITY, "shape_anisotropy": CV_SHAPE_ANISOTROPY,
+         "dist_to_interface": CV_DIST_TO_INTERFACE}
 
 # every symbol include/psg.h declares
 EXPORTS = ["psg_create", "psg_destroy", "psg_set_stream", "psg_last_error", "psg_set_layout", "psg_set_cvs",
@@ -39,7 +40,8 @@ class _CvDesc(C.Structure):
     _fields_ = [("type", C.c_int), ("n_groups", C.c_int), ("group_is_range", C.c_int * 4),
                 ("group_begin", C.c_int * 4), ("group_size", C.c_int * 4),
                 ("range_begin", C.c_longlong * 4), ("range_size", C.c_longlong * 4),
-                ("axis", C.c_int), ("period", C.c_double)]
+                ("axis", C.c_int), ("period", C.c_double), ("dti_sigma", C.c_double), ("dti_scope", C.c_double * 2),
+                ("dti_coeff", C.c_double), ("dti_bins", C.c_int)]
 
 
 _lib = None
@@ -180,7 +182,7 @@ class Context:
         self.R = n_replicas
 
     def set_cvs(self, cvs, slot_atom_idx=None, slot_weight=None, atom_weight=None):
-        """cvs: list of dicts {"type": CV_*, "groups": [("slots", begin, size) | ("range", first, n)], "axis", "period"}"""
+        """cvs: list of dicts {"type": CV_*, "groups": [("slots", begin, size) | ("range", first, n)], "axis", "period"[, "dti"]}"""
         arr = (_CvDesc * len(cvs))()
         for k, cv in enumerate(cvs):
             arr[k].type = cv["type"]
@@ -193,6 +195,10 @@ class Context:
                     arr[k].group_begin[g], arr[k].group_size[g] = int(grp[1]), int(grp[2])
             arr[k].axis = int(cv.get("axis", 0))
             arr[k].period = float(cv.get("period", 0.0))
+            if "dti" in cv:     # {"sigma", "scope": (lo, hi), "bins", "coeff"} of PSG_CV_DIST_TO_INTERFACE
+                d = cv["dti"]
+                arr[k].dti_sigma, arr[k].dti_coeff, arr[k].dti_bins = float(d["sigma"]), float(d["coeff"]), int(d["bins"])
+                arr[k].dti_scope[0], arr[k].dti_scope[1] = float(d["scope"][0]), float(d["scope"][1])
         if slot_atom_idx is None:
             sa, n_slots, per_rep = None, 0, 0
         else:

@@ -1068,6 +1068,83 @@ def test_distance_to_interface_matches_oracle(torch, psg, R, n_i, bins, axis):
 
 
 # ------------------------------------------------------------------------------------ error behaviour
+def test_distance_to_interface_as_a_cv_of_the_step(torch, psg):
+    """PSG_CV_DIST_TO_INTERFACE (Eq. 4-8, App. A) as a psg_cv_desc type: next to a Distance CV, under a harmonic
+    bias and under ABF, through psg_step (the separate kernels in sequence); value, bias and forces against the oracle's
+    pieces (its DistanceToInterface with derivatives, its harmonic / ABF stage, its Distance Jacobian)"""
+    rng = np.random.default_rng(31)
+    R, N, axis = 5, 1400, 2
+    mob = np.array([3, 9, 1200], np.int32)                    # the last mobile atom lies inside the interface range
+    mw = np.array([1.0, 2.5, 0.5], np.float32)
+    ib, ni = 40, 1300
+    dti = {"sigma": 0.25, "scope": (1.0, 5.0), "bins": 33, "coeff": 3.0}
+    pos = np.zeros((R, N, 4), np.float32)
+    pos[..., :3] = rng.uniform(0.0, 6.0, size=(R, N, 3))
+    pos[:, ib:ib + ni, axis] = np.where(rng.uniform(size=(R, ni)) < 0.5, rng.uniform(0.5, 2.8, size=(R, ni)), rng.uniform(2.8, 5.5, size=(R, ni)) * 0.7 + 1.0)
+    pos[..., 3] = 7.0
+    slots = np.concatenate([mob, [700, 701]]).astype(np.int32)          # slots 0..2 mobile, 3 and 4 the Distance pair
+    sw = np.concatenate([mw, [1.0, 1.0]]).astype(np.float32)
+    cvs = [{"type": psg.CV_DIST_TO_INTERFACE, "groups": [("slots", 0, 3), ("range", ib, ni)], "axis": axis, "period": 0.0, "dti": dti},
+           {"type": psg.CV_DISTANCE, "groups": [("slots", 3, 1), ("slots", 4, 1)], "axis": 0, "period": 0.0}]
+    o_dist = orc.System(R, N, N, 4, [{"type": orc.DISTANCE, "groups": [("slots", 0, 1), ("slots", 1, 1)], "axis": 0, "period": 0.0}],
+                        np.array([700, 701], np.int32), None, None)
+    xi_ref = np.zeros((R, 2))
+    jm, dx = [], []
+    for r in range(R):
+        x, j, d, _ = orc.dist_to_interface(pos[r], mob, mw, ib, ni, axis, dti["sigma"], dti["scope"], dti["bins"], dti["coeff"])
+        xi_ref[r, 0] = x; jm.append(j); dx.append(d)
+    xi_ref[:, 1] = o_dist.cv_eval(pos, want_jac=False)[:, 0]
+    f0 = (rng.standard_normal((R, N, 4)) * 50).astype(np.float32)
+
+    def forces_ref(dV):
+        f = f0[..., :3].astype(np.float64)
+        f = o_dist.apply_forces(pos, dV[:, 1:2], f)
+        for r in range(R):
+            np.add.at(f[r], mob, -dV[r, 0] * jm[r])
+            f[r, ib:ib + ni, axis] += -dV[r, 0] * dx[r]
+        return f
+
+    ctx = psg.Context(0)
+    ctx.set_layout(R, N, N, 4, 4)
+    ctx.set_cvs(cvs, slots, sw, None)
+    # -- harmonic
+    ks, cen = np.array([400.0, 150.0], np.float32), np.stack([np.linspace(-0.5, 0.5, R), np.full(R, 2.0)], axis=1).astype(np.float32)
+    ctx.set_harmonic(ks, cen)
+    d_f = dev(torch, f0)
+    n0 = ctx.launch_count()
+    ctx.step(dev(torch, pos), d_f, None, 1)
+    ctx.sync_check()
+    assert ctx.launch_count() - n0 == 6          # k_cv_eval, two interface kernels, k_harmonic, k_apply_sparse, k_dti_apply
+    out = {k: v.cpu().numpy() for k, v in ctx.read_step_outputs().items()}
+    assert_close(out["xi"], xi_ref, "xi (interface CV + distance)")
+    V, dV = orc.harmonic(xi_ref.astype(np.float32).astype(np.float64), ks, cen, np.zeros(2))
+    assert_close(out["V"], V, "V")
+    assert_close(out["dVdxi"], dV, "dV/dxi")
+    assert_forces_close(d_f.cpu().numpy()[..., :3], forces_ref(dV), f0[..., :3], "forces through the interface CV")
+    assert np.array_equal(d_f.cpu().numpy()[..., 3].view(np.uint32), f0[..., 3].view(np.uint32))
+    # -- ABF on the same two CVs: bins bit-exact, the mean force scattered through both Jacobians
+    lower, upper = np.array([-3.0, 0.0], np.float32), np.array([3.0, 9.0], np.float32)
+    shape, periodic = np.array([12, 9], np.int32), np.array([0, 0], np.int32)
+    ctx.set_abf(lower, upper, shape, periodic, 2)
+    fs = rng.normal(scale=10.0, size=(R, 2)).astype(np.float32)
+    d_f = dev(torch, f0)
+    ctx.step(dev(torch, pos), d_f, dev(torch, fs), 1)
+    ctx.sync_check()
+    out = {k: v.cpu().numpy() for k, v in ctx.read_step_outputs().items()}
+    hist, fsum = np.zeros(108, np.int32), np.zeros((108, 2), np.float64)
+    b, dVa = orc.abf_update(out["xi"], fs, lower, upper, shape, periodic, 2, hist, fsum)
+    assert np.array_equal(out["bin"], b) and (b >= 0).sum() >= 2     # (out-of-grid replicas get no mean force)
+    assert_close(out["dVdxi"], dVa, "ABF mean force")
+    assert_forces_close(d_f.cpu().numpy()[..., :3], forces_ref(dVa), f0[..., :3], "ABF forces through the interface CV")
+    # -- argument checks
+    bad = [dict(cvs[0], groups=[("range", 0, 3), ("range", ib, ni)]), cvs[1]]
+    with pytest.raises(psg.PsgError):
+        ctx.set_cvs(bad, slots, sw, None)
+    with pytest.raises(psg.PsgError):
+        ctx.set_cvs([cvs[0], dict(cvs[0], groups=[("slots", 3, 2), ("range", ib, ni)])], slots, sw, None)   # two of them
+    ctx.close()
+
+
 def test_argument_validation(torch, psg):
     ctx = psg.Context(0)
     with pytest.raises(psg.PsgError) as e:
