@@ -53,7 +53,7 @@ enum {
     PSG_CV_COM_COMPONENT = 4, /* AxisCV Component: barycenter coordinate along an axis  (L188) */
     PSG_CV_RGYR = 5,          /* RadiusofGyration: sqrt(sum w|r-c|^2 / sum w)           (L189) */
     PSG_CV_DISPLACEMENT = 6,  /* TwoPointCV Displacement c2 - c1: one CV per component (axis) (L185) */
-    /* Gyration-tensor shape CVs of ONE explicit group (L188-L189; reading R-SHAPE):
+    /* Gyration-tensor shape CVs of ONE group, explicit atoms or a contiguous range (L188-L189; reading R-SHAPE):
      * S = sum w (r - c)(r - c)^T / sum w, eigenvalues l1 >= l2 >= l3. */
     PSG_CV_PRINCIPAL_MOMENT = 7, /* AxisCV PrincipalMoment: l_axis, axis 0 = the largest               (L188) */
     PSG_CV_ASPHERICITY = 8,      /* l1 - (l2 + l3)/2                                                    (L189) */

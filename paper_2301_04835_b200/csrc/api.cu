@@ -101,7 +101,7 @@ int psg_create(psg_ctx** out, int device, void* cuda_stream) {
 static void free_all(psg_ctx* c) {
     dfree(c->d_slot_atom); dfree(c->d_slot_gid); dfree(c->d_slot_weight); dfree(c->d_atom_weight);
     dfree(c->d_xi); dfree(c->d_V); dfree(c->d_dVdxi); dfree(c->d_bin); dfree(c->d_V64);
-    dfree(c->d_jac); dfree(c->d_gdesc); dfree(c->d_rpart); dfree(c->d_arrive); dfree(c->d_rdesc); dfree(c->d_gbar); dfree(c->d_whist);
+    dfree(c->d_jac); dfree(c->d_gdesc); dfree(c->d_rpart); dfree(c->d_rpart2); dfree(c->d_gdesc_m); dfree(c->d_arrive); dfree(c->d_rdesc); dfree(c->d_gbar); dfree(c->d_whist);
     dfree(c->d_kspring); dfree(c->d_centers);
     dfree(c->md.hills); dfree(c->md.heights); dfree(c->md.n_hills); dfree(c->md.part);
     if (c->abf.own) { dfree(c->abf.hist); dfree(c->abf.fsum); }
@@ -167,7 +167,7 @@ int psg_set_cvs(psg_ctx* c, int n_cv, const psg_cv_desc* cvs, int n_slots, const
     cudaSetDevice(c->device);
     SysParams P = c->sys;
     P.n_cv = n_cv; P.n_slots = n_slots; P.per_rep = per_rep ? 1 : 0;
-    P.n_groups = 0; P.n_ranges = 0; P.any_rgyr = 0;
+    P.n_groups = 0; P.n_ranges = 0; P.any_rgyr = 0; P.any_shape_range = 0;
     P.has_box = 0; P.box[0] = P.box[1] = P.box[2] = 0.0;   // psg_set_box comes after psg_set_cvs
     P.span_begin = P.N; P.span_end = 0;
     std::vector<int> slot_gid(n_slots > 0 ? n_slots : 1, -1);
@@ -180,11 +180,11 @@ int psg_set_cvs(psg_ctx* c, int n_cv, const psg_cv_desc* cvs, int n_slots, const
             (d.axis < 0 || d.axis > 2))
             return fail(c, PSG_EINVAL, "psg_set_cvs: axis must be 0, 1 or 2");
         const bool shape = d.type >= PSG_CV_PRINCIPAL_MOMENT && d.type <= PSG_CV_SHAPE_ANISOTROPY;
-        if (shape && d.group_is_range[0]) return fail(c, PSG_EINVAL, "psg_set_cvs: gyration-tensor CVs take an explicit group");
         if (!(d.period >= 0.0)) return fail(c, PSG_EINVAL, "psg_set_cvs: period must be >= 0");
         CvDev& C = P.cv[k];
         C.type = d.type; C.n_groups = d.n_groups; C.axis = d.axis; C.period = d.period; C.gid0 = P.n_groups;
         if (d.type == PSG_CV_RGYR || shape) P.any_rgyr = 1;   // per-atom Jacobian depends on r_i - c: the generic kernels
+        if (shape && d.group_is_range[0]) P.any_shape_range = 1;
         const bool is_dti = d.type == PSG_CV_DIST_TO_INTERFACE;
         if (is_dti) {
             if (dti_k >= 0) return fail(c, PSG_EINVAL, "psg_set_cvs: at most one DistanceToInterface CV per ctx");
@@ -271,6 +271,8 @@ int psg_set_cvs(psg_ctx* c, int n_cv, const psg_cv_desc* cvs, int n_slots, const
     CK(c, dalloc(c->d_jac, R * (size_t)n_slots * 3));
     CK(c, dalloc(c->d_gdesc, R * P.n_groups * PSG_GDESC_DOUBLES));
     CK(c, dalloc(c->d_rpart, R * P.n_ranges * (size_t)P.range_blocks * PSG_MOM));
+    CK(c, dalloc(c->d_rpart2, P.any_shape_range ? R * P.n_ranges * (size_t)P.range_blocks * 6 : 0));
+    CK(c, dalloc(c->d_gdesc_m, P.any_shape_range ? R * P.n_groups * 6 : 0));
     CK(c, dalloc(c->d_arrive, 2 * R));
     CK(c, cudaMemset(c->d_arrive, 0, 2 * R * sizeof(unsigned)));
     CK(c, dalloc(c->d_whist, R * 2 * n_cv));

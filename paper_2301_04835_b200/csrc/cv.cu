@@ -91,18 +91,64 @@ __global__ void __launch_bounds__(PSG_RANGE_THREADS, 4) k_range_moments(const __
 }
 
 // --------------------------------------------------------------------------------------------
+// Second moments of the range groups that carry a gyration-tensor shape CV (PAPER.md:L188-L189 over large groups): per block
+// and group the six sums of w e e^T, e = r - (the group's first atom; with a box the nearest image), binary64. grid =
+// (range_blocks, R) like k_range_moments; only launched when such a CV exists.
+template <bool BOX>
+__global__ void __launch_bounds__(256) k_range_second(const __grid_constant__ SysParams P, const float* __restrict__ pos,
+                                                       double* __restrict__ rpart2) {
+    const int r = blockIdx.y, b = blockIdx.x, tid = threadIdx.x;
+    const float* p = pos + (long long)r * P.rstride * P.ps;
+    const long long t0 = P.span_begin + (long long)b * PSG_RANGE_TILE;
+    const long long t1 = t0 + PSG_RANGE_TILE < P.span_end ? t0 + PSG_RANGE_TILE : P.span_end;
+    __shared__ double red[8][6];
+    for (int q = 0; q < P.n_ranges; ++q) {
+        const GroupDev& G = P.grp[P.range_gid[q]];
+        if (!is_shape_cv(P.cv[G.cv].type)) continue;   // block-uniform
+        const long long gb = G.rbegin, ge = G.rbegin + G.rsize;
+        double m[6] = {0, 0, 0, 0, 0, 0};
+        if (t0 < ge && t1 > gb) {
+            const D3 first = load_pos(p, gb, P.ps);
+            for (long long a = t0 + tid; a < t1; a += 256) {
+                if (a < gb || a >= ge) continue;
+                const D3 x = load_pos(p, a, P.ps);
+                D3 e = x - first;
+                if (BOX) e = min_image(e, P.box);
+                const double w = P.atom_weight ? (double)__ldg(P.atom_weight + a) : 1.0;
+                m[0] += w * e.x * e.x; m[1] += w * e.x * e.y; m[2] += w * e.x * e.z;
+                m[3] += w * e.y * e.y; m[4] += w * e.y * e.z; m[5] += w * e.z * e.z;
+            }
+        }
+#pragma unroll
+        for (int i = 0; i < 6; ++i) m[i] = warp_sum(m[i]);
+        __syncthreads();
+        if ((tid & 31) == 0)
+#pragma unroll
+            for (int i = 0; i < 6; ++i) red[tid >> 5][i] = m[i];
+        __syncthreads();
+        if (tid < 6) {
+            double s = 0;
+#pragma unroll
+            for (int wq = 0; wq < 8; ++wq) s += red[wq][tid];   // fixed order
+            rpart2[(((long long)r * P.n_ranges + q) * P.range_blocks + b) * 6 + tid] = s;
+        }
+    }
+}
+
+// --------------------------------------------------------------------------------------------
 // One warp per replica. Writes xi (fp32), the compact Jacobian of explicit slots (fp32, to jac_user and/or
 // jac_cache) and the per-group descriptors gdesc[r][gid] = {v(3), c(3), coef, W} (fp64) for range groups.
 __global__ void __launch_bounds__(256) k_cv_eval(const __grid_constant__ SysParams P, const float* __restrict__ pos,
                                                   const double* __restrict__ rpart, float* __restrict__ xi,
                                                   float* __restrict__ jac_user, float* __restrict__ jac_cache,
-                                                  double* __restrict__ gdesc) {
+                                                  double* __restrict__ gdesc, const double* __restrict__ rpart2,
+                                                  double* __restrict__ gdesc_m) {
     __shared__ WarpCvSmem sm[8];
     const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
     const int r = blockIdx.x * 8 + wid;
     if (r >= P.R) return;
     WarpCvSmem& S = sm[wid];
-    warp_cv_eval<true>(P, r, pos, rpart, S, lane);
+    warp_cv_eval<true>(P, r, pos, rpart, S, lane, rpart2);
     if (lane < P.n_cv) xi[(long long)r * P.n_cv + lane] = (float)S.xi[lane];
     for (int s = lane; s < P.n_slots; s += 32) {
         D3 j = slot_jacobian(P, r, pos, S, s);
@@ -115,6 +161,11 @@ __global__ void __launch_bounds__(256) k_cv_eval(const __grid_constant__ SysPara
         d[0] = S.v[lane][0]; d[1] = S.v[lane][1]; d[2] = S.v[lane][2];
         d[3] = S.cen[lane][0]; d[4] = S.cen[lane][1]; d[5] = S.cen[lane][2];
         d[6] = S.coef[lane]; d[7] = S.cen[lane][3];
+        if (gdesc_m) {   // shape CVs over ranges: the matrix M of d xi / d r_i = w_i M (r_i - c)
+            double* m = gdesc_m + ((long long)r * P.n_groups + lane) * 6;
+#pragma unroll
+            for (int e = 0; e < 6; ++e) m[e] = S.sec[lane][e];
+        }
     }
 }
 
@@ -143,7 +194,7 @@ __global__ void __launch_bounds__(256) k_apply_sparse(const __grid_constant__ Sy
 template <bool BOX>
 __global__ void __launch_bounds__(256) k_apply_dense(const __grid_constant__ SysParams P, const float* __restrict__ pos,
                                                       const double* __restrict__ gdesc, const float* __restrict__ dVdxi,
-                                                      float* __restrict__ force) {
+                                                      float* __restrict__ force, const double* __restrict__ gdesc_m) {
     constexpr int PER = PSG_RANGE_TILE / 256;
     const int r = blockIdx.y, b = blockIdx.x, tid = threadIdx.x;
     const long long t0 = P.span_begin + (long long)b * PSG_RANGE_TILE;
@@ -151,6 +202,8 @@ __global__ void __launch_bounds__(256) k_apply_dense(const __grid_constant__ Sys
         s_k[PSG_MAX_RANGE_GROUPS];
     __shared__ long long s_b[PSG_MAX_RANGE_GROUPS], s_e[PSG_MAX_RANGE_GROUPS];
     __shared__ double s_first[PSG_MAX_RANGE_GROUPS][3], s_cd[PSG_MAX_RANGE_GROUPS][3];   // minimum image: first atom, centre
+    __shared__ float s_M[PSG_MAX_RANGE_GROUPS][6];   // shape CVs: -dV/dxi * M (symmetric), s_shape = 1
+    __shared__ int s_shape[PSG_MAX_RANGE_GROUPS];
     if (tid < P.n_ranges) {
         int gid = P.range_gid[tid];
         const GroupDev& G = P.grp[gid];
@@ -165,6 +218,12 @@ __global__ void __launch_bounds__(256) k_apply_dense(const __grid_constant__ Sys
         }
         s_k[tid] = (float)(dv * d[6]);
         s_b[tid] = G.rbegin; s_e[tid] = G.rbegin + G.rsize;
+        s_shape[tid] = gdesc_m != nullptr && d[6] == PSG_COEF_SHAPE;
+        if (s_shape[tid]) {
+            const double* m = gdesc_m + ((long long)r * P.n_groups + gid) * 6;
+#pragma unroll
+            for (int e = 0; e < 6; ++e) s_M[tid][e] = (float)(dv * m[e]);
+        }
         if (BOX) {
             const D3 f0 = load_pos(pos + (long long)r * P.rstride * P.ps, G.rbegin, P.ps);
             s_first[tid][0] = f0.x; s_first[tid][1] = f0.y; s_first[tid][2] = f0.z;
@@ -194,16 +253,24 @@ __global__ void __launch_bounds__(256) k_apply_dense(const __grid_constant__ Sys
             if (a >= s_b[q] && a < s_e[q]) {
                 any = true;
                 float k = s_k[q];
+                float dx, dy, dz;   // r_i - c_g
                 if (BOX) {   // r_i = the image nearest to the group's first atom, as in the moments
                     const D3 d = min_image(d3((double)px - s_first[q][0], (double)py - s_first[q][1], (double)pz - s_first[q][2]), P.box);
-                    ax += s_v[q][0] + k * (float)((s_first[q][0] + d.x) - s_cd[q][0]);
-                    ay += s_v[q][1] + k * (float)((s_first[q][1] + d.y) - s_cd[q][1]);
-                    az += s_v[q][2] + k * (float)((s_first[q][2] + d.z) - s_cd[q][2]);
-                    continue;
+                    dx = (float)((s_first[q][0] + d.x) - s_cd[q][0]);
+                    dy = (float)((s_first[q][1] + d.y) - s_cd[q][1]);
+                    dz = (float)((s_first[q][2] + d.z) - s_cd[q][2]);
+                } else {
+                    dx = (px - s_chi[q][0]) - s_clo[q][0]; dy = (py - s_chi[q][1]) - s_clo[q][1]; dz = (pz - s_chi[q][2]) - s_clo[q][2];
                 }
-                ax += s_v[q][0] + k * ((px - s_chi[q][0]) - s_clo[q][0]);
-                ay += s_v[q][1] + k * ((py - s_chi[q][1]) - s_clo[q][1]);
-                az += s_v[q][2] + k * ((pz - s_chi[q][2]) - s_clo[q][2]);
+                if (s_shape[q]) {   // gyration-tensor shape CV: w M (r - c), M symmetric
+                    ax += s_M[q][0] * dx + s_M[q][1] * dy + s_M[q][2] * dz;
+                    ay += s_M[q][1] * dx + s_M[q][3] * dy + s_M[q][4] * dz;
+                    az += s_M[q][2] * dx + s_M[q][4] * dy + s_M[q][5] * dz;
+                } else {
+                    ax += s_v[q][0] + k * dx;
+                    ay += s_v[q][1] + k * dy;
+                    az += s_v[q][2] + k * dz;
+                }
             }
         }
         if (!any) continue;
@@ -230,7 +297,14 @@ cudaError_t psg_launch_cv_eval(psg_ctx* c, const float* d_pos, float* d_xi, floa
         else k_range_moments<false><<<g, PSG_RANGE_THREADS, 0, c->stream>>>(P, d_pos, c->d_rpart);
         c->launches++;
     }
-    k_cv_eval<<<(P.R + 7) / 8, 256, 0, c->stream>>>(P, d_pos, c->d_rpart, d_xi, d_jac, c->d_jac, c->d_gdesc);
+    if (P.any_shape_range) {
+        dim3 g(P.range_blocks, P.R);
+        if (P.has_box) k_range_second<true><<<g, 256, 0, c->stream>>>(P, d_pos, c->d_rpart2);
+        else k_range_second<false><<<g, 256, 0, c->stream>>>(P, d_pos, c->d_rpart2);
+        c->launches++;
+    }
+    k_cv_eval<<<(P.R + 7) / 8, 256, 0, c->stream>>>(P, d_pos, c->d_rpart, d_xi, d_jac, c->d_jac, c->d_gdesc,
+                                                    P.any_shape_range ? c->d_rpart2 : nullptr, P.any_shape_range ? c->d_gdesc_m : nullptr);
     c->launches++;
     cudaError_t e = cudaGetLastError();
     // DistanceToInterface: k_cv_eval left 0 in its column and zero Jacobians for its mobile slots; its own kernels fill the column
@@ -247,8 +321,8 @@ cudaError_t psg_launch_apply(psg_ctx* c, const float* d_pos, const float* d_dVdx
     }
     if (P.n_ranges > 0) {
         dim3 g(P.range_blocks, P.R);
-        if (P.has_box) k_apply_dense<true><<<g, 256, 0, c->stream>>>(P, d_pos, c->d_gdesc, d_dVdxi, d_force);
-        else k_apply_dense<false><<<g, 256, 0, c->stream>>>(P, d_pos, c->d_gdesc, d_dVdxi, d_force);
+        if (P.has_box) k_apply_dense<true><<<g, 256, 0, c->stream>>>(P, d_pos, c->d_gdesc, d_dVdxi, d_force, P.any_shape_range ? c->d_gdesc_m : nullptr);
+        else k_apply_dense<false><<<g, 256, 0, c->stream>>>(P, d_pos, c->d_gdesc, d_dVdxi, d_force, P.any_shape_range ? c->d_gdesc_m : nullptr);
         c->launches++;
     }
     cudaError_t e = cudaGetLastError();

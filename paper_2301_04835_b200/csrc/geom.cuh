@@ -262,7 +262,8 @@ struct WarpCvSmem {
 // On return (after __syncwarp) sm.xi / sm.v / sm.coef / sm.cen are valid for the whole warp.
 template <bool JAC>
 __device__ __forceinline__ void warp_cv_eval(const SysParams& P, int r, const float* __restrict__ pos,
-                                             const double* __restrict__ rpart, WarpCvSmem& sm, int lane) {
+                                             const double* __restrict__ rpart, WarpCvSmem& sm, int lane,
+                                             const double* __restrict__ rpart2 = nullptr) {
     const float* p = pos + (long long)r * P.rstride * P.ps;
     // range groups: all lanes sum the block partials (fixed order => deterministic)
     for (int q = 0; q < P.n_ranges; ++q) {
@@ -279,6 +280,26 @@ __device__ __forceinline__ void warp_cv_eval(const SysParams& P, int r, const fl
             double iw = 1.0 / a[0];
             sm.cen[gid][0] = a[1] * iw; sm.cen[gid][1] = a[2] * iw; sm.cen[gid][2] = a[3] * iw; sm.cen[gid][3] = a[0];
             sm.m2[gid] = a[4];
+        }
+        // a gyration-tensor shape CV over this range: the six second moments about the range's first atom (k_range_second),
+        // S = sum w x'x'^T / W - c'c'^T with c' = c - first, as for explicit groups
+        const int gid_q = P.range_gid[q];
+        if (rpart2 && is_shape_cv(P.cv[P.grp[gid_q].cv].type)) {
+            const double* s2 = rpart2 + ((long long)r * P.n_ranges + q) * P.range_blocks * 6;
+            double e[6] = {0, 0, 0, 0, 0, 0};
+            for (int b = lane; b < P.range_blocks; b += 32) {
+#pragma unroll
+                for (int i = 0; i < 6; ++i) e[i] += __ldcg(s2 + (long long)b * 6 + i);
+            }
+#pragma unroll
+            for (int i = 0; i < 6; ++i) e[i] = warp_sum(e[i]);
+            if (lane == 0) {
+                const D3 first = load_pos(p, P.grp[gid_q].rbegin, P.ps);
+                const double iw = 1.0 / a[0];
+                const D3 cp = d3(a[1] * iw - first.x, a[2] * iw - first.y, a[3] * iw - first.z);
+                sm.sec[gid_q][0] = e[0] * iw - cp.x * cp.x; sm.sec[gid_q][1] = e[1] * iw - cp.x * cp.y; sm.sec[gid_q][2] = e[2] * iw - cp.x * cp.z;
+                sm.sec[gid_q][3] = e[3] * iw - cp.y * cp.y; sm.sec[gid_q][4] = e[4] * iw - cp.y * cp.z; sm.sec[gid_q][5] = e[5] * iw - cp.z * cp.z;
+            }
         }
     }
     // explicit groups: lane j gathers group j

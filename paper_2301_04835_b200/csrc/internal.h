@@ -41,6 +41,7 @@ struct SysParams {
     int ps, fs;                 // floats per atom in pos / force
     int n_cv, n_slots, per_rep, n_groups, n_ranges;
     int any_rgyr;
+    int any_shape_range;        // a gyration-tensor shape CV over a contiguous range: second moments from k_range_second
     int has_box;                // minimum-image convention on (psg_set_box); explicit groups only
     double box[3];              // orthorhombic box lengths, 0 = open in that direction
     CvDev cv[PSG_MAX_CV];
@@ -111,6 +112,8 @@ struct psg_ctx {
     float* d_jac = nullptr;          // [R][n_slots][3]
     double* d_gdesc = nullptr;       // [R][n_groups][PSG_GDESC_DOUBLES]
     double* d_rpart = nullptr;       // [R][n_ranges][range_blocks][PSG_MOM]
+    double* d_rpart2 = nullptr;      // [R][n_ranges][range_blocks][6]: second moments about the group's first atom (shape CVs over ranges)
+    double* d_gdesc_m = nullptr;     // [R][n_groups][6]: the symmetric matrix M of d xi / d r_i = w_i M (r_i - c) of such a group
     unsigned* d_arrive = nullptr;    // [2][R]: arrive / done counters of the fused range step (zero between launches)
     double* d_whist = nullptr;       // [R][2][n_cv]: W(t - dt), W(t - 2 dt) of the ABF force estimator
     bool est_first = true;           // the next psg_abf_estimate initialises the history

@@ -642,7 +642,7 @@ static int rs_blocks_per_sm(int device) {
 bool psg_range_step_supported(const psg_ctx* c, const float* d_pos, const float* d_force) {
     const SysParams& P = c->sys;
     if (c->range_step_off) return false;   // psg_set_tuning: take the separate kernels
-    if (!(c->method == PSG_METHOD_HARMONIC && !P.has_box && P.n_ranges > 0 && P.n_slots == 0 && P.ps == 4 && P.fs == 4 && P.rstride > 0 &&
+    if (!(c->method == PSG_METHOD_HARMONIC && !P.has_box && !P.any_shape_range && P.n_ranges > 0 && P.n_slots == 0 && P.ps == 4 && P.fs == 4 && P.rstride > 0 &&
           ((reinterpret_cast<uintptr_t>(d_pos) | reinterpret_cast<uintptr_t>(d_force)) & 15u) == 0 &&
           c->d_arrive != nullptr))
         return false;

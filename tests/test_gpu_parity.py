@@ -1315,11 +1315,60 @@ def test_shape_cv_metad_and_abf_steps(torch, psg):
     ctx.close()
 
 
+@pytest.mark.parametrize("boxed", [False, True])
+def test_shape_cvs_over_range_groups_match_oracle(torch, psg, boxed):
+    """gyration-tensor shape CVs over CONTIGUOUS RANGES (the polymer windows of config 3 are where PrincipalMoment /
+    Asphericity are used): second moments by k_range_second, Jacobian w_i M (r_i - c) applied by the
+    dense kernel; mass-weighted, overlapping ranges, next to an Rg CV, under a harmonic bias; with and without a box"""
+    rng = np.random.default_rng(77)
+    R, N = 3, 5003
+    xyz = np.cumsum(0.15 * rng.standard_normal((R, N, 3)) * np.array([1.6, 1.0, 0.6]), axis=1) + 40.0
+    pos = np.zeros((R, N, 4), np.float32)
+    pos[..., :3] = xyz
+    pos[..., 3] = 1.25
+    aw = rng.uniform(1.0, 12.0, size=N).astype(np.float32)
+    box = None
+    if boxed:
+        ext = float(np.ptp(xyz, axis=1).max())
+        box = np.ceil(np.array([2.4, 2.7, 2.2]) * ext)
+        pos[..., :3] = np.mod(xyz, box).astype(np.float32)
+        assert (np.abs(pos[..., :3] - xyz) > 1).any()
+    defs = [("asphericity", [("range", 0, N)], 0), ("principal_moment", [("range", 400, 3100)], 1), ("rgyr", [("range", 0, N)], 0),
+            ("shape_anisotropy", [("range", 2500, N - 2500)], 0)]
+    okind = {"asphericity": orc.ASPHERICITY, "principal_moment": orc.PRINCIPAL_MOMENT, "rgyr": orc.RGYR, "shape_anisotropy": orc.SHAPE_ANISOTROPY}
+    gkind = {"asphericity": psg.CV_ASPHERICITY, "principal_moment": psg.CV_PRINCIPAL_MOMENT, "rgyr": psg.CV_RGYR,
+             "shape_anisotropy": psg.CV_SHAPE_ANISOTROPY}
+    sysm = orc.System(R, N, N, 4, [{"type": okind[k], "groups": g, "axis": ax, "period": 0.0} for k, g, ax in defs], None, atom_weight=aw, box=box)
+    ctx = psg.Context(0)
+    ctx.set_layout(R, N, N, 4, 4)
+    ctx.set_cvs([{"type": gkind[k], "groups": g, "axis": ax, "period": 0.0} for k, g, ax in defs], None, None, aw)
+    if boxed:
+        ctx.set_box(box)
+    xi_ref = sysm.cv_eval(pos, want_jac=False)
+    ks = np.array([30.0, 20.0, 100.0, 500.0], np.float32)
+    cen = (xi_ref * rng.uniform(0.8, 1.2, size=xi_ref.shape)).astype(np.float32)
+    ctx.set_harmonic(ks, cen)
+    f0 = (rng.standard_normal((R, N, 4)) * 30).astype(np.float32)
+    d_f = dev(torch, f0)
+    ctx.step(dev(torch, pos), d_f, None, 1)
+    ctx.sync_check()
+    out = {k: v.cpu().numpy() for k, v in ctx.read_step_outputs().items()}
+    assert_close(out["xi"], xi_ref, "shape CVs over ranges: xi")
+    V, dV = orc.harmonic(xi_ref.astype(np.float32).astype(np.float64), ks, cen, np.zeros(4))
+    assert_close(out["V"], V, "V")
+    assert_close(out["dVdxi"], dV, "dV/dxi")
+    f_ref = sysm.apply_forces(pos, dV, f0[..., :3].astype(np.float64))
+    assert_forces_close(d_f.cpu().numpy()[..., :3], f_ref, f0[..., :3], "shape CVs over ranges: forces")
+    assert np.array_equal(d_f.cpu().numpy()[..., 3].view(np.uint32), f0[..., 3].view(np.uint32))
+    ctx.close()
+
+
 def test_shape_cv_argument_errors(torch, psg):
     ctx = psg.Context(0)
     ctx.set_layout(2, 30, 30, 4, 4)
-    with pytest.raises(psg.PsgError):      # a range group
-        ctx.set_cvs([{"type": psg.CV_ASPHERICITY, "groups": [("range", 0, 30)], "axis": 0, "period": 0.0}], np.zeros(0, np.int32))
+    ctx.set_cvs([{"type": psg.CV_ASPHERICITY, "groups": [("range", 0, 30)], "axis": 0, "period": 0.0}], np.zeros(0, np.int32))   # a range is fine
+    with pytest.raises(psg.PsgError):      # ... but not beyond the array
+        ctx.set_cvs([{"type": psg.CV_ASPHERICITY, "groups": [("range", 10, 30)], "axis": 0, "period": 0.0}], np.zeros(0, np.int32))
     with pytest.raises(psg.PsgError):      # which eigenvalue?
         ctx.set_cvs([{"type": psg.CV_PRINCIPAL_MOMENT, "groups": [("slots", 0, 5)], "axis": 3, "period": 0.0}], np.arange(5, dtype=np.int32))
     ctx.close()

@@ -133,3 +133,32 @@ def test_anisotropy_jacobian_is_smooth_through_degenerate_eigenvalues():
     t = np.trace(S)
     M = 3 * S / t ** 2 - 3 * np.trace(S @ S) / t ** 3 * np.eye(3)
     assert np.allclose(jac, (2.0 / 6.0) * xyz @ M.T, atol=1e-14)
+
+
+@pytest.mark.parametrize("cv_type,axis", SHAPES)
+def test_contiguous_range_group_equals_the_tensor_assembled_here(cv_type, axis):
+    """the same CVs over a contiguous atom range with per-atom weights (how a polymer window uses them): value against
+    numpy.linalg.eigvalsh of the tensor assembled here, forces against central finite differences of the value"""
+    rng = np.random.default_rng(21)
+    n, first = 60, 7
+    xyz = rng.standard_normal((first + n + 5, 3)) * np.array([2.0, 1.0, 0.5]) + 30.0
+    aw = rng.uniform(1.0, 9.0, size=len(xyz)).astype(np.float32)
+    pos = np.zeros((1, len(xyz), 4), np.float32)
+    pos[0, :, :3] = xyz
+    cv = {"type": cv_type, "groups": [("range", first, n)], "axis": axis, "period": 0.0}
+    s = orc.System(1, len(xyz), len(xyz), 4, [cv], None, atom_weight=aw)
+    lam = np.sort(np.linalg.eigvalsh(_tensor(pos[0, first:first + n, :3], aw[first:first + n])))[::-1]
+    b, c = lam[0] - 0.5 * (lam[1] + lam[2]), lam[1] - lam[2]
+    want = {orc.PRINCIPAL_MOMENT: lam[axis], orc.ASPHERICITY: b, orc.ACYLINDRICITY: c,
+            orc.SHAPE_ANISOTROPY: (b * b + 0.75 * c * c) / lam.sum() ** 2}[cv_type]
+    assert s.cv_eval(pos, want_jac=False)[0, 0] == pytest.approx(want, rel=1e-10)
+    f = s.apply_forces(pos, np.array([[1.0]]), np.zeros((1, len(xyz), 3)))       # F = -d xi / d r
+    assert np.all(f[0, :first] == 0) and np.all(f[0, first + n:] == 0)
+    h = 2.0 ** -9
+    for a in (first, first + 17, first + n - 1):
+        for x in range(3):
+            p, m = pos.copy(), pos.copy()
+            p[0, a, x] += h
+            m[0, a, x] -= h
+            d = (s.cv_eval(p, want_jac=False)[0, 0] - s.cv_eval(m, want_jac=False)[0, 0]) / (2 * h)
+            assert -f[0, a, x] == pytest.approx(d, rel=2e-5, abs=1e-7)
