@@ -41,7 +41,7 @@ __global__ void __launch_bounds__(256, 4) k_abf_step(const __grid_constant__ Sys
             const long long o = ((long long)r * P.n_slots + s) * 3;
             A.jac[o] = (float)j.x; A.jac[o + 1] = (float)j.y; A.jac[o + 2] = (float)j.z;
             // the force record phase 2 will update, requested into L2 now (the arrays are GBs: a cold miss otherwise)
-            const int atom = P.slot_atom[(P.per_rep ? (long long)r * P.n_slots : 0) + s];
+            const int atom = slot_atom_of(P, r, s);
             asm volatile("prefetch.global.L2 [%0];" ::"l"(A.force + ((long long)r * P.rstride + atom) * P.fs));
         }
         if (lane == 0) {
@@ -71,9 +71,9 @@ __global__ void __launch_bounds__(256, 4) k_abf_step(const __grid_constant__ Sys
         if (lane == 0) abf_mean_one(G, P.n_cv, A.bin_out[r], dV);
         __syncwarp();
         for (int s = lane; s < P.n_slots; s += 32) {
-            const int gid = P.slot_gid[s];
+            const int gid = P.slot_gid_c[s];
             const float dv = -dV[P.grp[gid].cv];
-            const int atom = P.slot_atom[(P.per_rep ? (long long)r * P.n_slots : 0) + s];
+            const int atom = slot_atom_of(P, r, s);
             float* f = A.force + ((long long)r * P.rstride + atom) * P.fs;
             const float* j = A.jac + ((long long)r * P.n_slots + s) * 3;
             force_add(f, dv * j[0], dv * j[1], dv * j[2], P.fs);

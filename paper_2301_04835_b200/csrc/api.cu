@@ -251,6 +251,7 @@ int psg_set_cvs(psg_ctx* c, int n_cv, const psg_cv_desc* cvs, int n_slots, const
         CK(c, cudaMemcpy(c->d_atom_weight, atom_weight, (size_t)P.N * sizeof(float), cudaMemcpyHostToDevice));
     }
     for (int i = 0; i < PSG_MAX_SLOTS; ++i) P.slot_atom_c[i] = (!per_rep && i < n_slots) ? slot_atom[i] : 0;
+    for (int i = 0; i < PSG_MAX_SLOTS; ++i) P.slot_gid_c[i] = (unsigned char)(i < n_slots ? slot_gid[i] : 0);
     P.simple_groups = (P.n_ranges == 0 && !P.any_rgyr) ? 1 : 0;
     for (int k = 0; k < PSG_MAX_CV; ++k)
         for (int g = 0; g < PSG_MAX_GROUPS; ++g) {

@@ -177,9 +177,9 @@ __global__ void __launch_bounds__(256) k_apply_sparse(const __grid_constant__ Sy
     long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     if (t >= (long long)P.R * P.n_slots) return;
     int r = (int)(t / P.n_slots), s = (int)(t % P.n_slots);
-    int gid = P.slot_gid[s];
+    int gid = P.slot_gid_c[s];
     float dv = -dVdxi[(long long)r * P.n_cv + P.grp[gid].cv];
-    int atom = P.slot_atom[(P.per_rep ? (long long)r * P.n_slots : 0) + s];
+    int atom = slot_atom_of(P, r, s);
     float* f = force + ((long long)r * P.rstride + atom) * P.fs;
     const float* j = jac + t * 3;
     force_add(f, dv * j[0], dv * j[1], dv * j[2], P.fs);

@@ -239,6 +239,12 @@ __device__ __forceinline__ double shape_from_eigenvalues(int type, int axis, con
 }
 #define PSG_COEF_SHAPE (-1.0)   // WarpCvSmem::coef of a shape-CV group: sec[] holds (2/W) sum_k g_k v_k v_k^T
 
+// atom of slot s of replica r: a shared index list is read from the kernel parameters (no global load ahead of the gather:
+// with a cold L2 the index load and the position load were two dependent DRAM round trips), a per-replica one from memory
+__device__ __forceinline__ int slot_atom_of(const SysParams& P, int r, int s) {
+    return P.per_rep ? __ldg(P.slot_atom + (long long)r * P.n_slots + s) : P.slot_atom_c[s];
+}
+
 __device__ __forceinline__ double warp_sum(double v) {
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
@@ -305,15 +311,14 @@ __device__ __forceinline__ void warp_cv_eval(const SysParams& P, int r, const fl
     // explicit groups: lane j gathers group j
     if (lane < P.n_groups && !P.grp[lane].is_range) {
         const GroupDev& G = P.grp[lane];
-        const int* sa = P.slot_atom + (P.per_rep ? (long long)r * P.n_slots : 0);
         double sx = 0, sy = 0, sz = 0, sw = 0, s2 = 0;
         double q[6] = {0, 0, 0, 0, 0, 0};
         const bool shape = is_shape_cv(P.cv[G.cv].type);
         const double* box = sys_box(P);
-        const D3 first = load_pos(p, sa[G.begin], P.ps);
+        const D3 first = load_pos(p, slot_atom_of(P, r, G.begin), P.ps);
         for (int i = 0; i < G.size; ++i) {
             int s = G.begin + i;
-            D3 x = load_pos(p, sa[s], P.ps);
+            D3 x = load_pos(p, slot_atom_of(P, r, s), P.ps);
             if (box) x = first + min_image(x - first, box);   // the image nearest to the group's first atom
             double w = P.slot_weight ? (double)P.slot_weight[s] : 1.0;
             sx += w * x.x; sy += w * x.y; sz += w * x.z; sw += w;
@@ -387,14 +392,13 @@ __device__ __forceinline__ void warp_cv_eval(const SysParams& P, int r, const fl
 // d(xi)/d(r_slot) for an explicit slot s (weight w_s) given the per-group vector
 __device__ __forceinline__ D3 slot_jacobian(const SysParams& P, int r, const float* __restrict__ pos,
                                             const WarpCvSmem& sm, int s) {
-    int gid = P.slot_gid[s];
+    int gid = P.slot_gid_c[s];
     double w = P.slot_weight ? (double)P.slot_weight[s] : 1.0;
     D3 j = d3(w * sm.v[gid][0], w * sm.v[gid][1], w * sm.v[gid][2]);
     if (sm.coef[gid] != 0.0) {   // explicit RGYR group: w (r - c) / (W Rg); shape-CV group: w M (r - c)
-        const int* sa = P.slot_atom + (P.per_rep ? (long long)r * P.n_slots : 0);
-        D3 x = load_pos(pos + (long long)r * P.rstride * P.ps, sa[s], P.ps);
+        D3 x = load_pos(pos + (long long)r * P.rstride * P.ps, slot_atom_of(P, r, s), P.ps);
         if (P.has_box) {
-            const D3 first = load_pos(pos + (long long)r * P.rstride * P.ps, sa[P.grp[gid].begin], P.ps);
+            const D3 first = load_pos(pos + (long long)r * P.rstride * P.ps, slot_atom_of(P, r, P.grp[gid].begin), P.ps);
             x = first + min_image(x - first, P.box);
         }
         const D3 d = d3(x.x - sm.cen[gid][0], x.y - sm.cen[gid][1], x.z - sm.cen[gid][2]);

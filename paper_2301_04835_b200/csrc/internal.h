@@ -50,6 +50,7 @@ struct SysParams {
     long long span_begin, span_end;          // union span of all range groups
     int range_blocks;                        // blocks per replica over the span
     int slot_atom_c[PSG_MAX_SLOTS];          // shared index list (per_rep == 0): read from kernel parameters
+    unsigned char slot_gid_c[PSG_MAX_SLOTS]; // global group id of a slot, from kernel parameters too (slot_gid is the device copy)
     // fast gather of the fused metadynamics step: when every group is ONE explicit atom (simple_groups), group g of CV k
     // is slot cv_slot[4 k + g] and, with a shared index list, atom cv_atom[4 k + g]; unused groups repeat group 0
     int simple_groups;

@@ -251,8 +251,8 @@ __global__ void __launch_bounds__(256) k_grid_step(const __grid_constant__ SysPa
     __syncwarp();
     for (int s = lane; s < P.n_slots; s += 32) {
         const D3 j = slot_jacobian(P, r, pos, S, s);
-        const float dv = -s_dv[wid][P.grp[P.slot_gid[s]].cv];
-        const int atom = P.slot_atom[(P.per_rep ? (long long)r * P.n_slots : 0) + s];
+        const float dv = -s_dv[wid][P.grp[P.slot_gid_c[s]].cv];
+        const int atom = slot_atom_of(P, r, s);
         float* f = force + ((long long)r * P.rstride + atom) * P.fs;
         force_add(f, dv * (float)j.x, dv * (float)j.y, dv * (float)j.z, P.fs);
     }
