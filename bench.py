@@ -59,8 +59,8 @@ def hill_eval_instr_f64(n_cv, n_periodic):
 
 # dram__bytes_read.sum + dram__bytes_write.sum of ONE launch of the dominant kernel, bytes, NOT measured in this run:
 # copied from the committed ncu --set full captures named here
-NCU_TRAFFIC = {1: (1.23e6, "profiles/r1b_hills_config1_ncu_full.md"), 2: (8.58e6, "profiles/r1b_abf_step_config2_ncu_full.md"),
-               3: (1.2412e9, "profiles/r1b_range_step_config3_ncu_full.md"), 4: (5.87e6, "profiles/r1b_hills_config4_ncu_full.md")}
+NCU_TRAFFIC = {1: (1.224e6, "profiles/r2_hills_config1_ncu_full.md"), 2: (8.58e6, "profiles/r1b_abf_step_config2_ncu_full.md"),
+               3: (1.2412e9, "profiles/r1b_range_step_config3_ncu_full.md"), 4: (5.98e6, "profiles/r2_hills_config4_ncu_full.md")}
 
 
 def _peaks():
