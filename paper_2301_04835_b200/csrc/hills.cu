@@ -102,17 +102,6 @@ __global__ void k_null_hills(int begin, int end, int rec, float4* __restrict__ h
 }
 
 // ---------------------------------------------------------------- host side
-#ifdef PSG_TRACE
-static long long* g_trace = nullptr;
-long long* psg_trace_buffer() {
-    if (!g_trace) { cudaMalloc(&g_trace, 4096 * 32 * sizeof(long long)); cudaMemset(g_trace, 0, 4096 * 32 * sizeof(long long)); }
-    return g_trace;
-}
-extern "C" int psg_debug_trace_clear() { return (int)cudaMemset(psg_trace_buffer(), 0, 4096 * 32 * sizeof(long long)); }
-extern "C" int psg_debug_trace(long long* host_out, int n_ctas) {
-    return (int)cudaMemcpy(host_out, psg_trace_buffer(), (size_t)n_ctas * 32 * sizeof(long long), cudaMemcpyDeviceToHost);
-}
-#endif
 bool psg_stream_capturing(const psg_ctx* c) {
     cudaStreamCaptureStatus st = cudaStreamCaptureStatusNone;
     if (cudaStreamIsCapturing(c->stream, &st) != cudaSuccess) { st = cudaStreamCaptureStatusNone; (void)cudaGetLastError(); }
@@ -162,9 +151,6 @@ static HillKernelArgs base_args(psg_ctx* c) {
     // launch may be replayed with a longer list than the one seen now, and after a CAPTURED deposit the replays grow the
     // list behind the host's back: in both cases the kernel reads the device counter.
     A.n_h_host = (psg_stream_capturing(c) || c->count_unknown) ? -1 : (int)c->nh_bound;
-#ifdef PSG_TRACE
-    A.trace = psg_trace_buffer();
-#endif
     return A;
 }
 

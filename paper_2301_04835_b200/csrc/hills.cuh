@@ -299,13 +299,6 @@ __device__ __forceinline__ void accumulate_f64(const float4* __restrict__ sm, co
     __syncwarp();
 }
 
-#ifdef PSG_TRACE
-#define PSG_CLK_EARLY(i) do { if (threadIdx.x == 0 && blockIdx.x == 0 && g_trace_slot) g_trace_slot[16 + (i)] = clock64() - g_clk0; } while (0)
-__device__ long long* g_trace_slot = nullptr;   // debug builds: the CTA's stamp row, set by thread 0
-__device__ long long g_clk0 = 0;
-#else
-#define PSG_CLK_EARLY(i) do { } while (0)
-#endif
 // lane-local CV of (replica r, CV k) for systems with explicit groups only; dc[g] = d xi / d c_g / W_g.
 template <bool JAC>
 __device__ __forceinline__ double thread_cv(const SysParams& P, int r, int k, const float* __restrict__ pos, D3* dc) {
@@ -317,7 +310,6 @@ __device__ __forceinline__ double thread_cv(const SysParams& P, int r, int k, co
     // Fast path (measured: the gather, not the arithmetic, was half of the prologue): every group a single unweighted
     // atom -- a single atom is its own barycenter -- so all indices are formed first and the four position loads are in
     // flight together instead of one dependent (index -> position) chain per group.
-    PSG_CLK_EARLY(3);
     bool single = !P.slot_weight;
 #pragma unroll
     for (int g = 0; g < 4; ++g)
@@ -329,22 +321,11 @@ __device__ __forceinline__ double thread_cv(const SysParams& P, int r, int k, co
             const int s = P.grp[C.gid0 + (g < C.n_groups ? g : 0)].begin;   // unused groups re-read group 0 (no branch)
             a[g] = P.per_rep ? sa[s] : P.slot_atom_c[s];                    // shared index lists come from kernel parameters
         }
-#ifdef PSG_TRACE
-        if (threadIdx.x == 0 && blockIdx.x == 0 && g_trace_slot) { long long t_ = clock64() - g_clk0 + (a[0] + a[1] + a[2] + a[3] == -12345 ? 1 : 0); g_trace_slot[16 + 4] = t_; }
-#endif
 #pragma unroll
         for (int g = 0; g < 4; ++g) {
             c[g] = load_pos(p, a[g], P.ps);
             W[g] = 1.0;
         }
-#ifdef PSG_TRACE
-        if (threadIdx.x == 0 && blockIdx.x == 0 && g_trace_slot) {   // thread 0: all four positions have arrived
-            long long t_;
-            asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t_) : "d"(c[0].x + c[1].x + c[2].x + c[3].x));
-            g_trace_slot[9] = t_;
-            g_trace_slot[16 + 5] = clock64() - g_clk0;
-        }
-#endif
     } else {
 #pragma unroll
         for (int g = 0; g < 4; ++g) {
@@ -409,20 +390,7 @@ struct HillKernelArgs {
     int Lc_host, n_chunks_host;   // the chunking for n_h_host (computed on the host: three integer divisions off the kernel's entry path)
     float inv_n_rt;          // 1 / (number of replica tiles), for the item -> (tile, chunk) split
     int simple;              // fused: every group one unweighted atom, no box: the lean gather (SysParams::cv_slot / cv_atom)
-#ifdef PSG_TRACE
-    long long* trace;        // [grid][8] clock64 stamps of the first item of every CTA (debug builds only)
-#endif
 };
-#ifdef PSG_TRACE
-#define PSG_TS 32
-#define PSG_CLK(i) do { if (threadIdx.x == 0 && blockIdx.x == 0 && g_trace_slot) g_trace_slot[16 + (i)] = clock64() - g_clk0; } while (0)
-#define PSG_STAMP(i) do { if (threadIdx.x == 0 && item == (int)blockIdx.x && A.trace) { long long t_; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t_)); A.trace[blockIdx.x * PSG_TS + (i)] = t_; } } while (0)
-#define PSG_STAMP_T(tidx, i) do { if (threadIdx.x == (tidx) && item == (int)blockIdx.x && A.trace) { long long t_; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t_)); A.trace[blockIdx.x * PSG_TS + (i)] = t_; } } while (0)
-#else
-#define PSG_STAMP(i) do { } while (0)
-#define PSG_STAMP_T(tidx, i) do { } while (0)
-#define PSG_CLK(i) do { } while (0)
-#endif
 
 // chunk length (a multiple of 32, at least 32) and number of chunks per replica tile for n_h hills on `grid` CTAs
 __host__ __device__ inline void hills_chunking(int n_h, int grid, int n_rt, int& Lc, int& n_chunks) {
@@ -475,9 +443,6 @@ __global__ void __launch_bounds__(HWARPS * 32, 1) k_hills(const __grid_constant_
     constexpr int SUBH = SUB / REC;   // hills per stage: a stage is always SUB x 16 bytes
     constexpr int NV = 1 + NCV;
     constexpr int NT = HWARPS * 32;
-#ifdef PSG_TRACE
-    if (threadIdx.x == 0 && blockIdx.x == 0) { g_clk0 = clock64(); g_trace_slot = A.trace; }
-#endif
     extern __shared__ __align__(128) unsigned char smem_raw[];
     constexpr int WACC = ((RT * NV + 31) / 32) * 32;   // per-warp binary64 totals (padded to whole butterfly passes)
     constexpr int PASSES = WACC / 32;
@@ -526,7 +491,6 @@ __global__ void __launch_bounds__(HWARPS * 32, 1) k_hills(const __grid_constant_
         hills_chunking(n_h, (int)gridDim.x, n_rt, Lc, n_chunks);
     }
     const int items = n_rt * n_chunks;
-    PSG_CLK(8);
     // One thread with no CV work of its own (lane 0 of the last warp) owns the barriers and the first TMA loads of an item;
     // nobody else touches them before the __syncthreads that follows the CV prologue.
     const bool producer = tid == NT - 32;
@@ -535,7 +499,6 @@ __global__ void __launch_bounds__(HWARPS * 32, 1) k_hills(const __grid_constant_
         for (int s = 0; s < STG; ++s) mbar_init(&full[s], 1);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
-    PSG_CLK(9);
     unsigned seq = 0;   // sub-tiles consumed so far by this CTA (stage = seq % STG, parity = (seq / STG) & 1)
 
     // Lean gather (every group a single unweighted atom, no box: the ADP dihedrals of PAPER.md:L81 and every BASELINE.json
@@ -593,8 +556,6 @@ __global__ void __launch_bounds__(HWARPS * 32, 1) k_hills(const __grid_constant_
         if (len > Lc) len = Lc;
         if (len < 0) len = 0;
         const int n_st = (len + SUBH - 1) / SUBH;
-        PSG_STAMP(0);
-        PSG_CLK(0);
         if (producer) {
             for (int t = 0; t < n_st && t < STG; ++t) {
                 int s = (seq + t) % STG;
@@ -603,8 +564,6 @@ __global__ void __launch_bounds__(HWARPS * 32, 1) k_hills(const __grid_constant_
                 tma_load_1d(stage + s * SUBH * REC, A.hills + (size_t)(h0 + t * SUBH) * REC, (uint32_t)cnt * REC * 16u, &full[s]);
             }
         }
-        PSG_STAMP(8);
-        PSG_CLK(1);
         // CV values (and per-group Jacobian vectors) of this tile's replicas; overlaps the first TMA loads
         if (A.fused && A.simple) {
             if (!lean_done) {
@@ -638,8 +597,6 @@ __global__ void __launch_bounds__(HWARPS * 32, 1) k_hills(const __grid_constant_
                         if (chunk == 0 && A.xi_out) A.xi_out[(long long)r * NCV + k] = v;
                     }
                     s_xi[k * TILE_R + rr] = v;
-                    PSG_STAMP(10);
-                    PSG_CLK(6);
                 } else if (r < R) {
                     D3 dc[4];
                     if (chunk == 0) prefetch_force_lines(P, r, k, A.force);
@@ -651,7 +608,6 @@ __global__ void __launch_bounds__(HWARPS * 32, 1) k_hills(const __grid_constant_
                             float* j = s_jv + (rr * P.n_groups + C.gid0 + g) * 3;
                             j[0] = (float)dc[g].x; j[1] = (float)dc[g].y; j[2] = (float)dc[g].z;
                         }
-                    PSG_STAMP_T(TILE_R * NCV, 11);
                 }
             }
         } else {
@@ -661,8 +617,6 @@ __global__ void __launch_bounds__(HWARPS * 32, 1) k_hills(const __grid_constant_
             }
         }
         __syncthreads();
-        PSG_STAMP(1);
-        PSG_CLK(7);
         const bool warp_active = r0 + w8 * RT < R;
         // Stage hand-back without a CTA-wide barrier (measured: the bare loop reaches 0.95 of the FFMA peak, the loop with a
         // barrier per 1,024 hills 0.80): warps drift freely; lane 0 counts its warp out of the stage with a shared-memory
@@ -710,7 +664,6 @@ __global__ void __launch_bounds__(HWARPS * 32, 1) k_hills(const __grid_constant_
             for (int t = 0; t < n_st; ++t) {
                 const int s = seq % STG;
                 if (!ready) mbar_wait(&full[s], (seq / STG) & 1);
-                if (t == 0) PSG_STAMP(12);
                 const int cnt = min(SUBH, len - t * SUBH);
                 if (warp_active) {
                     // a full sub-tile gets a compile-time trip count (the compiler then schedules across iterations)
@@ -757,10 +710,8 @@ __global__ void __launch_bounds__(HWARPS * 32, 1) k_hills(const __grid_constant_
             }
         }
         if (lane == 0 && pend_old == HWARPS - 1) s_cnt[PSG_PEND_VARS(NCV) ? pend_s : (int)((seq + STG - 1) % STG)] = 0;   // the item's last count-out (nothing left to refill)
-        PSG_STAMP(2);
         constexpr int TV = TILE_R * NV;
         __syncthreads();
-        PSG_STAMP(14);
         // Warps w8 and w8 + HHALF (the two halves of the chunk's hills) in fixed order -> this chunk's partial of the tile.
         // The CTA of chunk 0 FINISHES the tile: the others publish their partials and are done; it keeps its own on chip
         // and collects theirs.  A published value is ONE 64-bit word that carries its own valid flag -- the lowest mantissa
@@ -776,10 +727,8 @@ __global__ void __launch_bounds__(HWARPS * 32, 1) k_hills(const __grid_constant_
             if (finisher) s_out[t] = val;
             else __stcg(part_bits + (size_t)(chunk * n_rt + tile) * TV + t, (u64)__double_as_longlong(val) | 1ull);
         }
-        PSG_STAMP(3);
         if (finisher) {
             __syncthreads();
-            PSG_STAMP(4);
             // chunk partials in fixed order; two thread groups split the chunks so that more loads are in flight
             constexpr int PARTS = NT >= 2 * TV ? 2 : 1;
             constexpr int BATCH = 9;   // words in flight per thread (config 1: 18 chunks per tile = 2 groups x 9: one round trip)
@@ -829,7 +778,6 @@ __global__ void __launch_bounds__(HWARPS * 32, 1) k_hills(const __grid_constant_
             }
             if (A.fused) {
                 __syncthreads();
-                PSG_STAMP(5);
                 // forces: L2 reductions (atoms shared by CVs / walkers collide).  Lean gather: one thread per (replica, group),
                 // atom and Jacobian out of shared memory -- no global load between the last sum and the reductions
                 if (A.simple) {
@@ -858,12 +806,5 @@ __global__ void __launch_bounds__(HWARPS * 32, 1) k_hills(const __grid_constant_
             }
         }
         __syncthreads();   // s_xi / s_out / s_wacc are reused by the next item
-        PSG_STAMP(6);
-#ifdef PSG_TRACE
-        if (threadIdx.x == 0 && item == (int)blockIdx.x && A.trace) {
-            unsigned smid; asm volatile("mov.u32 %0, %%smid;" : "=r"(smid));
-            A.trace[blockIdx.x * PSG_TS + 7] = smid;
-        }
-#endif
     }
 }

@@ -174,6 +174,3 @@ cudaError_t psg_launch_range_step(psg_ctx* c, const float* d_pos, float* d_force
 bool psg_stream_capturing(const psg_ctx* c);
 size_t psg_hill_part_doubles(const psg_ctx* c, int* max_chunks_out, int* n_rtiles_out);
 
-#ifdef PSG_TRACE
-long long* psg_trace_buffer();   // debug builds: [4096][8] clock64 stamps
-#endif

@@ -56,9 +56,6 @@ struct RangeStepArgs {
     unsigned* done;         // [R]  slices whose forces are written
     float4* desc;           // [R][n_ranges][RS_DESC]
     int lag;                // items PA may run ahead of the B group
-#ifdef PSG_TRACE
-    long long* trace;
-#endif
 };
 
 __device__ __forceinline__ uint32_t rs_smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
@@ -107,21 +104,6 @@ __device__ __forceinline__ float4 rs_ld_relaxed_f4(const float4* p) {   // one 1
     return v;
 }
 
-#ifdef PSG_TRACE
-// debug builds: cycles each role spends waiting, summed over the launch, [grid][16] (lane 0 / thread 0 of the role)
-__device__ __forceinline__ long long rs_gt() { long long t; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t)); return t; }
-#define RS_GSTAMP(cond, i) do { if ((cond) && A.trace) A.trace[blockIdx.x * 32 + (i)] = rs_gt(); } while (0)
-#define RS_T0 long long rs_t0_ = clock64()
-#define RS_ACC(slot) do { rs_acc_[slot] += clock64() - rs_t0_; } while (0)
-#define RS_DECL long long rs_acc_[3] = {0, 0, 0}; const long long rs_start_ = clock64()
-#define RS_FLUSH(cond, base) do { if ((cond) && A.trace) { for (int z_ = 0; z_ < 3; ++z_) A.trace[blockIdx.x * 32 + (base) + z_] = rs_acc_[z_]; A.trace[blockIdx.x * 32 + (base) + 3] = clock64() - rs_start_; } } while (0)
-#else
-#define RS_GSTAMP(cond, i) do { } while (0)
-#define RS_T0 do { } while (0)
-#define RS_ACC(slot) do { } while (0)
-#define RS_DECL do { } while (0)
-#define RS_FLUSH(cond, base) do { } while (0)
-#endif
 
 struct RsShared {
     double red[RS_RED][RS_GT / 32][PSG_MAX_RANGE_GROUPS][PSG_MOM];   // A group -> T warps: per-warp partial moments
@@ -366,9 +348,6 @@ __device__ __forceinline__ void rs_tail(const SysParams& P, const RangeStepArgs&
 // B group, one item: force update of the slice; positions and forces out of shared memory, result streamed to global
 __device__ __forceinline__ void rs_phase_b(const SysParams& P, const RangeStepArgs& A, RsShared& S, const float4* __restrict__ sp,
                                            const float4* __restrict__ sf, const RsItem& I, int tid, int db, int r_next) {
-#ifdef PSG_TRACE
-    const long long rs_p0_ = clock64();
-#endif
     if (tid < P.n_ranges * RS_DESC) {
         // this thread's record was requested one item ago (cp.async, no registers held): in steady state it is already
         // here and the L2 round trip is off the critical path; poll only if the window was not finished yet
@@ -379,9 +358,6 @@ __device__ __forceinline__ void rs_phase_b(const SysParams& P, const RangeStepAr
         while (d.w != RS_TAG) {
             d = rs_ld_relaxed_f4(src);
             if (d.w != RS_TAG) __nanosleep(200);
-#ifdef PSG_TRACE
-            if (tid == 0 && A.trace) A.trace[blockIdx.x * 32 + 24] += 1;   // polls
-#endif
         }
         *mine = d;
         if (r_next >= 0) {
@@ -417,9 +393,6 @@ __device__ __forceinline__ void rs_phase_b(const SysParams& P, const RangeStepAr
         S.bfast[db] = fast && any;
     }
     rs_b_sync();
-#ifdef PSG_TRACE
-    if (tid == 0 && A.trace) A.trace[blockIdx.x * 32 + 25] += clock64() - rs_p0_;   // poll + group barrier
-#endif
     float4* f = reinterpret_cast<float4*>(A.force) + I.a0;
     const long long t0 = P.span_begin + (long long)I.s * RS_SLICE;
     // group-major, the thread's RS_PERB atoms side by side (independent chains); per atom the groups are still
@@ -490,8 +463,6 @@ __global__ void __launch_bounds__(RS_THREADS, 1) k_range_step(const __grid_const
     const long long items = (long long)P.R * P.range_blocks;
     const long long G = gridDim.x;
     const long long n_mine = blockIdx.x < items ? (items - blockIdx.x + G - 1) / G : 0;
-
-    RS_GSTAMP(tid == 0, 31);
     if (tid == 0) {
         for (int st = 0; st < RS_ASTAGES; ++st) { rs_mbar_init(&S.a_full[st], 1); rs_mbar_init(&S.a_empty[st], RS_GT / 32); }
         for (int st = 0; st < RS_BSTAGES; ++st) { rs_mbar_init(&S.b_full[st], 1); rs_mbar_init(&S.b_empty[st], RS_GTB / 32); }
@@ -511,32 +482,28 @@ __global__ void __launch_bounds__(RS_THREADS, 1) k_range_step(const __grid_const
         // ---------------- PA: positions -> ring A, at most `lag` items ahead of the B group
         if (lane == 0) {
             const uint64_t keep = rs_policy_evict_last();
-            RS_DECL;
             for (long long it = 0; it < n_mine; ++it) {
                 const int st = (int)(it % RS_ASTAGES);
-                { RS_T0; if (it >= RS_ASTAGES) rs_mbar_wait(&S.a_empty[st], (uint32_t)((it / RS_ASTAGES - 1) & 1)); RS_ACC(0); }
-                { RS_T0; while (it - S.b_prog > A.lag) __nanosleep(200); RS_ACC(1); }
+                if (it >= RS_ASTAGES) rs_mbar_wait(&S.a_empty[st], (uint32_t)((it / RS_ASTAGES - 1) & 1));
+                while (it - S.b_prog > A.lag) __nanosleep(200);
                 const RsItem I = rs_item(P, it, G);
                 rs_mbar_expect_tx(&S.a_full[st], I.bytes);
                 rs_tma_load_1d(ring_a + (size_t)st * RS_SLICE, reinterpret_cast<const float4*>(A.pos) + I.a0, I.bytes, &S.a_full[st], keep);
             }
-            RS_FLUSH(true, 0);
         }
     } else if (warp == 1) {
         // ---------------- PB: positions (L2) + forces -> ring B
         if (lane == 0) {
             const uint64_t once = rs_policy_evict_first();
-            RS_DECL;
             for (long long it = 0; it < n_mine; ++it) {
                 const int st = (int)(it % RS_BSTAGES);
-                { RS_T0; if (it >= RS_BSTAGES) rs_mbar_wait(&S.b_empty[st], (uint32_t)((it / RS_BSTAGES - 1) & 1)); RS_ACC(0); }
+                if (it >= RS_BSTAGES) rs_mbar_wait(&S.b_empty[st], (uint32_t)((it / RS_BSTAGES - 1) & 1));
                 const RsItem I = rs_item(P, it, G);
                 float4* dst = ring_b + (size_t)st * 2 * RS_SLICE;
                 rs_mbar_expect_tx(&S.b_full[st], 2u * I.bytes);
                 rs_tma_load_1d(dst, reinterpret_cast<const float4*>(A.pos) + I.a0, I.bytes, &S.b_full[st], once);
                 rs_tma_load_1d(dst + RS_SLICE, reinterpret_cast<const float4*>(A.force) + I.a0, I.bytes, &S.b_full[st], once);
             }
-            RS_FLUSH(true, 4);
         }
     } else if (warp == 2) {
         // ---------------- W: windows b, b + grid, ...
@@ -550,55 +517,41 @@ __global__ void __launch_bounds__(RS_THREADS, 1) k_range_step(const __grid_const
             }
             __syncwarp();
             __threadfence();
-#ifdef PSG_TRACE
-            const long long w0_ = clock64();
-#endif
             rs_window(P, A, S, (int)r, lane);
-#ifdef PSG_TRACE
-            if (lane == 0 && A.trace) { A.trace[blockIdx.x * 32 + 28] += clock64() - w0_; A.trace[blockIdx.x * 32 + 29] += 1; }
-#endif
         }
     } else if (warp < 3 + RS_NT) {
         // ---------------- T warp j: items j, j + RS_NT, ...
         const int j = warp - 3;
-        RS_DECL;
         for (long long it = j; it < n_mine; it += RS_NT) {
             const int buf = (int)(it % RS_RED);
             const RsItem I = rs_item(P, it, G);
-            { RS_T0; rs_mbar_wait(&S.red_full[buf], (uint32_t)((it / RS_RED) & 1)); RS_ACC(0); }
-            { RS_T0; rs_tail(P, A, S, I, buf, lane); RS_ACC(1); }
+            rs_mbar_wait(&S.red_full[buf], (uint32_t)((it / RS_RED) & 1));
+            rs_tail(P, A, S, I, buf, lane);
         }
-        RS_FLUSH(lane == 0, 8 + 4 * j);
     } else if (tid < RS_LEAD + RS_GT) {
         // ---------------- A group
         const int t = tid - RS_LEAD;
-        RS_DECL;
         for (long long it = 0; it < n_mine; ++it) {
             const int st = (int)(it % RS_ASTAGES), buf = (int)(it % RS_RED);
             const RsItem I = rs_item(P, it, G);
-            { RS_T0; rs_mbar_wait(&S.a_full[st], (uint32_t)((it / RS_ASTAGES) & 1)); RS_ACC(0); }
-            { RS_T0; if (it >= RS_RED) rs_mbar_wait(&S.red_empty[buf], (uint32_t)((it / RS_RED - 1) & 1)); RS_ACC(1); }
-            { RS_T0; rs_phase_a(P, S, ring_a + (size_t)st * RS_SLICE, I, buf, t); RS_ACC(2); }
+            rs_mbar_wait(&S.a_full[st], (uint32_t)((it / RS_ASTAGES) & 1));
+            if (it >= RS_RED) rs_mbar_wait(&S.red_empty[buf], (uint32_t)((it / RS_RED - 1) & 1));
+            rs_phase_a(P, S, ring_a + (size_t)st * RS_SLICE, I, buf, t);
             if ((t & 31) == 0) {
                 rs_mbar_arrive(&S.red_full[buf]);   // this warp's partials are in S.red[buf]
                 rs_mbar_arrive(&S.a_empty[st]);     // and it is done reading the stage
             }
         }
-        RS_FLUSH(t == 0, 16);
-        RS_GSTAMP(t == 0, 26);
     } else {
         // ---------------- B group
         const int t = tid - RS_LEAD - RS_GT;
-        RS_DECL;
         for (long long it = 0; it < n_mine; ++it) {
             const int st = (int)(it % RS_BSTAGES);
             const RsItem I = rs_item(P, it, G);
             const float4* sp = ring_b + (size_t)st * 2 * RS_SLICE;
-            { RS_T0; rs_mbar_wait(&S.b_full[st], (uint32_t)((it / RS_BSTAGES) & 1)); RS_ACC(0); }
-            RS_GSTAMP(t == 0 && it == 0, 27);
-            RS_GSTAMP(t == 0 && it == n_mine / 2, 14);
+            rs_mbar_wait(&S.b_full[st], (uint32_t)((it / RS_BSTAGES) & 1));
             const int r_next = it + 1 < n_mine ? rs_item(P, it + 1, G).r : -1;
-            { RS_T0; rs_phase_b(P, A, S, sp, sp + RS_SLICE, I, t, (int)(it % 3), r_next); RS_ACC(1); }
+            rs_phase_b(P, A, S, sp, sp + RS_SLICE, I, t, (int)(it % 3), r_next);
             __syncwarp();
             if ((t & 31) == 0) rs_mbar_arrive(&S.b_empty[st]);   // this warp is done reading the stage
             if (t == 0) {
@@ -612,8 +565,6 @@ __global__ void __launch_bounds__(RS_THREADS, 1) k_range_step(const __grid_const
                 }
             }
         }
-        RS_FLUSH(t == 0, 20);
-        RS_GSTAMP(t == 0, 30);
     }
 }
 
@@ -661,9 +612,6 @@ cudaError_t psg_launch_range_step(psg_ctx* c, const float* d_pos, float* d_force
     // B runs `lag` items behind A: long enough to cover the window dependency (several L2 round trips), short
     // enough that lag x grid x 32 KB of positions stays in L2 (10 x 148 x 32 KB = 47 MB of 126 MB; measured optimum)
     A.lag = c->range_lag > 0 ? c->range_lag : 10;
-#ifdef PSG_TRACE
-    A.trace = psg_trace_buffer();
-#endif
     long long items = (long long)P.R * P.range_blocks;
     long long grid = (long long)c->sm_count * max_blocks_per_sm;
     if (grid > items) grid = items;
