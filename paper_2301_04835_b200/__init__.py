@@ -6,12 +6,12 @@ arguments (ctypes): every step of the path runs in the kernels.  PyTorch is used
 memory and streams, nothing else.  There is no CPU fallback: if libpsg.so is missing or no
 CUDA device is present, calls raise.
 """
-from .psg import (Context, PsgError, load_library, lib_path, measure_alu_peak, configure_from_workload,
+from .psg import (Context, PsgError, load_library, lib_path, measure_alu_peak, configure_from_workload, range_rgyr_static,
                   CV_DISTANCE, CV_ANGLE, CV_DIHEDRAL, CV_COM_COMPONENT, CV_RGYR, CV_DISPLACEMENT,
                   CV_PRINCIPAL_MOMENT, CV_ASPHERICITY, CV_ACYLINDRICITY, CV_SHAPE_ANISOTROPY, CV_DIST_TO_INTERFACE,
                   HILLS_F32, HILLS_F64, METHOD_NONE, METHOD_HARMONIC, METHOD_METAD, METHOD_ABF, METHOD_METAD_GRID, EXPORTS)
 
-__all__ = ["Context", "PsgError", "load_library", "lib_path", "measure_alu_peak", "configure_from_workload",
+__all__ = ["Context", "PsgError", "load_library", "lib_path", "measure_alu_peak", "configure_from_workload", "range_rgyr_static",
            "CV_DISTANCE", "CV_ANGLE", "CV_DIHEDRAL", "CV_COM_COMPONENT", "CV_RGYR", "CV_DISPLACEMENT", "CV_PRINCIPAL_MOMENT",
            "CV_ASPHERICITY", "CV_ACYLINDRICITY", "CV_SHAPE_ANISOTROPY", "CV_DIST_TO_INTERFACE", "HILLS_F32", "HILLS_F64",
            "METHOD_NONE", "METHOD_HARMONIC", "METHOD_METAD", "METHOD_ABF", "METHOD_METAD_GRID", "EXPORTS"]

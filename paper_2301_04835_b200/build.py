@@ -13,7 +13,7 @@ ROOT = os.path.dirname(HERE)
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libpsg.so")
 SOURCES = ["api.cu", "cv.cu", "bias.cu", "range_step.cu", "abf_step.cu", "abf_estimate.cu", "interface_cv.cu", "metad_grid.cu", "hills.cu", "hills_n12.cu", "hills_n3a.cu", "hills_n3b.cu", "hills_n4.cu",
-           "microbench.cu"]
+           "microbench.cu", "noalloc.cu"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
               "-Xcompiler", "-fPIC", "--fmad=true", "-I", os.path.join(ROOT, "include"), "-I", CSRC]
 

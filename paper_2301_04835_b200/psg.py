@@ -27,7 +27,8 @@ EXPORTS = ["psg_create", "psg_destroy", "psg_set_stream", "psg_last_error", "psg
            "psg_set_abf", "psg_abf_state", "psg_cv_eval", "psg_bias_eval", "psg_deposit_hill", "psg_abf_update",
            "psg_abf_accumulate_delta", "psg_abf_apply_grid_delta", "psg_abf_estimate", "psg_abf_estimate_reset", "psg_apply_bias_forces", "psg_step", "psg_step_outputs", "psg_step_host", "psg_sync_check",
            "psg_interface_cv_set", "psg_interface_cv_eval", "psg_interface_cv_apply", "psg_hill_heights", "psg_append_hills", "psg_set_metad_grid", "psg_metad_grid_set",
-           "psg_metad_grid_deposit", "psg_metad_grid_eval", "psg_metad_grid_step", "psg_metad_grid_state", "psg_measure_alu_peak", "psg_launch_count", "psg_set_tuning"]
+           "psg_metad_grid_deposit", "psg_metad_grid_eval", "psg_metad_grid_step", "psg_metad_grid_state", "psg_measure_alu_peak", "psg_launch_count", "psg_set_tuning",
+           "psg_range_rgyr_static", "psg_static_last_error"]
 
 
 class PsgError(RuntimeError):
@@ -104,6 +105,9 @@ def load_library():
         L.psg_metad_grid_step.argtypes = [vp, vp, vp]
         L.psg_measure_alu_peak.argtypes = [i, i, C.POINTER(C.c_double)]
         L.psg_set_tuning.argtypes = [vp, i, i]
+        L.psg_range_rgyr_static.argtypes = [i, vp, vp, i, i, ll, ll, ll, vp, vp, vp]
+        L.psg_static_last_error.restype = C.c_char_p
+        L.psg_static_last_error.argtypes = []
         _lib = L
     return _lib
 
@@ -133,6 +137,27 @@ def measure_alu_peak(which: int, device: int = 0) -> float:
     if rc != 0:
         raise PsgError(rc, "psg_measure_alu_peak failed")
     return out.value
+
+
+def range_rgyr_static(pos, first_atom, n_group_atoms, weight=None, xi=None, center=None, device=0, stream=None):
+    """psg_range_rgyr_static (include/psg_static.h): radius of gyration of one contiguous atom range per replica, with no
+    allocation inside the library (static device scratch; limit PSG_STATIC_MAX_BLOCKS).  pos: CUDA float32 [R][stride][3|4];
+    weight: CUDA float32 [>= first + n] or None; xi: CUDA float32 [R] out; center: CUDA float64 [R][4] out or None.
+    stream: raw cudaStream_t, torch.cuda.Stream or None = torch's current stream.  Argument marshalling only."""
+    import torch
+    if stream is None:
+        stream = torch.cuda.current_stream(device).cuda_stream
+    elif hasattr(stream, "cuda_stream"):
+        stream = stream.cuda_stream
+    if pos.dim() != 3 or xi is None:
+        raise ValueError("pos must be [R][stride][3|4] and xi [R] must be given (this call allocates nothing)")
+    L = load_library()
+    rc = L.psg_range_rgyr_static(device, C.c_void_p(stream), _dp(pos, torch.float32), pos.shape[2], pos.shape[0], pos.shape[1],
+                                 int(first_atom), int(n_group_atoms), _dp(weight, torch.float32), _dp(xi, torch.float32),
+                                 _dp(center, torch.float64))
+    if rc != 0:
+        raise PsgError(rc, L.psg_static_last_error().decode())
+    return xi
 
 
 class Context:

@@ -9,7 +9,7 @@ import pytest
 
 ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
 HEADER = os.path.join(ROOT, "include", "psg.h")
-HEADERS = [HEADER, os.path.join(ROOT, "include", "psg_bench.h")]
+HEADERS = [HEADER, os.path.join(ROOT, "include", "psg_bench.h"), os.path.join(ROOT, "include", "psg_static.h")]
 
 
 @pytest.fixture(scope="module")
