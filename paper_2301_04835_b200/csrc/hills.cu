@@ -113,9 +113,9 @@ size_t psg_hill_part_doubles(const psg_ctx* c, int* max_chunks_out, int* n_rtile
     int n_rt = (c->sys.R + TILE_R - 1) / TILE_R;
     int cpt = hills_grid(c) / n_rt;
     if (cpt < 1) cpt = 1;
-    if (max_chunks_out) *max_chunks_out = cpt;
+    if (max_chunks_out) *max_chunks_out = cpt + 1;
     if (n_rtiles_out) *n_rtiles_out = n_rt;
-    return (size_t)cpt * n_rt * TILE_R * (1 + PSG_MAX_CV);
+    return (size_t)(cpt + 1) * n_rt * TILE_R * (1 + PSG_MAX_CV);   // + 1: the short last chunk of hills_spare_chunking
 }
 
 static cudaError_t launch_hills(psg_ctx* c, HillKernelArgs& A) {
@@ -131,7 +131,11 @@ static cudaError_t launch_hills(psg_ctx* c, HillKernelArgs& A) {
     const int n_rt = (c->sys.R + TILE_R - 1) / TILE_R;
     A.inv_n_rt = 1.0f / (float)n_rt;
     A.Lc_host = A.n_chunks_host = 0;
-    if (A.n_h_host >= 0) hills_chunking(A.n_h_host, grid, n_rt, A.Lc_host, A.n_chunks_host);
+    A.n_long = 0;
+    if (A.n_h_host >= 0) {
+        hills_chunking(A.n_h_host, grid, n_rt, A.Lc_host, A.n_chunks_host);
+        if (PSG_SPARE_CHUNKS(n_cv, c->md.precision == PSG_HILLS_F64)) hills_spare_chunking(A.n_h_host, grid, n_rt, A.Lc_host, A.n_chunks_host, A.n_long);
+    }
     A.simple = fused && c->sys.simple_groups && !c->sys.slot_weight && !c->sys.has_box;
     if (c->md.precision == PSG_HILLS_F64) return psg_hills_dispatch_f64(c, A, smem, grid);
     switch (n_cv) {

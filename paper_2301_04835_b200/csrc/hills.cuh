@@ -376,6 +376,10 @@ struct HillKernelArgs {
     const float* heights;    // W, as exported
     const int* n_hills;      // device counter (exact), read only when n_h_host < 0 (stream capture)
     int n_h_host;            // host upper bound of the count; records beyond the exact count are null (contribute 0)
+    int n_long;              // > 0: uneven chunking (hills_spare_chunking): CTA b < n_long runs item b only, the grid - n_long CTAs
+                             // behind them share the short last chunks of all tiles: items b, b + (grid - n_long), ...  (It sits in
+                             // the padding after n_h_host: the struct must not grow into another constant-cache line, whose cold
+                             // miss after an L2 flush costs the fused step 2 us.)
     double* part;
     const float* xi_in;      // not fused: [R][n_cv]
     float* V_out;            // nullable
@@ -401,6 +405,29 @@ __host__ __device__ inline void hills_chunking(int n_h, int grid, int n_rt, int&
     if (Lc < 32) Lc = 32;
     n_chunks = (n_h + Lc - 1) / Lc;
     if (n_chunks < 1) n_chunks = 1;
+}
+// Which instantiations take the uneven chunking below.  The hill loop sits at the 128-register limit and its code changes with
+// anything that is live across it: the 1- and 2-CV kernels lost 2 % to two extra moves with this in (config 1, whose chunks are
+// too short to gain anyway), the 3-CV kernel gained; the binary64-term kernels are left as they were measured.
+#ifndef PSG_SPARE_CHUNKS
+#define PSG_SPARE_CHUNKS(NCV, F64) ((NCV) >= 3 && !(F64))
+#endif
+// When the grid is not a multiple of the tile count, grid - cpt * n_rt CTAs would idle (config 4: 16 tiles x 9 chunks = 144 of
+// 148).  Host only: shorten the cpt long chunks of every tile and add one SHORT last chunk per tile; the spare CTAs run those,
+// m = ceil(n_rt / spare) each.  The short length x balances m (x + o) = (n_h - x) / cpt + o, o = the fixed cost of one item
+// (launch-to-loop, flushes, publish) in hills.  Returns false (nothing changed) when the long chunks are too short to gain.
+__host__ inline bool hills_spare_chunking(int n_h, int grid, int n_rt, int& Lc, int& n_chunks, int& n_long) {
+    const int cpt = grid / n_rt, spare = grid - cpt * n_rt;
+    if (cpt < 2 || spare <= 0 || n_chunks != cpt || Lc < 8192) return false;
+    const int m = (n_rt + spare - 1) / spare;
+    const double o = 600.0;
+    const double x = ((double)n_h / cpt + o - m * o) / (m + 1.0 / cpt);
+    if (x < 64.0) return false;
+    int L = (int)(((double)n_h - x) / cpt);
+    L = ((L + 31) / 32) * 32;
+    if (L >= Lc || n_h - cpt * L < 32) return false;
+    Lc = L; n_chunks = cpt + 1; n_long = cpt * n_rt;
+    return true;
 }
 __host__ __device__ inline size_t hills_wacc_doubles(int n_cv) { return (size_t)((RT * (1 + n_cv) + 31) / 32) * 32; }
 __host__ __device__ inline size_t hills_smem_bytes(int n_cv, int stages, int n_groups, bool fused) {
@@ -466,6 +493,7 @@ __global__ void __launch_bounds__(HWARPS * 32, 1) k_hills(const __grid_constant_
     // issued before anything else.  They are consumed BEFORE the item loop (lean_finish below): registers that stayed live
     // into the loop would be taken from the hill loop.
     static_assert(2 * TILE_R * NCV <= NT, "one pass of the CV prologue covers a tile");
+    static_assert(sizeof(HillKernelArgs) == 128, "HillKernelArgs is two 64-byte constant lines");
     const bool early = A.fused && A.simple && A.n_h_host >= 0 && (int)blockIdx.x < n_rt * A.n_chunks_host;   // CTA-uniform
     float4 pre[4];
     int pre_a[4];
@@ -547,7 +575,10 @@ __global__ void __launch_bounds__(HWARPS * 32, 1) k_hills(const __grid_constant_
         lean_done = true;
     }
 
-    for (int item = blockIdx.x; item < items; item += gridDim.x) {
+    // (the step is recomputed from the kernel parameters at the end of an item: a value kept live across the hill loop costs it
+    // moves; and only the instantiations that use the uneven chunking compile it: PSG_SPARE_CHUNKS)
+    for (int item = blockIdx.x; item < items;
+         item += (PSG_SPARE_CHUNKS(NCV, F64) && A.n_long > 0) ? ((int)blockIdx.x < A.n_long ? items : (int)gridDim.x - A.n_long) : (int)gridDim.x) {
         int tile, chunk;
         hills_item(item, n_rt, A.inv_n_rt, tile, chunk);
         const int r0 = tile * TILE_R;

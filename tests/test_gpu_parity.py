@@ -206,6 +206,29 @@ def test_hill_sum_f32_mode(torch, psg, n_cv, periodic, R, n_h):
     assert bad.mean() <= 0.05, f"literal fail fraction {bad.mean():.4f}"
 
 
+@pytest.mark.parametrize("n_cv,periodic,R,n_h", [(3, 3, 320, 250000), (4, 5, 130, 410000), (3, 0, 1024, 150000)])
+def test_hill_sum_uneven_chunking_on_the_spare_ctas(torch, psg, n_cv, periodic, R, n_h):
+    """Long hill lists on a tile count that does not divide the 148 CTAs (5, 3, 16 tiles): the 3- and 4-CV kernels shorten the
+    long chunks and let the spare CTAs run one short last chunk per tile (hills_spare_chunking): every hill exactly once."""
+    gV, gdV, V, dV, T = _hill_case(torch, psg, n_cv, periodic, R, n_h, 5, psg.HILLS_F32)
+    assert_close(gV, V, "V (f32 terms, uneven chunks)")
+    assert np.all(np.abs(gdV - dV) <= np.maximum(np.maximum(1e-5 * np.abs(dV), 1e-6), 2e-7 * T))
+    # a unit-height list with far-away walkers: V counts the hills that were summed (none twice, none dropped)
+    rng = np.random.default_rng(7)
+    ctx = psg.Context(0)
+    ctx.set_layout(R, 2 * n_cv, 2 * n_cv, 4, 4)
+    ctx.set_cvs([{"type": psg.CV_DISTANCE, "groups": [("slots", 2 * k, 1), ("slots", 2 * k + 1, 1)], "period": 0.0}
+                 for k in range(n_cv)], np.arange(2 * n_cv, dtype=np.int32))
+    ctx.set_metad(np.full(n_cv, 1.0e4, np.float32), 1.0, 0.0, n_h, 0)      # sigma so wide that every Gaussian is 1 to 1e-9
+    ctx.load_hills(dev(torch, rng.uniform(0.9, 1.1, size=(n_h, n_cv)).astype(np.float32)), dev(torch, np.ones(n_h, np.float32)))
+    d_V = torch.empty(R, device="cuda")
+    d_dV = torch.empty((R, n_cv), device="cuda")
+    ctx.bias_eval(dev(torch, np.ones((R, n_cv), np.float32)), d_V, d_dV)
+    ctx.sync_check()
+    assert np.all(np.abs(d_V.cpu().numpy().astype(np.float64) - n_h) <= 1e-5 * n_h), (d_V.min().item(), d_V.max().item(), n_h)
+    ctx.close()
+
+
 def test_hill_sum_empty_store_is_zero(torch, psg):
     gV, gdV, V, dV, T = _hill_case(torch, psg, 2, 3, 9, 0, 3, psg.HILLS_F32)
     assert np.all(gV == 0) and np.all(gdV == 0)
