@@ -121,7 +121,8 @@ size_t psg_hill_part_doubles(const psg_ctx* c, int* max_chunks_out, int* n_rtile
 static cudaError_t launch_hills(psg_ctx* c, HillKernelArgs& A) {
     const int n_cv = c->sys.n_cv;
     const bool fused = A.fused != 0;
-    // stages of 32 KB: as many as fit the SM's 227 KB (1 KB reserved per CTA), at most 6 (the binary64 accumulators are registers)
+    // stages of 64 KB: three of them fit the SM's 227 KB beside the per-warp totals for every n_cv and group count (the hand-back
+    // scheme wants 3: the refill of a stage is issued one sub-tile after its last reader left)
     int stages = PSG_HILL_MAX_STAGES;
     for (; stages > 3; --stages)
         if (hills_smem_bytes(n_cv, stages, c->sys.n_groups, fused) + 1024 <= 227 * 1024) break;

@@ -16,7 +16,7 @@
 //     MUFU.EX2 (one per replica), V += e, g_k += e d_k                                   (1 + NCV)
 // Binary32 partial sums (<= 64 hills per lane) are flushed into binary64 by a warp-wide transpose-reduction (31 shuffle +
 // add steps turn 32 per-lane values into one warp total per lane): the binary64 accumulators are ONE slot per lane (4 KB per CTA), not
-// 98-131 KB of shared memory, which leaves the SM's shared memory to the hill stages (up to 6 x 32 KB in flight).  Lanes (butterfly),
+// 98-131 KB of shared memory, which leaves the SM's shared memory to the hill stages (3 x 64 KB in flight).  Lanes (butterfly),
 // warps, then chunks are combined in binary64 in FIXED order (the CTA of a tile's chunk 0 collects the other chunks'
 // published partials, each word carrying its own valid flag), so results are bitwise reproducible.
 // FUSED: the CTA first evaluates the CVs (and Jacobians, kept in shared memory) of its tile from the engine's
@@ -30,7 +30,7 @@
 #define TILE_R PSG_HILL_TILE_R
 #define SUB PSG_HILL_SUB
 #ifndef PSG_FLUSH_EVERY
-#define PSG_FLUSH_EVERY 2        // sub-tiles (32 hills per lane each) between binary32 -> binary64 flushes
+#define PSG_FLUSH_EVERY 1        // sub-tiles (64 hills per lane each; 32 with 4 CVs) between binary32 -> binary64 flushes
 #endif
 #define MAGIC_RN 12582912.0f   // 1.5 * 2^23: (x + M) - M = rint(x) for |x| < 2^22
 
@@ -440,7 +440,7 @@ __host__ __device__ inline size_t hills_smem_bytes(int n_cv, int stages, int n_g
     return b;
 }
 #ifndef PSG_HILL_MAX_STAGES
-#define PSG_HILL_MAX_STAGES 6
+#define PSG_HILL_MAX_STAGES 3
 #endif
 
 // item -> (tile, chunk) without an integer division: a binary32 quotient, corrected by one (item < 2^24)
@@ -704,8 +704,9 @@ __global__ void __launch_bounds__(HWARPS * 32, 1) k_hills(const __grid_constant_
 #ifndef PSG_NO_EARLY_POLL
                 ready = t + 1 < n_st && mbar_test(&full[(seq + 1) % STG], ((seq + 1) / STG) & 1);
 #endif
-                // flush the binary32 partial sums (<= 64 hills per lane) into the lanes' binary64 registers; the four warps
-                // of a scheduler (wid mod 4) flush at different sub-tiles, so that the FMA pipe keeps work while one reduces
+                // flush the binary32 partial sums (<= 64 hills per lane) into the lanes' binary64 registers (with
+                // PSG_FLUSH_EVERY > 1 the four warps of a scheduler, wid mod 4, flush at different sub-tiles; with one flush per
+                // 64-hill sub-tile the warps drift apart by themselves)
 #ifdef PSG_NO_STAGGER
                 const int ph = 0;
 #else

@@ -19,7 +19,8 @@
 #endif
 #define PSG_HILL_HALF (PSG_HILL_WARPS / 2)
 #define PSG_HILL_TILE_R (PSG_HILL_RT * PSG_HILL_HALF)   // replicas per CTA tile (64): warp w and warp w + HALF own the same 8 replicas
-#define PSG_HILL_SUB 2048        // hills per shared-memory stage
+#define PSG_HILL_SUB 4096        // 16-byte hill records per shared-memory stage (64 KB): 64 hills per lane and pass of the hill loop; with 2,048 the
+                                 // loop's peeled entry / exit iterations and the per-stage bookkeeping cost config 1 5 % and config 4 0.5 %
 
 struct CvDev {
     int type, n_groups, axis, gid0;   // gid0: global id of this CV's first group
