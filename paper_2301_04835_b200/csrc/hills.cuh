@@ -774,18 +774,30 @@ __global__ void __launch_bounds__(HWARPS * 32, 1) k_hills(const __grid_constant_
                 for (int c = pt * cn; c < c1; c += BATCH) {
                     u64 w[BATCH];
 #pragma unroll
-                    for (int i = 0; i < BATCH; ++i)
+                    for (int i = 0; i < BATCH; ++i) {
+                        w[i] = 1ull;   // (own chunk / beyond the range: nothing to wait for)
                         if (c + i < c1 && c + i > 0) w[i] = __ldcg(src + (size_t)(c + i) * cstride);
+                    }
+                    // words that were not there yet are re-read TOGETHER, one round trip per pass (re-reading them one after
+                    // the other cost the finisher a round trip per late word)
+                    for (;;) {
+                        u64 all = ~0ull;
+#pragma unroll
+                        for (int i = 0; i < BATCH; ++i) all &= w[i];
+                        if (all & 1ull) break;
+#pragma unroll
+                        for (int i = 0; i < BATCH; ++i)
+                            if (!(w[i] & 1ull))
+                                asm volatile("ld.relaxed.gpu.global.u64 %0, [%1];" : "=l"(w[i]) : "l"(src + (size_t)(c + i) * cstride) : "memory");
+                    }
 #pragma unroll
                     for (int i = 0; i < BATCH; ++i) {
                         if (c + i >= c1) break;
                         if (c + i == 0) {
                             sum += s_out[v];   // this CTA's own chunk
                         } else {
-                            u64* q = src + (size_t)(c + i) * cstride;
-                            while (!(w[i] & 1ull)) asm volatile("ld.relaxed.gpu.global.u64 %0, [%1];" : "=l"(w[i]) : "l"(q) : "memory");
                             sum += __longlong_as_double((long long)w[i]);
-                            __stcg(q, 0ull);
+                            __stcg(src + (size_t)(c + i) * cstride, 0ull);
                         }
                     }
                 }
