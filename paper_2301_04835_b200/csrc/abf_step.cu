@@ -33,6 +33,12 @@ __global__ void __launch_bounds__(256, 4) k_abf_step(const __grid_constant__ Sys
     const int warps = gridDim.x * 8, gw = blockIdx.x * 8 + wid;
     WarpCvSmem& S = sm[wid];
 
+    // With at most one replica per warp (R <= resident warps: config 2's 4,096 on 4,736) the warp keeps what phase 2 needs ON
+    // CHIP across the barrier: lane 0 the bin, lane s the Jacobian of slot s (the first 32 slots; more go through the ctx
+    // cache).  Phase 2 is then ONE L2 round trip (the grid entry) instead of three (bin, grid entry, dV + Jacobian).
+    const bool one = A.phase == 0 && P.R <= warps;   // grid-uniform
+    int my_bin = -1;
+    float jx = 0.f, jy = 0.f, jz = 0.f;
     for (int r = gw; A.phase != 2 && r < P.R; r += warps) {
         warp_cv_eval<true>(P, r, A.pos, nullptr, S, lane);
         if (lane < P.n_cv) A.xi_out[(long long)r * P.n_cv + lane] = (float)S.xi[lane];
@@ -40,6 +46,7 @@ __global__ void __launch_bounds__(256, 4) k_abf_step(const __grid_constant__ Sys
             const D3 j = slot_jacobian(P, r, A.pos, S, s);
             const long long o = ((long long)r * P.n_slots + s) * 3;
             A.jac[o] = (float)j.x; A.jac[o + 1] = (float)j.y; A.jac[o + 2] = (float)j.z;
+            if (s == lane) { jx = (float)j.x; jy = (float)j.y; jz = (float)j.z; }
             // the force record phase 2 will update, requested into L2 now (the arrays are GBs: a cold miss otherwise)
             const int atom = slot_atom_of(P, r, s);
             asm volatile("prefetch.global.L2 [%0];" ::"l"(A.force + ((long long)r * P.rstride + atom) * P.fs));
@@ -48,7 +55,8 @@ __global__ void __launch_bounds__(256, 4) k_abf_step(const __grid_constant__ Sys
             float xi[PSG_MAX_CV];
 #pragma unroll
             for (int k = 0; k < PSG_MAX_CV; ++k) xi[k] = k < P.n_cv ? (float)S.xi[k] : 0.f;
-            A.bin_out[r] = abf_accumulate_one(G, P.n_cv, xi, A.fsample + (long long)r * P.n_cv);
+            my_bin = abf_accumulate_one(G, P.n_cv, xi, A.fsample + (long long)r * P.n_cv);
+            A.bin_out[r] = my_bin;
         }
         __syncwarp();
     }
@@ -68,6 +76,27 @@ __global__ void __launch_bounds__(256, 4) k_abf_step(const __grid_constant__ Sys
 
     for (int r = gw; r < P.R; r += warps) {
         float* dV = A.dV_out + (long long)r * P.n_cv;
+        if (one) {
+            float* sdv = reinterpret_cast<float*>(&S.xi[0]);   // this warp's scratch: phase 1 is over
+            if (lane == 0) {
+                abf_mean_one(G, P.n_cv, my_bin, sdv);
+                for (int k = 0; k < P.n_cv; ++k) dV[k] = sdv[k];
+            }
+            __syncwarp();
+            for (int s = lane; s < P.n_slots; s += 32) {
+                const int gid = P.slot_gid_c[s];
+                const float dv = -sdv[P.grp[gid].cv];
+                const int atom = slot_atom_of(P, r, s);
+                float* f = A.force + ((long long)r * P.rstride + atom) * P.fs;
+                if (s < 32) {
+                    force_add(f, dv * jx, dv * jy, dv * jz, P.fs);
+                } else {
+                    const float* j = A.jac + ((long long)r * P.n_slots + s) * 3;
+                    force_add(f, dv * j[0], dv * j[1], dv * j[2], P.fs);
+                }
+            }
+            continue;
+        }
         if (lane == 0) abf_mean_one(G, P.n_cv, A.bin_out[r], dV);
         __syncwarp();
         for (int s = lane; s < P.n_slots; s += 32) {
