@@ -117,6 +117,142 @@ __global__ void __launch_bounds__(256, 4) k_abf_step(const __grid_constant__ Sys
     }
 }
 
+// ---------------------------------------------------------------------------------------------------------------
+// The same step for the common layout (explicit groups, no box, point-group CVs): TWO THREADS per
+// (replica, CV) instead of a warp per replica.  One thread takes the value (sqrt / atan2 chain), another (in another warp) the
+// derivative (cv_jacobian_only: Newton-refined hardware reciprocals), so the two binary64 chains run side by side and a warp
+// instruction carries 32 of them: the warp-per-replica kernel issues every binary64 instruction for 2 live lanes, and with
+// 32 such warps per SM the FP64 pipe (16 lanes/clk per scheduler) is what phase 1 waits for (measured: 5.3-7.3 us of a
+// 13 us launch).  Each thread gathers the (few) atoms of its CV's groups itself.  The thread that owns the derivative keeps it
+// in registers across the barrier and scatters it.
+// LEAN_RB replicas per CTA; block = LEAN_RB x n_cv value threads followed by as many derivative threads (whole warps each: the
+// two roles are different code and would serialise inside a warp); grid = ceil(R / LEAN_RB), co-resident (cooperative launch).
+#define LEAN_RB 32
+__global__ void __launch_bounds__(LEAN_RB * PSG_MAX_CV * 2) k_abf_step_lean(const __grid_constant__ SysParams P, const __grid_constant__ AbfState G,
+                                                                          const __grid_constant__ AbfStepArgs A) {
+    __shared__ float s_xi[LEAN_RB][PSG_MAX_CV], s_dv[LEAN_RB][PSG_MAX_CV];
+    __shared__ int s_bin[LEAN_RB];
+    const int tid = threadIdx.x, n_cv = P.n_cv;
+    const int role = tid >= LEAN_RB * n_cv ? 1 : 0;   // role 0: value, 1: derivative
+    const int t = tid - role * LEAN_RB * n_cv, rl = t / n_cv, k = t - rl * n_cv;
+    const int r = blockIdx.x * LEAN_RB + rl;
+    const bool live = r < P.R;
+    const CvDev& C = P.cv[k];
+    float jf[4][3];   // derivative thread: d xi_k / d c_g / W_g, rounded to binary32 like the ctx cache
+    if (live) {
+        const float* p = A.pos + (long long)r * P.rstride * P.ps;
+        // group centres with the arithmetic of warp_cv_eval's gather (same sums, same order, same division: xi keeps its bits)
+        D3 c[4], dc[4];
+        double Wg[4];
+#pragma unroll
+        for (int g = 0; g < 4; ++g) {
+            c[g] = d3(0, 0, 0);
+            Wg[g] = 1.0;
+            if (g < C.n_groups) {
+                const GroupDev& Gd = P.grp[C.gid0 + g];
+                double sx = 0, sy = 0, sz = 0, sw = 0;
+#pragma unroll 4
+                for (int i = 0; i < Gd.size; ++i) {
+                    const int s = Gd.begin + i;
+                    const D3 x = load_pos(p, slot_atom_of(P, r, s), P.ps);
+                    const double w = P.slot_weight ? (double)P.slot_weight[s] : 1.0;
+                    sx += w * x.x; sy += w * x.y; sz += w * x.z; sw += w;
+                }
+                const double iw = 1.0 / sw;
+                c[g] = d3(sx * iw, sy * iw, sz * iw);
+                Wg[g] = sw;
+            }
+        }
+        if (role == 0) {
+            const float v = (float)cv_from_centers<false>(C.type, C.axis, c, dc, nullptr);
+            s_xi[rl][k] = v;
+            A.xi_out[(long long)r * n_cv + k] = v;
+        } else {
+            cv_jacobian_only(C.type, C.axis, c, dc);
+#pragma unroll
+            for (int g = 0; g < 4; ++g) {
+                const double iw = fast_rcp(Wg[g]);
+                jf[g][0] = (float)(dc[g].x * iw); jf[g][1] = (float)(dc[g].y * iw); jf[g][2] = (float)(dc[g].z * iw);
+                if (g < C.n_groups) {
+                    const GroupDev& Gd = P.grp[C.gid0 + g];
+                    for (int i = 0; i < Gd.size; ++i) {
+                        // the ctx cache, as after psg_cv_eval; and the force record phase 2 will update, requested into L2 now
+                        const int s = Gd.begin + i;
+                        const double w = P.slot_weight ? (double)P.slot_weight[s] : 1.0;
+                        const long long o = ((long long)r * P.n_slots + s) * 3;
+                        A.jac[o] = (float)(w * (dc[g].x * iw)); A.jac[o + 1] = (float)(w * (dc[g].y * iw)); A.jac[o + 2] = (float)(w * (dc[g].z * iw));
+                        asm volatile("prefetch.global.L2 [%0];" ::"l"(A.force + ((long long)r * P.rstride + slot_atom_of(P, r, s)) * P.fs));
+                    }
+                }
+            }
+        }
+    }
+    __syncthreads();
+    const bool owner = live && k == 0 && role == 0;   // one thread per replica bins and reads the grid
+    if (owner) {
+        float xi[PSG_MAX_CV];
+#pragma unroll
+        for (int q = 0; q < PSG_MAX_CV; ++q) xi[q] = q < n_cv ? s_xi[rl][q] : 0.f;
+        const int b = abf_accumulate_one(G, n_cv, xi, A.fsample + (long long)r * n_cv);
+        s_bin[rl] = b;
+        A.bin_out[r] = b;
+    }
+    // ---- grid barrier: every replica's atomics are performed before anyone reads the grid
+    __syncthreads();
+    if (tid == 0) {
+        __threadfence();
+        atomicAdd(A.bar, 1u);
+        unsigned n;
+        do {
+            asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(n) : "l"(A.bar) : "memory");
+        } while (n < gridDim.x);
+    }
+    __syncthreads();
+    if (owner) {
+        abf_mean_one(G, n_cv, s_bin[rl], s_dv[rl]);
+        for (int q = 0; q < n_cv; ++q) A.dV_out[(long long)r * n_cv + q] = s_dv[rl][q];
+    }
+    __syncthreads();
+    if (live && role == 1) {
+        const float dv = -s_dv[rl][k];
+#pragma unroll
+        for (int g = 0; g < 4; ++g)
+            if (g < C.n_groups) {
+                const GroupDev& Gd = P.grp[C.gid0 + g];
+                for (int i = 0; i < Gd.size; ++i) {
+                    const int s = Gd.begin + i;
+                    const float w = P.slot_weight ? P.slot_weight[s] : 1.f;
+                    force_add(A.force + ((long long)r * P.rstride + slot_atom_of(P, r, s)) * P.fs, dv * (w * jf[g][0]), dv * (w * jf[g][1]),
+                              dv * (w * jf[g][2]), P.fs);
+                }
+            }
+    }
+    // ---- the last CTA to leave re-arms the barrier for the next launch
+    if (tid == 0) {
+        const unsigned old = atomicAdd(A.bar + 1, 1u);
+        if (old == gridDim.x - 1) { A.bar[0] = 0u; A.bar[1] = 0u; }
+    }
+}
+
+// CTAs of the lean kernel that can be co-resident on the device (0 if it cannot be configured)
+static long long abf_lean_capacity(const psg_ctx* c, int threads) {
+    int n = 0;
+    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n, k_abf_step_lean, threads, 0) != cudaSuccess) n = 0;
+    (void)cudaGetLastError();
+    return (long long)n * c->sm_count;
+}
+
+static bool abf_lean_layout(const psg_ctx* c) {
+    const SysParams& P = c->sys;
+    if (P.n_ranges > 0 || P.any_rgyr || P.has_box || c->dti_cv >= 0 || P.n_cv < 1) return false;
+    for (int k = 0; k < P.n_cv; ++k) {
+        const int t = P.cv[k].type;
+        if (!(t == PSG_CV_DISTANCE || t == PSG_CV_ANGLE || t == PSG_CV_DIHEDRAL || t == PSG_CV_DISPLACEMENT || t == PSG_CV_COM_COMPONENT))
+            return false;
+    }
+    return true;
+}
+
 static int abf_blocks_per_sm(int device) {
     static int cache[PSG_MAX_DEVICES];
     static bool have[PSG_MAX_DEVICES] = {};
@@ -173,14 +309,26 @@ cudaError_t psg_launch_abf_step(psg_ctx* c, const float* d_pos, const float* d_f
     AbfStepArgs A{};
     A.pos = d_pos; A.fsample = d_fsample; A.force = d_force;
     A.xi_out = c->d_xi; A.bin_out = c->d_bin; A.dV_out = c->d_dVdxi; A.jac = c->d_jac; A.bar = c->d_gbar; A.phase = 0;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeCooperative;   // co-residency is what makes the grid barrier safe
+    attr[0].val.cooperative = 1;
+    if (abf_lean_layout(c)) {
+        const int threads = LEAN_RB * P.n_cv * 2;
+        const long long lgrid = (P.R + LEAN_RB - 1) / LEAN_RB;
+        if (lgrid <= abf_lean_capacity(c, threads)) {
+            cudaLaunchConfig_t cfg{};
+            cfg.gridDim = dim3((unsigned)lgrid); cfg.blockDim = dim3(threads); cfg.dynamicSmemBytes = 0; cfg.stream = c->stream;
+            cfg.attrs = attr; cfg.numAttrs = 1;
+            cudaError_t e = cudaLaunchKernelEx(&cfg, k_abf_step_lean, P, c->abf, A);
+            if (e == cudaSuccess) c->launches++;
+            return e;
+        }
+    }
     long long grid = (P.R + 7) / 8;
     const long long cap = (long long)c->sm_count * abf_blocks_per_sm(c->device);
     if (grid > cap) grid = cap;
     cudaLaunchConfig_t cfg{};
     cfg.gridDim = dim3((unsigned)grid); cfg.blockDim = dim3(256); cfg.dynamicSmemBytes = 0; cfg.stream = c->stream;
-    cudaLaunchAttribute attr[1];
-    attr[0].id = cudaLaunchAttributeCooperative;   // co-residency is what makes the grid barrier safe
-    attr[0].val.cooperative = 1;
     cfg.attrs = attr; cfg.numAttrs = 1;
     cudaError_t e = cudaLaunchKernelEx(&cfg, k_abf_step, P, c->abf, A);
     if (e == cudaSuccess) c->launches++;

@@ -591,6 +591,67 @@ def test_fused_abf_step_equals_unfused_calls(torch, psg, R, N):
     assert np.array_equal(a[3][..., 3].view(np.uint32), f0[..., 3].view(np.uint32))
 
 
+@pytest.mark.parametrize("ps", [3, 4])
+def test_fused_abf_step_two_threads_per_cv_kernel_on_weighted_groups(torch, psg, ps):
+    """k_abf_step_lean (explicit groups, no box, point-group CVs): weighted groups of 1..3 atoms, per-replica index lists,
+    angle + dihedral + component + distance on a 4-D grid, several steps with the grid filling up: xi, bins and histogram
+    against the oracle bit for bit, mean forces and forces within the tolerance; and the ctx Jacobian cache it leaves behind"""
+    rng = np.random.default_rng(23)
+    R, N = 75, 60        # 3 CTAs of 32 replicas, the last one ragged
+    groups = lambda b, sizes: [("slots", b + sum(sizes[:i]), sizes[i]) for i in range(len(sizes))]
+    cvs_n = [("angle", groups(0, [2, 1, 3]), 0.0, 0), ("dihedral", groups(6, [1, 2, 1, 1]), 2 * math.pi, 0),
+             ("component", groups(11, [3]), 0.0, 2), ("distance", groups(14, [1, 2]), 0.0, 0)]
+    ok = {"angle": orc.ANGLE, "dihedral": orc.DIHEDRAL, "component": orc.COMPONENT, "distance": orc.DISTANCE}
+    gk = {"angle": psg.CV_ANGLE, "dihedral": psg.CV_DIHEDRAL, "component": psg.CV_COM_COMPONENT, "distance": psg.CV_DISTANCE}
+    o_cvs = [{"type": ok[k], "groups": g, "axis": ax, "period": p} for k, g, p, ax in cvs_n]
+    g_cvs = [{"type": gk[k], "groups": g, "axis": ax, "period": p} for k, g, p, ax in cvs_n]
+    slot = np.stack([rng.permutation(N)[:17] for _ in range(R)]).astype(np.int32)
+    sw = rng.uniform(1, 16, size=17).astype(np.float32)
+    sysm = orc.System(R, N, N, ps, o_cvs, slot, sw, None)
+    lower = np.array([0.0, -math.pi, -2.5, 0.0], np.float32)
+    upper = np.array([math.pi, math.pi, 2.5, 4.0], np.float32)
+    shape, periodic, n_thr = np.array([4, 5, 3, 4], np.int32), np.array([0, 1, 0, 0], np.int32), 2
+    nb = int(np.prod(shape))
+    hist, fsum = np.zeros(nb, np.int32), np.zeros((nb, 4), np.float64)
+    ctx = psg.Context(0)
+    ctx.set_layout(R, N, N, ps, ps)
+    ctx.set_cvs(g_cvs, slot, sw, None)
+    ctx.set_abf(lower, upper, shape, periodic, n_thr)
+    f0 = np.zeros((R, N, ps), np.float32)
+    f0[..., :3] = rng.standard_normal((R, N, 3)) * 50
+    f_ref = f0[..., :3].astype(np.float64)
+    d_f = dev(torch, f0)
+    for step in range(1, 5):
+        pos = np.zeros((R, N, ps), np.float32)
+        pos[..., :3] = rng.normal(scale=0.9, size=(R, N, 3))
+        fs = rng.normal(scale=30.0, size=(R, 4)).astype(np.float32)
+        n0 = ctx.launch_count()
+        ctx.step(dev(torch, pos), d_f, dev(torch, fs), step)
+        ctx.sync_check()
+        assert ctx.launch_count() - n0 == 1
+        out = ctx.read_step_outputs()
+        xi_ref, jac_ref = sysm.cv_eval(pos)
+        b_ref, dV_ref = orc.abf_update(xi_ref.astype(np.float32), fs, lower, upper, shape, periodic, n_thr, hist, fsum)
+        f_ref = sysm.apply_forces(pos, dV_ref, f_ref)
+        assert_close(out["xi"].cpu().numpy(), xi_ref, f"xi, step {step}", period=np.array([0, 2 * math.pi, 0, 0]))
+        assert np.array_equal(out["bin"].cpu().numpy(), b_ref), f"bins, step {step}"
+        assert (b_ref >= 0).sum() >= R // 3
+        g = out["dVdxi"].cpu().numpy()
+        assert np.all(np.abs(g - dV_ref) <= np.maximum(1e-5 * np.abs(dV_ref), 1e-5)), f"mean force, step {step}"
+        assert_forces_close(d_f.cpu().numpy()[..., :3], f_ref, f0[..., :3], f"forces, step {step}")
+    hp, fp, nbins = ctx.abf_state()
+    from paper_2301_04835_b200.psg import _view
+    assert np.array_equal(_view(hp, (nb,), torch.int32, 0).cpu().numpy(), hist)
+    assert np.allclose(_view(fp, (nb, 4), torch.float32, 0).cpu().numpy(), fsum, rtol=1e-5, atol=1e-3)
+    # the Jacobian cache the fused step leaves (psg_apply_bias_forces would use it): the oracle's, slot by slot
+    d_jac = torch.empty((R, 17, 3), device="cuda")
+    d_xi = torch.empty((R, 4), device="cuda")
+    ctx.cv_eval(dev(torch, pos), d_xi, d_jac)
+    ctx.sync_check()
+    assert_close(d_jac.cpu().numpy(), jac_ref, "jacobian of the separate call")
+    ctx.close()
+
+
 def test_abf_shared_grid_split_over_two_contexts(torch, psg):
     """SURVEY 8(e), shared-grid ABF over several GPUs, on one: two contexts hold half of the replicas each, run
     psg_abf_accumulate_delta, exchange by summing the two delta grids (what the all-reduce does), and run
