@@ -8,6 +8,8 @@
 //            (red.global.add.f32: atoms shared between CVs or walkers collide)
 // The barrier is a counter in global memory, so the grid must be co-resident: the kernel is launched cooperatively
 // (the launch fails instead of hanging) with at most occupancy x SM-count CTAs; warps loop over replicas.
+// k_abf_step_lean (below) takes the whole step for the common layout: two threads per (replica, CV) instead of a warp per
+// replica.
 // Same arithmetic as k_cv_eval + k_abf_accumulate + k_abf_mean + k_apply_sparse: bins, counts, xi, dV/dxi and the
 // Jacobian are bit-identical to the separate calls; Fsum and forces differ only by the order of the atomics.
 #include "abf.cuh"
