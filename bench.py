@@ -59,7 +59,7 @@ def hill_eval_instr_f64(n_cv, n_periodic):
 
 # dram__bytes_read.sum + dram__bytes_write.sum of ONE launch of the dominant kernel, bytes, NOT measured in this run:
 # copied from the committed ncu --set full captures named here
-NCU_TRAFFIC = {1: (1.224e6, "profiles/r2_hills_config1_ncu_full.md"), 2: (8.58e6, "profiles/r1b_abf_step_config2_ncu_full.md"),
+NCU_TRAFFIC = {1: (1.224e6, "profiles/r2_hills_config1_ncu_full.md"), 2: (8.52e6, "profiles/r2b_abf_step_config2_ncu_full.md"),
                3: (1.2412e9, "profiles/r1b_range_step_config3_ncu_full.md"), 4: (5.98e6, "profiles/r2_hills_config4_ncu_full.md")}
 
 
@@ -528,7 +528,7 @@ class ConfigRun:
         else:
             bytes_step = float(w.R) * (8 * 32 + 3 * 32 + 8 * 32 * 2)   # sectors: 8 gathered, <= 3 grid RMW, 8 force RMW
             ach = bytes_step * n / (ms_total * 1e-3) / 1e9
-            r = {"bound": "hbm", "kernel": "k_abf_step (fused ABF step, one launch; latency-bound)", "achieved": ach,
+            r = {"bound": "hbm", "kernel": "k_abf_step_lean (fused ABF step, one launch; latency-bound)", "achieved": ach,
                  "peak": pk.hbm, "unit": "GB/s", "frac": ach / pk.hbm, "peak_source": pk.hbm_source,
                  "algorithmic_units_per_step": bytes_step, "algorithmic_units": "bytes (32 B sectors touched)"}
             model_us = bytes_step / (pk.hbm * 1e9) * 1e6
