@@ -121,11 +121,157 @@ __global__ void __launch_bounds__(128, 8) k_abf_estimate(const __grid_constant__
     }
 }
 
+// ---------------------------------------------------------------------------------------------------------------
+// The same estimator with ONE THREAD per (replica, CV) for explicit groups without a box and point-group CVs (the layout of
+// k_abf_step_lean, abf_step.cu): the thread gathers the atoms of its CV's groups, takes the derivative (cv_jacobian_only: the
+// estimator needs no CV value), forms its slots' Jacobians, its b_k = J_k . p and, after a barrier, row k of the Gram matrix;
+// the thread of CV 0 solves the n_cv x n_cv system.  A warp instruction then carries 32 chains instead of 1-8: the
+// warp-per-replica kernel above spends its time issuing binary64 instructions for a few live lanes (23 us for 4,096 replicas).
+#define EST_RB 16   // replicas per CTA; block = EST_RB x n_cv threads
+struct EstLeanRep {
+    double M[PSG_MAX_CV][PSG_MAX_CV + 1], W[PSG_MAX_CV];
+};
+__global__ void __launch_bounds__(EST_RB * PSG_MAX_CV) k_abf_estimate_lean(const __grid_constant__ SysParams P, const __grid_constant__ AbfEstArgs A) {
+    extern __shared__ __align__(16) unsigned char est_smem[];
+    const int ns = P.n_slots, n_cv = P.n_cv;
+    double* s_j = reinterpret_cast<double*>(est_smem);                       // [EST_RB][ns][3]
+    EstLeanRep* s_rep = reinterpret_cast<EstLeanRep*>(s_j + (size_t)EST_RB * ns * 3);
+    int* s_atom = reinterpret_cast<int*>(s_rep + EST_RB);                    // [EST_RB][ns]
+    int* s_cvk = s_atom + EST_RB * ns;                                       // [EST_RB][ns]
+    const int tid = threadIdx.x, rl = tid / n_cv, k = tid - rl * n_cv;
+    const int r = blockIdx.x * EST_RB + rl;
+    const bool live = r < P.R;
+    const CvDev& C = P.cv[k];
+    double* jr = s_j + (size_t)rl * ns * 3;
+    int* ar = s_atom + rl * ns;
+    int* kr = s_cvk + rl * ns;
+    EstLeanRep& S = s_rep[rl];
+    if (live) {
+        const float* p = A.pos + (long long)r * P.rstride * P.ps;
+        const float* v = A.vel + (long long)r * P.rstride * P.ps;
+        D3 c[4], dc[4];
+        double Wg[4];
+#pragma unroll
+        for (int g = 0; g < 4; ++g) {
+            c[g] = d3(0, 0, 0);
+            Wg[g] = 1.0;
+            if (g < C.n_groups) {
+                const GroupDev& Gd = P.grp[C.gid0 + g];
+                double sx = 0, sy = 0, sz = 0, sw = 0;
+#pragma unroll 4
+                for (int i = 0; i < Gd.size; ++i) {
+                    const int s = Gd.begin + i;
+                    const D3 x = load_pos(p, slot_atom_of(P, r, s), P.ps);
+                    const double w = P.slot_weight ? (double)P.slot_weight[s] : 1.0;
+                    sx += w * x.x; sy += w * x.y; sz += w * x.z; sw += w;
+                }
+                const double iw = 1.0 / sw;
+                c[g] = d3(sx * iw, sy * iw, sz * iw);
+                Wg[g] = sw;
+            }
+        }
+        cv_jacobian_only(C.type, C.axis, c, dc);
+        double b = 0.0;
+#pragma unroll
+        for (int g = 0; g < 4; ++g)
+            if (g < C.n_groups) {
+                const GroupDev& Gd = P.grp[C.gid0 + g];
+                const double iw = 1.0 / Wg[g];
+                for (int i = 0; i < Gd.size; ++i) {
+                    const int s = Gd.begin + i, a = slot_atom_of(P, r, s);
+                    const double w = P.slot_weight ? (double)P.slot_weight[s] : 1.0;
+                    const double jx = w * (dc[g].x * iw), jy = w * (dc[g].y * iw), jz = w * (dc[g].z * iw);
+                    jr[s * 3] = jx; jr[s * 3 + 1] = jy; jr[s * 3 + 2] = jz;
+                    ar[s] = a; kr[s] = k;
+                    const double m = (double)__ldg(A.mass + a);
+                    const double px = m * (double)v[(long long)a * P.ps], py = m * (double)v[(long long)a * P.ps + 1],
+                                 pz = m * (double)v[(long long)a * P.ps + 2];
+                    b += jx * px + jy * py + jz * pz;
+                }
+            }
+#pragma unroll
+        for (int l = 0; l <= PSG_MAX_CV; ++l) S.M[k][l] = 0.0;
+        S.M[k][n_cv] = b;
+    }
+    __syncthreads();
+    if (live) {
+        // row k of G = J J^T: this CV's slots against every slot on the same atom (an atom shared by two CVs couples them)
+#pragma unroll
+        for (int g = 0; g < 4; ++g)
+            if (g < C.n_groups) {
+                const GroupDev& Gd = P.grp[C.gid0 + g];
+                for (int i = 0; i < Gd.size; ++i) {
+                    const int s = Gd.begin + i, a = ar[s];
+                    for (int s2 = 0; s2 < ns; ++s2) {
+                        if (ar[s2] != a) continue;
+                        S.M[k][kr[s2]] += jr[s * 3] * jr[s2 * 3] + jr[s * 3 + 1] * jr[s2 * 3 + 1] + jr[s * 3 + 2] * jr[s2 * 3 + 2];
+                    }
+                }
+            }
+    }
+    __syncthreads();
+    if (live && k == 0) {
+        double (*M)[PSG_MAX_CV + 1] = S.M;
+        double* W = S.W;
+        bool ok = true;
+        for (int q = 0; q < PSG_MAX_CV; ++q) W[q] = 0.0;
+        for (int c0 = 0; c0 < n_cv && ok; ++c0) {   // Gaussian elimination, partial pivoting (as in k_abf_estimate)
+            int piv = c0;
+            for (int q = c0 + 1; q < n_cv; ++q)
+                if (fabs(M[q][c0]) > fabs(M[piv][c0])) piv = q;
+            if (!(fabs(M[piv][c0]) > 0.0)) { ok = false; break; }
+            if (piv != c0)
+                for (int l = 0; l <= n_cv; ++l) { double t = M[c0][l]; M[c0][l] = M[piv][l]; M[piv][l] = t; }
+            for (int q = c0 + 1; q < n_cv; ++q) {
+                const double f = M[q][c0] / M[c0][c0];
+                for (int l = c0; l <= n_cv; ++l) M[q][l] -= f * M[c0][l];
+            }
+        }
+        if (ok)
+            for (int q = n_cv - 1; q >= 0; --q) {
+                double t = M[q][n_cv];
+                for (int l = q + 1; l < n_cv; ++l) t -= M[q][l] * W[l];
+                W[q] = t / M[q][q];
+            }
+        double* h1 = A.whist + ((long long)r * 2 + 0) * n_cv;
+        double* h2 = A.whist + ((long long)r * 2 + 1) * n_cv;
+        for (int q = 0; q < n_cv; ++q) {
+            if (A.first) { h1[q] = W[q]; h2[q] = W[q]; }
+            const double dW = (1.5 * W[q] - 2.0 * h1[q] + 0.5 * h2[q]) / A.dt;
+            const double fb = A.fbias_prev ? (double)A.fbias_prev[(long long)r * n_cv + q] : 0.0;
+            A.fsample[(long long)r * n_cv + q] = (float)(dW + fb);
+            h2[q] = h1[q];
+            h1[q] = W[q];
+        }
+    }
+}
+
+static bool est_lean_layout(const psg_ctx* c) {
+    const SysParams& P = c->sys;
+    if (P.n_ranges > 0 || P.any_rgyr || P.has_box || c->dti_cv >= 0 || P.n_cv < 1 || P.n_slots < 1) return false;
+    for (int k = 0; k < P.n_cv; ++k) {
+        const int t = P.cv[k].type;
+        if (!(t == PSG_CV_DISTANCE || t == PSG_CV_ANGLE || t == PSG_CV_DIHEDRAL || t == PSG_CV_DISPLACEMENT || t == PSG_CV_COM_COMPONENT))
+            return false;
+    }
+    return true;
+}
+
 cudaError_t psg_launch_abf_estimate(psg_ctx* c, const float* d_pos, const float* d_vel, const float* d_mass, double dt,
                                     const float* d_fbias_prev, float* d_fsample) {
     AbfEstArgs A{};
     A.pos = d_pos; A.vel = d_vel; A.mass = d_mass; A.fbias_prev = d_fbias_prev; A.whist = c->d_whist; A.fsample = d_fsample;
     A.dt = dt; A.first = c->est_first ? 1 : 0;
+    if (est_lean_layout(c)) {
+        const int ns = c->sys.n_slots;
+        const size_t smem = (size_t)EST_RB * ns * 3 * sizeof(double) + EST_RB * sizeof(EstLeanRep) + (size_t)2 * EST_RB * ns * sizeof(int);
+        if (smem <= 48 * 1024) {
+            k_abf_estimate_lean<<<(c->sys.R + EST_RB - 1) / EST_RB, EST_RB * c->sys.n_cv, smem, c->stream>>>(c->sys, A);
+            c->launches++;
+            c->est_first = false;
+            return cudaGetLastError();
+        }
+    }
     int grid = (c->sys.R + 3) / 4;
     const int cap = c->sm_count * 8;
     if (grid > cap) grid = cap;

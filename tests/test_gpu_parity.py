@@ -643,6 +643,20 @@ def test_fused_abf_step_two_threads_per_cv_kernel_on_weighted_groups(torch, psg,
     from paper_2301_04835_b200.psg import _view
     assert np.array_equal(_view(hp, (nb,), torch.int32, 0).cpu().numpy(), hist)
     assert np.allclose(_view(fp, (nb, 4), torch.float32, 0).cpu().numpy(), fsum, rtol=1e-5, atol=1e-3)
+    # the estimator on the same layout (k_abf_estimate_lean: one thread per (replica, CV); the weighted groups share no atoms
+    # within a replica, the angle and the dihedral of one replica are coupled only through the solve)
+    mass = rng.uniform(1.0, 16.0, size=N).astype(np.float32)
+    whist = np.zeros((R, 2, 4))
+    d_fs = torch.empty((R, 4), device="cuda")
+    for est_step in range(3):
+        vel = np.zeros((R, N, ps), np.float32)
+        vel[..., :3] = rng.normal(scale=0.5, size=(R, N, 3))
+        fb = None if est_step == 0 else rng.normal(scale=20.0, size=(R, 4)).astype(np.float32)
+        ctx.abf_estimate(dev(torch, pos), dev(torch, vel), dev(torch, mass), 0.002, None if fb is None else dev(torch, fb), d_fs)
+        ctx.sync_check()
+        ref, Wref = sysm.abf_estimate(pos, vel, mass, 0.002, fb, whist, first=(est_step == 0))
+        tol = np.maximum(np.maximum(1e-5 * np.abs(ref), 1e-6), 4e-7 * np.abs(Wref).max(axis=0) / 0.002)
+        assert np.all(np.abs(d_fs.cpu().numpy() - ref) <= tol), f"estimator step {est_step}: max err {np.abs(d_fs.cpu().numpy() - ref).max()}"
     # the Jacobian cache the fused step leaves (psg_apply_bias_forces would use it): the oracle's, slot by slot
     d_jac = torch.empty((R, 17, 3), device="cuda")
     d_xi = torch.empty((R, 4), device="cuda")
