@@ -151,25 +151,7 @@ __global__ void __launch_bounds__(EST_RB * PSG_MAX_CV) k_abf_estimate_lean(const
         const float* v = A.vel + (long long)r * P.rstride * P.ps;
         D3 c[4], dc[4];
         double Wg[4];
-#pragma unroll
-        for (int g = 0; g < 4; ++g) {
-            c[g] = d3(0, 0, 0);
-            Wg[g] = 1.0;
-            if (g < C.n_groups) {
-                const GroupDev& Gd = P.grp[C.gid0 + g];
-                double sx = 0, sy = 0, sz = 0, sw = 0;
-#pragma unroll 4
-                for (int i = 0; i < Gd.size; ++i) {
-                    const int s = Gd.begin + i;
-                    const D3 x = load_pos(p, slot_atom_of(P, r, s), P.ps);
-                    const double w = P.slot_weight ? (double)P.slot_weight[s] : 1.0;
-                    sx += w * x.x; sy += w * x.y; sz += w * x.z; sw += w;
-                }
-                const double iw = 1.0 / sw;
-                c[g] = d3(sx * iw, sy * iw, sz * iw);
-                Wg[g] = sw;
-            }
-        }
+        thread_group_centres(P, r, C, p, c, Wg);
         cv_jacobian_only(C.type, C.axis, c, dc);
         double b = 0.0;
 #pragma unroll
@@ -246,23 +228,12 @@ __global__ void __launch_bounds__(EST_RB * PSG_MAX_CV) k_abf_estimate_lean(const
     }
 }
 
-static bool est_lean_layout(const psg_ctx* c) {
-    const SysParams& P = c->sys;
-    if (P.n_ranges > 0 || P.any_rgyr || P.has_box || c->dti_cv >= 0 || P.n_cv < 1 || P.n_slots < 1) return false;
-    for (int k = 0; k < P.n_cv; ++k) {
-        const int t = P.cv[k].type;
-        if (!(t == PSG_CV_DISTANCE || t == PSG_CV_ANGLE || t == PSG_CV_DIHEDRAL || t == PSG_CV_DISPLACEMENT || t == PSG_CV_COM_COMPONENT))
-            return false;
-    }
-    return true;
-}
-
 cudaError_t psg_launch_abf_estimate(psg_ctx* c, const float* d_pos, const float* d_vel, const float* d_mass, double dt,
                                     const float* d_fbias_prev, float* d_fsample) {
     AbfEstArgs A{};
     A.pos = d_pos; A.vel = d_vel; A.mass = d_mass; A.fbias_prev = d_fbias_prev; A.whist = c->d_whist; A.fsample = d_fsample;
     A.dt = dt; A.first = c->est_first ? 1 : 0;
-    if (est_lean_layout(c)) {
+    if (psg_lean_layout(c)) {
         const int ns = c->sys.n_slots;
         const size_t smem = (size_t)EST_RB * ns * 3 * sizeof(double) + EST_RB * sizeof(EstLeanRep) + (size_t)2 * EST_RB * ns * sizeof(int);
         if (smem <= 48 * 1024) {

@@ -143,28 +143,9 @@ __global__ void __launch_bounds__(LEAN_RB * PSG_MAX_CV * 2) k_abf_step_lean(cons
     float jf[4][3];   // derivative thread: d xi_k / d c_g / W_g, rounded to binary32 like the ctx cache
     if (live) {
         const float* p = A.pos + (long long)r * P.rstride * P.ps;
-        // group centres with the arithmetic of warp_cv_eval's gather (same sums, same order, same division: xi keeps its bits)
         D3 c[4], dc[4];
         double Wg[4];
-#pragma unroll
-        for (int g = 0; g < 4; ++g) {
-            c[g] = d3(0, 0, 0);
-            Wg[g] = 1.0;
-            if (g < C.n_groups) {
-                const GroupDev& Gd = P.grp[C.gid0 + g];
-                double sx = 0, sy = 0, sz = 0, sw = 0;
-#pragma unroll 4
-                for (int i = 0; i < Gd.size; ++i) {
-                    const int s = Gd.begin + i;
-                    const D3 x = load_pos(p, slot_atom_of(P, r, s), P.ps);
-                    const double w = P.slot_weight ? (double)P.slot_weight[s] : 1.0;
-                    sx += w * x.x; sy += w * x.y; sz += w * x.z; sw += w;
-                }
-                const double iw = 1.0 / sw;
-                c[g] = d3(sx * iw, sy * iw, sz * iw);
-                Wg[g] = sw;
-            }
-        }
+        thread_group_centres(P, r, C, p, c, Wg);   // (the arithmetic of warp_cv_eval's gather: xi keeps its bits)
         if (role == 0) {
             const float v = (float)cv_from_centers<false>(C.type, C.axis, c, dc, nullptr);
             s_xi[rl][k] = v;
@@ -244,17 +225,6 @@ static long long abf_lean_capacity(const psg_ctx* c, int threads) {
     return (long long)n * c->sm_count;
 }
 
-static bool abf_lean_layout(const psg_ctx* c) {
-    const SysParams& P = c->sys;
-    if (P.n_ranges > 0 || P.any_rgyr || P.has_box || c->dti_cv >= 0 || P.n_cv < 1) return false;
-    for (int k = 0; k < P.n_cv; ++k) {
-        const int t = P.cv[k].type;
-        if (!(t == PSG_CV_DISTANCE || t == PSG_CV_ANGLE || t == PSG_CV_DIHEDRAL || t == PSG_CV_DISPLACEMENT || t == PSG_CV_COM_COMPONENT))
-            return false;
-    }
-    return true;
-}
-
 static int abf_blocks_per_sm(int device) {
     static int cache[PSG_MAX_DEVICES];
     static bool have[PSG_MAX_DEVICES] = {};
@@ -314,7 +284,7 @@ cudaError_t psg_launch_abf_step(psg_ctx* c, const float* d_pos, const float* d_f
     cudaLaunchAttribute attr[1];
     attr[0].id = cudaLaunchAttributeCooperative;   // co-residency is what makes the grid barrier safe
     attr[0].val.cooperative = 1;
-    if (abf_lean_layout(c)) {
+    if (psg_lean_layout(c)) {
         const int threads = LEAN_RB * P.n_cv * 2;
         const long long lgrid = (P.R + LEAN_RB - 1) / LEAN_RB;
         if (lgrid <= abf_lean_capacity(c, threads)) {

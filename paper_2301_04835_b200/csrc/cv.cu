@@ -170,6 +170,46 @@ __global__ void __launch_bounds__(256) k_cv_eval(const __grid_constant__ SysPara
 }
 
 // --------------------------------------------------------------------------------------------
+// psg_cv_eval for the common layout (psg_lean_layout: explicit groups, no box, point-group CVs): TWO THREADS per (replica, CV),
+// in different warps, one for the value (sqrt / atan2 chain), one for the derivative (cv_jacobian_only), each gathering the few
+// atoms of its CV's groups itself.  A binary64 warp instruction then carries 32 chains; the warp-per-replica kernel above issues
+// each of them for the 1-4 lanes that own a CV.  Same xi bits; the Jacobian agrees to ~1 ulp of binary64 before
+// it is rounded to binary32.
+#define CVL_RB 32   // replicas per CTA: CVL_RB x n_cv value threads followed by as many derivative threads (whole warps)
+__global__ void __launch_bounds__(CVL_RB * PSG_MAX_CV * 2) k_cv_eval_lean(const __grid_constant__ SysParams P, const float* __restrict__ pos,
+                                                                        float* __restrict__ xi, float* __restrict__ jac_user,
+                                                                        float* __restrict__ jac_cache) {
+    const int n_cv = P.n_cv, tid = threadIdx.x;
+    const int role = tid >= CVL_RB * n_cv ? 1 : 0;
+    const int t = tid - role * CVL_RB * n_cv, rl = t / n_cv, k = t - rl * n_cv;
+    const int r = blockIdx.x * CVL_RB + rl;
+    if (r >= P.R) return;
+    const CvDev& C = P.cv[k];
+    D3 c[4], dc[4];
+    double Wg[4];
+    thread_group_centres(P, r, C, pos + (long long)r * P.rstride * P.ps, c, Wg);
+    if (role == 0) {
+        xi[(long long)r * n_cv + k] = (float)cv_from_centers<false>(C.type, C.axis, c, dc, nullptr);
+        return;
+    }
+    cv_jacobian_only(C.type, C.axis, c, dc);
+#pragma unroll
+    for (int g = 0; g < 4; ++g)
+        if (g < C.n_groups) {
+            const GroupDev& Gd = P.grp[C.gid0 + g];
+            const double iw = 1.0 / Wg[g];
+            for (int i = 0; i < Gd.size; ++i) {
+                const int s = Gd.begin + i;
+                const double w = P.slot_weight ? (double)P.slot_weight[s] : 1.0;
+                const float jx = (float)(w * (dc[g].x * iw)), jy = (float)(w * (dc[g].y * iw)), jz = (float)(w * (dc[g].z * iw));
+                const long long o = ((long long)r * P.n_slots + s) * 3;
+                if (jac_user) { jac_user[o] = jx; jac_user[o + 1] = jy; jac_user[o + 2] = jz; }
+                jac_cache[o] = jx; jac_cache[o + 1] = jy; jac_cache[o + 2] = jz;
+            }
+        }
+}
+
+// --------------------------------------------------------------------------------------------
 // Sparse scatter: thread per (replica, slot). Atoms shared between CVs (6, 8, 14 of phi/psi) or between
 // walkers of a shared array collide, hence L2 reductions (force_add: red.global.add.v2.f32 + one scalar per float4 record).
 __global__ void __launch_bounds__(256) k_apply_sparse(const __grid_constant__ SysParams P, const float* __restrict__ jac,
@@ -302,6 +342,11 @@ cudaError_t psg_launch_cv_eval(psg_ctx* c, const float* d_pos, float* d_xi, floa
         if (P.has_box) k_range_second<true><<<g, 256, 0, c->stream>>>(P, d_pos, c->d_rpart2);
         else k_range_second<false><<<g, 256, 0, c->stream>>>(P, d_pos, c->d_rpart2);
         c->launches++;
+    }
+    if (psg_lean_layout(c)) {
+        k_cv_eval_lean<<<(P.R + CVL_RB - 1) / CVL_RB, CVL_RB * P.n_cv * 2, 0, c->stream>>>(P, d_pos, d_xi, d_jac, c->d_jac);
+        c->launches++;
+        return cudaGetLastError();
     }
     k_cv_eval<<<(P.R + 7) / 8, 256, 0, c->stream>>>(P, d_pos, c->d_rpart, d_xi, d_jac, c->d_jac, c->d_gdesc,
                                                     P.any_shape_range ? c->d_rpart2 : nullptr, P.any_shape_range ? c->d_gdesc_m : nullptr);

@@ -389,6 +389,32 @@ __device__ __forceinline__ void warp_cv_eval(const SysParams& P, int r, const fl
     __syncwarp();
 }
 
+// The centres (and total weights) of the groups of CV C of replica r, gathered by ONE thread with the arithmetic of
+// warp_cv_eval's gather (same sums, same order, same division: a CV value computed from them keeps its bits).  Explicit groups,
+// no box.  Used by the thread-per-(replica, CV) kernels.
+__device__ __forceinline__ void thread_group_centres(const SysParams& P, int r, const CvDev& C, const float* __restrict__ p, D3 (&c)[4],
+                                                     double (&Wg)[4]) {
+#pragma unroll
+    for (int g = 0; g < 4; ++g) {
+        c[g] = d3(0, 0, 0);
+        Wg[g] = 1.0;
+        if (g < C.n_groups) {
+            const GroupDev& Gd = P.grp[C.gid0 + g];
+            double sx = 0, sy = 0, sz = 0, sw = 0;
+#pragma unroll 4
+            for (int i = 0; i < Gd.size; ++i) {
+                const int s = Gd.begin + i;
+                const D3 x = load_pos(p, slot_atom_of(P, r, s), P.ps);
+                const double w = P.slot_weight ? (double)P.slot_weight[s] : 1.0;
+                sx += w * x.x; sy += w * x.y; sz += w * x.z; sw += w;
+            }
+            const double iw = 1.0 / sw;
+            c[g] = d3(sx * iw, sy * iw, sz * iw);
+            Wg[g] = sw;
+        }
+    }
+}
+
 // d(xi)/d(r_slot) for an explicit slot s (weight w_s) given the per-group vector
 __device__ __forceinline__ D3 slot_jacobian(const SysParams& P, int r, const float* __restrict__ pos,
                                             const WarpCvSmem& sm, int s) {

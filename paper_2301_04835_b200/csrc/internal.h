@@ -174,4 +174,15 @@ bool psg_range_step_supported(const psg_ctx* c, const float* d_pos, const float*
 cudaError_t psg_launch_range_step(psg_ctx* c, const float* d_pos, float* d_force);   // fused harmonic step over range groups
 bool psg_stream_capturing(const psg_ctx* c);
 size_t psg_hill_part_doubles(const psg_ctx* c, int* max_chunks_out, int* n_rtiles_out);
-
+// The layout the thread-per-(replica, CV) kernels cover (k_cv_eval_lean, k_abf_step_lean, k_abf_estimate_lean): explicit groups
+// only, no minimum-image box, no DistanceToInterface CV, every CV a point-group CV (no Rg, no shape CV).
+inline bool psg_lean_layout(const psg_ctx* c) {
+    const SysParams& P = c->sys;
+    if (P.n_ranges > 0 || P.any_rgyr || P.has_box || c->dti_cv >= 0 || P.n_cv < 1 || P.n_slots < 1) return false;
+    for (int k = 0; k < P.n_cv; ++k) {
+        const int t = P.cv[k].type;
+        if (!(t == PSG_CV_DISTANCE || t == PSG_CV_ANGLE || t == PSG_CV_DIHEDRAL || t == PSG_CV_DISPLACEMENT || t == PSG_CV_COM_COMPONENT))
+            return false;
+    }
+    return true;
+}
