@@ -613,15 +613,16 @@ def test_fused_abf_step_two_threads_per_cv_kernel_on_weighted_groups(torch, psg,
     shape, periodic, n_thr = np.array([4, 5, 3, 4], np.int32), np.array([0, 1, 0, 0], np.int32), 2
     nb = int(np.prod(shape))
     hist, fsum = np.zeros(nb, np.int32), np.zeros((nb, 4), np.float64)
+    abs_sum = np.zeros((nb, 4))                                   # sum of |f| per bin: what bounds the rounding of the device's Fsum
+    slot_cv = np.array([0] * 6 + [1] * 5 + [2] * 3 + [3] * 3)     # CV that owns each of the 17 slots
     ctx = psg.Context(0)
     ctx.set_layout(R, N, N, ps, ps)
     ctx.set_cvs(g_cvs, slot, sw, None)
     ctx.set_abf(lower, upper, shape, periodic, n_thr)
     f0 = np.zeros((R, N, ps), np.float32)
     f0[..., :3] = rng.standard_normal((R, N, 3)) * 50
-    f_ref = f0[..., :3].astype(np.float64)
-    d_f = dev(torch, f0)
     for step in range(1, 5):
+        d_f = dev(torch, f0)      # a fresh force array per step: the tolerance of a binary32 += is relative to ITS operands
         pos = np.zeros((R, N, ps), np.float32)
         pos[..., :3] = rng.normal(scale=0.9, size=(R, N, 3))
         fs = rng.normal(scale=30.0, size=(R, 4)).astype(np.float32)
@@ -632,13 +633,22 @@ def test_fused_abf_step_two_threads_per_cv_kernel_on_weighted_groups(torch, psg,
         out = ctx.read_step_outputs()
         xi_ref, jac_ref = sysm.cv_eval(pos)
         b_ref, dV_ref = orc.abf_update(xi_ref.astype(np.float32), fs, lower, upper, shape, periodic, n_thr, hist, fsum)
-        f_ref = sysm.apply_forces(pos, dV_ref, f_ref)
+        f_ref = sysm.apply_forces(pos, dV_ref, f0[..., :3].astype(np.float64))
         assert_close(out["xi"].cpu().numpy(), xi_ref, f"xi, step {step}", period=np.array([0, 2 * math.pi, 0, 0]))
         assert np.array_equal(out["bin"].cpu().numpy(), b_ref), f"bins, step {step}"
         assert (b_ref >= 0).sum() >= R // 3
+        # Fsum is a binary32 sum built by atomics in any order (the oracle's is binary64): the mean force of a bin carries
+        # ~ulp32 of sum |f| over the bin's samples, divided by the count, and the forces inherit it through the Jacobian
+        inb = b_ref >= 0
+        np.add.at(abs_sum, b_ref[inb], np.abs(fs[inb]).astype(np.float64))
+        dv_tol = np.zeros((R, 4))
+        dv_tol[inb] = 4e-7 * abs_sum[b_ref[inb]] / np.maximum(hist[b_ref[inb]], n_thr)[:, None]
         g = out["dVdxi"].cpu().numpy()
-        assert np.all(np.abs(g - dV_ref) <= np.maximum(1e-5 * np.abs(dV_ref), 1e-5)), f"mean force, step {step}"
-        assert_forces_close(d_f.cpu().numpy()[..., :3], f_ref, f0[..., :3], f"forces, step {step}")
+        assert np.all(np.abs(g - dV_ref) <= np.maximum(np.maximum(1e-5 * np.abs(dV_ref), 1e-6), dv_tol)), f"mean force, step {step}"
+        extra = np.zeros((R, N, 3))
+        for sl in range(17):
+            extra[np.arange(R), slot[:, sl]] += dv_tol[:, slot_cv[sl]][:, None] * np.abs(jac_ref[:, sl])
+        assert_forces_close(d_f.cpu().numpy()[..., :3], f_ref, f0[..., :3], f"forces, step {step}", extra)
     hp, fp, nbins = ctx.abf_state()
     from paper_2301_04835_b200.psg import _view
     assert np.array_equal(_view(hp, (nb,), torch.int32, 0).cpu().numpy(), hist)
